@@ -1,0 +1,69 @@
+"""Seeded synthetic workloads — the five BASELINE.json configs as plain parameter sets.
+
+This module is the ONLY thing the CUDA path's callers and the oracle's callers share.  It holds no
+arithmetic of the method (no Philox, no update rule, no heights): just sizes, probabilities, seeds and the
+integer record-time lists.  Everything else (initial lattices, disorder masks, turning points) is derived
+from the seed independently by each implementation.
+
+Record times: t_0 = 1, t_k = max(t_{k-1}+1, floor(T^(k/(K-1)) + 0.5)), last forced to T.
+The lists below are frozen literals; tests/test_workloads.py checks the rule reproduces them.
+"""
+from __future__ import annotations
+
+import math
+
+
+def log_spaced_times(T: int, K: int) -> list[int]:
+    ts = [1]
+    for k in range(1, K):
+        v = int(math.floor(T ** (k / (K - 1)) + 0.5))
+        ts.append(max(ts[-1] + 1, v))
+    ts[-1] = T
+    return ts
+
+
+_T40_1E4 = [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 13, 17, 22, 27, 35, 44, 55, 70, 89, 113, 143, 180, 229, 289, 367,
+            464, 588, 744, 943, 1194, 1512, 1914, 2424, 3070, 3888, 4924, 6236, 7897, 10000]
+_T50_1E5 = [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 13, 17, 21, 27, 34, 43, 54, 69, 87, 110, 139, 176, 222, 281, 356,
+            450, 569, 720, 910, 1151, 1456, 1842, 2330, 2947, 3728, 4715, 5964, 7543, 9541, 12068, 15264, 19307,
+            24421, 30888, 39069, 49417, 62506, 79060, 100000]
+_T20_1E3 = [1, 2, 3, 4, 5, 6, 9, 13, 18, 26, 38, 55, 78, 113, 162, 234, 336, 483, 695, 1000]
+
+# BASELINE.json `configs`[0..4]  (numbered 1..5 as in SURVEY.md §8(d)).
+CONFIGS = {
+    1: dict(name="config1_kpz_L64_S16_p1", kind="kpz", L=64, S=16, p=1.0, q=0.0, disorder=None, n_mcs=1000,
+            record_times=[1, 2, 4, 8, 16, 32, 64, 128, 256, 512, 1000], seed=1),
+    2: dict(name="config2_kpz_L8192_S1024_p075_q025", kind="kpz", L=8192, S=1024, p=0.75, q=0.25, disorder=None,
+            n_mcs=10_000, record_times=_T40_1E4, seed=2),
+    # disorder = (prob_slow_p, p_slow, prob_slow_q, q_slow)
+    3: dict(name="config3_disorder_L16384_S512", kind="kpz", L=16384, S=512, p=1.0, q=0.0,
+            disorder=(0.1, 0.5, 0.0, 0.0), n_mcs=100_000, record_times=_T50_1E5, seed=3),
+    4: dict(name="config4_stream_L2p28_S1_p09_q01", kind="kpz", L=1 << 28, S=1, p=0.9, q=0.1, disorder=None,
+            n_mcs=1000, record_times=_T20_1E3, seed=4),
+    5: dict(name="config5_lanes_L16384_S256", kind="lanes", L=16384, S=256, p_a=1.0, p_b=1.0, rho0=0.3,
+            turn_prob=0.05, turn_period=100, omega=0.1, n_mcs=100_000, record_times=_T50_1E5, seed=5),
+    # Auxiliary streamed runs: same kernel as config 4, dyadic rates (bandwidth-bound).
+    "4-aux-i": dict(name="config4aux1_stream_L2p28_p075_q025", kind="kpz", L=1 << 28, S=1, p=0.75, q=0.25,
+                    disorder=None, n_mcs=1000, record_times=_T20_1E3, seed=4),
+    "4-aux-ii": dict(name="config4aux2_stream_L2p32_p075_q025", kind="kpz", L=1 << 32, S=1, p=0.75, q=0.25,
+                     disorder=None, n_mcs=200, record_times=[1, 2, 4, 8, 16, 32, 64, 128, 200], seed=4),
+}
+
+
+def site_updates(cfg: dict, n_mcs: int | None = None, nsamples: int | None = None) -> int:
+    """Site updates of a run: L per MCS per sample; the two-lane model counts both lanes."""
+    n = cfg["n_mcs"] if n_mcs is None else n_mcs
+    s = cfg["S"] if nsamples is None else nsamples
+    lanes = 2 if cfg["kind"] == "lanes" else 1
+    return lanes * cfg["L"] * s * n
+
+
+def truncated(cfg: dict, n_mcs: int, nsamples: int | None = None, first_sample: int = 0) -> dict:
+    """The same workload cut to n_mcs steps / nsamples samples starting at global sample `first_sample`."""
+    c = dict(cfg)
+    c["n_mcs"] = n_mcs
+    c["record_times"] = [t for t in cfg["record_times"] if t <= n_mcs]
+    if nsamples is not None:
+        c["S"] = nsamples
+    c["first_sample"] = first_sample
+    return c
