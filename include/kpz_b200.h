@@ -1,0 +1,136 @@
+/*
+ * include/kpz_b200.h — C ABI of libkpz_b200.so: the B200 (sm_100a) hot path of arxiv/paper_1012_0385.
+ *
+ * What the library computes (citations: PAPER.md:<line> = /root/reference/PAPER.md; DESIGN §R<n> = the numbered
+ * readings in DESIGN.md §1):
+ *   - the two-sub-lattice Monte-Carlo sweep of the 1+1D RSOS/KPZ model in ASEP lattice-gas form on periodic
+ *     rings, site-dependent rates p_i, q_i with quenched bimodal disorder (PAPER.md:151-155,
+ *     Eq. 8), randomness from counter-based Philox4x32-10;
+ *   - heights h_x and the exact integer sums behind the width W of Eq. 3 at listed record
+ *     times, W^2 averaged over samples;
+ *   - the two-lane opposite-direction model with turning points.
+ *
+ * Conventions
+ *   - Every function returns 0 (KPZ_OK) or a negative error code; no exception or abort crosses the ABI.
+ *     kpz_last_error() returns a thread-local text for the last failing call.
+ *   - Pointers named d_* are DEVICE pointers, all others are HOST pointers.  The caller (PyTorch) allocates
+ *     all device memory — the workspace handed to *_create and every d_* output — and owns the CUDA stream;
+ *     the handle borrows them and they must outlive it.  The library performs no device allocation.
+ *   - All work is enqueued on the stream given at create time; only the calls documented "syncs" wait for it.
+ *   - Lattice / mask words use the NATURAL layout: bit (i & 31) of word (i >> 5) is site i; a sample occupies
+ *     L/32 consecutive uint32 words; samples are consecutive.  (Internally rings are kept de-interleaved.)
+ *   - L must be a multiple of 64, L >= 64.  Handles are not thread-safe; distinct handles are independent.
+ */
+#ifndef KPZ_B200_H
+#define KPZ_B200_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KPZ_OK 0
+#define KPZ_EINVAL (-1)       /* NULL pointer, L odd or < 4, probability outside [0,1], nsamples < 1, bad record times */
+#define KPZ_EUNSUPPORTED (-2) /* L not a multiple of 64, size beyond a path's limit, sum-of-squares overflow guard */
+#define KPZ_ENOMEM (-3)       /* workspace / output capacity too small */
+#define KPZ_ECUDA (-4)        /* CUDA launch or runtime error; text in kpz_last_error() */
+
+typedef struct kpz_sim kpz_sim;     /* opaque */
+typedef struct lanes_sim lanes_sim; /* opaque */
+
+/* Eq. 8: a site is "slow" with probability prob_slow_*, independently per site and sample
+ * (DESIGN §R8); slow sites use p_slow / q_slow instead of p / q. */
+typedef struct {
+  double prob_slow_p;
+  double p_slow;
+  double prob_slow_q;
+  double q_slow;
+} kpz_disorder;
+
+typedef struct {
+  int32_t first_sample; /* global index of sample 0 of this handle (part of the RNG key); default 0 */
+  int32_t offset_mode;  /* 0 = sub-lattice offset drawn per pass, 1 = alternating 0,1 */
+  int32_t path;         /* 0 auto, 1 force the on-chip per-sample kernel (K1), 2 force the streamed kernel (K3) */
+} kpz_options;
+
+#define KPZ_PATH_AUTO 0
+#define KPZ_PATH_ONCHIP 1
+#define KPZ_PATH_STREAM 2
+
+/* ---- KPZ / ASEP ring ensemble ----------------------------------------------------------------------------- */
+
+/* Bytes of device workspace kpz_create needs for these sizes (max_records = capacity of the record list). */
+int kpz_workspace_bytes(int64_t L, int32_t nsamples, const kpz_disorder* disorder, const kpz_options* opt,
+                        int32_t max_records, size_t* bytes);
+
+/* Create an ensemble of nsamples rings of L sites: flat start n_i = i & 1, rates p (forward) and
+ * q (backward), optional disorder (NULL = none), Philox key = seed.  d_workspace: device memory of at least
+ * kpz_workspace_bytes(...) bytes, 256-byte aligned.  cuda_stream: a cudaStream_t (NULL = default stream).
+ * Enqueues the initialisation kernels; does not sync. */
+int kpz_create(kpz_sim** out, int64_t L, int32_t nsamples, double p, double q, const kpz_disorder* disorder,
+               uint64_t seed, const kpz_options* opt, int32_t max_records, void* d_workspace, size_t workspace_bytes,
+               void* cuda_stream);
+
+/* Record times (host array): strictly increasing absolute MCS counts, t[0] > current time, nt <= max_records
+ * (DESIGN §R7).  Replaces the list and clears captured records. */
+int kpz_set_record_times(kpz_sim*, const int64_t* t, int32_t nt);
+
+/* Advance every sample by n_mcs Monte-Carlo steps (one MCS = two sub-lattice passes), capturing
+ * (sum h, sum h^2) per sample at every record time passed.  Asynchronous on the stream.
+ * run(a); run(b) is bit-identical to run(a+b). */
+int kpz_run(kpz_sim*, int64_t n_mcs);
+
+int kpz_time(const kpz_sim*, int64_t* t); /* MCS done so far (host value; no sync) */
+
+/* Copy the occupation bits out / in (device buffers, natural layout, nsamples * L/32 words).  Async. */
+int kpz_lattice(kpz_sim*, uint32_t* d_words);
+int kpz_set_lattice(kpz_sim*, const uint32_t* d_words);
+/* Quenched disorder tags, same layout; either pointer may be NULL.  Async. */
+int kpz_disorder_masks(kpz_sim*, uint32_t* d_slow_p, uint32_t* d_slow_q);
+int kpz_set_disorder_masks(kpz_sim*, const uint32_t* d_slow_p, const uint32_t* d_slow_q);
+
+/* Heights of one sample: d_h[x] = sum_{i<=x} (2 n_i - 1), x = 0..L-1, L int32 values
+ * on the device.  Async. */
+int kpz_heights(kpz_sim*, int32_t sample, int32_t* d_h);
+
+/* Records captured so far (host outputs; SYNCS the stream).  nt: in = capacity of the arrays, out = count.
+ * t[nt]; sum_h, sum_h2 [nt][nsamples] exact int64 (Eq. 3 sums); w2_mean[nt] = mean over samples of
+ * (L*sum_h2 - sum_h^2)/L^2.  Any output pointer may be NULL. */
+int kpz_roughness(kpz_sim*, int32_t* nt, int64_t* t, int64_t* sum_h, int64_t* sum_h2, double* w2_mean);
+
+int kpz_destroy(kpz_sim*);
+
+/* ---- two-lane opposite-direction model -------------------------------------------------- */
+
+int lanes_workspace_bytes(int64_t L, int32_t nsamples, int32_t max_records, size_t* bytes);
+
+/* Two rings of L sites per sample; lane A hops right with p_a, lane B hops left with p_b under the same
+ * sub-lattice schedule; initial occupation Bernoulli(rho0) per site per lane; each site is a turning point with
+ * probability turn_prob, redrawn every turn_period MCS (0 = never); at a turning point a particle changes lane
+ * with probability omega if the target site is empty. */
+int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, double p_b, double rho0, double turn_prob,
+                 int64_t turn_period, double omega, uint64_t seed, const kpz_options* opt, int32_t max_records,
+                 void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+int lanes_set_record_times(lanes_sim*, const int64_t* t, int32_t nt);
+int lanes_run(lanes_sim*, int64_t n_mcs);
+int lanes_time(const lanes_sim*, int64_t* t);
+/* Occupations of lanes A, B and the current turning-point mask (device, natural layout, any may be NULL). Async. */
+int lanes_state(lanes_sim*, uint32_t* d_a, uint32_t* d_b, uint32_t* d_turn);
+int lanes_set_state(lanes_sim*, const uint32_t* d_a, const uint32_t* d_b, const uint32_t* d_turn);
+/* Hop counts J_A, J_B and lane populations at the record times (host; SYNCS). */
+int lanes_currents(lanes_sim*, int32_t* nt, int64_t* t, int64_t* j_a, int64_t* j_b, int64_t* n_a, int64_t* n_b);
+/* Epoch-end occupancy counts [nsamples][L] per lane (device, uint32) and the snapshot count. SYNCS. */
+int lanes_profile(lanes_sim*, uint32_t* d_occ_a, uint32_t* d_occ_b, int64_t* nsnap);
+int lanes_destroy(lanes_sim*);
+
+/* ---- diagnostics ------------------------------------------------------------------------------------------ */
+const char* kpz_strerror(int code);
+const char* kpz_last_error(void);        /* thread-local detail of the last failing call */
+int64_t kpz_kernel_launches(void);       /* kernels launched by this library in this process so far */
+/* Which kernel family a handle's kpz_run uses: 1 = on-chip per-sample (K1), 2 = streamed (K3). */
+int kpz_path(const kpz_sim*, int32_t* path);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

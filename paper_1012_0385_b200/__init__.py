@@ -1,0 +1,12 @@
+"""paper_1012_0385_b200 — B200-native (sm_100a) KPZ/ASEP lattice-gas sweep behind a C ABI (include/kpz_b200.h).
+
+    from paper_1012_0385_b200 import KpzSim, LanesSim
+
+The package holds only what the hot path needs: csrc/ (CUDA kernels + C ABI), build.py (nvcc, in-tree) and
+binding.py (ctypes marshalling).  There is no CPU fallback.
+"""
+from .binding import (KPZ_PATH_AUTO, KPZ_PATH_ONCHIP, KPZ_PATH_STREAM, KpzError, KpzSim, LanesSim, kernel_launches,
+                      load_library, words_from_numpy, words_to_numpy)
+
+__all__ = ["KpzSim", "LanesSim", "KpzError", "load_library", "kernel_launches", "words_to_numpy", "words_from_numpy",
+           "KPZ_PATH_AUTO", "KPZ_PATH_ONCHIP", "KPZ_PATH_STREAM"]

@@ -1,0 +1,612 @@
+// kpz_api.cu — host side of the KPZ/ASEP ring ensemble: the kpz_* entry points of include/kpz_b200.h.
+// Validation, workspace carving, kernel dispatch.  Every step of the path runs in the kernels; this file only
+// launches them.  There is no CPU fallback: without a CUDA device every call that needs one fails with KPZ_ECUDA.
+#include <algorithm>
+#include <atomic>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "kpz_k1.cuh"
+#include "kpz_k3.cuh"
+#include "kpz_util.cuh"
+
+namespace kpz {
+
+// ---- error plumbing ------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+static std::atomic<long long> g_launches{0};
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+void count_launch(int n) { g_launches += n; }
+
+static int grid_for(size_t n, int block = 256) {
+  size_t g = (n + block - 1) / block;
+  return (int)std::min<size_t>(std::max<size_t>(g, 1), 148 * 16);
+}
+
+}  // namespace kpz
+
+using namespace kpz;
+
+struct kpz_sim {
+  int64_t L = 0;
+  int32_t S = 0;
+  int32_t max_records = 0;
+  int32_t path = 0;  // 1 = K1, 2 = K3
+  bool has_disorder = false, has_sp = false, has_sq = false;
+  KpzDev dev{};
+  cudaStream_t stream = nullptr;
+  // workspace carve-up (device)
+  uint32_t *E = nullptr, *O = nullptr, *E2 = nullptr, *O2 = nullptr;
+  uint32_t *SPE = nullptr, *SPO = nullptr, *SQE = nullptr, *SQO = nullptr;
+  long long *rec_t = nullptr, *rec_sum_h = nullptr, *rec_sum_h2 = nullptr;
+  int* scratch = nullptr;
+  size_t scratch_ints = 0;
+  unsigned char* k3off = nullptr;  // [(chunk+1)][S] offsets of a chunk of passes; row 0 = frame of the stored lattice
+  int* tiles = nullptr;            // [S][ntiles]
+  int ntiles = 0;
+  // host state
+  int64_t t = 0;
+  int frame = 0;  // K3: frame of the stored lattice (always 0 between calls)
+  std::vector<int64_t> rec_times;
+  int32_t nrec = 0;  // records captured (times <= t)
+};
+
+namespace {
+
+constexpr int kK3ChunkPasses = 4096;  // offsets are drawn for this many passes at a time
+
+struct Layout {
+  size_t off_E, off_O, off_E2, off_O2, off_SPE, off_SPO, off_SQE, off_SQO, off_rec_t, off_h, off_h2, off_scratch, total;
+  size_t off_k3off, off_tiles;
+  int PW, PWp, U, ntiles;
+  size_t scratch_ints;
+};
+
+int choose_path(int64_t L, const kpz_options* opt, int* path) {
+  const int64_t U = (L / 64 + 3) / 4;
+  int want = opt ? opt->path : KPZ_PATH_AUTO;
+  if (want == KPZ_PATH_AUTO) want = (U <= 1024) ? KPZ_PATH_ONCHIP : KPZ_PATH_STREAM;
+  if (want == KPZ_PATH_ONCHIP && U > 1024)
+    return fail(KPZ_EUNSUPPORTED, "on-chip path holds at most 262144 sites per sample (L=%lld)", (long long)L);
+  if (want != KPZ_PATH_ONCHIP && want != KPZ_PATH_STREAM) return fail(KPZ_EINVAL, "options.path must be 0, 1 or 2");
+  *path = want;
+  return KPZ_OK;
+}
+
+int validate_sizes(int64_t L, int32_t S, int32_t max_records) {
+  if (L < 4 || (L & 1) || S < 1 || max_records < 0) return fail(KPZ_EINVAL, "need even L >= 4, nsamples >= 1, max_records >= 0");
+  if (L % 64 != 0) return fail(KPZ_EUNSUPPORTED, "the CUDA path needs L to be a multiple of 64 (L=%lld)", (long long)L);
+  if (L > ((int64_t)1 << 36)) return fail(KPZ_EUNSUPPORTED, "L too large");
+  if ((L / 64) * (int64_t)S > ((int64_t)1 << 31) - 8) return fail(KPZ_EUNSUPPORTED, "nsamples * L too large");
+  return KPZ_OK;
+}
+
+Layout make_layout(int64_t L, int32_t S, bool disorder, int path, int32_t max_records) {
+  Layout y{};
+  y.PW = (int)(L / 64);
+  y.PWp = (y.PW + 3) / 4 * 4;
+  y.U = y.PWp / 4;
+  const size_t plane = align_up((size_t)S * y.PWp * 4, 256);
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    size_t o = off;
+    off += align_up(bytes, 256);
+    return o;
+  };
+  y.off_E = take(plane);
+  y.off_O = take(plane);
+  y.off_E2 = y.off_O2 = 0;
+  if (path == KPZ_PATH_STREAM) {
+    y.off_E2 = take(plane);
+    y.off_O2 = take(plane);
+  }
+  y.off_SPE = y.off_SPO = y.off_SQE = y.off_SQO = 0;
+  if (disorder) {
+    y.off_SPE = take(plane);
+    y.off_SPO = take(plane);
+    y.off_SQE = take(plane);
+    y.off_SQO = take(plane);
+  }
+  y.off_rec_t = take((size_t)std::max(max_records, 1) * 8);
+  y.off_h = take((size_t)std::max(max_records, 1) * S * 8);
+  y.off_h2 = take((size_t)std::max(max_records, 1) * S * 8);
+  y.scratch_ints = (size_t)y.PW + 8192;
+  y.off_scratch = take(y.scratch_ints * 4);
+  y.ntiles = (y.U + 255) / 256;
+  y.off_k3off = y.off_tiles = 0;
+  if (path == KPZ_PATH_STREAM) {
+    y.off_k3off = take((size_t)(kK3ChunkPasses + 1) * S);
+    y.off_tiles = take((size_t)S * y.ntiles * 4);
+  }
+  y.total = off;
+  return y;
+}
+
+// ---- K1 dispatch ---------------------------------------------------------------------------------------
+using K1Fn = void (*)(const KpzDev, const KpzRunArgs);
+
+template <bool SW, bool PARTIAL, int DIS>
+K1Fn k1_pick_nps(int nps) {
+  if (PARTIAL) return kpz_k1_kernel<SW, PARTIAL, DIS, -1>;
+  switch (nps) {
+    case 0: return kpz_k1_kernel<SW, false, DIS, 0>;
+    case 1: return kpz_k1_kernel<SW, false, DIS, 1>;
+    case 2: return kpz_k1_kernel<SW, false, DIS, 2>;
+    default: return kpz_k1_kernel<SW, false, DIS, -1>;
+  }
+}
+template <bool SW, bool PARTIAL>
+K1Fn k1_pick_dis(int dis, int nps) {
+  switch (dis) {
+    case 0: return k1_pick_nps<SW, PARTIAL, 0>(nps);
+    case 1: return k1_pick_nps<SW, PARTIAL, 1>(nps);
+    default: return k1_pick_nps<SW, PARTIAL, 2>(nps);
+  }
+}
+K1Fn k1_pick(bool single_warp, bool partial, int dis, int nps) {
+  if (single_warp) return partial ? k1_pick_dis<true, true>(dis, nps) : k1_pick_dis<true, false>(dis, nps);
+  return partial ? k1_pick_dis<false, true>(dis, nps) : k1_pick_dis<false, false>(dis, nps);
+}
+
+void refresh_planes(kpz_sim* sim) {
+  int np = std::max(planes_needed(sim->dev.thr[0]), planes_needed(sim->dev.thr[2]));
+  if (sim->has_sp) np = std::max(np, planes_needed(sim->dev.thr[1]));
+  if (sim->has_sq) np = std::max(np, planes_needed(sim->dev.thr[3]));
+  sim->dev.nplanes = np;
+  sim->dev.SPE = sim->has_sp || sim->has_sq ? sim->SPE : nullptr;
+  sim->dev.SPO = sim->has_sp || sim->has_sq ? sim->SPO : nullptr;
+  sim->dev.SQE = sim->has_sq ? sim->SQE : nullptr;
+  sim->dev.SQO = sim->has_sq ? sim->SQO : nullptr;
+}
+
+
+// ---- K3 dispatch and driver ------------------------------------------------------------------------------
+using K3Fn = void (*)(const KpzDev, const K3Pass);
+
+template <bool PARTIAL, int DIS>
+K3Fn k3_pick_nps(int nps) {
+  if (PARTIAL) return k3_pass_kernel<PARTIAL, DIS, -1>;
+  switch (nps) {
+    case 0: return k3_pass_kernel<false, DIS, 0>;
+    case 1: return k3_pass_kernel<false, DIS, 1>;
+    case 2: return k3_pass_kernel<false, DIS, 2>;
+    default: return k3_pass_kernel<false, DIS, -1>;
+  }
+}
+template <bool PARTIAL>
+K3Fn k3_pick_dis(int dis, int nps) {
+  switch (dis) {
+    case 0: return k3_pick_nps<PARTIAL, 0>(nps);
+    case 1: return k3_pick_nps<PARTIAL, 1>(nps);
+    default: return k3_pick_nps<PARTIAL, 2>(nps);
+  }
+}
+
+int k3_launch_pass(kpz_sim* sim, K3Fn fn, const unsigned char* fin, const unsigned char* fo, long long m, int pass) {
+  KpzDev D = sim->dev;
+  K3Pass A{};
+  A.Ein = sim->E;
+  A.Oin = sim->O;
+  A.Eout = sim->E2;
+  A.Oout = sim->O2;
+  A.fin = fin;
+  A.fo = fo;
+  A.m = m;
+  A.pass = pass;
+  const size_t nunits = (size_t)D.S * D.U;
+  fn<<<(unsigned)((nunits + 255) / 256), 256, 0, sim->stream>>>(D, A);
+  KPZ_LAUNCH_CHECK("k3_pass_kernel");
+  std::swap(sim->E, sim->E2);
+  std::swap(sim->O, sim->O2);
+  sim->dev.E = sim->E;
+  sim->dev.O = sim->O;
+  return KPZ_OK;
+}
+
+int k3_record(kpz_sim* sim, int ri) {
+  const KpzDev& D = sim->dev;
+  const bool partial = (D.PW % 4) != 0;
+  const int nt = sim->ntiles;
+  unsigned long long* oh = (unsigned long long*)(sim->rec_sum_h + (size_t)ri * D.S);
+  unsigned long long* oh2 = (unsigned long long*)(sim->rec_sum_h2 + (size_t)ri * D.S);
+  KPZ_CUDA_CHECK(cudaMemsetAsync(oh, 0, (size_t)D.S * 8, sim->stream));
+  KPZ_CUDA_CHECK(cudaMemsetAsync(oh2, 0, (size_t)D.S * 8, sim->stream));
+  if (partial) k3_tile_totals<true><<<D.S * nt, 256, 0, sim->stream>>>(sim->E, sim->O, D.S, D.U, D.PW, D.PWp, nt, sim->tiles);
+  else k3_tile_totals<false><<<D.S * nt, 256, 0, sim->stream>>>(sim->E, sim->O, D.S, D.U, D.PW, D.PWp, nt, sim->tiles);
+  KPZ_LAUNCH_CHECK("k3_tile_totals");
+  k3_scan_tiles<<<D.S, 1024, 0, sim->stream>>>(sim->tiles, nt);
+  KPZ_LAUNCH_CHECK("k3_scan_tiles");
+  if (partial) k3_tile_sums<true><<<D.S * nt, 256, 0, sim->stream>>>(sim->E, sim->O, D.S, D.U, D.PW, D.PWp, nt, sim->tiles, oh, oh2);
+  else k3_tile_sums<false><<<D.S * nt, 256, 0, sim->stream>>>(sim->E, sim->O, D.S, D.U, D.PW, D.PWp, nt, sim->tiles, oh, oh2);
+  KPZ_LAUNCH_CHECK("k3_tile_sums");
+  return KPZ_OK;
+}
+
+// The stored lattice is in frame 0 on entry and on exit.  Inside, the frame of each sample follows its offsets;
+// row r of k3off holds the offsets of pass (chunk start + r - 1), row 0 the frame the chunk starts in.
+int k3_run(kpz_sim* sim, int64_t n_mcs) {
+  const KpzDev& D0 = sim->dev;
+  const int S = D0.S;
+  const bool partial = (D0.PW % 4) != 0;
+  const int dis = sim->has_sq ? 2 : sim->has_sp ? 1 : 0;
+  K3Fn fn = partial ? k3_pick_dis<true>(dis, D0.nplanes) : k3_pick_dis<false>(dis, D0.nplanes);
+  const int nt = (int)sim->rec_times.size();
+  int ri = sim->nrec;
+  const long long pass_begin = 2 * (long long)sim->t, pass_end = 2 * (long long)(sim->t + n_mcs);
+  bool frame_dirty = false;  // some sample may be in frame 1
+  const unsigned char* prev_row = nullptr;  // device row with the current frames (nullptr = all zero)
+  for (long long c0 = pass_begin; c0 < pass_end; c0 += kK3ChunkPasses) {
+    const int np = (int)std::min<long long>(kK3ChunkPasses, pass_end - c0);
+    // row 0 := current frames, rows 1..np := offsets
+    k3_copy_row<<<grid_for(S), 256, 0, sim->stream>>>(sim->k3off, frame_dirty ? prev_row : nullptr, S);
+    KPZ_LAUNCH_CHECK("k3_copy_row");
+    k3_offsets<<<grid_for((size_t)np * S), 256, 0, sim->stream>>>(D0.keys, D0.first_sample, S, c0, np, D0.offset_mode,
+                                                                 sim->k3off);
+    KPZ_LAUNCH_CHECK("k3_offsets");
+    // the copy above read prev_row (= last row of this same buffer) before k3_offsets overwrites it only if
+    // np rows do not reach it; keep it safe by staging through row 0 first (stream order guarantees it).
+    int fin_row = 0;
+    for (int k = 0; k < np; ++k) {
+      const long long gp = c0 + k;
+      const long long m = gp >> 1;
+      const int pass = (int)(gp & 1);
+      int rc = k3_launch_pass(sim, fn, sim->k3off + (size_t)fin_row * S, sim->k3off + (size_t)(k + 1) * S, m, pass);
+      if (rc) return rc;
+      fin_row = k + 1;
+      frame_dirty = true;
+      if (pass == 1 && ri < nt && sim->rec_times[ri] == m + 1) {
+        // bring every sample to frame 0 (no update), then reduce
+        rc = k3_launch_pass(sim, fn, sim->k3off + (size_t)fin_row * S, nullptr, m, pass);
+        if (rc) return rc;
+        // from now on the stored frame is 0: point fin at a zero row (row 0 rewritten to zero)
+        k3_copy_row<<<grid_for(S), 256, 0, sim->stream>>>(sim->k3off, nullptr, S);
+        KPZ_LAUNCH_CHECK("k3_copy_row");
+        fin_row = 0;
+        frame_dirty = false;
+        rc = k3_record(sim, ri);
+        if (rc) return rc;
+        ++ri;
+      }
+    }
+    prev_row = sim->k3off + (size_t)fin_row * S;
+    if (fin_row == 0) frame_dirty = false;
+  }
+  if (frame_dirty) {
+    int rc = k3_launch_pass(sim, fn, prev_row, nullptr, 0, 0);
+    if (rc) return rc;
+  }
+  return KPZ_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* kpz_strerror(int code) {
+  switch (code) {
+    case KPZ_OK: return "ok";
+    case KPZ_EINVAL: return "invalid argument";
+    case KPZ_EUNSUPPORTED: return "unsupported size or configuration";
+    case KPZ_ENOMEM: return "workspace or output capacity too small";
+    case KPZ_ECUDA: return "CUDA error";
+    default: return "unknown error";
+  }
+}
+const char* kpz_last_error(void) { return kpz::g_err; }
+int64_t kpz_kernel_launches(void) { return (int64_t)kpz::g_launches.load(); }
+
+int kpz_workspace_bytes(int64_t L, int32_t nsamples, const kpz_disorder* disorder, const kpz_options* opt,
+                        int32_t max_records, size_t* bytes) {
+  if (!bytes) return fail(KPZ_EINVAL, "bytes is NULL");
+  int rc = validate_sizes(L, nsamples, max_records);
+  if (rc) return rc;
+  int path;
+  rc = choose_path(L, opt, &path);
+  if (rc) return rc;
+  *bytes = make_layout(L, nsamples, disorder != nullptr, path, max_records).total;
+  return KPZ_OK;
+}
+
+int kpz_create(kpz_sim** out, int64_t L, int32_t nsamples, double p, double q, const kpz_disorder* disorder,
+               uint64_t seed, const kpz_options* opt, int32_t max_records, void* d_workspace, size_t workspace_bytes,
+               void* cuda_stream) {
+  if (!out) return fail(KPZ_EINVAL, "out is NULL");
+  *out = nullptr;
+  int rc = validate_sizes(L, nsamples, max_records);
+  if (rc) return rc;
+  if (!valid_prob(p) || !valid_prob(q)) return fail(KPZ_EINVAL, "p and q must lie in [0,1]");
+  kpz_disorder d{0.0, p, 0.0, q};
+  if (disorder) {
+    d = *disorder;
+    if (!valid_prob(d.prob_slow_p) || !valid_prob(d.p_slow) || !valid_prob(d.prob_slow_q) || !valid_prob(d.q_slow))
+      return fail(KPZ_EINVAL, "disorder probabilities must lie in [0,1]");
+  }
+  kpz_options o{0, 0, 0};
+  if (opt) o = *opt;
+  if (o.first_sample < 0 || (o.offset_mode != 0 && o.offset_mode != 1))
+    return fail(KPZ_EINVAL, "options: first_sample >= 0, offset_mode in {0,1}");
+  int path;
+  rc = choose_path(L, &o, &path);
+  if (rc) return rc;
+  if (!d_workspace) return fail(KPZ_EINVAL, "d_workspace is NULL");
+  if (((uintptr_t)d_workspace & 255) != 0) return fail(KPZ_EINVAL, "d_workspace must be 256-byte aligned");
+  const Layout y = make_layout(L, nsamples, disorder != nullptr, path, max_records);
+  if (workspace_bytes < y.total)
+    return fail(KPZ_ENOMEM, "workspace has %zu bytes, %zu needed", workspace_bytes, y.total);
+
+  kpz_sim* sim = new (std::nothrow) kpz_sim();
+  if (!sim) return fail(KPZ_ENOMEM, "host allocation failed");
+  sim->L = L;
+  sim->S = nsamples;
+  sim->max_records = max_records;
+  sim->path = path;
+  sim->has_disorder = disorder != nullptr;
+  sim->has_sp = disorder && d.prob_slow_p > 0.0;
+  sim->has_sq = disorder && d.prob_slow_q > 0.0;
+  sim->stream = (cudaStream_t)cuda_stream;
+  char* base = (char*)d_workspace;
+  sim->E = (uint32_t*)(base + y.off_E);
+  sim->O = (uint32_t*)(base + y.off_O);
+  if (path == KPZ_PATH_STREAM) {
+    sim->E2 = (uint32_t*)(base + y.off_E2);
+    sim->O2 = (uint32_t*)(base + y.off_O2);
+  }
+  if (disorder) {
+    sim->SPE = (uint32_t*)(base + y.off_SPE);
+    sim->SPO = (uint32_t*)(base + y.off_SPO);
+    sim->SQE = (uint32_t*)(base + y.off_SQE);
+    sim->SQO = (uint32_t*)(base + y.off_SQO);
+  }
+  sim->rec_t = (long long*)(base + y.off_rec_t);
+  sim->rec_sum_h = (long long*)(base + y.off_h);
+  sim->rec_sum_h2 = (long long*)(base + y.off_h2);
+  sim->scratch = (int*)(base + y.off_scratch);
+  sim->scratch_ints = y.scratch_ints;
+  sim->ntiles = y.ntiles;
+  if (path == KPZ_PATH_STREAM) {
+    sim->k3off = (unsigned char*)(base + y.off_k3off);
+    sim->tiles = (int*)(base + y.off_tiles);
+  }
+
+  KpzDev& D = sim->dev;
+  D.keys = make_keys(seed);
+  D.thr[0] = make_thresh(p);
+  D.thr[1] = make_thresh(d.p_slow);
+  D.thr[2] = make_thresh(q);
+  D.thr[3] = make_thresh(d.q_slow);
+  D.offset_mode = o.offset_mode;
+  D.first_sample = o.first_sample;
+  D.S = nsamples;
+  D.PW = y.PW;
+  D.PWp = y.PWp;
+  D.U = y.U;
+  D.E = sim->E;
+  D.O = sim->O;
+  refresh_planes(sim);
+
+  const size_t nwords = (size_t)nsamples * y.PWp;
+  k_init_flat<<<grid_for(nwords), 256, 0, sim->stream>>>(sim->E, sim->O, nsamples, y.PW, y.PWp);
+  {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+      delete sim;
+      return fail(KPZ_ECUDA, "launch k_init_flat: %s", cudaGetErrorString(e));
+    }
+    count_launch();
+  }
+  if (disorder) {
+    const size_t ng = (size_t)nsamples * ((y.PW + 1) / 2);
+    if (y.PWp != y.PW) {  // pad words of the mask rows must be zero
+      for (uint32_t* m : {sim->SPE, sim->SPO, sim->SQE, sim->SQO}) {
+        k_zero_words<<<grid_for(nwords), 256, 0, sim->stream>>>(m, nwords);
+        count_launch();
+      }
+    }
+    k_site_mask_eo<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_SLOW_P, make_thresh(d.prob_slow_p),
+                                                              o.first_sample, nsamples, y.PW, y.PWp, sim->SPE, sim->SPO);
+    k_site_mask_eo<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_SLOW_Q, make_thresh(d.prob_slow_q),
+                                                              o.first_sample, nsamples, y.PW, y.PWp, sim->SQE, sim->SQO);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+      delete sim;
+      return fail(KPZ_ECUDA, "launch k_site_mask_eo: %s", cudaGetErrorString(e));
+    }
+    count_launch(2);
+  }
+  *out = sim;
+  return KPZ_OK;
+}
+
+int kpz_destroy(kpz_sim* sim) {
+  delete sim;
+  return KPZ_OK;
+}
+
+int kpz_path(const kpz_sim* sim, int32_t* path) {
+  if (!sim || !path) return fail(KPZ_EINVAL, "NULL argument");
+  *path = sim->path;
+  return KPZ_OK;
+}
+
+int kpz_time(const kpz_sim* sim, int64_t* t) {
+  if (!sim || !t) return fail(KPZ_EINVAL, "NULL argument");
+  *t = sim->t;
+  return KPZ_OK;
+}
+
+int kpz_set_record_times(kpz_sim* sim, const int64_t* t, int32_t nt) {
+  if (!sim || nt < 0 || (nt > 0 && !t)) return fail(KPZ_EINVAL, "bad record-time list");
+  if (nt > sim->max_records) return fail(KPZ_ENOMEM, "%d record times but max_records=%d", nt, sim->max_records);
+  for (int32_t k = 0; k < nt; ++k) {
+    if (t[k] < 1 || (k == 0 ? t[k] <= sim->t : t[k] <= t[k - 1]))
+      return fail(KPZ_EINVAL, "record times must be strictly increasing and later than the current time");
+    // |h| <= min(L, 1 + 8 t); refuse when L * bound^2 could overflow int64
+    const long double bound = std::min<long double>((long double)sim->L, 1.0L + 8.0L * (long double)t[k]);
+    if ((long double)sim->L * bound * bound >= 9.0e18L)
+      return fail(KPZ_EUNSUPPORTED, "sum of h^2 could overflow int64 at t=%lld for L=%lld", (long long)t[k], (long long)sim->L);
+    if (sim->path == KPZ_PATH_STREAM && bound >= 2147483647.0L)
+      return fail(KPZ_EUNSUPPORTED, "heights could overflow int32 at t=%lld", (long long)t[k]);
+  }
+  sim->rec_times.assign(t, t + nt);
+  sim->nrec = 0;
+  if (nt > 0) {
+    // stream-ordered copy from a staging vector that outlives the call: use a synchronous-safe pageable copy
+    KPZ_CUDA_CHECK(cudaMemcpyAsync(sim->rec_t, sim->rec_times.data(), (size_t)nt * 8, cudaMemcpyHostToDevice, sim->stream));
+    KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
+  }
+  return KPZ_OK;
+}
+
+int kpz_run(kpz_sim* sim, int64_t n_mcs) {
+  if (!sim || n_mcs < 0) return fail(KPZ_EINVAL, "bad arguments");
+  if (n_mcs == 0) return KPZ_OK;
+  if (((uint64_t)(sim->t + n_mcs) >> 54) != 0) return fail(KPZ_EUNSUPPORTED, "time beyond 2^54 MCS");
+  const int32_t nt = (int32_t)sim->rec_times.size();
+  int rc = KPZ_OK;
+  if (sim->path == KPZ_PATH_ONCHIP) {
+    KpzRunArgs A{};
+    A.t0 = sim->t;
+    A.n_mcs = n_mcs;
+    A.rec_t = sim->rec_t;
+    A.rec_begin = sim->nrec;
+    A.nt = nt;
+    A.rec_sum_h = sim->rec_sum_h;
+    A.rec_sum_h2 = sim->rec_sum_h2;
+    const KpzDev& D = sim->dev;
+    const bool single = D.U <= 32;
+    const bool partial = (D.PW % 4) != 0;
+    const int dis = sim->has_sq ? 2 : sim->has_sp ? 1 : 0;
+    K1Fn fn = k1_pick(single, partial, dis, D.nplanes);
+    const int block = (D.U + 31) / 32 * 32;
+    fn<<<sim->S, block, 0, sim->stream>>>(D, A);
+    KPZ_LAUNCH_CHECK("kpz_k1_kernel");
+  } else {
+    rc = k3_run(sim, n_mcs);
+    if (rc) return rc;
+  }
+  sim->t += n_mcs;
+  while (sim->nrec < nt && sim->rec_times[sim->nrec] <= sim->t) sim->nrec++;
+  return KPZ_OK;
+}
+
+int kpz_lattice(kpz_sim* sim, uint32_t* d_words) {
+  if (!sim || !d_words) return fail(KPZ_EINVAL, "NULL argument");
+  const KpzDev& D = sim->dev;
+  k_eo_to_nat<<<grid_for((size_t)D.S * D.PW), 256, 0, sim->stream>>>(sim->E, sim->O, D.S, D.PW, D.PWp, d_words);
+  KPZ_LAUNCH_CHECK("k_eo_to_nat");
+  return KPZ_OK;
+}
+
+int kpz_set_lattice(kpz_sim* sim, const uint32_t* d_words) {
+  if (!sim || !d_words) return fail(KPZ_EINVAL, "NULL argument");
+  const KpzDev& D = sim->dev;
+  k_nat_to_eo<<<grid_for((size_t)D.S * D.PW), 256, 0, sim->stream>>>(d_words, D.S, D.PW, D.PWp, sim->E, sim->O);
+  KPZ_LAUNCH_CHECK("k_nat_to_eo");
+  return KPZ_OK;
+}
+
+int kpz_disorder_masks(kpz_sim* sim, uint32_t* d_slow_p, uint32_t* d_slow_q) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  const KpzDev& D = sim->dev;
+  const size_t n = (size_t)D.S * D.PW;
+  if (d_slow_p) {
+    if (sim->has_disorder) k_eo_to_nat<<<grid_for(n), 256, 0, sim->stream>>>(sim->SPE, sim->SPO, D.S, D.PW, D.PWp, d_slow_p);
+    else k_zero_words<<<grid_for(2 * n), 256, 0, sim->stream>>>(d_slow_p, 2 * n);
+    KPZ_LAUNCH_CHECK("disorder_masks(p)");
+  }
+  if (d_slow_q) {
+    if (sim->has_disorder) k_eo_to_nat<<<grid_for(n), 256, 0, sim->stream>>>(sim->SQE, sim->SQO, D.S, D.PW, D.PWp, d_slow_q);
+    else k_zero_words<<<grid_for(2 * n), 256, 0, sim->stream>>>(d_slow_q, 2 * n);
+    KPZ_LAUNCH_CHECK("disorder_masks(q)");
+  }
+  return KPZ_OK;
+}
+
+int kpz_set_disorder_masks(kpz_sim* sim, const uint32_t* d_slow_p, const uint32_t* d_slow_q) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  if (!sim->has_disorder) return fail(KPZ_EINVAL, "handle was created without a disorder description");
+  const KpzDev& D = sim->dev;
+  const size_t n = (size_t)D.S * D.PW;
+  if (d_slow_p) {
+    k_nat_to_eo<<<grid_for(n), 256, 0, sim->stream>>>(d_slow_p, D.S, D.PW, D.PWp, sim->SPE, sim->SPO);
+    KPZ_LAUNCH_CHECK("set_disorder_masks(p)");
+    sim->has_sp = true;
+  }
+  if (d_slow_q) {
+    k_nat_to_eo<<<grid_for(n), 256, 0, sim->stream>>>(d_slow_q, D.S, D.PW, D.PWp, sim->SQE, sim->SQO);
+    KPZ_LAUNCH_CHECK("set_disorder_masks(q)");
+    sim->has_sq = true;
+  }
+  refresh_planes(sim);
+  return KPZ_OK;
+}
+
+int kpz_heights(kpz_sim* sim, int32_t sample, int32_t* d_h) {
+  if (!sim || !d_h || sample < 0 || sample >= sim->S) return fail(KPZ_EINVAL, "bad arguments");
+  if (sim->L > 0x7FFFFFFF) return fail(KPZ_EUNSUPPORTED, "heights need L < 2^31");
+  const KpzDev& D = sim->dev;
+  const uint32_t* E = sim->E + (size_t)sample * D.PWp;
+  const uint32_t* O = sim->O + (size_t)sample * D.PWp;
+  k_group_totals<<<grid_for(D.PW), 256, 0, sim->stream>>>(E, O, D.PW, sim->scratch);
+  KPZ_LAUNCH_CHECK("k_group_totals");
+  k_exclusive_scan_1block<<<1, 1024, 0, sim->stream>>>(sim->scratch, D.PW);
+  KPZ_LAUNCH_CHECK("k_exclusive_scan_1block");
+  k_heights_expand<<<grid_for(D.PW, 128), 128, 0, sim->stream>>>(E, O, sim->scratch, D.PW, d_h);
+  KPZ_LAUNCH_CHECK("k_heights_expand");
+  return KPZ_OK;
+}
+
+int kpz_roughness(kpz_sim* sim, int32_t* nt, int64_t* t, int64_t* sum_h, int64_t* sum_h2, double* w2_mean) {
+  if (!sim || !nt) return fail(KPZ_EINVAL, "NULL argument");
+  if (*nt < sim->nrec) return fail(KPZ_ENOMEM, "capacity %d < %d records", *nt, sim->nrec);
+  const int32_t n = sim->nrec;
+  const size_t cells = (size_t)n * sim->S;
+  std::vector<int64_t> h, h2;
+  int64_t* ph = sum_h;
+  int64_t* ph2 = sum_h2;
+  if (n > 0) {
+    if (!ph) {
+      h.resize(cells);
+      ph = h.data();
+    }
+    if (!ph2) {
+      h2.resize(cells);
+      ph2 = h2.data();
+    }
+    KPZ_CUDA_CHECK(cudaMemcpyAsync(ph, sim->rec_sum_h, cells * 8, cudaMemcpyDeviceToHost, sim->stream));
+    KPZ_CUDA_CHECK(cudaMemcpyAsync(ph2, sim->rec_sum_h2, cells * 8, cudaMemcpyDeviceToHost, sim->stream));
+  }
+  KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
+  for (int32_t k = 0; k < n; ++k) {
+    if (t) t[k] = sim->rec_times[k];
+    if (w2_mean) {
+      // Eq. 3 squared per sample, averaged over samples
+      double acc = 0.0;
+      for (int32_t s = 0; s < sim->S; ++s) {
+        const __int128 s1 = ph[(size_t)k * sim->S + s], s2 = ph2[(size_t)k * sim->S + s];
+        const __int128 num = (__int128)sim->L * s2 - s1 * s1;
+        acc += (double)num / ((double)sim->L * (double)sim->L);
+      }
+      w2_mean[k] = acc / (double)sim->S;
+    }
+  }
+  *nt = n;
+  return KPZ_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,262 @@
+// lanes_api.cu — host side of the two-lane model: the lanes_* entry points of include/kpz_b200.h.
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "lanes_k4.cuh"
+
+using namespace kpz;
+
+struct lanes_sim {
+  int64_t L = 0;
+  int32_t S = 0;
+  int32_t max_records = 0;
+  LanesDev dev{};
+  cudaStream_t stream = nullptr;
+  long long* rec_t = nullptr;
+  long long* rec = nullptr;  // [4][max_records][S] (plane stride = nt * S of the current list)
+  int64_t t = 0;
+  std::vector<int64_t> rec_times;
+  int32_t nrec = 0;
+};
+
+namespace {
+
+struct LLayout {
+  size_t off_A, off_B, off_T, off_JA, off_JB, off_occA, off_occB, off_rec_t, off_rec, total;
+  int W, Wp, U;
+};
+
+int lanes_validate(int64_t L, int32_t S, int32_t max_records) {
+  if (L < 4 || (L & 1) || S < 1 || max_records < 0) return fail(KPZ_EINVAL, "need even L >= 4, nsamples >= 1, max_records >= 0");
+  if (L % 64 != 0) return fail(KPZ_EUNSUPPORTED, "the CUDA path needs L to be a multiple of 64 (L=%lld)", (long long)L);
+  if (L > 262144) return fail(KPZ_EUNSUPPORTED, "the two-lane kernel holds at most 262144 sites per lane on chip (L=%lld)", (long long)L);
+  if ((int64_t)S * L > ((int64_t)1 << 33)) return fail(KPZ_EUNSUPPORTED, "nsamples * L too large");
+  return KPZ_OK;
+}
+
+LLayout lanes_layout(int64_t L, int32_t S, int32_t max_records) {
+  LLayout y{};
+  y.W = (int)(L / 32);
+  y.Wp = (y.W + 7) / 8 * 8;
+  y.U = y.Wp / 8;
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    size_t o = off;
+    off += align_up(bytes, 256);
+    return o;
+  };
+  const size_t plane = (size_t)S * y.Wp * 4;
+  y.off_A = take(plane);
+  y.off_B = take(plane);
+  y.off_T = take(plane);
+  y.off_JA = take((size_t)S * 8);
+  y.off_JB = take((size_t)S * 8);
+  y.off_occA = take((size_t)S * L * 4);
+  y.off_occB = take((size_t)S * L * 4);
+  y.off_rec_t = take((size_t)std::max(max_records, 1) * 8);
+  y.off_rec = take((size_t)4 * std::max(max_records, 1) * S * 8);
+  y.total = off;
+  return y;
+}
+
+int grid_for(size_t n, int block = 256) {
+  size_t g = (n + block - 1) / block;
+  return (int)std::min<size_t>(std::max<size_t>(g, 1), 148 * 16);
+}
+
+}  // namespace
+
+extern "C" {
+
+int lanes_workspace_bytes(int64_t L, int32_t nsamples, int32_t max_records, size_t* bytes) {
+  if (!bytes) return fail(KPZ_EINVAL, "bytes is NULL");
+  int rc = lanes_validate(L, nsamples, max_records);
+  if (rc) return rc;
+  *bytes = lanes_layout(L, nsamples, max_records).total;
+  return KPZ_OK;
+}
+
+int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, double p_b, double rho0, double turn_prob,
+                 int64_t turn_period, double omega, uint64_t seed, const kpz_options* opt, int32_t max_records,
+                 void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return fail(KPZ_EINVAL, "out is NULL");
+  *out = nullptr;
+  int rc = lanes_validate(L, nsamples, max_records);
+  if (rc) return rc;
+  if (!valid_prob(p_a) || !valid_prob(p_b) || !valid_prob(rho0) || !valid_prob(turn_prob) || !valid_prob(omega) ||
+      turn_period < 0)
+    return fail(KPZ_EINVAL, "probabilities must lie in [0,1] and turn_period >= 0");
+  kpz_options o{0, 0, 0};
+  if (opt) o = *opt;
+  if (o.first_sample < 0 || (o.offset_mode != 0 && o.offset_mode != 1))
+    return fail(KPZ_EINVAL, "options: first_sample >= 0, offset_mode in {0,1}");
+  if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(KPZ_EINVAL, "d_workspace must be non-NULL and 256-byte aligned");
+  const LLayout y = lanes_layout(L, nsamples, max_records);
+  if (workspace_bytes < y.total) return fail(KPZ_ENOMEM, "workspace has %zu bytes, %zu needed", workspace_bytes, y.total);
+  lanes_sim* sim = new (std::nothrow) lanes_sim();
+  if (!sim) return fail(KPZ_ENOMEM, "host allocation failed");
+  sim->L = L;
+  sim->S = nsamples;
+  sim->max_records = max_records;
+  sim->stream = (cudaStream_t)cuda_stream;
+  char* base = (char*)d_workspace;
+  LanesDev& D = sim->dev;
+  D.keys = make_keys(seed);
+  D.t_pa = make_thresh(p_a);
+  D.t_pb = make_thresh(p_b);
+  D.t_turn = make_thresh(turn_prob);
+  D.t_omega = make_thresh(omega);
+  D.np_a = planes_needed(D.t_pa);
+  D.np_b = planes_needed(D.t_pb);
+  D.np_w = planes_needed(D.t_omega);
+  D.offset_mode = o.offset_mode;
+  D.first_sample = o.first_sample;
+  D.S = nsamples;
+  D.W = y.W;
+  D.Wp = y.Wp;
+  D.U = y.U;
+  D.period = turn_period;
+  D.A = (uint32_t*)(base + y.off_A);
+  D.B = (uint32_t*)(base + y.off_B);
+  D.T = (uint32_t*)(base + y.off_T);
+  D.JA = (unsigned long long*)(base + y.off_JA);
+  D.JB = (unsigned long long*)(base + y.off_JB);
+  D.occA = (uint32_t*)(base + y.off_occA);
+  D.occB = (uint32_t*)(base + y.off_occB);
+  sim->rec_t = (long long*)(base + y.off_rec_t);
+  sim->rec = (long long*)(base + y.off_rec);
+
+  cudaError_t e = cudaMemsetAsync(base, 0, y.off_rec_t, sim->stream);  // lattices (incl. pad words), counters, profile
+  if (e != cudaSuccess) {
+    delete sim;
+    return fail(KPZ_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+  }
+  const Thresh t_rho = make_thresh(rho0);
+  const size_t ng = (size_t)nsamples * ((y.W + 3) / 4);
+  k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_INIT_A, t_rho, 0, o.first_sample, nsamples, y.W, y.Wp, D.A);
+  k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_INIT_B, t_rho, 0, o.first_sample, nsamples, y.W, y.Wp, D.B);
+  k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_TURN, D.t_turn, 0, o.first_sample, nsamples, y.W, y.Wp, D.T);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    delete sim;
+    return fail(KPZ_ECUDA, "launch k_site_mask_nat: %s", cudaGetErrorString(e));
+  }
+  count_launch(3);
+  *out = sim;
+  return KPZ_OK;
+}
+
+int lanes_destroy(lanes_sim* sim) {
+  delete sim;
+  return KPZ_OK;
+}
+
+int lanes_time(const lanes_sim* sim, int64_t* t) {
+  if (!sim || !t) return fail(KPZ_EINVAL, "NULL argument");
+  *t = sim->t;
+  return KPZ_OK;
+}
+
+int lanes_set_record_times(lanes_sim* sim, const int64_t* t, int32_t nt) {
+  if (!sim || nt < 0 || (nt > 0 && !t)) return fail(KPZ_EINVAL, "bad record-time list");
+  if (nt > sim->max_records) return fail(KPZ_ENOMEM, "%d record times but max_records=%d", nt, sim->max_records);
+  for (int32_t k = 0; k < nt; ++k)
+    if (t[k] < 1 || (k == 0 ? t[k] <= sim->t : t[k] <= t[k - 1]))
+      return fail(KPZ_EINVAL, "record times must be strictly increasing and later than the current time");
+  sim->rec_times.assign(t, t + nt);
+  sim->nrec = 0;
+  if (nt > 0) {
+    KPZ_CUDA_CHECK(cudaMemcpyAsync(sim->rec_t, sim->rec_times.data(), (size_t)nt * 8, cudaMemcpyHostToDevice, sim->stream));
+    KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
+  }
+  return KPZ_OK;
+}
+
+int lanes_run(lanes_sim* sim, int64_t n_mcs) {
+  if (!sim || n_mcs < 0) return fail(KPZ_EINVAL, "bad arguments");
+  if (n_mcs == 0) return KPZ_OK;
+  if (((uint64_t)(sim->t + n_mcs) >> 54) != 0) return fail(KPZ_EUNSUPPORTED, "time beyond 2^54 MCS");
+  const LanesDev& D = sim->dev;
+  const int32_t nt = (int32_t)sim->rec_times.size();
+  LanesRunArgs A{};
+  A.t0 = sim->t;
+  A.n_mcs = n_mcs;
+  A.rec_t = sim->rec_t;
+  A.rec_begin = sim->nrec;
+  A.nt = nt;
+  A.rec = sim->rec;
+  const bool single = D.U <= 32;
+  const bool partial = (D.W % 8) != 0;
+  const int block = (D.U + 31) / 32 * 32;
+  if (single) {
+    if (partial) lanes_k4_kernel<true, true><<<sim->S, block, 0, sim->stream>>>(D, A);
+    else lanes_k4_kernel<true, false><<<sim->S, block, 0, sim->stream>>>(D, A);
+  } else {
+    if (partial) lanes_k4_kernel<false, true><<<sim->S, block, 0, sim->stream>>>(D, A);
+    else lanes_k4_kernel<false, false><<<sim->S, block, 0, sim->stream>>>(D, A);
+  }
+  KPZ_LAUNCH_CHECK("lanes_k4_kernel");
+  sim->t += n_mcs;
+  while (sim->nrec < nt && sim->rec_times[sim->nrec] <= sim->t) sim->nrec++;
+  return KPZ_OK;
+}
+
+int lanes_state(lanes_sim* sim, uint32_t* d_a, uint32_t* d_b, uint32_t* d_turn) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  const LanesDev& D = sim->dev;
+  const size_t n = (size_t)D.S * D.W;
+  const uint32_t* src[3] = {D.A, D.B, D.T};
+  uint32_t* dst[3] = {d_a, d_b, d_turn};
+  for (int k = 0; k < 3; ++k)
+    if (dst[k]) {
+      k_copy_rows<<<grid_for(n), 256, 0, sim->stream>>>(src[k], D.S, D.W, D.Wp, D.W, dst[k]);
+      KPZ_LAUNCH_CHECK("k_copy_rows");
+    }
+  return KPZ_OK;
+}
+
+int lanes_set_state(lanes_sim* sim, const uint32_t* d_a, const uint32_t* d_b, const uint32_t* d_turn) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  const LanesDev& D = sim->dev;
+  const size_t n = (size_t)D.S * D.W;
+  const uint32_t* src[3] = {d_a, d_b, d_turn};
+  uint32_t* dst[3] = {D.A, D.B, D.T};
+  for (int k = 0; k < 3; ++k)
+    if (src[k]) {
+      k_copy_rows<<<grid_for(n), 256, 0, sim->stream>>>(src[k], D.S, D.W, D.W, D.Wp, dst[k]);
+      KPZ_LAUNCH_CHECK("k_copy_rows");
+    }
+  return KPZ_OK;
+}
+
+int lanes_currents(lanes_sim* sim, int32_t* nt, int64_t* t, int64_t* j_a, int64_t* j_b, int64_t* n_a, int64_t* n_b) {
+  if (!sim || !nt) return fail(KPZ_EINVAL, "NULL argument");
+  if (*nt < sim->nrec) return fail(KPZ_ENOMEM, "capacity %d < %d records", *nt, sim->nrec);
+  const int32_t n = sim->nrec;
+  const size_t cells = (size_t)n * sim->S;
+  const size_t plane = sim->rec_times.size() * (size_t)sim->S;
+  int64_t* dst[4] = {j_a, j_b, n_a, n_b};
+  if (n > 0)
+    for (int k = 0; k < 4; ++k)
+      if (dst[k])
+        KPZ_CUDA_CHECK(cudaMemcpyAsync(dst[k], sim->rec + k * plane, cells * 8, cudaMemcpyDeviceToHost, sim->stream));
+  KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
+  for (int32_t k = 0; k < n; ++k)
+    if (t) t[k] = sim->rec_times[k];
+  *nt = n;
+  return KPZ_OK;
+}
+
+int lanes_profile(lanes_sim* sim, uint32_t* d_occ_a, uint32_t* d_occ_b, int64_t* nsnap) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  const size_t bytes = (size_t)sim->S * sim->L * 4;
+  if (d_occ_a) KPZ_CUDA_CHECK(cudaMemcpyAsync(d_occ_a, sim->dev.occA, bytes, cudaMemcpyDeviceToDevice, sim->stream));
+  if (d_occ_b) KPZ_CUDA_CHECK(cudaMemcpyAsync(d_occ_b, sim->dev.occB, bytes, cudaMemcpyDeviceToDevice, sim->stream));
+  KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
+  if (nsnap) *nsnap = sim->dev.period > 0 ? sim->t / sim->dev.period : 0;
+  return KPZ_OK;
+}
+
+}  // extern "C"

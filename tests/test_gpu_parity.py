@@ -1,0 +1,360 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle, bit for bit, on the
+same seeds — lattice words, disorder masks, int32 heights, exact sums, hop counts, populations, profiles.
+
+Run on the B200 box with:  python -m pytest tests -m gpu
+"""
+import numpy as np
+import pytest
+
+import workloads
+from oracle import kpzref as R
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def K():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1012_0385_b200 as pkg
+    pkg.load_library()
+    return pkg
+
+
+def run_both_kpz(K, L, S, p, q, disorder=None, seed=1, first_sample=0, offset_mode=0, path=0, times=(), chunks=(),
+                 start=None, check_heights=(0,)):
+    """Run oracle and CUDA path on the same parameters; compare everything; return the GPU records."""
+    total = sum(chunks)
+    ref = R.KpzRef(L, S, p, q, disorder=disorder, seed=seed, first_sample=first_sample, offset_mode=offset_mode)
+    gpu = K.KpzSim(L, S, p, q, disorder=disorder, seed=seed, first_sample=first_sample, offset_mode=offset_mode,
+                   path=path, max_records=max(len(times), 1))
+    if start is not None:
+        ref.set_lattice(start)
+        gpu.set_lattice(K.words_from_numpy(start, gpu.device))
+    if disorder is not None:
+        rp, rq = ref.disorder_masks()
+        gp, gq = gpu.disorder_masks()
+        assert np.array_equal(K.words_to_numpy(gp), rp), "slow-p masks differ"
+        assert np.array_equal(K.words_to_numpy(gq), rq), "slow-q masks differ"
+    times = [t for t in times if t <= total]
+    ref.set_record_times(times)
+    gpu.set_record_times(times)
+    assert np.array_equal(K.words_to_numpy(gpu.lattice()), ref.lattice()), "initial lattices differ"
+    done = 0
+    for n in chunks:
+        ref.run(n)
+        gpu.run(n)
+        done += n
+        assert gpu.time == ref.time == done
+        assert np.array_equal(K.words_to_numpy(gpu.lattice()), ref.lattice()), f"lattices differ at t={done}"
+    rr, gr = ref.roughness(), gpu.roughness()
+    assert list(gr["t"]) == list(rr["t"]) == times
+    assert np.array_equal(gr["sum_h"], rr["sum_h"]), "sum h differs"
+    assert np.array_equal(gr["sum_h2"], rr["sum_h2"]), "sum h^2 differs"
+    assert np.array_equal(gr["w2_mean"], rr["w2_mean"]) or np.allclose(gr["w2_mean"], rr["w2_mean"], rtol=1e-15, atol=0)
+    for s in check_heights:
+        if s < S:
+            assert np.array_equal(gpu.heights(s).cpu().numpy(), ref.heights(s)), f"heights of sample {s} differ"
+    return gpu, gr
+
+
+# ---------------------------------------------------------------------------------------------------------
+# random numbers
+# ---------------------------------------------------------------------------------------------------------
+
+def _hooks():
+    import ctypes as C
+    from paper_1012_0385_b200 import binding
+    return C.CDLL(binding.HOOKS_PATH)
+
+
+def test_device_philox_matches_curand_and_oracle(K):
+    import ctypes as C
+    hooks = _hooks()
+    rng = np.random.default_rng(0)
+    n = 4096
+    ctr = rng.integers(0, 2**32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0
+    ctr[1] = 0xFFFFFFFF
+    seed = 0x299F31D0A4093822
+    d_ctr = K.words_from_numpy(ctr, "cuda")
+    ours = torch.zeros((n, 4), dtype=torch.int32, device="cuda")
+    cur = torch.zeros((n, 4), dtype=torch.int32, device="cuda")
+    rc = hooks.kpz_test_philox_dump(C.c_uint64(seed), C.c_void_p(d_ctr.data_ptr()), n, C.c_void_p(ours.data_ptr()),
+                                    C.c_void_p(cur.data_ptr()), None)
+    assert rc == 0
+    torch.cuda.synchronize()
+    ours, cur = K.words_to_numpy(ours), K.words_to_numpy(cur)
+    assert np.array_equal(ours, cur), "product Philox differs from cuRAND's curand_Philox4x32_10"
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    for i in list(range(8)) + [n - 1]:
+        assert list(ours[i]) == R.philox4x32_10(list(ctr[i]), key)
+    # the published known-answer vector with key 0
+    z = torch.zeros((1, 4), dtype=torch.int32, device="cuda")
+    o2 = torch.zeros((1, 4), dtype=torch.int32, device="cuda")
+    c2 = torch.zeros((1, 4), dtype=torch.int32, device="cuda")
+    assert hooks.kpz_test_philox_dump(C.c_uint64(0), C.c_void_p(z.data_ptr()), 1, C.c_void_p(o2.data_ptr()),
+                                      C.c_void_p(c2.data_ptr()), None) == 0
+    torch.cuda.synchronize()
+    assert list(K.words_to_numpy(o2)[0]) == [0x6627E8D5, 0xE169C58D, 0xBC57AC4C, 0x9B00DBD8]
+
+
+@pytest.mark.parametrize("prob", [0.0, 1.0, 0.5, 0.1, 0.05, 0.3, 0.999999])
+def test_device_bernoulli_masks_match_oracle_uniforms(K, prob):
+    import ctypes as C
+    hooks = _hooks()
+    ng, seed, tag, sample, tk = 6, 99, R.TAGS["TURN"], 5, (1 << 33) + 7
+    out = torch.zeros((ng, 4), dtype=torch.int32, device="cuda")
+    assert hooks.kpz_test_bernoulli(C.c_uint64(seed), tag, C.c_double(prob), sample, C.c_longlong(tk), ng,
+                                    C.c_void_p(out.data_ptr()), None) == 0
+    torch.cuda.synchronize()
+    bits = R.unpack_words(K.words_to_numpy(out).reshape(1, -1), ng * 128)[0]
+    T = R.threshold(prob)
+    want = np.array([R.uniform(seed, tag, sample, tk, 0, e) < T for e in range(ng * 128)], dtype=np.uint8)
+    assert np.array_equal(bits, want)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# K1 (on-chip) — the five configs' KPZ members and edge sizes
+# ---------------------------------------------------------------------------------------------------------
+
+def test_config1_in_full(K):
+    c = workloads.CONFIGS[1]
+    gpu, r = run_both_kpz(K, c["L"], c["S"], c["p"], c["q"], seed=c["seed"], times=c["record_times"],
+                          chunks=[c["n_mcs"]], check_heights=range(c["S"]))
+    assert gpu.path == K.KPZ_PATH_ONCHIP
+    assert np.all(r["sum_h2"] == 32) and np.all(np.abs(r["sum_h"]) == 32) and np.all(r["w2_mean"] == 0.25)
+
+
+def test_config2_all_records_on_a_sample_subset(K):
+    c = workloads.CONFIGS[2]
+    run_both_kpz(K, c["L"], 48, c["p"], c["q"], seed=c["seed"], times=c["record_times"], chunks=[300],
+                 check_heights=(0, 47))
+
+
+def test_config2_first_and_last_sample_full_length(K):
+    c = workloads.CONFIGS[2]
+    for fs in (0, c["S"] - 1):
+        run_both_kpz(K, c["L"], 1, c["p"], c["q"], seed=c["seed"], first_sample=fs, times=c["record_times"],
+                     chunks=[c["n_mcs"]])
+
+
+def test_config2_sample_k_of_full_launch_equals_solo_oracle_run(K):
+    # the launch configuration bench.py times (S=1024 CTAs), shortened; samples picked across the grid
+    c = workloads.CONFIGS[2]
+    n, times = 200, [t for t in c["record_times"] if t <= 200]
+    gpu = K.KpzSim(c["L"], c["S"], c["p"], c["q"], seed=c["seed"], max_records=len(times))
+    gpu.set_record_times(times)
+    gpu.run(n)
+    lat = K.words_to_numpy(gpu.lattice())
+    r = gpu.roughness()
+    for k in (0, 1, 147, 148, 511, 1023):
+        ref = R.KpzRef(c["L"], 1, c["p"], c["q"], seed=c["seed"], first_sample=k)
+        ref.set_record_times(times)
+        ref.run(n)
+        assert np.array_equal(lat[k], ref.lattice()[0])
+        rr = ref.roughness()
+        assert np.array_equal(r["sum_h"][:, k], rr["sum_h"][:, 0]) and np.array_equal(r["sum_h2"][:, k], rr["sum_h2"][:, 0])
+    # properties that hold for every sample at any size: conservation and h_{L-1} = 2N - L = 0
+    bits = R.unpack_words(lat, c["L"])
+    assert np.all(bits.sum(axis=1) == c["L"] // 2)
+
+
+def test_config3_disorder_subset(K):
+    c = workloads.CONFIGS[3]
+    run_both_kpz(K, c["L"], 12, c["p"], c["q"], disorder=c["disorder"], seed=c["seed"], times=c["record_times"],
+                 chunks=[150], check_heights=(0, 11))
+    run_both_kpz(K, c["L"], 1, c["p"], c["q"], disorder=c["disorder"], seed=c["seed"], first_sample=c["S"] - 1,
+                 times=c["record_times"], chunks=[400])
+
+
+@pytest.mark.parametrize("L", [64, 128, 192, 256, 320, 2048, 2112, 8192, 8448, 12288, 16384, 40960, 262144])
+def test_k1_sizes_ragged_tails_and_multi_warp(K, L):
+    S = 3 if L <= 40960 else 1
+    n = 24 if L <= 40960 else 6
+    times = sorted({1, 2, 5, 6, n})
+    rng = np.random.default_rng(L)
+    start = R.pack_sites((rng.random((S, L)) < 0.5).astype(np.uint8))
+    run_both_kpz(K, L, S, 0.75, 0.25, seed=L, times=times, chunks=[2, 4, n - 6], start=start, path=1)
+    # non-dyadic rates: dynamic plane count with early exit
+    run_both_kpz(K, L, S, 0.9, 0.1, seed=L + 1, times=times, chunks=[n], path=1)
+
+
+@pytest.mark.parametrize("p,q,dis", [
+    (1.0, 0.0, (0.1, 0.5, 0.0, 0.0)),          # config-3 style: one plane, slow-p only
+    (0.8, 0.0, (0.5, 0.16, 0.0, 0.0)),         # the paper's p=0.8, Q=0.5
+    (0.5, 0.5, (0.5, 0.1, 0.5, 0.1)),          # Q-SSEP, r=0.2
+    (0.75, 0.25, (0.3, 0.25, 0.6, 1.0)),       # slow-q "always"
+    (0.3, 0.7, (0.2, 0.0, 0.2, 0.0)),          # slow = blocked
+    (0.0, 0.0, None), (1.0, 1.0, None), (0.5, 0.0, None), (0.0, 0.5, None),
+])
+@pytest.mark.parametrize("L", [448, 16384])
+def test_k1_rate_classes(K, L, p, q, dis):
+    rng = np.random.default_rng(7)
+    start = R.pack_sites((rng.random((2, L)) < 0.4).astype(np.uint8))
+    run_both_kpz(K, L, 2, p, q, disorder=dis, seed=11, times=[3, 20], chunks=[20], start=start)
+
+
+def test_k1_alternating_offsets_and_resume(K):
+    run_both_kpz(K, 4096, 2, 0.8, 0.0, seed=5, offset_mode=1, times=[1, 7, 33], chunks=[1, 1, 15, 16, 17])
+    run_both_kpz(K, 4096, 2, 0.75, 0.25, seed=5, first_sample=77, times=[16, 17, 48, 50], chunks=[15, 2, 31, 2])
+
+
+def test_k1_explicit_disorder_masks(K):
+    L, S = 1024, 2
+    rng = np.random.default_rng(3)
+    mp = R.pack_sites((rng.random((S, L)) < 0.3).astype(np.uint8))
+    mq = R.pack_sites((rng.random((S, L)) < 0.6).astype(np.uint8))
+    ref = R.KpzRef(L, S, 0.75, 0.5, disorder=(0.0, 0.25, 0.0, 0.125), seed=4)
+    gpu = K.KpzSim(L, S, 0.75, 0.5, disorder=(0.0, 0.25, 0.0, 0.125), seed=4)
+    ref.set_disorder_masks(mp, mq)
+    gpu.set_disorder_masks(K.words_from_numpy(mp, gpu.device), K.words_from_numpy(mq, gpu.device))
+    gp, gq = gpu.disorder_masks()
+    assert np.array_equal(K.words_to_numpy(gp), mp) and np.array_equal(K.words_to_numpy(gq), mq)
+    ref.run(30)
+    gpu.run(30)
+    assert np.array_equal(K.words_to_numpy(gpu.lattice()), ref.lattice())
+
+
+# ---------------------------------------------------------------------------------------------------------
+# K3 (streamed) — config 4's path
+# ---------------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("L,S", [(64, 2), (320, 3), (4096, 3), (65536 + 64, 2), (1 << 18, 1)])
+def test_k3_forced_on_small_rings(K, L, S):
+    rng = np.random.default_rng(L)
+    start = R.pack_sites((rng.random((S, L)) < 0.5).astype(np.uint8))
+    n = 12 if L < 100000 else 5
+    gpu, _ = run_both_kpz(K, L, S, 0.9, 0.1, seed=4, times=[1, 2, 4, n], chunks=[3, n - 3], start=start, path=2)
+    assert gpu.path == K.KPZ_PATH_STREAM
+    run_both_kpz(K, L, S, 0.75, 0.25, disorder=(0.2, 0.25, 0.3, 0.5), seed=5, times=[2, n], chunks=[n], path=2)
+
+
+def test_k3_equals_k1_at_2p16(K):
+    L, c = 1 << 16, workloads.CONFIGS[4]
+    sims = []
+    for path in (1, 2):
+        g = K.KpzSim(L, 2, c["p"], c["q"], seed=c["seed"], path=path, max_records=8)
+        g.set_record_times([1, 10, 100, 150])
+        g.run(150)
+        sims.append((K.words_to_numpy(g.lattice()), g.roughness()))
+    assert np.array_equal(sims[0][0], sims[1][0])
+    for k in ("sum_h", "sum_h2"):
+        assert np.array_equal(sims[0][1][k], sims[1][1][k])
+
+
+def test_config4_path_at_2p20_vs_oracle(K):
+    c = workloads.CONFIGS[4]
+    gpu, _ = run_both_kpz(K, 1 << 20, 1, c["p"], c["q"], seed=c["seed"], times=c["record_times"], chunks=[26])
+    assert gpu.path == K.KPZ_PATH_STREAM
+
+
+def test_config4_full_size_first_steps_and_invariants(K):
+    c = workloads.CONFIGS[4]
+    L = c["L"]
+    gpu = K.KpzSim(L, 1, c["p"], c["q"], seed=c["seed"], max_records=8)
+    assert gpu.path == K.KPZ_PATH_STREAM
+    times = [1, 2]
+    gpu.set_record_times(times)
+    gpu.run(2)
+    ref = R.KpzRef(L, 1, c["p"], c["q"], seed=c["seed"])
+    ref.set_record_times(times)
+    ref.run(2)
+    assert np.array_equal(K.words_to_numpy(gpu.lattice()), ref.lattice())
+    gr, rr = gpu.roughness(), ref.roughness()
+    assert np.array_equal(gr["sum_h"], rr["sum_h"]) and np.array_equal(gr["sum_h2"], rr["sum_h2"])
+    # longer run at full size: properties that hold at any size
+    gpu.set_record_times([20])
+    gpu.run(18)
+    lat = gpu.lattice()
+    h = gpu.heights(0)
+    assert int(h[-1].item()) == 0                                  # h_{L-1} = 2N - L = 0 at half filling
+    r = gpu.roughness()
+    assert r["sum_h"][0, 0] == int(h.sum(dtype=torch.int64).item())
+    assert r["sum_h2"][0, 0] == int((h.to(torch.int64) ** 2).sum().item())
+    del lat
+
+
+# ---------------------------------------------------------------------------------------------------------
+# K4 (two-lane)
+# ---------------------------------------------------------------------------------------------------------
+
+def run_both_lanes(K, L, S, p_a, p_b, rho0, turn_prob, period, omega, seed, times, chunks, first_sample=0,
+                   offset_mode=0):
+    total = sum(chunks)
+    times = [t for t in times if t <= total]
+    ref = R.LanesRef(L, S, p_a, p_b, rho0, turn_prob, period, omega, seed=seed, first_sample=first_sample,
+                     offset_mode=offset_mode)
+    gpu = K.LanesSim(L, S, p_a, p_b, rho0, turn_prob, period, omega, seed=seed, first_sample=first_sample,
+                     offset_mode=offset_mode, max_records=max(len(times), 1))
+    ref.set_record_times(times)
+    gpu.set_record_times(times)
+
+    def same_state(tag):
+        for name, g, r in zip("AB T".replace(" ", ""), gpu.state(), ref.state()):
+            assert np.array_equal(K.words_to_numpy(g), r), f"{name} differs {tag}"
+    same_state("initially")
+    done = 0
+    for n in chunks:
+        ref.run(n)
+        gpu.run(n)
+        done += n
+        assert gpu.time == ref.time == done
+        same_state(f"at t={done}")
+    gc, rc = gpu.currents(), ref.currents()
+    assert list(gc["t"]) == list(rc["t"]) == times
+    for k in ("j_a", "j_b", "n_a", "n_b"):
+        assert np.array_equal(gc[k], rc[k]), k
+    ga, gb, gn = gpu.profile()
+    ra, rb, rn = ref.profile()
+    assert gn == rn
+    assert np.array_equal(K.words_to_numpy(ga), ra) and np.array_equal(K.words_to_numpy(gb), rb)
+    return gpu, gc
+
+
+def test_config5_subset(K):
+    c = workloads.CONFIGS[5]
+    gpu, cur = run_both_lanes(K, c["L"], 6, c["p_a"], c["p_b"], c["rho0"], c["turn_prob"], c["turn_period"], c["omega"],
+                              c["seed"], c["record_times"], [100, 1, 199])
+    assert cur["j_a"][-1].min() > 0
+    run_both_lanes(K, c["L"], 1, c["p_a"], c["p_b"], c["rho0"], c["turn_prob"], c["turn_period"], c["omega"],
+                   c["seed"], c["record_times"], [450], first_sample=c["S"] - 1)
+
+
+@pytest.mark.parametrize("L", [64, 192, 256, 8192, 8192 + 64, 40960])
+def test_lanes_sizes(K, L):
+    run_both_lanes(K, L, 2, 1.0, 1.0, 0.3, 0.2, 5, 0.3, seed=L, times=[1, 4, 5, 17], chunks=[4, 1, 12])
+
+
+@pytest.mark.parametrize("p_a,p_b,omega,tp", [(0.5, 0.5, 0.8, 0.5), (0.75, 0.25, 0.1, 0.05), (0.9, 0.6, 1.0, 1.0),
+                                              (1.0, 0.0, 0.0, 0.3), (0.3, 1.0, 0.5, 0.0)])
+def test_lanes_rates(K, p_a, p_b, omega, tp):
+    run_both_lanes(K, 2048, 2, p_a, p_b, 0.45, tp, 7, omega, seed=9, times=[2, 7, 8, 30], chunks=[30])
+    run_both_lanes(K, 2048, 2, p_a, p_b, 0.45, tp, 0, omega, seed=9, times=[30], chunks=[30], offset_mode=1)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# error behaviour through the ABI
+# ---------------------------------------------------------------------------------------------------------
+
+def test_error_codes(K):
+    g = K.KpzSim(128, 1, 0.5, 0.5, max_records=2)
+    with pytest.raises(K.KpzError) as e:
+        g.set_record_times([1, 2, 3])
+    assert e.value.code == -3
+    with pytest.raises(K.KpzError) as e:
+        g.set_record_times([2, 2])
+    assert e.value.code == -1
+    g.run(5)
+    with pytest.raises(K.KpzError) as e:
+        g.set_record_times([5])
+    assert e.value.code == -1
+    with pytest.raises(K.KpzError) as e:
+        K.KpzSim(100, 1, 0.5, 0.5)
+    assert e.value.code == -2
+    with pytest.raises(K.KpzError) as e:
+        g.set_disorder_masks(g.lattice())
+    assert e.value.code == -1
+    assert K.kernel_launches() > 0
