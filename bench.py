@@ -1,0 +1,389 @@
+#!/usr/bin/env python
+"""bench.py — site-update throughput of the KPZ/ASEP hot path on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|4|5|4-aux-i|4-aux-ii] [--impl reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: reset to the
+initial state (a1), run the configuration's full number of MCS with its record times (a2-a7 / a9), records left in
+device memory.  The default workload is BASELINE.json `configs[1]` (config 2: KPZ ring L=8192, 1024 samples,
+p=0.75/q=0.25, 10^4 MCS, 40 record times), the configuration the metric is quoted on.
+
+value      site updates / s (GSU/s) of the whole job, device-timed (CUDA events on the launching stream), inputs
+           resident in HBM when the timed region starts.
+e2e        same metric through the C ABI with HOST buffers: pinned initial lattice -> device, kpz_set_lattice,
+           kpz_run, kpz_roughness (records -> host) and the final lattice -> pinned host, all inside the timed region.
+roofline   the dominant kernel against the bound DESIGN.md §6 derives for it.
+cpu_baseline  the oracle (oracle/, as it stands) on one host core over a bounded sample of the same workload.
+
+N > 1 (torchrun): every rank runs the same workload on its own samples (first_sample = rank * S): weak scaling, no
+collective on the data path; time = max over ranks.
+
+--impl reference times the CPU oracle (there is no reference implementation to install: /root/reference holds only
+the paper's text).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "site_updates_per_sec"
+UNIT = "GSU/s"
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# roofline model: algorithmic cost per site-update of the dominant kernel of each workload
+# ---------------------------------------------------------------------------------------------------------------
+SM_COUNT = 148
+# integer thread-instructions per site-update of the on-chip sweep (DESIGN.md §6.1 derives these from the
+# algorithm: Philox rounds for the bit-planes the thresholds need + pair logic + frame change)
+ALU_OPS_PER_SU = {2: 1.08, 3: 0.73, 5: 0.47}
+# streamed sweep: one read + one write of the bit-packed ring per sub-lattice pass = 2 passes * 2 * 1/8 B
+STREAM_BYTES_PER_SU = 0.5
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            with open(path) as f:
+                d = json.load(f)
+            return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+        except Exception:
+            pass
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# clock sampling during the timed region (NVML; nvidia-smi as a fallback)
+# ---------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+               0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        self._h = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            phys = index
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            if vis:
+                try:
+                    phys = int(vis.split(",")[index])
+                except Exception:
+                    phys = index
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._h = None
+
+    def _loop(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+                for bit, name in self.REASONS.items():
+                    if r & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.004)
+
+    def start(self):
+        if self._h is not None:
+            self._thread = threading.Thread(target=self._loop, daemon=True)
+            self._thread.start()
+
+    def stop(self):
+        if self._thread is not None:
+            self._stop.set()
+            self._thread.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unsampled"]}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# CPU oracle legs
+# ---------------------------------------------------------------------------------------------------------------
+def _oracle_sim(cfg, nsamples, first_sample=0):
+    from oracle import kpzref as R  # test infrastructure: only the cpu_baseline / reference legs load it
+    if cfg["kind"] == "lanes":
+        return R.LanesRef(cfg["L"], nsamples, cfg["p_a"], cfg["p_b"], cfg["rho0"], cfg["turn_prob"], cfg["turn_period"],
+                          cfg["omega"], seed=cfg["seed"], first_sample=first_sample)
+    return R.KpzRef(cfg["L"], nsamples, cfg["p"], cfg["q"], disorder=cfg["disorder"], seed=cfg["seed"],
+                    first_sample=first_sample)
+
+
+def oracle_sample_shape(cfg, target_su):
+    """A bounded sample of the workload: whole samples first, then a prefix of the MCS; about target_su site updates."""
+    per_mcs = (2 if cfg["kind"] == "lanes" else 1) * cfg["L"]
+    n_mcs = int(max(1, min(cfg["n_mcs"], target_su // per_mcs)))
+    nsamp = int(max(1, min(cfg["S"], target_su // (per_mcs * n_mcs))))
+    return nsamp, n_mcs
+
+
+def time_oracle(cfg, nsamp, n_mcs, first_sample=0):
+    sim = _oracle_sim(cfg, nsamp, first_sample)
+    sim.set_record_times([t for t in cfg["record_times"] if t <= n_mcs])
+    t0 = time.perf_counter()
+    sim.run(n_mcs)
+    if cfg["kind"] == "lanes":
+        sim.currents()
+    else:
+        sim.roughness()
+    dt = time.perf_counter() - t0
+    sim.close()
+    return workloads.site_updates(cfg, n_mcs, nsamp) / dt / 1e9, dt
+
+
+def run_reference(args, cfg, cfg_key):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    nsamp, n_mcs = oracle_sample_shape(cfg, 8_000_000)   # ~1 s of one host core per step
+    for w in range(args.warmup):
+        time_oracle(cfg, nsamp, n_mcs, first_sample=w)
+    t_total, su = 0.0, 0
+    for k in range(args.steps):
+        _, dt = time_oracle(cfg, nsamp, n_mcs, first_sample=args.warmup + k)
+        t_total += dt
+        su += workloads.site_updates(cfg, n_mcs, nsamp)
+    value = su / t_total / 1e9
+    sample = f"{nsamp} sample(s) x {n_mcs} MCS of {cfg['name']} per step (of {cfg['S']} x {cfg['n_mcs']})"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t_total / max(args.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": cfg["name"], "config_key": str(cfg_key), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# CUDA path
+# ---------------------------------------------------------------------------------------------------------------
+def make_sim(pkg, cfg, first_sample):
+    nrec = len(cfg["record_times"])
+    if cfg["kind"] == "lanes":
+        sim = pkg.LanesSim(cfg["L"], cfg["S"], cfg["p_a"], cfg["p_b"], cfg["rho0"], cfg["turn_prob"], cfg["turn_period"],
+                           cfg["omega"], seed=cfg["seed"], first_sample=first_sample, max_records=nrec)
+    else:
+        sim = pkg.KpzSim(cfg["L"], cfg["S"], cfg["p"], cfg["q"], disorder=cfg["disorder"], seed=cfg["seed"],
+                         first_sample=first_sample, max_records=nrec)
+    sim.set_record_times(cfg["record_times"])
+    return sim
+
+
+def run_cuda(args, cfg, cfg_key):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1012_0385_b200 as pkg
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    pkg.load_library()
+
+    n_mcs = cfg["n_mcs"] if args.mcs is None else args.mcs
+    if args.mcs is not None:
+        cfg = workloads.truncated(cfg, n_mcs)
+    su_step = workloads.site_updates(cfg)
+    sim = make_sim(pkg, cfg, first_sample=rank * cfg["S"])      # global sample indices: results independent of N
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def step(ev=None):
+        if ev:
+            ev[0].record(stream)
+        sim.reset()
+        if ev:
+            ev[1].record(stream)
+        sim.run(n_mcs)
+        if ev:
+            ev[2].record(stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        flush.fill_(1)
+        step()
+    barrier()
+
+    sampler = ClockSampler(local_rank)
+    events = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    launches0 = pkg.kernel_launches()
+    sampler.start()
+    wall0 = time.perf_counter()
+    for k in range(args.steps):
+        flush.fill_(k & 0xFF)          # L2 flush between timed iterations (outside the events)
+        step(events[k])
+    barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    launches = pkg.kernel_launches() - launches0
+    t_step = [e[0].elapsed_time(e[2]) for e in events]       # ms, reset + run
+    t_run = [e[1].elapsed_time(e[2]) for e in events]        # ms, kpz_run / lanes_run only
+    t_total = torch.tensor([sum(t_step), sum(t_run)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_total, op=dist.ReduceOp.MAX)
+    ms_total, ms_run_total = float(t_total[0]), float(t_total[1])
+    value = world * su_step * args.steps / (ms_total * 1e-3) / 1e9
+
+    # ---- e2e: host buffers through the C ABI ------------------------------------------------------------------
+    e2e = None
+    if cfg["kind"] == "kpz":
+        nw = cfg["L"] // 32
+        import numpy as np
+        h_in = torch.from_numpy(np.full((cfg["S"], nw), 0xAAAAAAAA, dtype=np.uint32).view(np.int32)).pin_memory()
+        h_out = torch.empty((cfg["S"], nw), dtype=torch.int32).pin_memory()
+        d_in = torch.empty((cfg["S"], nw), dtype=torch.int32, device=dev)
+        d_out = torch.empty((cfg["S"], nw), dtype=torch.int32, device=dev)
+
+        def e2e_step():
+            sim.reset()
+            d_in.copy_(h_in, non_blocking=True)
+            sim.set_lattice(d_in)
+            sim.run(n_mcs)
+            sim.lattice(out=d_out)
+            h_out.copy_(d_out, non_blocking=True)
+            return sim.roughness()        # syncs; records -> host
+
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            rec = e2e_step()
+        barrier()
+        dt = time.perf_counter() - t0
+        tt = torch.tensor([dt], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        rec_bytes = int(rec["sum_h"].nbytes + rec["sum_h2"].nbytes)
+        e2e = {"value": world * su_step * args.steps / float(tt[0]) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": int(h_in.numel() * 4), "d2h_bytes_per_step": int(h_out.numel() * 4) + rec_bytes}
+    else:
+        def e2e_step():
+            sim.reset()
+            sim.run(n_mcs)
+            a, b, _ = sim.state()
+            ha, hb = a.cpu(), b.cpu()
+            return sim.currents(), ha, hb
+
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            cur, ha, hb = e2e_step()
+        barrier()
+        dt = time.perf_counter() - t0
+        tt = torch.tensor([dt], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * su_step * args.steps / float(tt[0]) / 1e9, "unit": UNIT, "h2d_bytes_per_step": 0,
+               "d2h_bytes_per_step": int(ha.numel() * 4 + hb.numel() * 4 + 4 * cur["j_a"].nbytes),
+               "note": "the two-lane initial state is generated on the device from the seed; no host input exists"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel -------------------------------------------------------------------
+    peaks = measured_peaks()
+    path = sim.path if cfg["kind"] == "kpz" else 1
+    ms_run = ms_run_total / args.steps
+    if path == 2:
+        # streamed sweep: 2*n_mcs pass kernels per run; per launch one read + one write of the ring
+        n_launch = 2 * n_mcs
+        bytes_launch = 2 * cfg["S"] * cfg["L"] / 8
+        achieved = bytes_launch * n_launch / (ms_run * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "k3_pass_kernel", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+                "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
+    else:
+        ops = ALU_OPS_PER_SU.get(cfg_key if isinstance(cfg_key, int) else -1, 1.08)
+        peak = SM_COUNT * 4 * 32 * peaks["sm_max_mhz"] * 1e6 / 1e12      # T thread-instr/s at 1 warp-instr/clk/SMSP
+        achieved = ops * su_step / (ms_run * 1e-3) / 1e12
+        roof = {"bound": "alu", "kernel": "kpz_k1_kernel" if cfg["kind"] == "kpz" else "lanes_k4_kernel",
+                "achieved": achieved, "peak": peak, "unit": "Tinstr/s", "frac": achieved / peak, "traffic": None,
+                "peak_source": f"148 SM x 4 SMSP x 32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max clock)",
+                "algorithmic_instr_per_site_update": ops}
+
+    # ---- CPU oracle on a bounded sample (one host core) -------------------------------------------------------
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        nsamp, nm = oracle_sample_shape(cfg, 150_000_000)      # ~15 s at ~1e7 site updates/s
+        v, dt = time_oracle(cfg, nsamp, nm)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
+               "sample": f"{nsamp} sample(s) x {nm} MCS of {cfg['name']} (of {cfg['S']} x {cfg['n_mcs']})"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32", "data": "synthetic",
+        "config": {"workload": cfg["name"], "config_key": str(cfg_key), "L": cfg["L"], "samples_per_gpu": cfg["S"],
+                   "n_mcs": n_mcs, "records": len(cfg["record_times"]), "path": {1: "on-chip K1", 2: "streamed K3"}[path]
+                   if cfg["kind"] == "kpz" else "two-lane K4", "l2": "flushed between timed steps (256 MiB fill)",
+                   "parallelism": f"samples x{world}"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
+        "ms_run_per_step": ms_run, "wall_s_timed_region": wall,
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", default="2")
+    ap.add_argument("--mcs", type=int, default=None, help="truncate the run to this many MCS (diagnostics only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    key = int(args.config) if args.config.isdigit() else args.config
+    cfg = dict(workloads.CONFIGS[key])
+    if args.impl == "reference":
+        return run_reference(args, cfg, key)
+    return run_cuda(args, cfg, key)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -82,6 +82,10 @@ int kpz_run(kpz_sim*, int64_t n_mcs);
 
 int kpz_time(const kpz_sim*, int64_t* t); /* MCS done so far (host value; no sync) */
 
+/* Back to the state right after kpz_create: flat lattice, disorder tags regenerated from the seed, t = 0,
+ * captured records dropped (the record-time list is kept).  Enqueues the initialisation kernels; async. */
+int kpz_reset(kpz_sim*);
+
 /* Copy the occupation bits out / in (device buffers, natural layout, nsamples * L/32 words).  Async. */
 int kpz_lattice(kpz_sim*, uint32_t* d_words);
 int kpz_set_lattice(kpz_sim*, const uint32_t* d_words);
@@ -114,6 +118,7 @@ int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, doubl
 int lanes_set_record_times(lanes_sim*, const int64_t* t, int32_t nt);
 int lanes_run(lanes_sim*, int64_t n_mcs);
 int lanes_time(const lanes_sim*, int64_t* t);
+int lanes_reset(lanes_sim*); /* as kpz_reset: initial occupations, epoch-0 turning points, zero counters; async */
 /* Occupations of lanes A, B and the current turning-point mask (device, natural layout, any may be NULL). Async. */
 int lanes_state(lanes_sim*, uint32_t* d_a, uint32_t* d_b, uint32_t* d_turn);
 int lanes_set_state(lanes_sim*, const uint32_t* d_a, const uint32_t* d_b, const uint32_t* d_turn);

@@ -46,6 +46,7 @@ SIGNATURES = {
     "kpz_set_record_times": (C.c_int, [_P, C.POINTER(C.c_int64), C.c_int32]),
     "kpz_run": (C.c_int, [_P, C.c_int64]),
     "kpz_time": (C.c_int, [_P, C.POINTER(C.c_int64)]),
+    "kpz_reset": (C.c_int, [_P]),
     "kpz_lattice": (C.c_int, [_P, _P]),
     "kpz_set_lattice": (C.c_int, [_P, _P]),
     "kpz_disorder_masks": (C.c_int, [_P, _P, _P]),
@@ -59,6 +60,7 @@ SIGNATURES = {
     "lanes_set_record_times": (C.c_int, [_P, C.POINTER(C.c_int64), C.c_int32]),
     "lanes_run": (C.c_int, [_P, C.c_int64]),
     "lanes_time": (C.c_int, [_P, C.POINTER(C.c_int64)]),
+    "lanes_reset": (C.c_int, [_P]),
     "lanes_state": (C.c_int, [_P, _P, _P, _P]),
     "lanes_set_state": (C.c_int, [_P, _P, _P, _P]),
     "lanes_currents": (C.c_int, [_P, C.POINTER(C.c_int32), _P, _P, _P, _P, _P]),
@@ -171,6 +173,9 @@ class KpzSim:
     def run(self, n_mcs):
         _chk(load_library().kpz_run(self._h, int(n_mcs)), "kpz_run")
 
+    def reset(self):
+        _chk(load_library().kpz_reset(self._h), "kpz_reset")
+
     def lattice(self, out=None):
         """Occupation words [S][L/32] (natural layout) as a device tensor (int32 storage of the uint32 words)."""
         if out is None:
@@ -258,6 +263,9 @@ class LanesSim:
 
     def run(self, n_mcs):
         _chk(load_library().lanes_run(self._h, int(n_mcs)), "lanes_run")
+
+    def reset(self):
+        _chk(load_library().lanes_reset(self._h), "lanes_reset")
 
     def state(self):
         a, b, tn = [torch.empty((self.S, self.nw), dtype=torch.int32, device=self.device) for _ in range(3)]

@@ -48,6 +48,8 @@ struct kpz_sim {
   int32_t max_records = 0;
   int32_t path = 0;  // 1 = K1, 2 = K3
   bool has_disorder = false, has_sp = false, has_sq = false;
+  bool has_sp0 = false, has_sq0 = false;  // as created (kpz_reset restores them)
+  kpz_disorder dis{};
   KpzDev dev{};
   cudaStream_t stream = nullptr;
   // workspace carve-up (device)
@@ -174,6 +176,30 @@ void refresh_planes(kpz_sim* sim) {
   sim->dev.SQO = sim->has_sq ? sim->SQO : nullptr;
 }
 
+
+// a1: flat start and the quenched disorder tags (Eq. 8) — the kernels kpz_create and kpz_reset enqueue.
+int init_state(kpz_sim* sim) {
+  const KpzDev& D = sim->dev;
+  const size_t nwords = (size_t)D.S * D.PWp;
+  k_init_flat<<<grid_for(nwords), 256, 0, sim->stream>>>(sim->E, sim->O, D.S, D.PW, D.PWp);
+  KPZ_LAUNCH_CHECK("k_init_flat");
+  if (sim->has_disorder) {
+    const size_t ng = (size_t)D.S * ((D.PW + 1) / 2);
+    if (D.PWp != D.PW) {  // pad words of the mask rows must be zero
+      for (uint32_t* m : {sim->SPE, sim->SPO, sim->SQE, sim->SQO}) {
+        k_zero_words<<<grid_for(nwords), 256, 0, sim->stream>>>(m, nwords);
+        KPZ_LAUNCH_CHECK("k_zero_words");
+      }
+    }
+    k_site_mask_eo<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_SLOW_P, make_thresh(sim->dis.prob_slow_p),
+                                                              D.first_sample, D.S, D.PW, D.PWp, sim->SPE, sim->SPO);
+    KPZ_LAUNCH_CHECK("k_site_mask_eo");
+    k_site_mask_eo<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_SLOW_Q, make_thresh(sim->dis.prob_slow_q),
+                                                              D.first_sample, D.S, D.PW, D.PWp, sim->SQE, sim->SQO);
+    KPZ_LAUNCH_CHECK("k_site_mask_eo");
+  }
+  return KPZ_OK;
+}
 
 // ---- K3 dispatch and driver ------------------------------------------------------------------------------
 using K3Fn = void (*)(const KpzDev, const K3Pass);
@@ -358,6 +384,8 @@ int kpz_create(kpz_sim** out, int64_t L, int32_t nsamples, double p, double q, c
   sim->has_disorder = disorder != nullptr;
   sim->has_sp = disorder && d.prob_slow_p > 0.0;
   sim->has_sq = disorder && d.prob_slow_q > 0.0;
+  sim->has_sp0 = sim->has_sp;
+  sim->has_sq0 = sim->has_sq;
   sim->stream = (cudaStream_t)cuda_stream;
   char* base = (char*)d_workspace;
   sim->E = (uint32_t*)(base + y.off_E);
@@ -399,34 +427,11 @@ int kpz_create(kpz_sim** out, int64_t L, int32_t nsamples, double p, double q, c
   D.O = sim->O;
   refresh_planes(sim);
 
-  const size_t nwords = (size_t)nsamples * y.PWp;
-  k_init_flat<<<grid_for(nwords), 256, 0, sim->stream>>>(sim->E, sim->O, nsamples, y.PW, y.PWp);
-  {
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) {
-      delete sim;
-      return fail(KPZ_ECUDA, "launch k_init_flat: %s", cudaGetErrorString(e));
-    }
-    count_launch();
-  }
-  if (disorder) {
-    const size_t ng = (size_t)nsamples * ((y.PW + 1) / 2);
-    if (y.PWp != y.PW) {  // pad words of the mask rows must be zero
-      for (uint32_t* m : {sim->SPE, sim->SPO, sim->SQE, sim->SQO}) {
-        k_zero_words<<<grid_for(nwords), 256, 0, sim->stream>>>(m, nwords);
-        count_launch();
-      }
-    }
-    k_site_mask_eo<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_SLOW_P, make_thresh(d.prob_slow_p),
-                                                              o.first_sample, nsamples, y.PW, y.PWp, sim->SPE, sim->SPO);
-    k_site_mask_eo<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_SLOW_Q, make_thresh(d.prob_slow_q),
-                                                              o.first_sample, nsamples, y.PW, y.PWp, sim->SQE, sim->SQO);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) {
-      delete sim;
-      return fail(KPZ_ECUDA, "launch k_site_mask_eo: %s", cudaGetErrorString(e));
-    }
-    count_launch(2);
+  sim->dis = d;
+  rc = init_state(sim);
+  if (rc) {
+    delete sim;
+    return rc;
   }
   *out = sim;
   return KPZ_OK;
@@ -434,6 +439,19 @@ int kpz_create(kpz_sim** out, int64_t L, int32_t nsamples, double p, double q, c
 
 int kpz_destroy(kpz_sim* sim) {
   delete sim;
+  return KPZ_OK;
+}
+
+int kpz_reset(kpz_sim* sim) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  sim->has_sp = sim->has_sp0;
+  sim->has_sq = sim->has_sq0;
+  refresh_planes(sim);
+  int rc = init_state(sim);
+  if (rc) return rc;
+  sim->t = 0;
+  sim->nrec = 0;
+  sim->frame = 0;
   return KPZ_OK;
 }
 

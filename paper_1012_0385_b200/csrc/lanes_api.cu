@@ -19,6 +19,9 @@ struct lanes_sim {
   int64_t t = 0;
   std::vector<int64_t> rec_times;
   int32_t nrec = 0;
+  char* base = nullptr;   // workspace start
+  size_t zero_bytes = 0;  // lattices (incl. pad words), counters and profile sit in [base, base + zero_bytes)
+  Thresh t_rho{};
 };
 
 namespace {
@@ -66,9 +69,32 @@ int grid_for(size_t n, int block = 256) {
   return (int)std::min<size_t>(std::max<size_t>(g, 1), 148 * 16);
 }
 
+// Initial occupations, epoch-0 turning points (§R13), zero counters and profile.
+int lanes_init_state(lanes_sim* sim) {
+  const LanesDev& D = sim->dev;
+  KPZ_CUDA_CHECK(cudaMemsetAsync(sim->base, 0, sim->zero_bytes, sim->stream));
+  const size_t ng = (size_t)D.S * ((D.W + 3) / 4);
+  k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_INIT_A, sim->t_rho, 0, D.first_sample, D.S, D.W, D.Wp, D.A);
+  KPZ_LAUNCH_CHECK("k_site_mask_nat");
+  k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_INIT_B, sim->t_rho, 0, D.first_sample, D.S, D.W, D.Wp, D.B);
+  KPZ_LAUNCH_CHECK("k_site_mask_nat");
+  k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_TURN, D.t_turn, 0, D.first_sample, D.S, D.W, D.Wp, D.T);
+  KPZ_LAUNCH_CHECK("k_site_mask_nat");
+  return KPZ_OK;
+}
+
 }  // namespace
 
 extern "C" {
+
+int lanes_reset(lanes_sim* sim) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  int rc = lanes_init_state(sim);
+  if (rc) return rc;
+  sim->t = 0;
+  sim->nrec = 0;
+  return KPZ_OK;
+}
 
 int lanes_workspace_bytes(int64_t L, int32_t nsamples, int32_t max_records, size_t* bytes) {
   if (!bytes) return fail(KPZ_EINVAL, "bytes is NULL");
@@ -128,22 +154,14 @@ int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, doubl
   sim->rec_t = (long long*)(base + y.off_rec_t);
   sim->rec = (long long*)(base + y.off_rec);
 
-  cudaError_t e = cudaMemsetAsync(base, 0, y.off_rec_t, sim->stream);  // lattices (incl. pad words), counters, profile
-  if (e != cudaSuccess) {
+  sim->zero_bytes = y.off_rec_t;
+  sim->base = base;
+  sim->t_rho = make_thresh(rho0);
+  rc = lanes_init_state(sim);
+  if (rc) {
     delete sim;
-    return fail(KPZ_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+    return rc;
   }
-  const Thresh t_rho = make_thresh(rho0);
-  const size_t ng = (size_t)nsamples * ((y.W + 3) / 4);
-  k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_INIT_A, t_rho, 0, o.first_sample, nsamples, y.W, y.Wp, D.A);
-  k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_INIT_B, t_rho, 0, o.first_sample, nsamples, y.W, y.Wp, D.B);
-  k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_TURN, D.t_turn, 0, o.first_sample, nsamples, y.W, y.Wp, D.T);
-  e = cudaGetLastError();
-  if (e != cudaSuccess) {
-    delete sim;
-    return fail(KPZ_ECUDA, "launch k_site_mask_nat: %s", cudaGetErrorString(e));
-  }
-  count_launch(3);
   *out = sim;
   return KPZ_OK;
 }

@@ -335,6 +335,36 @@ def test_lanes_rates(K, p_a, p_b, omega, tp):
     run_both_lanes(K, 2048, 2, p_a, p_b, 0.45, tp, 0, omega, seed=9, times=[30], chunks=[30], offset_mode=1)
 
 
+def test_reset_reproduces_a_fresh_run(K):
+    c = workloads.CONFIGS[3]
+    times = [2, 9, 30]
+    g = K.KpzSim(2048, 3, c["p"], c["q"], disorder=c["disorder"], seed=c["seed"], max_records=3)
+    g.set_record_times(times)
+    g.run(30)
+    first = (K.words_to_numpy(g.lattice()).copy(), g.roughness())
+    g.reset()
+    assert g.time == 0 and len(g.roughness()["t"]) == 0
+    ref = R.KpzRef(2048, 3, c["p"], c["q"], disorder=c["disorder"], seed=c["seed"])
+    assert np.array_equal(K.words_to_numpy(g.lattice()), ref.lattice())
+    g.run(30)
+    assert np.array_equal(K.words_to_numpy(g.lattice()), first[0])
+    r = g.roughness()
+    assert np.array_equal(r["sum_h"], first[1]["sum_h"]) and np.array_equal(r["sum_h2"], first[1]["sum_h2"])
+    ref.set_record_times(times)
+    ref.run(30)
+    assert np.array_equal(first[0], ref.lattice())
+    c5 = workloads.CONFIGS[5]
+    l = K.LanesSim(2048, 2, 1.0, 1.0, c5["rho0"], c5["turn_prob"], 10, c5["omega"], seed=5, max_records=2)
+    l.set_record_times([7, 25])
+    l.run(25)
+    s1, c1, p1 = [K.words_to_numpy(x).copy() for x in l.state()], l.currents(), [K.words_to_numpy(x).copy() for x in l.profile()[:2]]
+    l.reset()
+    l.run(25)
+    s2, c2, p2 = [K.words_to_numpy(x) for x in l.state()], l.currents(), [K.words_to_numpy(x) for x in l.profile()[:2]]
+    assert all(np.array_equal(a, b) for a, b in zip(s1, s2)) and all(np.array_equal(a, b) for a, b in zip(p1, p2))
+    assert all(np.array_equal(c1[k], c2[k]) for k in ("j_a", "j_b", "n_a", "n_b"))
+
+
 # ---------------------------------------------------------------------------------------------------------
 # error behaviour through the ABI
 # ---------------------------------------------------------------------------------------------------------
