@@ -135,6 +135,13 @@ int64_t kpz_kernel_launches(void);       /* kernels launched by this library in 
 /* Which kernel family a handle's kpz_run uses: 1 = on-chip per-sample (K1), 2 = streamed (K3). */
 int kpz_path(const kpz_sim*, int32_t* path);
 
+/* The on-chip sweep kernel is specialised at run time (NVRTC) on the ring size and the acceptance thresholds
+ * (DESIGN §5); the environment variable KPZ_B200_JIT=0 selects the statically compiled generic kernels instead.
+ * kpz_jit_check compiles - without loading, so it needs no GPU - the kernel kpz_run would use for these parameters
+ * and returns the size of its sm_100a cubin (0 when that configuration runs on a statically compiled kernel). */
+int kpz_jit_check(int64_t L, double p, double q, const kpz_disorder* disorder, const kpz_options* opt,
+                  size_t* cubin_bytes);
+
 #ifdef __cplusplus
 }
 #endif

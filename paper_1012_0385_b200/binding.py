@@ -70,6 +70,8 @@ SIGNATURES = {
     "kpz_last_error": (C.c_char_p, []),
     "kpz_kernel_launches": (C.c_int64, []),
     "kpz_path": (C.c_int, [_P, C.POINTER(C.c_int32)]),
+    "kpz_jit_check": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.POINTER(Disorder), C.POINTER(Options),
+                                C.POINTER(C.c_size_t)]),
 }
 
 
@@ -115,6 +117,16 @@ def _times(t):
 
 def kernel_launches() -> int:
     return int(load_library().kpz_kernel_launches())
+
+
+def jit_check(L, p, q, disorder=None, offset_mode=0, path=KPZ_PATH_AUTO) -> int:
+    """kpz_jit_check: compile (no GPU needed) the specialised sweep kernel for these parameters; cubin size in bytes."""
+    d = None if disorder is None else Disorder(*[float(x) for x in disorder])
+    o = Options(0, int(offset_mode), int(path))
+    n = C.c_size_t()
+    _chk(load_library().kpz_jit_check(int(L), float(p), float(q), C.byref(d) if d is not None else None, C.byref(o),
+                                      C.byref(n)), "kpz_jit_check")
+    return int(n.value)
 
 
 class KpzSim:

@@ -7,7 +7,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/kpz_b200.h"
-#include "philox.cuh"
+#include "sweep_types.cuh"
 
 namespace kpz {
 
@@ -34,11 +34,6 @@ void count_launch(int n = 1);
 inline bool valid_prob(double x) { return x >= 0.0 && x <= 1.0; }
 inline uint64_t threshold(double x) { return (uint64_t)std::floor(x * 4294967296.0); }
 
-// A threshold as the kernels see it: `always` (T = 2^32), else the 32-bit value (0 = never).
-struct Thresh {
-  uint32_t value;   // low 32 bits of T
-  uint32_t always;  // 1 if T == 2^32
-};
 inline Thresh make_thresh(double x) {
   uint64_t T = threshold(x);
   Thresh t;

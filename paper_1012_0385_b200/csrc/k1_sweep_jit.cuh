@@ -1,0 +1,467 @@
+// k1_sweep_jit.cuh — K1 v2: the on-chip per-sample sweep specialised at run time (NVRTC, see jit.cu) on the
+// ring size and on the four acceptance thresholds (north_star (1),(3)).
+//
+// Why specialise.  The sweep is integer work on two pipes: Philox needs 20 IMAD.WIDE per call (fmaheavy pipe,
+// measured 0.25 warp-instr/clk/SMSP on B200) and 20 LOP3 (alu pipe, 0.5/clk); the pair logic is LOP3 only.  With
+// thresholds known at compile time the lazy MSB-first comparison U < T folds into a fixed boolean
+// function of the few bit-planes T needs, so the logic costs ~4 LOP3 per 32 pairs instead of ~15, the plane count
+// is a constant, and the Philox calls of the NEXT MCS (counter-based, state-independent) are issued in the same
+// basic block as the logic of the current one: the kernel runs at the IMAD.WIDE rate of the Philox rounds.
+//
+// Compile-time configuration (all -D macros, set by jit.cu):
+//   K1J_PW            pair-words (64-site groups) per sample = L/64
+//   K1J_T0..K1J_T3    thresholds T(p), T(p_slow), T(q), T(q_slow) as integers in [0, 2^32]
+//   K1J_DIS           0 no disorder tags, 1 slow-p tags, 2 slow-p and slow-q tags
+//   K1J_OFFSET_MODE   0 drawn offsets, 1 alternating
+//
+// Layout on chip: as K1 v1 (kpz_k1.cuh): thread = one unit = 128 pairs = one Philox supergroup, 4 even-site words
+// P[4] and 4 odd-site words Q[4] in registers; frame 0 pairs (P,Q) = sites (2k,2k+1), frame 1 pairs (Q,P') with P'
+// = P shifted by one even site.  The lattice is in frame 0 at every MCS boundary.
+#pragma once
+#include "sweep_types.cuh"
+
+#ifndef K1J_PW
+#error "k1_sweep_jit.cuh needs K1J_PW, K1J_T0..3, K1J_DIS, K1J_OFFSET_MODE"
+#endif
+
+namespace kpz {
+namespace k1j {
+
+constexpr int PW = K1J_PW;
+constexpr int PWp = (PW + 3) / 4 * 4;
+constexpr int U = PWp / 4;
+constexpr bool SINGLE_WARP = U <= 32;
+constexpr bool PARTIAL = (PW % 4) != 0;
+constexpr int DIS = K1J_DIS;
+constexpr int NTHREADS = (U + 31) / 32 * 32;
+constexpr uint64_t T0 = K1J_T0, T1 = K1J_T1, T2 = K1J_T2, T3 = K1J_T3;
+constexpr uint64_t kOne = 1ull << 32;
+
+// bit-planes U < T can depend on: 0 for T in {0, 2^32}, else 32 - ctz(T)
+__host__ __device__ constexpr int planes_of(uint64_t T) {
+  if (T == 0 || T >= kOne) return 0;
+  int z = 0;
+  while (!((T >> z) & 1ull)) ++z;
+  return 32 - z;
+}
+__host__ __device__ constexpr int cmax(int a, int b) { return a > b ? a : b; }
+constexpr int NPS = cmax(cmax(planes_of(T0), planes_of(T2)),
+                         cmax(DIS >= 1 ? planes_of(T1) : 0, DIS >= 2 ? planes_of(T3) : 0));
+constexpr int NPSA = NPS > 0 ? NPS : 1;  // array extent
+
+// The random bit-planes of one MCS of one unit: r[pass][plane][word].
+struct Planes {
+  uint32_t r[2][NPSA][4];
+};
+
+__device__ __forceinline__ void draw_planes(Planes& R, const PhiloxKeys& K, uint32_t G, uint32_t gs, long long m) {
+  const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
+#pragma unroll
+  for (int pass = 0; pass < 2; ++pass) {
+#pragma unroll
+    for (int pl = 0; pl < NPS; ++pl) {
+      const uint4 v = philox4x32_10(G, gs, tlo, ctr3(TAG_PAIR, (uint32_t)pass, (uint32_t)pl, thi), K);
+      R.r[pass][pl][0] = v.x;
+      R.r[pass][pl][1] = v.y;
+      R.r[pass][pl][2] = v.z;
+      R.r[pass][pl][3] = v.w;
+    }
+  }
+}
+
+// [U < T] for the 32 pairs of word w, MSB first; T is a constant so this folds to a fixed boolean function.
+template <uint64_t T>
+__device__ __forceinline__ uint32_t accept(const uint32_t (&r)[NPSA][4], int w) {
+  if (T >= kOne) return ~0u;
+  if (T == 0) return 0u;
+  constexpr int np = planes_of(T);
+  uint32_t lt = 0u, eq = ~0u;
+#pragma unroll
+  for (int pl = 0; pl < np; ++pl) {
+    const uint32_t x = r[pl][w];
+    if ((T >> (31 - pl)) & 1ull) {
+      lt |= eq & ~x;
+      eq &= x;
+    } else {
+      eq &= ~x;
+    }
+  }
+  return lt;
+}
+
+// ---- pair logic as explicit LOP3s --------------------------------------------------------------------------------
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t d;
+  asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(d) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+  return d;
+}
+
+// [U < T] for one pair whose leading plane bits are r0, r1 (compile-time evaluation of the same MSB-first rule).
+__host__ __device__ constexpr int accept_bits(uint64_t T, int r0, int r1) {
+  if (T >= kOne) return 1;
+  if (T == 0) return 0;
+  const int np = planes_of(T);
+  for (int pl = 0; pl < np && pl < 2; ++pl) {
+    const int t = (int)((T >> (31 - pl)) & 1ull), x = pl == 0 ? r0 : r1;
+    if (t && !x) return 1;
+    if (t != x) return 0;
+  }
+  return 0;
+}
+// On an active pair (a != b) the side a alone tells which move is attempted: a = 1 forward with the p class of the
+// a site, a = 0 backward with the q class of the b site.  sel = "the attempted move is accepted".
+__host__ __device__ constexpr int sel_bit(int a, int spa, int sqb, int r0, int r1) {
+  return a ? accept_bits(spa ? T1 : T0, r0, r1) : accept_bits(sqb ? T3 : T2, r0, r1);
+}
+// When sel depends on at most three words (a + tags + planes) it is ONE LOP3 with this table; inputs in the order
+// a, [spa], [sqb], [plane 0], [plane 1].
+constexpr int SEL_NVARS = 1 + (DIS >= 1) + (DIS >= 2) + NPS;
+__host__ __device__ constexpr int sel_lut() {
+  int lut = 0;
+  for (int i = 0; i < 8; ++i) {
+    const int in[3] = {(i >> 2) & 1, (i >> 1) & 1, i & 1};
+    int k = 1, spa = 0, sqb = 0, r0 = 0, r1 = 0;
+    if (DIS >= 1) spa = in[k < 3 ? k : 2], ++k;
+    if (DIS >= 2) sqb = in[k < 3 ? k : 2], ++k;
+    if (NPS >= 1) r0 = in[k < 3 ? k : 2], ++k;
+    if (NPS >= 2) r1 = in[k < 3 ? k : 2], ++k;
+    lut |= sel_bit(in[0], spa, sqb, r0, r1) << i;
+  }
+  return lut;
+}
+
+// One sub-lattice pass: a = departure side of a forward hop, b = the other side (§R3).
+__device__ __forceinline__ void pass_logic(uint32_t (&a)[4], uint32_t (&b)[4], const uint32_t (&spa)[4],
+                                           const uint32_t (&sqb)[4], const uint32_t (&r)[NPSA][4]) {
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    uint32_t sel;
+    if constexpr (SEL_NVARS <= 3) {
+      uint32_t in[3] = {a[w], 0u, 0u};
+      int k = 1;
+      if (DIS >= 1) in[k++] = spa[w];
+      if (DIS >= 2) in[k++] = sqb[w];
+      if (NPS >= 1) in[k++] = r[0][w];
+      if (NPS >= 2) in[k++] = r[NPS >= 2 ? 1 : 0][w];
+      sel = lop3<sel_lut()>(in[0], in[1], in[2]);
+    } else {
+      uint32_t selp = accept<T0>(r, w), selq = accept<T2>(r, w);
+      if (DIS >= 1) selp = (selp & ~spa[w]) | (accept<T1>(r, w) & spa[w]);
+      if (DIS >= 2) selq = (selq & ~sqb[w]) | (accept<T3>(r, w) & sqb[w]);
+      sel = lop3<0xCA>(a[w], selp, selq);  // a ? selp : selq
+    }
+    const uint32_t na = lop3<0xD8>(a[w], b[w], sel);  // a ^ ((a ^ b) & sel)
+    const uint32_t nb = lop3<0xE4>(a[w], b[w], sel);  // b ^ ((a ^ b) & sel)
+    a[w] = na;
+    b[w] = nb;
+  }
+}
+
+// ---- neighbour word exchange (a5): the value held by unit `src` of this sample ---------------------------------
+__device__ __forceinline__ uint32_t unit_exchange(uint32_t mine, int src, uint32_t* halo, int& parity) {
+  if (SINGLE_WARP) {
+    return __shfl_sync(0xFFFFFFFFu, mine, src);
+  } else {
+    uint32_t* slot = halo + parity * NTHREADS;
+    slot[threadIdx.x] = mine;
+    __syncthreads();
+    const uint32_t v = slot[src];
+    parity ^= 1;
+    return v;
+  }
+}
+
+struct Unit {
+  int nw;   // valid words of this unit (4, fewer in the last unit of a ragged ring, 0 for an idle lane)
+  int nxt;  // unit holding the next 256 sites (ring closure: the last unit's successor is unit 0)
+  int prv;
+};
+
+// frame 0 -> 1: P'[w] = P[w] >> 1 | next << 31
+__device__ __forceinline__ void frame_up(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity) {
+  const uint32_t h = unit_exchange(P[0], un.nxt, halo, parity);
+  if (!PARTIAL) {
+    P[0] = __funnelshift_r(P[0], P[1], 1);
+    P[1] = __funnelshift_r(P[1], P[2], 1);
+    P[2] = __funnelshift_r(P[2], P[3], 1);
+    P[3] = __funnelshift_r(P[3], h, 1);
+  } else {
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const uint32_t next = (w + 1 < un.nw) ? P[w + 1 < 4 ? w + 1 : 3] : h;
+      P[w] = (w < un.nw) ? __funnelshift_r(P[w], next, 1) : 0u;
+    }
+  }
+}
+// frame 1 -> 0: P[w] = P'[w] << 1 | prev >> 31
+__device__ __forceinline__ void frame_down(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity) {
+  uint32_t last = P[3];
+  if (PARTIAL) last = un.nw >= 4 ? P[3] : un.nw == 3 ? P[2] : un.nw == 2 ? P[1] : P[0];
+  const uint32_t h = unit_exchange(last, un.prv, halo, parity);
+  if (!PARTIAL) {
+    P[3] = __funnelshift_l(P[2], P[3], 1);
+    P[2] = __funnelshift_l(P[1], P[2], 1);
+    P[1] = __funnelshift_l(P[0], P[1], 1);
+    P[0] = __funnelshift_l(h, P[0], 1);
+  } else {
+#pragma unroll
+    for (int w = 3; w >= 0; --w) {
+      const uint32_t prev = (w > 0) ? P[w > 0 ? w - 1 : 0] : h;
+      P[w] = (w < un.nw) ? __funnelshift_l(prev, P[w], 1) : 0u;
+    }
+  }
+}
+
+// Quenched tags in the frames the passes use them in.
+struct Tags {
+  uint32_t spa0[4];  // slow-p at even sites  (a side of frame 0)
+  uint32_t spa1[4];  // slow-p at odd sites   (a side of frame 1)
+  uint32_t sqb0[4];  // slow-q at odd sites   (b side of frame 0)
+  uint32_t sqb1[4];  // slow-q at even sites, shifted to frame 1 (b side of frame 1)
+};
+
+// One MCS with the offsets (O0, O1) of its two passes known at compile time; frame 0 on entry and exit.
+template <int O0, int O1>
+__device__ __forceinline__ void mcs_logic(uint32_t (&P)[4], uint32_t (&Q)[4], const Tags& G, const Planes& R,
+                                          const Unit& un, uint32_t* halo, int& parity) {
+  if (O0) frame_up(P, un, halo, parity);
+  if (O0) pass_logic(Q, P, G.spa1, G.sqb1, R.r[0]);
+  else pass_logic(P, Q, G.spa0, G.sqb0, R.r[0]);
+  if (O1 && !O0) frame_up(P, un, halo, parity);
+  if (!O1 && O0) frame_down(P, un, halo, parity);
+  if (O1) pass_logic(Q, P, G.spa1, G.sqb1, R.r[1]);
+  else pass_logic(P, Q, G.spa0, G.sqb0, R.r[1]);
+  if (O1) frame_down(P, un, halo, parity);
+}
+
+// ---- K2 fused: heights h_x = inclusive prefix of (2n-1), exact sums per sample (a6, a7) -----------
+// 8 sites at a time through a 256-entry table in shared memory: index = 4 even-site bits | 4 odd-site bits << 4
+// (site order e0,o0,e1,o1,...); entry = (r8+8) | (s1+36)<<5 | s2<<12 with r_k the height after k sites relative to
+// the height before the byte, s1 = sum r_k, s2 = sum r_k^2.
+__device__ __forceinline__ uint32_t height_lut_entry(int idx) {
+  int r = 0, s1 = 0, s2 = 0;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    r += 2 * ((idx >> k) & 1) - 1;
+    s1 += r;
+    s2 += r * r;
+    r += 2 * ((idx >> (4 + k)) & 1) - 1;
+    s1 += r;
+    s2 += r * r;
+  }
+  return (uint32_t)(r + 8) | ((uint32_t)(s1 + 36) << 5) | ((uint32_t)s2 << 12);
+}
+
+// Sums over this unit's sites of the heights relative to the site before the unit (|r| <= 256, s2 <= 2^24).
+__device__ __forceinline__ void unit_relative_sums(const uint32_t (&P)[4], const uint32_t (&Q)[4], int nw,
+                                                   const uint32_t* lut, int& r_out, int& s1_out, int& s2_out) {
+  int r = 0, s1 = 0, s2 = 0;
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    if (!PARTIAL || w < nw) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const uint32_t idx = ((P[w] >> (4 * k)) & 15u) | (((Q[w] >> (4 * k)) & 15u) << 4);
+        const uint32_t v = lut[idx];
+        const int d = (int)(v & 31u) - 8, a1 = (int)((v >> 5) & 127u) - 36, a2 = (int)(v >> 12);
+        s1 += 8 * r + a1;
+        s2 += 8 * r * r + 2 * r * a1 + a2;
+        r += d;
+      }
+    }
+  }
+  r_out = r;
+  s1_out = s1;
+  s2_out = s2;
+}
+
+__device__ __forceinline__ void record_sums(const uint32_t (&P)[4], const uint32_t (&Q)[4], int nw,
+                                            const uint32_t* lut, long long* scratch, long long* out_h,
+                                            long long* out_h2) {
+  int r = 0, s1 = 0, s2 = 0;
+  if (nw > 0) unit_relative_sums(P, Q, nw, lut, r, s1, s2);
+  const int lane = threadIdx.x & 31;
+  int incl = r;  // inclusive scan of the unit totals: the height before unit u is the sum over units < u
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+    if (lane >= d) incl += v;
+  }
+  long long base = (long long)(incl - r);
+  if (!SINGLE_WARP) {
+    const int warp = threadIdx.x >> 5;
+    int* wtot = reinterpret_cast<int*>(scratch + 64);
+    __syncthreads();
+    if (lane == 31) wtot[warp] = incl;
+    __syncthreads();
+    int add = 0;
+    for (int k = 0; k < warp; ++k) add += wtot[k];
+    base += add;
+  }
+  const long long n = 64LL * nw;
+  long long H = n * base + (long long)s1;
+  long long H2 = n * base * base + 2LL * base * (long long)s1 + (long long)s2;
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) {
+    H += __shfl_down_sync(0xFFFFFFFFu, H, d);
+    H2 += __shfl_down_sync(0xFFFFFFFFu, H2, d);
+  }
+  if (SINGLE_WARP) {
+    if (lane == 0) {
+      *out_h = H;
+      *out_h2 = H2;
+    }
+  } else {
+    const int warp = threadIdx.x >> 5;
+    if (lane == 0) {
+      scratch[warp] = H;
+      scratch[32 + warp] = H2;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      long long a = 0, b = 0;
+      for (int k = 0; k < NTHREADS / 32; ++k) {
+        a += scratch[k];
+        b += scratch[32 + k];
+      }
+      *out_h = a;
+      *out_h2 = b;
+    }
+  }
+}
+
+// Offsets of the 32 passes of the 16 MCS starting at (m & ~15): lane l draws (mcs = base + l/2, pass = l & 1) and a
+// ballot packs them: bit 2k+pass of the result = offset of pass `pass` of MCS base+k.
+__device__ __forceinline__ uint32_t draw_offsets16(const PhiloxKeys& K, uint32_t gs, long long m) {
+  const int lane = threadIdx.x & 31;
+  const unsigned long long mb = ((unsigned long long)m & ~15ull) + (unsigned)(lane >> 1);
+  const uint4 w = philox4x32_10(0u, gs, (uint32_t)mb, ctr3(TAG_OFFSET, lane & 1, 0, (uint32_t)(mb >> 32)), K);
+  return __ballot_sync(0xFFFFFFFFu, w.x & 1u);
+}
+
+struct Ctx {
+  uint32_t P[4], Q[4];
+  Tags tags;
+  Unit un;
+  uint32_t gs;   // global sample index (Philox counter c1)
+  uint32_t G;    // supergroup index of this unit (Philox counter c0)
+  int parity;
+  uint32_t offbits;
+};
+
+// MCS m: draw the planes of MCS m+1 into Rn, then apply MCS m with the planes Rc drawn one step earlier.  Both sit
+// in one basic block per offset combination, so the scheduler overlaps the Philox rounds with the pair logic.
+__device__ __forceinline__ void mcs_step(Ctx& c, const Planes& Rc, Planes& Rn, const PhiloxKeys& K, long long m,
+                                         uint32_t* halo) {
+  if (K1J_OFFSET_MODE == 1) {
+    draw_planes(Rn, K, c.G, c.gs, m + 1);
+    mcs_logic<0, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
+  } else {
+    const uint32_t code = (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
+    switch (code) {
+      case 0:
+        draw_planes(Rn, K, c.G, c.gs, m + 1);
+        mcs_logic<0, 0>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
+        break;
+      case 1:
+        draw_planes(Rn, K, c.G, c.gs, m + 1);
+        mcs_logic<1, 0>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
+        break;
+      case 2:
+        draw_planes(Rn, K, c.G, c.gs, m + 1);
+        mcs_logic<0, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
+        break;
+      default:
+        draw_planes(Rn, K, c.G, c.gs, m + 1);
+        mcs_logic<1, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
+        break;
+    }
+  }
+}
+
+}  // namespace k1j
+}  // namespace kpz
+
+// grid = S samples, block = NTHREADS; thread u = unit u (idle when u >= U, but it joins every barrier / shuffle).
+extern "C" __global__ void __launch_bounds__(kpz::k1j::NTHREADS)
+kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::KpzRunArgs A) {
+  using namespace kpz;
+  using namespace kpz::k1j;
+  __shared__ uint32_t halo[SINGLE_WARP ? 1 : 2 * NTHREADS];
+  __shared__ long long scratch[SINGLE_WARP ? 1 : 96];
+  __shared__ uint32_t lut[256];
+  for (int i = threadIdx.x; i < 256; i += NTHREADS) lut[i] = height_lut_entry(i);
+  __syncthreads();
+
+  const int s = blockIdx.x;
+  const int u = threadIdx.x;
+  const bool active = u < U;
+  Ctx c;
+  c.un.nw = !active ? 0 : (PARTIAL ? min(4, PW - 4 * u) : 4);
+  c.un.nxt = (u + 1 >= U) ? 0 : u + 1;
+  c.un.prv = (u == 0) ? U - 1 : u - 1;
+  c.gs = (uint32_t)(D.first_sample + s);
+  c.G = (uint32_t)u;
+  c.parity = 0;
+  c.offbits = 0;
+  const unsigned long long row = (unsigned long long)s * PWp + 4ull * (active ? u : 0);
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    c.P[w] = c.Q[w] = 0u;
+    c.tags.spa0[w] = c.tags.spa1[w] = c.tags.sqb0[w] = c.tags.sqb1[w] = 0u;
+  }
+  if (active) {
+    const uint4 e = *reinterpret_cast<const uint4*>(D.E + row);
+    const uint4 o = *reinterpret_cast<const uint4*>(D.O + row);
+    c.P[0] = e.x; c.P[1] = e.y; c.P[2] = e.z; c.P[3] = e.w;
+    c.Q[0] = o.x; c.Q[1] = o.y; c.Q[2] = o.z; c.Q[3] = o.w;
+    if (DIS >= 1) {
+      const uint4 x = *reinterpret_cast<const uint4*>(D.SPE + row);
+      const uint4 y = *reinterpret_cast<const uint4*>(D.SPO + row);
+      c.tags.spa0[0] = x.x; c.tags.spa0[1] = x.y; c.tags.spa0[2] = x.z; c.tags.spa0[3] = x.w;
+      c.tags.spa1[0] = y.x; c.tags.spa1[1] = y.y; c.tags.spa1[2] = y.z; c.tags.spa1[3] = y.w;
+    }
+    if (DIS >= 2) {
+      const uint4 x = *reinterpret_cast<const uint4*>(D.SQO + row);
+      const uint4 y = *reinterpret_cast<const uint4*>(D.SQE + row);
+      c.tags.sqb0[0] = x.x; c.tags.sqb0[1] = x.y; c.tags.sqb0[2] = x.z; c.tags.sqb0[3] = x.w;
+      c.tags.sqb1[0] = y.x; c.tags.sqb1[1] = y.y; c.tags.sqb1[2] = y.z; c.tags.sqb1[3] = y.w;
+    }
+  }
+  if (DIS >= 2) frame_up(c.tags.sqb1, c.un, halo, c.parity);  // b side of frame 1 = the NEXT even site
+
+  int ri = A.rec_begin;
+  long long next_rec = ri < A.nt ? A.rec_t[ri] : -1;
+  const long long t_end = A.t0 + A.n_mcs;
+  long long m = A.t0;
+  if (K1J_OFFSET_MODE == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+
+  Planes RA, RB;
+  draw_planes(RA, D.keys, c.G, c.gs, m);
+
+  auto after_mcs = [&]() {  // m has been advanced: t = m
+    if (m == next_rec) {
+      record_sums(c.P, c.Q, c.un.nw, lut, scratch, A.rec_sum_h + (size_t)ri * D.S + s,
+                  A.rec_sum_h2 + (size_t)ri * D.S + s);
+      ++ri;
+      next_rec = ri < A.nt ? A.rec_t[ri] : -1;
+    }
+    if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+  };
+
+  while (m < t_end) {
+    mcs_step(c, RA, RB, D.keys, m, halo);
+    ++m;
+    after_mcs();
+    if (m >= t_end) break;
+    mcs_step(c, RB, RA, D.keys, m, halo);
+    ++m;
+    after_mcs();
+  }
+
+  if (active) {
+    *reinterpret_cast<uint4*>(D.E + row) = make_uint4(c.P[0], c.P[1], c.P[2], c.P[3]);
+    *reinterpret_cast<uint4*>(D.O + row) = make_uint4(c.Q[0], c.Q[1], c.Q[2], c.Q[3]);
+  }
+}

@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "common.cuh"
+#include "jit.h"
 #include "kpz_k1.cuh"
 #include "kpz_k3.cuh"
 #include "kpz_util.cuh"
@@ -164,6 +165,35 @@ K1Fn k1_pick(bool single_warp, bool partial, int dis, int nps) {
   if (single_warp) return partial ? k1_pick_dis<true, true>(dis, nps) : k1_pick_dis<true, false>(dis, nps);
   return partial ? k1_pick_dis<false, true>(dis, nps) : k1_pick_dis<false, false>(dis, nps);
 }
+
+// ---- K1 v2: the sweep specialised at run time on (L, thresholds, tags, offset mode) — k1_sweep_jit.cuh ----------
+// Fixed plane counts only: beyond kK1JitMaxPlanes planes (non-dyadic rates) the lazily evaluated generic kernel
+// (kpz_k1.cuh) needs fewer Philox calls.
+constexpr int kK1JitMaxPlanes = 6;
+
+std::vector<std::string> k1_jit_defines(const KpzDev& D, int dis) {
+  auto T = [&](int c) -> unsigned long long {
+    return D.thr[c].always ? (1ull << 32) : (unsigned long long)D.thr[c].value;
+  };
+  char buf[64];
+  std::vector<std::string> d;
+  snprintf(buf, sizeof buf, "K1J_PW=%d", D.PW);
+  d.push_back(buf);
+  for (int c = 0; c < 4; ++c) {
+    // classes a kernel variant never reads are normalised so that equal kernels share one cache entry
+    unsigned long long t = T(c);
+    if ((c == 1 && dis < 1) || (c == 3 && dis < 2)) t = 0;
+    snprintf(buf, sizeof buf, "K1J_T%d=0x%llxull", c, t);
+    d.push_back(buf);
+  }
+  snprintf(buf, sizeof buf, "K1J_DIS=%d", dis);
+  d.push_back(buf);
+  snprintf(buf, sizeof buf, "K1J_OFFSET_MODE=%d", D.offset_mode);
+  d.push_back(buf);
+  return d;
+}
+
+bool k1_use_jit(const KpzDev& D) { return jit_enabled() && D.nplanes <= kK1JitMaxPlanes; }
 
 void refresh_planes(kpz_sim* sim) {
   int np = std::max(planes_needed(sim->dev.thr[0]), planes_needed(sim->dev.thr[2]));
@@ -437,6 +467,41 @@ int kpz_create(kpz_sim** out, int64_t L, int32_t nsamples, double p, double q, c
   return KPZ_OK;
 }
 
+int kpz_jit_check(int64_t L, double p, double q, const kpz_disorder* disorder, const kpz_options* opt,
+                  size_t* cubin_bytes) {
+  if (!cubin_bytes) return fail(KPZ_EINVAL, "cubin_bytes is NULL");
+  *cubin_bytes = 0;
+  int rc = validate_sizes(L, 1, 0);
+  if (rc) return rc;
+  if (!valid_prob(p) || !valid_prob(q)) return fail(KPZ_EINVAL, "p and q must lie in [0,1]");
+  kpz_disorder d{0.0, p, 0.0, q};
+  if (disorder) d = *disorder;
+  if (!valid_prob(d.prob_slow_p) || !valid_prob(d.p_slow) || !valid_prob(d.prob_slow_q) || !valid_prob(d.q_slow))
+    return fail(KPZ_EINVAL, "disorder probabilities must lie in [0,1]");
+  int path;
+  rc = choose_path(L, opt, &path);
+  if (rc) return rc;
+  if (path != KPZ_PATH_ONCHIP) return KPZ_OK;
+  kpz_sim tmp;
+  tmp.has_sp = disorder && d.prob_slow_p > 0.0;
+  tmp.has_sq = disorder && d.prob_slow_q > 0.0;
+  KpzDev& D = tmp.dev;
+  D.thr[0] = make_thresh(p);
+  D.thr[1] = make_thresh(d.p_slow);
+  D.thr[2] = make_thresh(q);
+  D.thr[3] = make_thresh(d.q_slow);
+  D.offset_mode = opt ? opt->offset_mode : 0;
+  D.PW = (int)(L / 64);
+  refresh_planes(&tmp);
+  if (!k1_use_jit(D)) return KPZ_OK;
+  std::vector<char> cubin;
+  rc = jit_compile("k1_sweep_jit.cuh", "kpz_k1_sweep_jit", k1_jit_defines(D, tmp.has_sq ? 2 : tmp.has_sp ? 1 : 0), &cubin,
+                   nullptr);
+  if (rc) return rc;
+  *cubin_bytes = cubin.size();
+  return KPZ_OK;
+}
+
 int kpz_destroy(kpz_sim* sim) {
   delete sim;
   return KPZ_OK;
@@ -509,10 +574,19 @@ int kpz_run(kpz_sim* sim, int64_t n_mcs) {
     const bool single = D.U <= 32;
     const bool partial = (D.PW % 4) != 0;
     const int dis = sim->has_sq ? 2 : sim->has_sp ? 1 : 0;
-    K1Fn fn = k1_pick(single, partial, dis, D.nplanes);
     const int block = (D.U + 31) / 32 * 32;
-    fn<<<sim->S, block, 0, sim->stream>>>(D, A);
-    KPZ_LAUNCH_CHECK("kpz_k1_kernel");
+    if (k1_use_jit(D)) {
+      void* kfn = nullptr;
+      rc = jit_get("k1_sweep_jit.cuh", "kpz_k1_sweep_jit", k1_jit_defines(D, dis), &kfn);
+      if (rc) return rc;
+      void* args[] = {(void*)&D, (void*)&A};
+      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(sim->S), dim3(block), args, 0, sim->stream));
+      KPZ_LAUNCH_CHECK("kpz_k1_sweep_jit");
+    } else {
+      K1Fn fn = k1_pick(single, partial, dis, D.nplanes);
+      fn<<<sim->S, block, 0, sim->stream>>>(D, A);
+      KPZ_LAUNCH_CHECK("kpz_k1_kernel");
+    }
   } else {
     rc = k3_run(sim, n_mcs);
     if (rc) return rc;

@@ -17,34 +17,6 @@
 
 namespace kpz {
 
-struct KpzDev {
-  PhiloxKeys keys;
-  Thresh thr[4];  // classes: 0 = p, 1 = p_slow, 2 = q, 3 = q_slow
-  int32_t nplanes;
-  int32_t offset_mode;
-  int32_t first_sample;
-  int32_t S;
-  int32_t PW;   // 64-site groups (pair-words) per sample = L/64
-  int32_t PWp;  // row stride in words, multiple of 4
-  int32_t U;    // units per sample = PWp/4
-  uint32_t* E;  // [S][PWp] even-site words (frame 0)
-  uint32_t* O;  // [S][PWp] odd-site words
-  const uint32_t* SPE;  // slow-p tags at even / odd sites, same layout (nullptr = none)
-  const uint32_t* SPO;
-  const uint32_t* SQE;
-  const uint32_t* SQO;
-};
-
-struct KpzRunArgs {
-  long long t0;      // MCS already done
-  long long n_mcs;   // MCS to do
-  const long long* rec_t;  // [nt] record times (device)
-  int32_t rec_begin;       // first record index with time > t0
-  int32_t nt;
-  long long* rec_sum_h;    // [nt][S]
-  long long* rec_sum_h2;   // [nt][S]
-};
-
 // -------------------------------------------------------------------------------------------------------
 // One sub-lattice pass on a unit held in the right frame: a = departure side of a forward hop, b = the other.
 // (1,0) -> (0,1) iff U < T(p or p_slow at a);  (0,1) -> (1,0) iff U < T(q or q_slow at b)   (§R3).

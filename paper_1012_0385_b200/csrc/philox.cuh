@@ -1,8 +1,7 @@
 // philox.cuh — device/host Philox4x32-10 and the method's counter packing (§R4).
 // Product code (CUDA path).  Shares nothing with oracle/.
 #pragma once
-#include <cstdint>
-#include <cuda_runtime.h>
+#include "rtc_prelude.cuh"
 
 namespace kpz {
 
@@ -32,6 +31,7 @@ struct PhiloxKeys {
   uint32_t k1[10];
 };
 
+#ifndef __CUDACC_RTC__
 inline PhiloxKeys make_keys(uint64_t seed) {
   PhiloxKeys K;
   uint32_t a = (uint32_t)(seed & 0xFFFFFFFFull), b = (uint32_t)(seed >> 32);
@@ -43,6 +43,7 @@ inline PhiloxKeys make_keys(uint64_t seed) {
   }
   return K;
 }
+#endif
 
 // c3 = tag<<28 | pass<<27 | plane<<22 | time_hi(22 bits)
 __host__ __device__ __forceinline__ uint32_t ctr3(uint32_t tag, uint32_t pass, uint32_t plane, uint32_t time_hi) {
