@@ -13,6 +13,7 @@
 //   K1J_T0..K1J_T3    thresholds T(p), T(p_slow), T(q), T(q_slow) as integers in [0, 2^32]
 //   K1J_DIS           0 no disorder tags, 1 slow-p tags, 2 slow-p and slow-q tags
 //   K1J_OFFSET_MODE   0 drawn offsets, 1 alternating
+//   K1J_VARIANT       code shape of the drawn-offset sweep (see pass_branchfree)
 //
 // Layout on chip: as K1 v1 (kpz_k1.cuh): thread = one unit = 128 pairs = one Philox supergroup, 4 even-site words
 // P[4] and 4 odd-site words Q[4] in registers; frame 0 pairs (P,Q) = sites (2k,2k+1), frame 1 pairs (Q,P') with P'
@@ -20,6 +21,9 @@
 #pragma once
 #include "sweep_types.cuh"
 
+#ifndef K1J_VARIANT
+#define K1J_VARIANT 1  // 0: one code path per offset pair (4-way switch); 1: branch-free
+#endif
 #ifndef K1J_PW
 #error "k1_sweep_jit.cuh needs K1J_PW, K1J_T0..3, K1J_DIS, K1J_OFFSET_MODE"
 #endif
@@ -131,26 +135,31 @@ __host__ __device__ constexpr int sel_lut() {
   return lut;
 }
 
-// One sub-lattice pass: a = departure side of a forward hop, b = the other side (§R3).
+// sel for one word: a = departure side of a forward hop; spa / sqb = the tags of the pair's a / b site.
+__device__ __forceinline__ uint32_t select_word(uint32_t a, uint32_t spa, uint32_t sqb, const uint32_t (&r)[NPSA][4],
+                                                int w) {
+  if constexpr (SEL_NVARS <= 3) {
+    uint32_t in[3] = {a, 0u, 0u};
+    int k = 1;
+    if (DIS >= 1) in[k++] = spa;
+    if (DIS >= 2) in[k++] = sqb;
+    if (NPS >= 1) in[k++] = r[0][w];
+    if (NPS >= 2) in[k++] = r[NPS >= 2 ? 1 : 0][w];
+    return lop3<sel_lut()>(in[0], in[1], in[2]);
+  } else {
+    uint32_t selp = accept<T0>(r, w), selq = accept<T2>(r, w);
+    if (DIS >= 1) selp = lop3<0xCA>(spa, accept<T1>(r, w), selp);  // spa ? slow : normal
+    if (DIS >= 2) selq = lop3<0xCA>(sqb, accept<T3>(r, w), selq);
+    return lop3<0xCA>(a, selp, selq);  // a ? selp : selq
+  }
+}
+
+// One sub-lattice pass with the roles known at compile time (§R3).
 __device__ __forceinline__ void pass_logic(uint32_t (&a)[4], uint32_t (&b)[4], const uint32_t (&spa)[4],
                                            const uint32_t (&sqb)[4], const uint32_t (&r)[NPSA][4]) {
 #pragma unroll
   for (int w = 0; w < 4; ++w) {
-    uint32_t sel;
-    if constexpr (SEL_NVARS <= 3) {
-      uint32_t in[3] = {a[w], 0u, 0u};
-      int k = 1;
-      if (DIS >= 1) in[k++] = spa[w];
-      if (DIS >= 2) in[k++] = sqb[w];
-      if (NPS >= 1) in[k++] = r[0][w];
-      if (NPS >= 2) in[k++] = r[NPS >= 2 ? 1 : 0][w];
-      sel = lop3<sel_lut()>(in[0], in[1], in[2]);
-    } else {
-      uint32_t selp = accept<T0>(r, w), selq = accept<T2>(r, w);
-      if (DIS >= 1) selp = (selp & ~spa[w]) | (accept<T1>(r, w) & spa[w]);
-      if (DIS >= 2) selq = (selq & ~sqb[w]) | (accept<T3>(r, w) & sqb[w]);
-      sel = lop3<0xCA>(a[w], selp, selq);  // a ? selp : selq
-    }
+    const uint32_t sel = select_word(a[w], spa[w], sqb[w], r, w);
     const uint32_t na = lop3<0xD8>(a[w], b[w], sel);  // a ^ ((a ^ b) & sel)
     const uint32_t nb = lop3<0xE4>(a[w], b[w], sel);  // b ^ ((a ^ b) & sel)
     a[w] = na;
@@ -179,36 +188,39 @@ struct Unit {
 };
 
 // frame 0 -> 1: P'[w] = P[w] >> 1 | next << 31
-__device__ __forceinline__ void frame_up(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity) {
+// (sh = 1; sh = 0 leaves P as it is: the branch-free sweep passes the offset itself)
+__device__ __forceinline__ void frame_up(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity,
+                                         uint32_t sh = 1u) {
   const uint32_t h = unit_exchange(P[0], un.nxt, halo, parity);
   if (!PARTIAL) {
-    P[0] = __funnelshift_r(P[0], P[1], 1);
-    P[1] = __funnelshift_r(P[1], P[2], 1);
-    P[2] = __funnelshift_r(P[2], P[3], 1);
-    P[3] = __funnelshift_r(P[3], h, 1);
+    P[0] = __funnelshift_r(P[0], P[1], sh);
+    P[1] = __funnelshift_r(P[1], P[2], sh);
+    P[2] = __funnelshift_r(P[2], P[3], sh);
+    P[3] = __funnelshift_r(P[3], h, sh);
   } else {
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
       const uint32_t next = (w + 1 < un.nw) ? P[w + 1 < 4 ? w + 1 : 3] : h;
-      P[w] = (w < un.nw) ? __funnelshift_r(P[w], next, 1) : 0u;
+      P[w] = (w < un.nw) ? __funnelshift_r(P[w], next, sh) : 0u;
     }
   }
 }
 // frame 1 -> 0: P[w] = P'[w] << 1 | prev >> 31
-__device__ __forceinline__ void frame_down(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity) {
+__device__ __forceinline__ void frame_down(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity,
+                                           uint32_t sh = 1u) {
   uint32_t last = P[3];
   if (PARTIAL) last = un.nw >= 4 ? P[3] : un.nw == 3 ? P[2] : un.nw == 2 ? P[1] : P[0];
   const uint32_t h = unit_exchange(last, un.prv, halo, parity);
   if (!PARTIAL) {
-    P[3] = __funnelshift_l(P[2], P[3], 1);
-    P[2] = __funnelshift_l(P[1], P[2], 1);
-    P[1] = __funnelshift_l(P[0], P[1], 1);
-    P[0] = __funnelshift_l(h, P[0], 1);
+    P[3] = __funnelshift_l(P[2], P[3], sh);
+    P[2] = __funnelshift_l(P[1], P[2], sh);
+    P[1] = __funnelshift_l(P[0], P[1], sh);
+    P[0] = __funnelshift_l(h, P[0], sh);
   } else {
 #pragma unroll
     for (int w = 3; w >= 0; --w) {
       const uint32_t prev = (w > 0) ? P[w > 0 ? w - 1 : 0] : h;
-      P[w] = (w < un.nw) ? __funnelshift_l(prev, P[w], 1) : 0u;
+      P[w] = (w < un.nw) ? __funnelshift_l(prev, P[w], sh) : 0u;
     }
   }
 }
@@ -233,6 +245,30 @@ __device__ __forceinline__ void mcs_logic(uint32_t (&P)[4], uint32_t (&Q)[4], co
   if (O1) pass_logic(Q, P, G.spa1, G.sqb1, R.r[1]);
   else pass_logic(P, Q, G.spa0, G.sqb0, R.r[1]);
   if (O1) frame_down(P, un, halo, parity);
+}
+
+// Branch-free form (K1J_VARIANT 1): the offset o of a pass is a run-time, warp-uniform value.  P goes to frame o by
+// a funnel shift by o bits, the a side is picked by a mask (P and Q enter the update symmetrically, so only the
+// rate selection needs to know which of them is a), and P returns to frame 0 by the opposite shift: the whole
+// MCS is one basic block, which the scheduler fills with the Philox rounds of the next MCS.
+__device__ __forceinline__ void pass_branchfree(uint32_t (&P)[4], uint32_t (&Q)[4], const Tags& G,
+                                                const uint32_t (&r)[NPSA][4], const Unit& un, uint32_t o,
+                                                uint32_t* halo, int& parity) {
+  const uint32_t M = 0u - o;  // all ones in frame 1
+  frame_up(P, un, halo, parity, o);
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    const uint32_t a = lop3<0xCA>(M, Q[w], P[w]);  // frame 1: a = odd site (Q); frame 0: a = even site (P)
+    uint32_t spa = 0u, sqb = 0u;
+    if (DIS >= 1) spa = lop3<0xCA>(M, G.spa1[w], G.spa0[w]);
+    if (DIS >= 2) sqb = lop3<0xCA>(M, G.sqb1[w], G.sqb0[w]);
+    const uint32_t sel = select_word(a, spa, sqb, r, w);
+    const uint32_t np = lop3<0xD8>(P[w], Q[w], sel);
+    const uint32_t nq = lop3<0xE4>(P[w], Q[w], sel);
+    P[w] = np;
+    Q[w] = nq;
+  }
+  frame_down(P, un, halo, parity, o);
 }
 
 // ---- K2 fused: heights h_x = inclusive prefix of (2n-1), exact sums per sample (a6, a7) -----------
@@ -357,6 +393,11 @@ __device__ __forceinline__ void mcs_step(Ctx& c, const Planes& Rc, Planes& Rn, c
   if (K1J_OFFSET_MODE == 1) {
     draw_planes(Rn, K, c.G, c.gs, m + 1);
     mcs_logic<0, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
+  } else if (K1J_VARIANT == 1) {
+    const uint32_t code = (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
+    draw_planes(Rn, K, c.G, c.gs, m + 1);
+    pass_branchfree(c.P, c.Q, c.tags, Rc.r[0], c.un, code & 1u, halo, c.parity);
+    pass_branchfree(c.P, c.Q, c.tags, Rc.r[1], c.un, code >> 1, halo, c.parity);
   } else {
     const uint32_t code = (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
     switch (code) {

@@ -3,7 +3,9 @@
 // launches them.  There is no CPU fallback: without a CUDA device every call that needs one fails with KPZ_ECUDA.
 #include <algorithm>
 #include <atomic>
+#include <cstdlib>
 #include <cstring>
+#include <string>
 #include <new>
 #include <vector>
 
@@ -190,6 +192,10 @@ std::vector<std::string> k1_jit_defines(const KpzDev& D, int dis) {
   d.push_back(buf);
   snprintf(buf, sizeof buf, "K1J_OFFSET_MODE=%d", D.offset_mode);
   d.push_back(buf);
+  if (const char* v = std::getenv("KPZ_B200_K1_VARIANT")) {  // tuning knob: code shape of the sweep (k1_sweep_jit.cuh)
+    snprintf(buf, sizeof buf, "K1J_VARIANT=%d", atoi(v));
+    d.push_back(buf);
+  }
   return d;
 }
 
