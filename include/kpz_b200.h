@@ -141,6 +141,8 @@ int kpz_path(const kpz_sim*, int32_t* path);
  * and returns the size of its sm_100a cubin (0 when that configuration runs on a statically compiled kernel). */
 int kpz_jit_check(int64_t L, double p, double q, const kpz_disorder* disorder, const kpz_options* opt,
                   size_t* cubin_bytes);
+int lanes_jit_check(int64_t L, double p_a, double p_b, double turn_prob, int64_t turn_period, double omega,
+                    const kpz_options* opt, size_t* cubin_bytes); /* same for the two-lane kernel */
 
 #ifdef __cplusplus
 }

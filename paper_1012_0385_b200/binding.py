@@ -72,6 +72,8 @@ SIGNATURES = {
     "kpz_path": (C.c_int, [_P, C.POINTER(C.c_int32)]),
     "kpz_jit_check": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.POINTER(Disorder), C.POINTER(Options),
                                 C.POINTER(C.c_size_t)]),
+    "lanes_jit_check": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int64, C.c_double,
+                                  C.POINTER(Options), C.POINTER(C.c_size_t)]),
 }
 
 
@@ -126,6 +128,15 @@ def jit_check(L, p, q, disorder=None, offset_mode=0, path=KPZ_PATH_AUTO) -> int:
     n = C.c_size_t()
     _chk(load_library().kpz_jit_check(int(L), float(p), float(q), C.byref(d) if d is not None else None, C.byref(o),
                                       C.byref(n)), "kpz_jit_check")
+    return int(n.value)
+
+
+def lanes_jit_check(L, p_a, p_b, turn_prob, turn_period, omega, offset_mode=0) -> int:
+    """lanes_jit_check: compile (no GPU needed) the specialised two-lane kernel; cubin size in bytes."""
+    o = Options(0, int(offset_mode), 0)
+    n = C.c_size_t()
+    _chk(load_library().lanes_jit_check(int(L), float(p_a), float(p_b), float(turn_prob), int(turn_period),
+                                        float(omega), C.byref(o), C.byref(n)), "lanes_jit_check")
     return int(n.value)
 
 

@@ -1,0 +1,418 @@
+// k4_lanes_jit.cuh — K4 v2: two-lane opposite-direction lattice gas with turning points, specialised at run time
+// (NVRTC, jit.cu) on the ring size and the four thresholds (north_star (4); PAPER.md:253-275;
+// DESIGN §R12-R17).  One CTA per sample, persistent over the whole lanes_run.
+//
+// Layout on chip: NATURAL bit order (bit i&31 of word i>>5 = site i), because the dominant random streams of this
+// model are per SITE (lane changes, turning points): one Philox call is one bit-plane of 128 consecutive sites = 4
+// natural words.  A thread owns exactly one such supergroup: 4 words of lane A, lane B and the turning-point mask
+// in registers (L=16384: 128 threads = 4 warps per sample, 1024 warps on the chip for config 5).
+//   * in-lane hops are word-local bit logic: with sh = (X >> 1 | next word << 31), lane A (right) hops where
+//     X & ~sh & pairmask(o), lane B (left) where ~X & sh & pairmask(o); offset 1 needs bit 0 of the next thread's
+//     word 0 and sends one carry bit back (ring closure = wrap-around of that exchange);
+//   * lane changes: live = turn & source & ~target; U < T(omega) is evaluated MSB-first over bit-planes: the first
+//     K4J_EAGER planes of both lane-change steps of MCS m+1 are drawn while MCS m is processed (counter-based, state
+//     independent), deeper planes only while some live site of the warp is still undecided, two planes per trip;
+//   * hop counters by POPC of two merged hop words (hops of one pass sit on one bit parity), occupancy profile at
+//     epoch ends by warp-transposed, coalesced red.global.add.
+//
+// Compile-time configuration (-D, set by lanes_api.cu): K4J_W = L/32, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN
+// (thresholds in [0, 2^32]), K4J_OFFSET_MODE, K4J_EAGER.
+#pragma once
+#include "sweep_types.cuh"
+
+#ifndef K4J_W
+#error "k4_lanes_jit.cuh needs K4J_W, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN, K4J_OFFSET_MODE"
+#endif
+#ifndef K4J_EAGER
+#define K4J_EAGER 2
+#endif
+
+namespace kpz {
+namespace k4j {
+
+constexpr int W = K4J_W;
+constexpr int U = (W + 3) / 4;
+constexpr bool SINGLE_WARP = U <= 32;
+constexpr bool PARTIAL = (W % 4) != 0;
+constexpr int NTHREADS = (U + 31) / 32 * 32;
+constexpr uint64_t TPA = K4J_TPA, TPB = K4J_TPB, TOMEGA = K4J_TOMEGA, TTURN = K4J_TTURN;
+constexpr uint64_t kOne = 1ull << 32;
+constexpr uint32_t FULL = 0xFFFFFFFFu;
+
+__host__ __device__ constexpr int planes_of(uint64_t T) {
+  if (T == 0 || T >= kOne) return 0;
+  int z = 0;
+  while (!((T >> z) & 1ull)) ++z;
+  return 32 - z;
+}
+constexpr int NPW = planes_of(TOMEGA);
+constexpr int EAGER = K4J_EAGER < NPW ? K4J_EAGER : NPW;
+constexpr int EAGERA = EAGER > 0 ? EAGER : 1;
+
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t d;
+  asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(d) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+  return d;
+}
+
+// One MSB-first comparison step with plane `pl` of the uniforms (R = that plane's bits): lt = already decided
+// U < T, eq = prefix still equal to T's.
+template <uint64_t T>
+__device__ __forceinline__ void plane_step(uint32_t (&lt)[4], uint32_t (&eq)[4], const uint32_t (&R)[4], int pl) {
+  const uint32_t tb = 0u - (uint32_t)((T >> (31 - pl)) & 1ull);
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    lt[w] |= eq[w] & tb & ~R[w];
+    eq[w] &= ~(R[w] ^ tb);
+  }
+}
+
+// Finish U < T for the still-undecided elements `eq` of supergroup G of stream c3 (tag | pass | time_hi), starting at
+// plane pl0.  Two planes per trip, trips are warp-uniform (a warp leaves when none of its lanes is undecided).
+template <uint64_t T>
+__device__ __forceinline__ void resolve(uint32_t (&lt)[4], uint32_t (&eq)[4], const PhiloxKeys& K, uint32_t G,
+                                        uint32_t gs, uint32_t tlo, uint32_t c3, int pl0) {
+  constexpr int NP = planes_of(T);
+#pragma unroll 1
+  for (int pl = pl0; pl < NP; pl += 2) {
+    if (!__any_sync(FULL, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u)) break;
+    const uint4 v0 = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)pl << 22), K);
+    const uint4 v1 = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)(pl + 1 < 32 ? pl + 1 : 31) << 22), K);
+    const uint32_t R0[4] = {v0.x, v0.y, v0.z, v0.w};
+    const uint32_t R1[4] = {v1.x, v1.y, v1.z, v1.w};
+    plane_step<T>(lt, eq, R0, pl);
+    if (pl + 1 < NP) plane_step<T>(lt, eq, R1, pl + 1);
+  }
+}
+
+// [U < T] over the `live` elements of one supergroup, from plane 0.
+template <uint64_t T>
+__device__ __forceinline__ void lazy_less(uint32_t (&lt)[4], const uint32_t (&live)[4], const PhiloxKeys& K, uint32_t G,
+                                          uint32_t gs, uint32_t tlo, uint32_t c3) {
+  uint32_t eq[4];
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    lt[w] = (T >= kOne) ? live[w] : 0u;
+    eq[w] = (T >= kOne || T == 0) ? 0u : live[w];
+  }
+  if (T > 0 && T < kOne) resolve<T>(lt, eq, K, G, gs, tlo, c3, 0);
+}
+
+// ---- bit gathers between site order and pair order ------------------------------------------------------------------
+__device__ __forceinline__ uint32_t compress_even(uint32_t x) {  // even-position bits -> low 16 bits
+  x &= 0x55555555u;
+  x = (x | (x >> 1)) & 0x33333333u;
+  x = (x | (x >> 2)) & 0x0F0F0F0Fu;
+  x = (x | (x >> 4)) & 0x00FF00FFu;
+  x = (x | (x >> 8)) & 0x0000FFFFu;
+  return x;
+}
+__device__ __forceinline__ uint32_t spread_even(uint32_t x) {  // low 16 bits -> even positions
+  x &= 0x0000FFFFu;
+  x = (x | (x << 8)) & 0x00FF00FFu;
+  x = (x | (x << 4)) & 0x0F0F0F0Fu;
+  x = (x | (x << 2)) & 0x33333333u;
+  x = (x | (x << 1)) & 0x55555555u;
+  return x;
+}
+
+// ---- neighbour exchange: the value held by thread `src` of this sample ---------------------------------------------
+__device__ __forceinline__ uint32_t unit_exchange(uint32_t mine, int src, uint32_t* halo, int& parity) {
+  if (SINGLE_WARP) {
+    return __shfl_sync(FULL, mine, src);
+  } else {
+    uint32_t* slot = halo + parity * NTHREADS;
+    slot[threadIdx.x] = mine;
+    __syncthreads();
+    const uint32_t v = slot[src];
+    parity ^= 1;
+    return v;
+  }
+}
+
+struct Unit {
+  int u;     // supergroup index of this thread within the sample
+  int nwn;   // valid words (4; 2 in the last thread of a ragged ring; 0 for an idle lane)
+  int nxt, prv;
+  uint32_t gs;  // global sample index
+};
+
+// In-lane pass of one lane: RIGHT (lane A): (1,0)->(0,1) on pairs (a, a+1); else (lane B) (0,1)->(1,0).
+// o = offset of the pass; next0 = bit 0 of the next thread's word 0 (old value; only used when o = 1).
+// Returns the carry: 1 if the hop over this thread's last pair flips bit 0 of the next thread (o = 1 only).
+template <bool RIGHT, uint64_t TP>
+__device__ __forceinline__ uint32_t lane_pass(uint32_t (&X)[4], const Unit& un, uint32_t o, uint32_t next0,
+                                              const PhiloxKeys& K, uint32_t tag, uint32_t tlo, uint32_t c3time,
+                                              unsigned long long& hops) {
+  uint32_t hop[4];
+  const uint32_t amask = o ? 0xAAAAAAAAu : 0x55555555u;
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    uint32_t nx = (w < 3) ? X[w < 3 ? w + 1 : 3] : next0;
+    if (PARTIAL) nx = (w + 1 < un.nwn) ? nx : next0;
+    const uint32_t sh = __funnelshift_r(X[w], nx, 1);
+    hop[w] = RIGHT ? lop3<0x20>(X[w], sh, amask) : lop3<0x08>(X[w], sh, amask);  // X & ~sh & m : ~X & sh & m
+    if (PARTIAL) hop[w] = (w < un.nwn) ? hop[w] : 0u;
+  }
+  if (TP < kOne) {
+    // candidates in PAIR order (in-lane uniforms are per pair): this thread's 64 pairs are words
+    // 2(u&1), 2(u&1)+1 of pair supergroup u>>1
+    const uint32_t lv0 = compress_even(hop[0] >> o) | (compress_even(hop[1] >> o) << 16);
+    const uint32_t lv1 = compress_even(hop[2] >> o) | (compress_even(hop[3] >> o) << 16);
+    const bool hi = (un.u & 1) != 0;
+    uint32_t live[4] = {hi ? 0u : lv0, hi ? 0u : lv1, hi ? lv0 : 0u, hi ? lv1 : 0u};
+    uint32_t acc[4];
+    lazy_less<TP>(acc, live, K, (uint32_t)(un.u >> 1), un.gs, tlo, ctr3(tag, 0, 0, 0) | c3time);
+    const uint32_t a0 = hi ? acc[2] : acc[0], a1 = hi ? acc[3] : acc[1];
+    hop[0] = spread_even(a0) << o;
+    hop[1] = spread_even(a0 >> 16) << o;
+    hop[2] = spread_even(a1) << o;
+    hop[3] = spread_even(a1 >> 16) << o;
+  }
+  // a hop flips both sites of its pair: hop | hop << 1, the bit shifted out of a word enters the next one
+  uint32_t out;
+  if (!PARTIAL) {
+    X[3] ^= hop[3] | __funnelshift_l(hop[2], hop[3], 1);
+    X[2] ^= hop[2] | __funnelshift_l(hop[1], hop[2], 1);
+    X[1] ^= hop[1] | __funnelshift_l(hop[0], hop[1], 1);
+    X[0] ^= hop[0] | (hop[0] << 1);
+    out = hop[3] >> 31;
+  } else {
+    uint32_t carry = 0;
+    out = 0;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      X[w] ^= hop[w] | (hop[w] << 1) | carry;
+      carry = hop[w] >> 31;
+      if (w + 1 == un.nwn) {  // the carry of the last valid word leaves the thread
+        out = carry;
+        carry = 0;
+      }
+    }
+  }
+  // hops of one pass sit on one bit parity, so two hop words merge into one POPC
+  hops += __popc(hop[0] | __funnelshift_l(hop[1], hop[1], 1)) + __popc(hop[2] | __funnelshift_l(hop[3], hop[3], 1));
+  return out;
+}
+
+// The eager planes of the two lane-change steps of one MCS: r[step][plane][word].
+struct Eager {
+  uint32_t r[2][EAGERA][4];
+};
+
+__device__ __forceinline__ void draw_eager(Eager& E, const PhiloxKeys& K, const Unit& un, long long m) {
+  const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
+#pragma unroll
+  for (int st = 0; st < 2; ++st) {
+#pragma unroll
+    for (int pl = 0; pl < EAGER; ++pl) {
+      const uint4 v = philox4x32_10((uint32_t)un.u, un.gs, tlo,
+                                    ctr3(st == 0 ? TAG_SWITCH_AB : TAG_SWITCH_BA, 0, (uint32_t)pl, thi), K);
+      E.r[st][pl][0] = v.x;
+      E.r[st][pl][1] = v.y;
+      E.r[st][pl][2] = v.z;
+      E.r[st][pl][3] = v.w;
+    }
+  }
+}
+
+// Lane changes at turning points: SRC -> DST where turn & SRC & ~DST and U < T(omega).
+__device__ __forceinline__ void lane_change(uint32_t (&SRC)[4], uint32_t (&DST)[4], const uint32_t (&T)[4],
+                                            const uint32_t (&r)[EAGERA][4], const PhiloxKeys& K, const Unit& un,
+                                            uint32_t tag, uint32_t tlo, uint32_t thi) {
+  uint32_t lt[4], eq[4];
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    const uint32_t live = lop3<0x20>(SRC[w], DST[w], T[w]);  // SRC & ~DST & T
+    lt[w] = (TOMEGA >= kOne) ? live : 0u;
+    eq[w] = (TOMEGA >= kOne || TOMEGA == 0) ? 0u : live;
+  }
+  if (TOMEGA > 0 && TOMEGA < kOne) {
+#pragma unroll
+    for (int pl = 0; pl < EAGER; ++pl) plane_step<TOMEGA>(lt, eq, r[pl], pl);
+    if (EAGER < NPW) resolve<TOMEGA>(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
+  }
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    SRC[w] ^= lt[w];
+    DST[w] ^= lt[w];
+  }
+}
+
+// Quenched-per-epoch turning-point mask of this thread's supergroup: all 128 sites are live.
+__device__ __forceinline__ void draw_turn(uint32_t (&T)[4], const PhiloxKeys& K, const Unit& un,
+                                          unsigned long long epoch) {
+  const uint32_t live[4] = {FULL, FULL, FULL, FULL};
+  lazy_less<TTURN>(T, live, K, (uint32_t)un.u, un.gs, (uint32_t)epoch, ctr3(TAG_TURN, 0, 0, (uint32_t)(epoch >> 32)));
+#pragma unroll
+  for (int w = 0; w < 4; ++w) T[w] = (w < un.nwn) ? T[w] : 0u;
+}
+
+// Epoch-end occupancy profile: occ[site] += bit.  The warp transposes its 32 x 4 words so that lane l
+// adds the bits of sites 32 j + l: every red.global.add of the warp covers 128 consecutive bytes.
+__device__ __forceinline__ void add_profile(const uint32_t (&X)[4], uint32_t* occ_sample) {
+  const int lane = threadIdx.x & 31;
+  const int warp_base = (threadIdx.x & ~31) * 128;  // first site of this warp
+#pragma unroll 1
+  for (int t = 0; t < 32; ++t) {
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const uint32_t v = __shfl_sync(FULL, X[w], t);
+      const int site = warp_base + 128 * t + 32 * w + lane;
+      if (((v >> lane) & 1u) && site < 32 * W) atomicAdd(occ_sample + site, 1u);
+    }
+  }
+}
+
+__device__ __forceinline__ uint32_t draw_offsets16(const PhiloxKeys& K, uint32_t gs, long long m) {
+  const int lane = threadIdx.x & 31;
+  const unsigned long long mb = ((unsigned long long)m & ~15ull) + (unsigned)(lane >> 1);
+  const uint4 w = philox4x32_10(0u, gs, (uint32_t)mb, ctr3(TAG_OFFSET, lane & 1, 0, (uint32_t)(mb >> 32)), K);
+  return __ballot_sync(FULL, w.x & 1u);
+}
+
+}  // namespace k4j
+}  // namespace kpz
+
+// grid = S samples, block = NTHREADS; thread u = supergroup u (idle when u >= U, but it joins every barrier / shuffle).
+extern "C" __global__ void __launch_bounds__(kpz::k4j::NTHREADS)
+lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constant__ kpz::LanesRunArgs R) {
+  using namespace kpz;
+  using namespace kpz::k4j;
+  __shared__ uint32_t halo[SINGLE_WARP ? 1 : 2 * NTHREADS];
+  __shared__ unsigned long long red[SINGLE_WARP ? 1 : 4 * 32];
+  const int s = blockIdx.x;
+  const int lane = threadIdx.x & 31;
+  Unit un;
+  un.u = threadIdx.x;
+  const bool active = un.u < U;
+  un.nwn = !active ? 0 : (PARTIAL ? min(4, W - 4 * un.u) : 4);
+  un.nxt = (un.u + 1 >= U) ? 0 : un.u + 1;
+  un.prv = (un.u == 0) ? U - 1 : un.u - 1;
+  un.gs = (uint32_t)(D.first_sample + s);
+  const unsigned long long row = (unsigned long long)s * D.Wp + 4ull * (active ? un.u : 0);
+  int parity = 0;
+
+  uint32_t A[4] = {0, 0, 0, 0}, B[4] = {0, 0, 0, 0}, T[4] = {0, 0, 0, 0};
+  if (active) {
+    const uint4 a = *reinterpret_cast<const uint4*>(D.A + row);
+    const uint4 b = *reinterpret_cast<const uint4*>(D.B + row);
+    const uint4 t = *reinterpret_cast<const uint4*>(D.T + row);
+    A[0] = a.x; A[1] = a.y; A[2] = a.z; A[3] = a.w;
+    B[0] = b.x; B[1] = b.y; B[2] = b.z; B[3] = b.w;
+    T[0] = t.x; T[1] = t.y; T[2] = t.z; T[3] = t.w;
+  }
+  unsigned long long jA = 0, jB = 0;
+  int ri = R.rec_begin;
+  long long next_rec = ri < R.nt ? R.rec_t[ri] : -1;
+  const long long t_end = R.t0 + R.n_mcs;
+  const long long period = D.period;
+  long long m = R.t0;
+  // epoch bookkeeping without a 64-bit division per MCS
+  long long epoch = period > 0 ? m / period : 0;
+  long long in_epoch = period > 0 ? m - epoch * period : 0;  // m mod period
+  uint32_t offbits = 0;
+  if (K4J_OFFSET_MODE == 0) offbits = draw_offsets16(D.keys, un.gs, m);
+
+  auto block_sum4 = [&](unsigned long long v0, unsigned long long v1, unsigned long long v2, unsigned long long v3,
+                        unsigned long long (&out)[4]) {
+    unsigned long long v[4] = {v0, v1, v2, v3};
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+#pragma unroll
+      for (int d = 16; d >= 1; d >>= 1) v[k] += __shfl_down_sync(FULL, v[k], d);
+    if (SINGLE_WARP) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k) out[k] = v[k];  // valid in lane 0
+    } else {
+      const int warp = threadIdx.x >> 5;
+      __syncthreads();
+      if (lane == 0)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) red[k * 32 + warp] = v[k];
+      __syncthreads();
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        unsigned long long a = 0;
+        for (int w = 0; w < NTHREADS / 32; ++w) a += red[k * 32 + w];
+        out[k] = a;
+      }
+    }
+  };
+
+  Eager EA, EB;
+  draw_eager(EA, D.keys, un, m);
+
+  // One MCS m with the eager lane-change planes Ec drawn one step earlier; draws those of MCS m+1 into En.
+  auto mcs = [&](const Eager& Ec, Eager& En) {
+    const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
+    if (period > 0 && m > 0 && in_epoch == 0) draw_turn(T, D.keys, un, (unsigned long long)epoch);
+    draw_eager(En, D.keys, un, m + 1);
+#pragma unroll
+    for (int pass = 0; pass < 2; ++pass) {
+      const uint32_t o = K4J_OFFSET_MODE ? (uint32_t)pass : ((offbits >> (2 * ((int)m & 15) + pass)) & 1u);
+      // in-lane hops of both lanes with the same offset
+      uint32_t nx = 0;
+      if (o) {
+        nx = unit_exchange((A[0] & 1u) | ((B[0] & 1u) << 1), un.nxt, halo, parity);
+        if (!active) nx = 0;  // idle threads hold all-zero words and must not see a neighbour bit
+      }
+      const uint32_t c3t = ((uint32_t)pass << 27) | thi;
+      const uint32_t cA = lane_pass<true, TPA>(A, un, o, nx & 1u, D.keys, TAG_PAIR, tlo, c3t, jA);
+      const uint32_t cB = lane_pass<false, TPB>(B, un, o, nx >> 1, D.keys, TAG_PAIR_B, tlo, c3t, jB);
+      if (o) {
+        const uint32_t in = unit_exchange(cA | (cB << 1), un.prv, halo, parity);
+        if (active) {
+          A[0] ^= in & 1u;
+          B[0] ^= in >> 1;
+        }
+      }
+      // lane changes at turning points: A->B after pass 0, B->A after pass 1
+      if (pass == 0) lane_change(A, B, T, Ec.r[0], D.keys, un, TAG_SWITCH_AB, tlo, thi);
+      else lane_change(B, A, T, Ec.r[1], D.keys, un, TAG_SWITCH_BA, tlo, thi);
+    }
+    ++m;  // t = m from here on
+    if (period > 0 && ++in_epoch == period) {
+      in_epoch = 0;
+      ++epoch;
+      add_profile(A, D.occA + (size_t)s * 32 * W);  // occupancy profile at epoch ends
+      add_profile(B, D.occB + (size_t)s * 32 * W);
+    }
+    if (m == next_rec) {
+      unsigned long long tot[4];
+      block_sum4(jA, jB, (unsigned long long)(__popc(A[0]) + __popc(A[1]) + __popc(A[2]) + __popc(A[3])),
+                 (unsigned long long)(__popc(B[0]) + __popc(B[1]) + __popc(B[2]) + __popc(B[3])), tot);
+      if (threadIdx.x == 0) {
+        const size_t cell = (size_t)ri * D.S + s, plane = (size_t)R.nt * D.S;
+        R.rec[cell] = (long long)(D.JA[s] + tot[0]);
+        R.rec[plane + cell] = (long long)(D.JB[s] + tot[1]);
+        R.rec[2 * plane + cell] = (long long)tot[2];
+        R.rec[3 * plane + cell] = (long long)tot[3];
+      }
+      ++ri;
+      next_rec = ri < R.nt ? R.rec_t[ri] : -1;
+    }
+    if (K4J_OFFSET_MODE == 0 && ((int)m & 15) == 0) offbits = draw_offsets16(D.keys, un.gs, m);
+  };
+
+  while (m < t_end) {
+    mcs(EA, EB);
+    if (m >= t_end) break;
+    mcs(EB, EA);
+  }
+
+  {
+    unsigned long long tot[4];
+    block_sum4(jA, jB, 0, 0, tot);
+    if (threadIdx.x == 0) {
+      D.JA[s] += tot[0];
+      D.JB[s] += tot[1];
+    }
+  }
+  if (active) {
+    *reinterpret_cast<uint4*>(D.A + row) = make_uint4(A[0], A[1], A[2], A[3]);
+    *reinterpret_cast<uint4*>(D.B + row) = make_uint4(B[0], B[1], B[2], B[3]);
+    *reinterpret_cast<uint4*>(D.T + row) = make_uint4(T[0], T[1], T[2], T[3]);
+  }
+}

@@ -1,9 +1,12 @@
 // lanes_api.cu — host side of the two-lane model: the lanes_* entry points of include/kpz_b200.h.
 #include <algorithm>
+#include <cstdlib>
 #include <new>
+#include <string>
 #include <vector>
 
 #include "common.cuh"
+#include "jit.h"
 #include "lanes_k4.cuh"
 
 using namespace kpz;
@@ -62,6 +65,32 @@ LLayout lanes_layout(int64_t L, int32_t S, int32_t max_records) {
   y.off_rec = take((size_t)4 * std::max(max_records, 1) * S * 8);
   y.total = off;
   return y;
+}
+
+// ---- K4 v2: kernel specialised at run time on (L, thresholds, offset mode) — k4_lanes_jit.cuh ---------------------
+bool k4_use_jit(const LanesDev& D) { return jit_enabled() && (D.W + 3) / 4 <= 1024; }
+
+std::vector<std::string> k4_jit_defines(const LanesDev& D) {
+  auto T = [](const Thresh& t) -> unsigned long long { return t.always ? (1ull << 32) : (unsigned long long)t.value; };
+  char buf[64];
+  std::vector<std::string> d;
+  snprintf(buf, sizeof buf, "K4J_W=%d", D.W);
+  d.push_back(buf);
+  snprintf(buf, sizeof buf, "K4J_TPA=0x%llxull", T(D.t_pa));
+  d.push_back(buf);
+  snprintf(buf, sizeof buf, "K4J_TPB=0x%llxull", T(D.t_pb));
+  d.push_back(buf);
+  snprintf(buf, sizeof buf, "K4J_TOMEGA=0x%llxull", T(D.t_omega));
+  d.push_back(buf);
+  snprintf(buf, sizeof buf, "K4J_TTURN=0x%llxull", D.period > 0 ? T(D.t_turn) : 0ull);  // never redrawn without a period
+  d.push_back(buf);
+  snprintf(buf, sizeof buf, "K4J_OFFSET_MODE=%d", D.offset_mode);
+  d.push_back(buf);
+  if (const char* v = std::getenv("KPZ_B200_K4_EAGER")) {  // tuning knob: lane-change planes drawn one MCS ahead
+    snprintf(buf, sizeof buf, "K4J_EAGER=%d", atoi(v));
+    d.push_back(buf);
+  }
+  return d;
 }
 
 int grid_for(size_t n, int block = 256) {
@@ -166,6 +195,30 @@ int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, doubl
   return KPZ_OK;
 }
 
+int lanes_jit_check(int64_t L, double p_a, double p_b, double turn_prob, int64_t turn_period, double omega,
+                    const kpz_options* opt, size_t* cubin_bytes) {
+  if (!cubin_bytes) return fail(KPZ_EINVAL, "cubin_bytes is NULL");
+  *cubin_bytes = 0;
+  int rc = lanes_validate(L, 1, 0);
+  if (rc) return rc;
+  if (!valid_prob(p_a) || !valid_prob(p_b) || !valid_prob(turn_prob) || !valid_prob(omega) || turn_period < 0)
+    return fail(KPZ_EINVAL, "probabilities must lie in [0,1] and turn_period >= 0");
+  LanesDev D{};
+  D.t_pa = make_thresh(p_a);
+  D.t_pb = make_thresh(p_b);
+  D.t_turn = make_thresh(turn_prob);
+  D.t_omega = make_thresh(omega);
+  D.offset_mode = opt ? opt->offset_mode : 0;
+  D.W = (int)(L / 32);
+  D.period = turn_period;
+  if (!k4_use_jit(D)) return KPZ_OK;
+  std::vector<char> cubin;
+  rc = jit_compile("k4_lanes_jit.cuh", "lanes_k4_sweep_jit", k4_jit_defines(D), &cubin, nullptr);
+  if (rc) return rc;
+  *cubin_bytes = cubin.size();
+  return KPZ_OK;
+}
+
 int lanes_destroy(lanes_sim* sim) {
   delete sim;
   return KPZ_OK;
@@ -208,7 +261,14 @@ int lanes_run(lanes_sim* sim, int64_t n_mcs) {
   const bool single = D.U <= 32;
   const bool partial = (D.W % 8) != 0;
   const int block = (D.U + 31) / 32 * 32;
-  if (single) {
+  if (k4_use_jit(D)) {
+    void* kfn = nullptr;
+    int rc = jit_get("k4_lanes_jit.cuh", "lanes_k4_sweep_jit", k4_jit_defines(D), &kfn);
+    if (rc) return rc;
+    void* args[] = {(void*)&D, (void*)&A};
+    const int block4 = ((D.W + 3) / 4 + 31) / 32 * 32;  // one thread per 128-site supergroup
+    KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(sim->S), dim3(block4), args, 0, sim->stream));
+  } else if (single) {
     if (partial) lanes_k4_kernel<true, true><<<sim->S, block, 0, sim->stream>>>(D, A);
     else lanes_k4_kernel<true, false><<<sim->S, block, 0, sim->stream>>>(D, A);
   } else {

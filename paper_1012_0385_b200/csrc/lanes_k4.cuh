@@ -14,33 +14,6 @@
 
 namespace kpz {
 
-struct LanesDev {
-  PhiloxKeys keys;
-  Thresh t_pa, t_pb, t_turn, t_omega;
-  int32_t np_a, np_b, np_w;  // planes needed by the in-lane thresholds and by omega
-  int32_t offset_mode;
-  int32_t first_sample;
-  int32_t S;
-  int32_t W;    // natural words per sample = L/32
-  int32_t Wp;   // row stride, multiple of 8
-  int32_t U;    // units per sample = Wp/8
-  long long period;
-  uint32_t* A;  // [S][Wp]
-  uint32_t* B;
-  uint32_t* T;  // turning-point mask of the current epoch
-  unsigned long long* JA;  // [S] hops so far
-  unsigned long long* JB;
-  uint32_t* occA;  // [S][L] epoch-end occupancy counts
-  uint32_t* occB;
-};
-
-struct LanesRunArgs {
-  long long t0, n_mcs;
-  const long long* rec_t;
-  int32_t rec_begin, nt;
-  long long* rec;  // [4][nt][S]: J_A, J_B, N_A, N_B
-};
-
 // Initial occupations / turning points in natural layout: thread = one supergroup of 128 sites.
 __global__ void k_site_mask_nat(const __grid_constant__ PhiloxKeys K, uint32_t tag, Thresh T, long long timekey,
                                 int first_sample, int S, int W, int Wp, uint32_t* M) {

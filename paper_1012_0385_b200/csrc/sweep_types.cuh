@@ -39,4 +39,32 @@ struct KpzRunArgs {
   long long* rec_sum_h2;   // [nt][S]
 };
 
+// ---- two-lane model (lanes_k4.cuh, k4_lanes_jit.cuh) ---------------------------------------------------------------
+struct LanesDev {
+  PhiloxKeys keys;
+  Thresh t_pa, t_pb, t_turn, t_omega;
+  int32_t np_a, np_b, np_w;  // planes needed by the in-lane thresholds and by omega
+  int32_t offset_mode;
+  int32_t first_sample;
+  int32_t S;
+  int32_t W;    // natural words per sample = L/32
+  int32_t Wp;   // row stride, multiple of 8
+  int32_t U;    // units per sample = Wp/8
+  long long period;
+  uint32_t* A;  // [S][Wp]
+  uint32_t* B;
+  uint32_t* T;  // turning-point mask of the current epoch
+  unsigned long long* JA;  // [S] hops so far
+  unsigned long long* JB;
+  uint32_t* occA;  // [S][L] epoch-end occupancy counts
+  uint32_t* occB;
+};
+
+struct LanesRunArgs {
+  long long t0, n_mcs;
+  const long long* rec_t;
+  int32_t rec_begin, nt;
+  long long* rec;  // [4][nt][S]: J_A, J_B, N_A, N_B
+};
+
 }  // namespace kpz
