@@ -16,7 +16,7 @@
 //     epoch ends by warp-transposed, coalesced red.global.add.
 //
 // Compile-time configuration (-D, set by lanes_api.cu): K4J_W = L/32, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN
-// (thresholds in [0, 2^32]), K4J_OFFSET_MODE, K4J_EAGER.
+// (thresholds in [0, 2^32]), K4J_OFFSET_MODE, K4J_EAGER, K4J_TAIL.
 #pragma once
 #include "sweep_types.cuh"
 
@@ -24,7 +24,10 @@
 #error "k4_lanes_jit.cuh needs K4J_W, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN, K4J_OFFSET_MODE"
 #endif
 #ifndef K4J_EAGER
-#define K4J_EAGER 2
+#define K4J_EAGER 4
+#endif
+#ifndef K4J_TAIL
+#define K4J_TAIL 0  // 0: two more planes per trip (resolve); 1: plane-parallel tail (resolve_tail; measured slower: serial)
 #endif
 
 namespace kpz {
@@ -86,6 +89,44 @@ __device__ __forceinline__ void resolve(uint32_t (&lt)[4], uint32_t (&eq)[4], co
   }
 }
 
+// Plane-parallel tail: after the eager planes only a few elements of a warp are still undecided (live * 2^-EAGER).
+// For each lane that still holds one, the WHOLE warp draws the remaining planes of that lane's supergroup at once
+// (lane l draws plane pl0 + l), a ballot per undecided element assembles the rest of its uniform, and one integer
+// comparison with the rest of T finishes it: one Philox call of the warp per undecided supergroup instead of two
+// per pair of planes.  Same result as resolve<T>() by construction (U < T with an equal prefix <=> suffix(U) <
+// suffix(T)).  `u0` = supergroup index of lane 0 of this warp.
+template <uint64_t T>
+__device__ __forceinline__ void resolve_tail(uint32_t (&lt)[4], uint32_t (&eq)[4], const PhiloxKeys& K, uint32_t u0,
+                                             uint32_t gs, uint32_t tlo, uint32_t c3, int pl0) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t t_suffix = (uint32_t)T & (pl0 > 0 ? (0xFFFFFFFFu >> pl0) : 0xFFFFFFFFu);
+  uint32_t todo = __ballot_sync(FULL, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u);
+  while (todo) {
+    const int src = __ffs(todo) - 1;
+    todo &= todo - 1;
+    const int pl = pl0 + lane;
+    const uint4 v = philox4x32_10(u0 + (uint32_t)src, gs, tlo, c3 | ((uint32_t)(pl < 32 ? pl : 31) << 22), K);
+    const uint32_t R[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      uint32_t e = __shfl_sync(FULL, eq[w], src);  // the owner's undecided elements of word w (warp-uniform)
+      uint32_t acc = 0u;
+      while (e) {
+        const int k = __ffs(e) - 1;
+        e &= e - 1;
+        // bit l of the ballot = plane pl0 + l of this element's uniform = bit 31 - pl0 - l of U
+        const uint32_t planes = __ballot_sync(FULL, ((R[w] >> k) & 1u) != 0u && pl < 32);
+        const uint32_t u_suffix = __brev(planes) >> pl0;
+        acc |= (u_suffix < t_suffix ? 1u : 0u) << k;
+      }
+      if (lane == src) {
+        lt[w] |= acc;
+        eq[w] = 0u;
+      }
+    }
+  }
+}
+
 // [U < T] over the `live` elements of one supergroup, from plane 0.
 template <uint64_t T>
 __device__ __forceinline__ void lazy_less(uint32_t (&lt)[4], const uint32_t (&live)[4], const PhiloxKeys& K, uint32_t G,
@@ -128,6 +169,22 @@ __device__ __forceinline__ uint32_t unit_exchange(uint32_t mine, int src, uint32
     const uint32_t v = slot[src];
     parity ^= 1;
     return v;
+  }
+}
+
+// Same, reading the values of two threads after one publication (one barrier).
+__device__ __forceinline__ void unit_exchange2(uint32_t mine, int src1, int src2, uint32_t& v1, uint32_t& v2,
+                                               uint32_t* halo, int& parity) {
+  if (SINGLE_WARP) {
+    v1 = __shfl_sync(FULL, mine, src1);
+    v2 = __shfl_sync(FULL, mine, src2);
+  } else {
+    uint32_t* slot = halo + parity * NTHREADS;
+    slot[threadIdx.x] = mine;
+    __syncthreads();
+    v1 = slot[src1];
+    v2 = slot[src2];
+    parity ^= 1;
   }
 }
 
@@ -231,7 +288,10 @@ __device__ __forceinline__ void lane_change(uint32_t (&SRC)[4], uint32_t (&DST)[
   if (TOMEGA > 0 && TOMEGA < kOne) {
 #pragma unroll
     for (int pl = 0; pl < EAGER; ++pl) plane_step<TOMEGA>(lt, eq, r[pl], pl);
-    if (EAGER < NPW) resolve<TOMEGA>(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
+    if (EAGER < NPW) {
+      if (K4J_TAIL) resolve_tail<TOMEGA>(lt, eq, K, (uint32_t)(un.u & ~31), un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
+      else resolve<TOMEGA>(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
+    }
   }
 #pragma unroll
   for (int w = 0; w < 4; ++w) {
@@ -353,19 +413,42 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
     for (int pass = 0; pass < 2; ++pass) {
       const uint32_t o = K4J_OFFSET_MODE ? (uint32_t)pass : ((offbits >> (2 * ((int)m & 15) + pass)) & 1u);
       // in-lane hops of both lanes with the same offset
-      uint32_t nx = 0;
-      if (o) {
-        nx = unit_exchange((A[0] & 1u) | ((B[0] & 1u) << 1), un.nxt, halo, parity);
-        if (!active) nx = 0;  // idle threads hold all-zero words and must not see a neighbour bit
-      }
       const uint32_t c3t = ((uint32_t)pass << 27) | thi;
-      const uint32_t cA = lane_pass<true, TPA>(A, un, o, nx & 1u, D.keys, TAG_PAIR, tlo, c3t, jA);
-      const uint32_t cB = lane_pass<false, TPB>(B, un, o, nx >> 1, D.keys, TAG_PAIR_B, tlo, c3t, jB);
-      if (o) {
-        const uint32_t in = unit_exchange(cA | (cB << 1), un.prv, halo, parity);
-        if (active) {
-          A[0] ^= in & 1u;
-          B[0] ^= in >> 1;
+      if (TPA >= kOne && TPB >= kOne) {
+        // rate 1 in both lanes (config 5): the hop over a thread boundary is decided by old bits alone,
+        // so both sides compute it from ONE exchange: first bits go to the previous thread, last bits to the next
+        uint32_t nx = 0, in = 0;
+        if (o) {
+          uint32_t lastA = A[3], lastB = B[3];
+          if (PARTIAL) {
+            lastA = un.nwn >= 4 ? A[3] : A[1];
+            lastB = un.nwn >= 4 ? B[3] : B[1];
+          }
+          const uint32_t mine = (A[0] & 1u) | ((B[0] & 1u) << 1) | ((lastA >> 31) << 2) | ((lastB >> 31) << 3);
+          uint32_t vn, vp;
+          unit_exchange2(mine, un.nxt, un.prv, vn, vp, halo, parity);
+          nx = active ? (vn & 3u) : 0u;  // idle threads hold all-zero words and must not see a neighbour bit
+          // lane A: particle on the previous thread's last site, hole on my first; lane B: the other way round
+          in = active ? (((vp >> 2) & ~A[0] & 1u) | ((~(vp >> 3) & B[0] & 1u) << 1)) : 0u;
+        }
+        lane_pass<true, TPA>(A, un, o, nx & 1u, D.keys, TAG_PAIR, tlo, c3t, jA);
+        lane_pass<false, TPB>(B, un, o, nx >> 1, D.keys, TAG_PAIR_B, tlo, c3t, jB);
+        A[0] ^= in & 1u;
+        B[0] ^= in >> 1;
+      } else {
+        uint32_t nx = 0;
+        if (o) {
+          nx = unit_exchange((A[0] & 1u) | ((B[0] & 1u) << 1), un.nxt, halo, parity);
+          if (!active) nx = 0;
+        }
+        const uint32_t cA = lane_pass<true, TPA>(A, un, o, nx & 1u, D.keys, TAG_PAIR, tlo, c3t, jA);
+        const uint32_t cB = lane_pass<false, TPB>(B, un, o, nx >> 1, D.keys, TAG_PAIR_B, tlo, c3t, jB);
+        if (o) {
+          const uint32_t in = unit_exchange(cA | (cB << 1), un.prv, halo, parity);
+          if (active) {
+            A[0] ^= in & 1u;
+            B[0] ^= in >> 1;
+          }
         }
       }
       // lane changes at turning points: A->B after pass 0, B->A after pass 1
