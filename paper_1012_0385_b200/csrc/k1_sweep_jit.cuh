@@ -24,6 +24,9 @@
 #ifndef K1J_VARIANT
 #define K1J_VARIANT 1  // 0: one code path per offset pair (4-way switch); 1: branch-free
 #endif
+#ifndef K1J_EAGER
+#define K1J_EAGER 6  // GENERAL path: planes drawn one MCS ahead; deeper planes are evaluated lazily
+#endif
 #ifndef K1J_PW
 #error "k1_sweep_jit.cuh needs K1J_PW, K1J_T0..3, K1J_DIS, K1J_OFFSET_MODE"
 #endif
@@ -51,9 +54,16 @@ __host__ __device__ constexpr int planes_of(uint64_t T) {
 __host__ __device__ constexpr int cmax(int a, int b) { return a > b ? a : b; }
 constexpr int NPS = cmax(cmax(planes_of(T0), planes_of(T2)),
                          cmax(DIS >= 1 ? planes_of(T1) : 0, DIS >= 2 ? planes_of(T3) : 0));
-constexpr int NPSA = NPS > 0 ? NPS : 1;  // array extent
+// Rate selection "sel" of a pair depends on a (which side holds the particle), the tags and the planes.  With at most
+// three such words it is ONE LOP3 (select_word); otherwise the GENERAL path compares plane by plane: the first NEAG
+// planes are drawn one MCS ahead like everything else, deeper planes only while some active pair of the warp is
+// still undecided (lazy, two planes per trip) - this is how non-dyadic rates such as p = 0.8 or 0.9 run.
+constexpr int SEL_NVARS = 1 + (DIS >= 1) + (DIS >= 2) + NPS;
+constexpr bool GENERAL = SEL_NVARS > 3;
+constexpr int NEAG = !GENERAL ? NPS : (NPS < K1J_EAGER ? NPS : K1J_EAGER);
+constexpr int NPSA = NEAG > 0 ? NEAG : 1;  // array extent
 
-// The random bit-planes of one MCS of one unit: r[pass][plane][word].
+// The eagerly drawn random bit-planes of one MCS of one unit: r[pass][plane][word].
 struct Planes {
   uint32_t r[2][NPSA][4];
 };
@@ -63,7 +73,7 @@ __device__ __forceinline__ void draw_planes(Planes& R, const PhiloxKeys& K, uint
 #pragma unroll
   for (int pass = 0; pass < 2; ++pass) {
 #pragma unroll
-    for (int pl = 0; pl < NPS; ++pl) {
+    for (int pl = 0; pl < NEAG; ++pl) {
       const uint4 v = philox4x32_10(G, gs, tlo, ctr3(TAG_PAIR, (uint32_t)pass, (uint32_t)pl, thi), K);
       R.r[pass][pl][0] = v.x;
       R.r[pass][pl][1] = v.y;
@@ -71,26 +81,6 @@ __device__ __forceinline__ void draw_planes(Planes& R, const PhiloxKeys& K, uint
       R.r[pass][pl][3] = v.w;
     }
   }
-}
-
-// [U < T] for the 32 pairs of word w, MSB first; T is a constant so this folds to a fixed boolean function.
-template <uint64_t T>
-__device__ __forceinline__ uint32_t accept(const uint32_t (&r)[NPSA][4], int w) {
-  if (T >= kOne) return ~0u;
-  if (T == 0) return 0u;
-  constexpr int np = planes_of(T);
-  uint32_t lt = 0u, eq = ~0u;
-#pragma unroll
-  for (int pl = 0; pl < np; ++pl) {
-    const uint32_t x = r[pl][w];
-    if ((T >> (31 - pl)) & 1ull) {
-      lt |= eq & ~x;
-      eq &= x;
-    } else {
-      eq &= ~x;
-    }
-  }
-  return lt;
 }
 
 // ---- pair logic as explicit LOP3s --------------------------------------------------------------------------------
@@ -120,7 +110,6 @@ __host__ __device__ constexpr int sel_bit(int a, int spa, int sqb, int r0, int r
 }
 // When sel depends on at most three words (a + tags + planes) it is ONE LOP3 with this table; inputs in the order
 // a, [spa], [sqb], [plane 0], [plane 1].
-constexpr int SEL_NVARS = 1 + (DIS >= 1) + (DIS >= 2) + NPS;
 __host__ __device__ constexpr int sel_lut() {
   int lut = 0;
   for (int i = 0; i < 8; ++i) {
@@ -135,22 +124,76 @@ __host__ __device__ constexpr int sel_lut() {
   return lut;
 }
 
-// sel for one word: a = departure side of a forward hop; spa / sqb = the tags of the pair's a / b site.
+// sel for one word (LUT path only): a = departure side of a forward hop; spa / sqb = the tags of the pair's a / b site.
 __device__ __forceinline__ uint32_t select_word(uint32_t a, uint32_t spa, uint32_t sqb, const uint32_t (&r)[NPSA][4],
                                                 int w) {
-  if constexpr (SEL_NVARS <= 3) {
-    uint32_t in[3] = {a, 0u, 0u};
-    int k = 1;
-    if (DIS >= 1) in[k++] = spa;
-    if (DIS >= 2) in[k++] = sqb;
-    if (NPS >= 1) in[k++] = r[0][w];
-    if (NPS >= 2) in[k++] = r[NPS >= 2 ? 1 : 0][w];
-    return lop3<sel_lut()>(in[0], in[1], in[2]);
-  } else {
-    uint32_t selp = accept<T0>(r, w), selq = accept<T2>(r, w);
-    if (DIS >= 1) selp = lop3<0xCA>(spa, accept<T1>(r, w), selp);  // spa ? slow : normal
-    if (DIS >= 2) selq = lop3<0xCA>(sqb, accept<T3>(r, w), selq);
-    return lop3<0xCA>(a, selp, selq);  // a ? selp : selq
+  uint32_t in[3] = {a, 0u, 0u};
+  int k = 1;
+  if (DIS >= 1) in[k < 3 ? k++ : 2] = spa;
+  if (DIS >= 2) in[k < 3 ? k++ : 2] = sqb;
+  if (NPS >= 1) in[k < 3 ? k++ : 2] = r[0][w];
+  if (NPS >= 2) in[k < 3 ? k++ : 2] = r[NEAG >= 2 ? 1 : 0][w];
+  return lop3<sel_lut()>(in[0], in[1], in[2]);
+}
+
+// GENERAL path.  Elements whose rate class c (0 = p, 1 = p_slow, 2 = q, 3 = q_slow) has bit b_c set; the b_c are
+// compile-time constants for the eager planes and warp-uniform values in the lazy loop.
+__device__ __forceinline__ uint32_t class_mask(uint32_t a, uint32_t spa, uint32_t sqb, uint32_t b0, uint32_t b1,
+                                               uint32_t b2, uint32_t b3) {
+  const uint32_t B0 = 0u - b0, B1 = 0u - b1, B2 = 0u - b2, B3 = 0u - b3;
+  const uint32_t mp = DIS >= 1 ? ((spa & B1) | (~spa & B0)) : B0;
+  const uint32_t mq = DIS >= 2 ? ((sqb & B3) | (~sqb & B2)) : B2;
+  return (a & mp) | (~a & mq);
+}
+__host__ __device__ constexpr uint32_t tbit(uint64_t T, int pl) { return (uint32_t)((T >> (31 - pl)) & 1ull); }
+__host__ __device__ constexpr uint32_t is_always(uint64_t T) { return T >= kOne ? 1u : 0u; }
+__host__ __device__ constexpr uint32_t is_partial(uint64_t T) { return (T > 0 && T < kOne) ? 1u : 0u; }
+
+// flips of the 32 pairs of each word of one pass: x = active pairs, a = side holding the particle's departure site.
+__device__ __forceinline__ void general_flips(uint32_t (&lt)[4], const uint32_t (&x)[4], const uint32_t (&a)[4],
+                                              const uint32_t (&spa)[4], const uint32_t (&sqb)[4],
+                                              const uint32_t (&r)[NPSA][4], const PhiloxKeys& K, uint32_t G, uint32_t gs,
+                                              uint32_t tlo, uint32_t c3) {
+  uint32_t eq[4];
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    lt[w] = x[w] & class_mask(a[w], spa[w], sqb[w], is_always(T0), is_always(T1), is_always(T2), is_always(T3));
+    eq[w] = x[w] & class_mask(a[w], spa[w], sqb[w], is_partial(T0), is_partial(T1), is_partial(T2), is_partial(T3));
+  }
+#pragma unroll
+  for (int pl = 0; pl < NEAG; ++pl) {
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const uint32_t tb = class_mask(a[w], spa[w], sqb[w], tbit(T0, pl), tbit(T1, pl), tbit(T2, pl), tbit(T3, pl));
+      lt[w] |= eq[w] & tb & ~r[pl][w];
+      eq[w] &= ~(r[pl][w] ^ tb);
+    }
+  }
+  if (NEAG < NPS) {
+#pragma unroll 1
+    for (int pl = NEAG; pl < NPS; pl += 2) {
+      if (!__any_sync(0xFFFFFFFFu, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u)) break;
+      const int pl1 = pl + 1 < 32 ? pl + 1 : 31;
+      const uint4 v0 = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)pl << 22), K);
+      const uint4 v1 = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)pl1 << 22), K);
+      const uint32_t R0[4] = {v0.x, v0.y, v0.z, v0.w};
+      const uint32_t R1[4] = {v1.x, v1.y, v1.z, v1.w};
+      const uint32_t s0 = 31 - pl, s1 = 31 - pl1;
+      const bool second = pl + 1 < NPS;
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        uint32_t tb = class_mask(a[w], spa[w], sqb[w], (uint32_t)(T0 >> s0) & 1u, (uint32_t)(T1 >> s0) & 1u,
+                                 (uint32_t)(T2 >> s0) & 1u, (uint32_t)(T3 >> s0) & 1u);
+        lt[w] |= eq[w] & tb & ~R0[w];
+        eq[w] &= ~(R0[w] ^ tb);
+        if (second) {
+          tb = class_mask(a[w], spa[w], sqb[w], (uint32_t)(T0 >> s1) & 1u, (uint32_t)(T1 >> s1) & 1u,
+                          (uint32_t)(T2 >> s1) & 1u, (uint32_t)(T3 >> s1) & 1u);
+          lt[w] |= eq[w] & tb & ~R1[w];
+          eq[w] &= ~(R1[w] ^ tb);
+        }
+      }
+    }
   }
 }
 
@@ -253,20 +296,38 @@ __device__ __forceinline__ void mcs_logic(uint32_t (&P)[4], uint32_t (&Q)[4], co
 // MCS is one basic block, which the scheduler fills with the Philox rounds of the next MCS.
 __device__ __forceinline__ void pass_branchfree(uint32_t (&P)[4], uint32_t (&Q)[4], const Tags& G,
                                                 const uint32_t (&r)[NPSA][4], const Unit& un, uint32_t o,
-                                                uint32_t* halo, int& parity) {
+                                                uint32_t* halo, int& parity, const PhiloxKeys& K, uint32_t Gu,
+                                                uint32_t gs, uint32_t tlo, uint32_t c3) {
   const uint32_t M = 0u - o;  // all ones in frame 1
   frame_up(P, un, halo, parity, o);
+  if constexpr (!GENERAL) {
 #pragma unroll
-  for (int w = 0; w < 4; ++w) {
-    const uint32_t a = lop3<0xCA>(M, Q[w], P[w]);  // frame 1: a = odd site (Q); frame 0: a = even site (P)
-    uint32_t spa = 0u, sqb = 0u;
-    if (DIS >= 1) spa = lop3<0xCA>(M, G.spa1[w], G.spa0[w]);
-    if (DIS >= 2) sqb = lop3<0xCA>(M, G.sqb1[w], G.sqb0[w]);
-    const uint32_t sel = select_word(a, spa, sqb, r, w);
-    const uint32_t np = lop3<0xD8>(P[w], Q[w], sel);
-    const uint32_t nq = lop3<0xE4>(P[w], Q[w], sel);
-    P[w] = np;
-    Q[w] = nq;
+    for (int w = 0; w < 4; ++w) {
+      const uint32_t a = lop3<0xCA>(M, Q[w], P[w]);  // frame 1: a = odd site (Q); frame 0: a = even site (P)
+      uint32_t spa = 0u, sqb = 0u;
+      if (DIS >= 1) spa = lop3<0xCA>(M, G.spa1[w], G.spa0[w]);
+      if (DIS >= 2) sqb = lop3<0xCA>(M, G.sqb1[w], G.sqb0[w]);
+      const uint32_t sel = select_word(a, spa, sqb, r, w);
+      const uint32_t np = lop3<0xD8>(P[w], Q[w], sel);
+      const uint32_t nq = lop3<0xE4>(P[w], Q[w], sel);
+      P[w] = np;
+      Q[w] = nq;
+    }
+  } else {
+    uint32_t a[4], x[4], spa[4], sqb[4], lt[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      a[w] = lop3<0xCA>(M, Q[w], P[w]);
+      x[w] = P[w] ^ Q[w];
+      spa[w] = DIS >= 1 ? lop3<0xCA>(M, G.spa1[w], G.spa0[w]) : 0u;
+      sqb[w] = DIS >= 2 ? lop3<0xCA>(M, G.sqb1[w], G.sqb0[w]) : 0u;
+    }
+    general_flips(lt, x, a, spa, sqb, r, K, Gu, gs, tlo, c3);
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      P[w] ^= lt[w];
+      Q[w] ^= lt[w];
+    }
   }
   frame_down(P, un, halo, parity, o);
 }
@@ -390,14 +451,17 @@ struct Ctx {
 // in one basic block per offset combination, so the scheduler overlaps the Philox rounds with the pair logic.
 __device__ __forceinline__ void mcs_step(Ctx& c, const Planes& Rc, Planes& Rn, const PhiloxKeys& K, long long m,
                                          uint32_t* halo) {
-  if (K1J_OFFSET_MODE == 1) {
+  const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
+  if (K1J_OFFSET_MODE == 1 && !GENERAL) {
     draw_planes(Rn, K, c.G, c.gs, m + 1);
     mcs_logic<0, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
-  } else if (K1J_VARIANT == 1) {
-    const uint32_t code = (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
+  } else if (K1J_VARIANT == 1 || GENERAL) {
+    const uint32_t code = K1J_OFFSET_MODE == 1 ? 2u : (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
     draw_planes(Rn, K, c.G, c.gs, m + 1);
-    pass_branchfree(c.P, c.Q, c.tags, Rc.r[0], c.un, code & 1u, halo, c.parity);
-    pass_branchfree(c.P, c.Q, c.tags, Rc.r[1], c.un, code >> 1, halo, c.parity);
+    pass_branchfree(c.P, c.Q, c.tags, Rc.r[0], c.un, code & 1u, halo, c.parity, K, c.G, c.gs, tlo,
+                    ctr3(TAG_PAIR, 0u, 0u, thi));
+    pass_branchfree(c.P, c.Q, c.tags, Rc.r[1], c.un, code >> 1, halo, c.parity, K, c.G, c.gs, tlo,
+                    ctr3(TAG_PAIR, 1u, 0u, thi));
   } else {
     const uint32_t code = (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
     switch (code) {

@@ -169,10 +169,8 @@ K1Fn k1_pick(bool single_warp, bool partial, int dis, int nps) {
 }
 
 // ---- K1 v2: the sweep specialised at run time on (L, thresholds, tags, offset mode) — k1_sweep_jit.cuh ----------
-// Fixed plane counts only: beyond kK1JitMaxPlanes planes (non-dyadic rates) the lazily evaluated generic kernel
-// (kpz_k1.cuh) needs fewer Philox calls.
-constexpr int kK1JitMaxPlanes = 6;
-
+// Every threshold set runs on it: up to three selection inputs fold into one LOP3, anything else (tags + planes,
+// non-dyadic rates) takes its GENERAL path with eagerly drawn leading planes and a lazy tail.
 std::vector<std::string> k1_jit_defines(const KpzDev& D, int dis) {
   auto T = [&](int c) -> unsigned long long {
     return D.thr[c].always ? (1ull << 32) : (unsigned long long)D.thr[c].value;
@@ -199,7 +197,7 @@ std::vector<std::string> k1_jit_defines(const KpzDev& D, int dis) {
   return d;
 }
 
-bool k1_use_jit(const KpzDev& D) { return jit_enabled() && D.nplanes <= kK1JitMaxPlanes; }
+bool k1_use_jit(const KpzDev&) { return jit_enabled(); }
 
 void refresh_planes(kpz_sim* sim) {
   int np = std::max(planes_needed(sim->dev.thr[0]), planes_needed(sim->dev.thr[2]));
