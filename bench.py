@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — site-update throughput of the KPZ/ASEP hot path on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|4|5|4-aux-i|4-aux-ii] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|5|4-aux-i|4-aux-ii|4-aux-i-blocked] [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: reset to the
 initial state (a1), run the configuration's full number of MCS with its record times (a2-a7 / a9), records left in
@@ -44,11 +44,23 @@ UNIT = "GSU/s"
 # roofline model: algorithmic cost per site-update of the dominant kernel of each workload
 # ---------------------------------------------------------------------------------------------------------------
 SM_COUNT = 148
-# integer thread-instructions per site-update of the on-chip sweep (DESIGN.md §6.1 derives these from the
-# algorithm: Philox rounds for the bit-planes the thresholds need + pair logic + frame change)
-ALU_OPS_PER_SU = {2: 1.08, 3: 0.73, 5: 0.47}
+# alu-pipe slots per site update of the on-chip / blocked sweeps and the two-lane kernel: one slot =
+# one LOP3 / SHF / IMAD.WIDE lane-instruction; the pipe takes 0.5 warp-instructions per clock and SMSP (measured).
+#   Philox call = 34 slots per 128 elements and plane; pair logic 3 LOP3 per 32 pairs and pass; 4 SHF per MCS.
+ALU_SLOTS_PER_SU = {
+    1: (2 * 4 * 3 + 4) / 256,                       # p=1, q=0: no plane, logic only
+    2: (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,          # 2 planes
+    3: (2 * 1 * 34 + 2 * 4 * 3 + 4) / 256,          # 1 plane (slow sites only)
+    4: (2 * 7.33 * (34 + 12) + 2 * 4 * 3 + 4) / 256,  # 32-plane thresholds: log2(64)+1.33 planes per unit and pass
+    5: (2 * 2.0 * 34 + 2 * 2 * 4 * 5 + 2 * 4 * 4) / 256,  # two-lane: lane changes dominate
+    "4-aux-i": (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,
+    "4-aux-ii": (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,
+    "4-aux-i-blocked": (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,
+}
+ALU_SLOTS_PER_CLK_SMSP = 0.5
 # streamed sweep: one read + one write of the bit-packed ring per sub-lattice pass = 2 passes * 2 * 1/8 B
 STREAM_BYTES_PER_SU = 0.5
+PATH_NAMES = {1: "on-chip K1", 2: "streamed K3 (one launch per pass)", 3: "blocked stream K3T (32 MCS per launch)"}
 
 
 def measured_peaks():
@@ -192,7 +204,7 @@ def make_sim(pkg, cfg, first_sample):
                            cfg["omega"], seed=cfg["seed"], first_sample=first_sample, max_records=nrec)
     else:
         sim = pkg.KpzSim(cfg["L"], cfg["S"], cfg["p"], cfg["q"], disorder=cfg["disorder"], seed=cfg["seed"],
-                         first_sample=first_sample, max_records=nrec)
+                         first_sample=first_sample, max_records=nrec, path=cfg.get("path", 0))
     sim.set_record_times(cfg["record_times"])
     return sim
 
@@ -335,13 +347,16 @@ def run_cuda(args, cfg, cfg_key):
                 "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
                 "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
     else:
-        ops = ALU_OPS_PER_SU.get(cfg_key if isinstance(cfg_key, int) else -1, 1.08)
-        peak = SM_COUNT * 4 * 32 * peaks["sm_max_mhz"] * 1e6 / 1e12      # T thread-instr/s at 1 warp-instr/clk/SMSP
-        achieved = ops * su_step / (ms_run * 1e-3) / 1e12
-        roof = {"bound": "alu", "kernel": "kpz_k1_kernel" if cfg["kind"] == "kpz" else "lanes_k4_kernel",
-                "achieved": achieved, "peak": peak, "unit": "Tinstr/s", "frac": achieved / peak, "traffic": None,
-                "peak_source": f"148 SM x 4 SMSP x 32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max clock)",
-                "algorithmic_instr_per_site_update": ops}
+        slots = ALU_SLOTS_PER_SU.get(cfg_key, ALU_SLOTS_PER_SU[2])
+        peak = SM_COUNT * 4 * ALU_SLOTS_PER_CLK_SMSP * 32 * peaks["sm_max_mhz"] * 1e6 / 1e12   # T lane-slots/s
+        achieved = slots * su_step / (ms_run * 1e-3) / 1e12
+        kname = {1: "kpz_k1_sweep_jit", 3: "kpz_k3t_sweep_jit"}.get(path, "kpz_k1_sweep_jit") if cfg["kind"] == "kpz" \
+            else "lanes_k4_sweep_jit"
+        roof = {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "Tslot/s",
+                "frac": achieved / peak, "traffic": None,
+                "peak_source": f"148 SM x 4 SMSP x 0.5 alu-pipe warp-instr/clk (measured) x 32 lanes x "
+                               f"{peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max clock)",
+                "algorithmic_slots_per_site_update": slots}
 
     # ---- CPU oracle on a bounded sample (one host core) -------------------------------------------------------
     cpu = None
@@ -356,8 +371,7 @@ def run_cuda(args, cfg, cfg_key):
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u32", "data": "synthetic",
         "config": {"workload": cfg["name"], "config_key": str(cfg_key), "L": cfg["L"], "samples_per_gpu": cfg["S"],
-                   "n_mcs": n_mcs, "records": len(cfg["record_times"]), "path": {1: "on-chip K1", 2: "streamed K3"}[path]
-                   if cfg["kind"] == "kpz" else "two-lane K4", "l2": "flushed between timed steps (256 MiB fill)",
+                   "n_mcs": n_mcs, "records": len(cfg["record_times"]), "path": PATH_NAMES[path] if cfg["kind"] == "kpz" else "two-lane K4", "l2": "flushed between timed steps (256 MiB fill)",
                    "parallelism": f"samples x{world}"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
         "ms_run_per_step": ms_run, "wall_s_timed_region": wall,

@@ -50,12 +50,14 @@ typedef struct {
 typedef struct {
   int32_t first_sample; /* global index of sample 0 of this handle (part of the RNG key); default 0 */
   int32_t offset_mode;  /* 0 = sub-lattice offset drawn per pass, 1 = alternating 0,1 */
-  int32_t path;         /* 0 auto, 1 force the on-chip per-sample kernel (K1), 2 force the streamed kernel (K3) */
+  int32_t path;         /* 0 auto, 1 on-chip per-sample kernel (K1), 2 streamed pass by pass (K3), 3 streamed in
+                           temporally blocked chunks (K3T); auto = 1 up to 262144 sites per ring, else 3 */
 } kpz_options;
 
 #define KPZ_PATH_AUTO 0
 #define KPZ_PATH_ONCHIP 1
 #define KPZ_PATH_STREAM 2
+#define KPZ_PATH_BLOCKED 3
 
 /* ---- KPZ / ASEP ring ensemble ----------------------------------------------------------------------------- */
 
@@ -132,7 +134,7 @@ int lanes_destroy(lanes_sim*);
 const char* kpz_strerror(int code);
 const char* kpz_last_error(void);        /* thread-local detail of the last failing call */
 int64_t kpz_kernel_launches(void);       /* kernels launched by this library in this process so far */
-/* Which kernel family a handle's kpz_run uses: 1 = on-chip per-sample (K1), 2 = streamed (K3). */
+/* Which kernel family a handle's kpz_run uses: 1 = on-chip per-sample (K1), 2 = streamed (K3), 3 = blocked (K3T). */
 int kpz_path(const kpz_sim*, int32_t* path);
 
 /* The on-chip sweep kernel is specialised at run time (NVRTC) on the ring size and the acceptance thresholds

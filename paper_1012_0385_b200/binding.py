@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libkpz_b200.so")
 HOOKS_PATH = os.path.join(HERE, "libkpz_b200_testhooks.so")
 
-KPZ_PATH_AUTO, KPZ_PATH_ONCHIP, KPZ_PATH_STREAM = 0, 1, 2
+KPZ_PATH_AUTO, KPZ_PATH_ONCHIP, KPZ_PATH_STREAM, KPZ_PATH_BLOCKED = 0, 1, 2, 3
 
 
 class KpzError(RuntimeError):

@@ -37,7 +37,12 @@ namespace k1j {
 constexpr int PW = K1J_PW;
 constexpr int PWp = (PW + 3) / 4 * 4;
 constexpr int U = PWp / 4;
-constexpr bool SINGLE_WARP = U <= 32;
+#ifdef K1J_TILE
+constexpr bool TILE = true;   // K3T: a warp sweeps a 32-unit window of a long ring (kpz_k3t_sweep_jit below)
+#else
+constexpr bool TILE = false;
+#endif
+constexpr bool SINGLE_WARP = TILE || U <= 32;
 constexpr bool PARTIAL = (PW % 4) != 0;
 constexpr int DIS = K1J_DIS;
 constexpr int NTHREADS = (U + 31) / 32 * 32;
@@ -488,6 +493,7 @@ __device__ __forceinline__ void mcs_step(Ctx& c, const Planes& Rc, Planes& Rn, c
 }  // namespace k1j
 }  // namespace kpz
 
+#ifndef K1J_TILE
 // grid = S samples, block = NTHREADS; thread u = unit u (idle when u >= U, but it joins every barrier / shuffle).
 extern "C" __global__ void __launch_bounds__(kpz::k1j::NTHREADS)
 kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::KpzRunArgs A) {
@@ -570,3 +576,73 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
     *reinterpret_cast<uint4*>(D.O + row) = make_uint4(c.Q[0], c.Q[1], c.Q[2], c.Q[3]);
   }
 }
+#else  // K1J_TILE
+// ---- K3T: temporally blocked sweep of rings beyond on-chip memory (north_star (2)) --------------------
+// The ring streams through HBM once per CHUNK of up to 32 MCS instead of once per pass.  A warp loads a window of 32
+// consecutive units (lane l holds unit tile*30 - 1 + l mod U), sweeps it exactly like K1 with the neighbour words of
+// the window's two ends left undefined, and stores the 30 interior units to the ping-pong buffer.  A pass moves
+// information by one site, so after k passes only the outer k+1 sites of the window are contaminated: the two end
+// units (256 sites each) absorb up to 127 MCS.  The random numbers are counter-based - keyed by the GLOBAL unit index
+// - so the halo units a neighbouring warp recomputes are bit-identical, and the result equals the pass-by-pass sweep.
+extern "C" __global__ void __launch_bounds__(128)
+kpz_k3t_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::K3TArgs A) {
+  using namespace kpz;
+  using namespace kpz::k1j;
+  constexpr int TI = 30;  // interior units per window
+  constexpr int NT = (U + TI - 1) / TI;
+  const int lane = threadIdx.x & 31;
+  const long long wid = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (wid >= (long long)D.S * NT) return;  // whole warps leave; the kernel has no block-wide barrier
+  const int s = (int)(wid / NT), tile = (int)(wid % NT);
+  int g = (tile * TI - 1 + lane) % U;
+  if (g < 0) g += U;
+  Ctx c;
+  c.un.nw = PARTIAL ? min(4, PW - 4 * g) : 4;
+  c.un.nxt = lane < 31 ? lane + 1 : 31;
+  c.un.prv = lane > 0 ? lane - 1 : 0;
+  c.gs = (uint32_t)(D.first_sample + s);
+  c.G = (uint32_t)g;
+  c.parity = 0;
+  c.offbits = 0;
+  const unsigned long long row = (unsigned long long)s * PWp + 4ull * g;
+  {
+    const uint4 e = *reinterpret_cast<const uint4*>(D.E + row);
+    const uint4 o = *reinterpret_cast<const uint4*>(D.O + row);
+    c.P[0] = e.x; c.P[1] = e.y; c.P[2] = e.z; c.P[3] = e.w;
+    c.Q[0] = o.x; c.Q[1] = o.y; c.Q[2] = o.z; c.Q[3] = o.w;
+  }
+#pragma unroll
+  for (int w = 0; w < 4; ++w) c.tags.spa0[w] = c.tags.spa1[w] = c.tags.sqb0[w] = c.tags.sqb1[w] = 0u;
+  if (DIS >= 1) {
+    const uint4 x = *reinterpret_cast<const uint4*>(D.SPE + row);
+    const uint4 y = *reinterpret_cast<const uint4*>(D.SPO + row);
+    c.tags.spa0[0] = x.x; c.tags.spa0[1] = x.y; c.tags.spa0[2] = x.z; c.tags.spa0[3] = x.w;
+    c.tags.spa1[0] = y.x; c.tags.spa1[1] = y.y; c.tags.spa1[2] = y.z; c.tags.spa1[3] = y.w;
+  }
+  if (DIS >= 2) {
+    const uint4 x = *reinterpret_cast<const uint4*>(D.SQO + row);
+    const uint4 y = *reinterpret_cast<const uint4*>(D.SQE + row);
+    c.tags.sqb0[0] = x.x; c.tags.sqb0[1] = x.y; c.tags.sqb0[2] = x.z; c.tags.sqb0[3] = x.w;
+    c.tags.sqb1[0] = y.x; c.tags.sqb1[1] = y.y; c.tags.sqb1[2] = y.z; c.tags.sqb1[3] = y.w;
+    frame_up(c.tags.sqb1, c.un, nullptr, c.parity);  // lane 31's incoming word is undefined: it is a halo unit
+  }
+  const long long t_end = A.t0 + A.n_mcs;
+  long long m = A.t0;
+  if (K1J_OFFSET_MODE == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+  Planes RA, RB;
+  draw_planes(RA, D.keys, c.G, c.gs, m);
+  while (m < t_end) {
+    mcs_step(c, RA, RB, D.keys, m, nullptr);
+    ++m;
+    if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+    if (m >= t_end) break;
+    mcs_step(c, RB, RA, D.keys, m, nullptr);
+    ++m;
+    if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+  }
+  if (lane >= 1 && lane <= TI && tile * TI + lane - 1 < U) {
+    *reinterpret_cast<uint4*>(A.Eout + row) = make_uint4(c.P[0], c.P[1], c.P[2], c.P[3]);
+    *reinterpret_cast<uint4*>(A.Oout + row) = make_uint4(c.Q[0], c.Q[1], c.Q[2], c.Q[3]);
+  }
+}
+#endif  // K1J_TILE

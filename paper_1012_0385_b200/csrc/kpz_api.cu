@@ -85,10 +85,13 @@ struct Layout {
 int choose_path(int64_t L, const kpz_options* opt, int* path) {
   const int64_t U = (L / 64 + 3) / 4;
   int want = opt ? opt->path : KPZ_PATH_AUTO;
-  if (want == KPZ_PATH_AUTO) want = (U <= 1024) ? KPZ_PATH_ONCHIP : KPZ_PATH_STREAM;
+  if (want == KPZ_PATH_AUTO) want = (U <= 1024) ? KPZ_PATH_ONCHIP : (jit_enabled() ? KPZ_PATH_BLOCKED : KPZ_PATH_STREAM);
   if (want == KPZ_PATH_ONCHIP && U > 1024)
     return fail(KPZ_EUNSUPPORTED, "on-chip path holds at most 262144 sites per sample (L=%lld)", (long long)L);
-  if (want != KPZ_PATH_ONCHIP && want != KPZ_PATH_STREAM) return fail(KPZ_EINVAL, "options.path must be 0, 1 or 2");
+  if (want != KPZ_PATH_ONCHIP && want != KPZ_PATH_STREAM && want != KPZ_PATH_BLOCKED)
+    return fail(KPZ_EINVAL, "options.path must be 0, 1, 2 or 3");
+  if (want == KPZ_PATH_BLOCKED && !jit_enabled())
+    return fail(KPZ_EUNSUPPORTED, "the blocked streamed path is compiled at run time (KPZ_B200_JIT=0 disables it)");
   *path = want;
   return KPZ_OK;
 }
@@ -116,7 +119,7 @@ Layout make_layout(int64_t L, int32_t S, bool disorder, int path, int32_t max_re
   y.off_E = take(plane);
   y.off_O = take(plane);
   y.off_E2 = y.off_O2 = 0;
-  if (path == KPZ_PATH_STREAM) {
+  if (path == KPZ_PATH_STREAM || path == KPZ_PATH_BLOCKED) {
     y.off_E2 = take(plane);
     y.off_O2 = take(plane);
   }
@@ -134,7 +137,7 @@ Layout make_layout(int64_t L, int32_t S, bool disorder, int path, int32_t max_re
   y.off_scratch = take(y.scratch_ints * 4);
   y.ntiles = (y.U + 255) / 256;
   y.off_k3off = y.off_tiles = 0;
-  if (path == KPZ_PATH_STREAM) {
+  if (path == KPZ_PATH_STREAM || path == KPZ_PATH_BLOCKED) {
     y.off_k3off = take((size_t)(kK3ChunkPasses + 1) * S);
     y.off_tiles = take((size_t)S * y.ntiles * 4);
   }
@@ -353,6 +356,49 @@ int k3_run(kpz_sim* sim, int64_t n_mcs) {
   return KPZ_OK;
 }
 
+// ---- K3T: temporally blocked streamed sweep (k1_sweep_jit.cuh, K1J_TILE) --------------------------------------------
+// One launch per chunk of up to kK3TChunk MCS (chunks end at record times); the lattice is in frame 0 between launches.
+constexpr long long kK3TChunk = 32;
+
+int k3t_run(kpz_sim* sim, int64_t n_mcs) {
+  const int dis = sim->has_sq ? 2 : sim->has_sp ? 1 : 0;
+  std::vector<std::string> defs = k1_jit_defines(sim->dev, dis);
+  defs.push_back("K1J_TILE=1");
+  void* kfn = nullptr;
+  int rc = jit_get("k1_sweep_jit.cuh", "kpz_k3t_sweep_jit", defs, &kfn);
+  if (rc) return rc;
+  const int nt = (int)sim->rec_times.size();
+  int ri = sim->nrec;
+  long long t = sim->t;
+  const long long t_end = sim->t + n_mcs;
+  const long long ntiles = ((long long)sim->dev.U + 29) / 30;
+  const long long nwarps = ntiles * sim->S;
+  while (t < t_end) {
+    long long n = std::min<long long>(kK3TChunk, t_end - t);
+    if (ri < nt && sim->rec_times[ri] - t < n) n = sim->rec_times[ri] - t;
+    KpzDev D = sim->dev;
+    K3TArgs A{};
+    A.Eout = sim->E2;
+    A.Oout = sim->O2;
+    A.t0 = t;
+    A.n_mcs = n;
+    void* args[] = {(void*)&D, (void*)&A};
+    KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((unsigned)((nwarps + 3) / 4)), dim3(128), args, 0, sim->stream));
+    KPZ_LAUNCH_CHECK("kpz_k3t_sweep_jit");
+    std::swap(sim->E, sim->E2);
+    std::swap(sim->O, sim->O2);
+    sim->dev.E = sim->E;
+    sim->dev.O = sim->O;
+    t += n;
+    if (ri < nt && sim->rec_times[ri] == t) {
+      rc = k3_record(sim, ri);
+      if (rc) return rc;
+      ++ri;
+    }
+  }
+  return KPZ_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -424,7 +470,7 @@ int kpz_create(kpz_sim** out, int64_t L, int32_t nsamples, double p, double q, c
   char* base = (char*)d_workspace;
   sim->E = (uint32_t*)(base + y.off_E);
   sim->O = (uint32_t*)(base + y.off_O);
-  if (path == KPZ_PATH_STREAM) {
+  if (path == KPZ_PATH_STREAM || path == KPZ_PATH_BLOCKED) {
     sim->E2 = (uint32_t*)(base + y.off_E2);
     sim->O2 = (uint32_t*)(base + y.off_O2);
   }
@@ -440,7 +486,7 @@ int kpz_create(kpz_sim** out, int64_t L, int32_t nsamples, double p, double q, c
   sim->scratch = (int*)(base + y.off_scratch);
   sim->scratch_ints = y.scratch_ints;
   sim->ntiles = y.ntiles;
-  if (path == KPZ_PATH_STREAM) {
+  if (path == KPZ_PATH_STREAM || path == KPZ_PATH_BLOCKED) {
     sim->k3off = (unsigned char*)(base + y.off_k3off);
     sim->tiles = (int*)(base + y.off_tiles);
   }
@@ -485,7 +531,7 @@ int kpz_jit_check(int64_t L, double p, double q, const kpz_disorder* disorder, c
   int path;
   rc = choose_path(L, opt, &path);
   if (rc) return rc;
-  if (path != KPZ_PATH_ONCHIP) return KPZ_OK;
+  if (path == KPZ_PATH_STREAM) return KPZ_OK;
   kpz_sim tmp;
   tmp.has_sp = disorder && d.prob_slow_p > 0.0;
   tmp.has_sq = disorder && d.prob_slow_q > 0.0;
@@ -499,7 +545,9 @@ int kpz_jit_check(int64_t L, double p, double q, const kpz_disorder* disorder, c
   refresh_planes(&tmp);
   if (!k1_use_jit(D)) return KPZ_OK;
   std::vector<char> cubin;
-  rc = jit_compile("k1_sweep_jit.cuh", "kpz_k1_sweep_jit", k1_jit_defines(D, tmp.has_sq ? 2 : tmp.has_sp ? 1 : 0), &cubin,
+  std::vector<std::string> defs = k1_jit_defines(D, tmp.has_sq ? 2 : tmp.has_sp ? 1 : 0);
+  if (path == KPZ_PATH_BLOCKED) defs.push_back("K1J_TILE=1");
+  rc = jit_compile("k1_sweep_jit.cuh", path == KPZ_PATH_BLOCKED ? "kpz_k3t_sweep_jit" : "kpz_k1_sweep_jit", defs, &cubin,
                    nullptr);
   if (rc) return rc;
   *cubin_bytes = cubin.size();
@@ -546,7 +594,7 @@ int kpz_set_record_times(kpz_sim* sim, const int64_t* t, int32_t nt) {
     const long double bound = std::min<long double>((long double)sim->L, 1.0L + 8.0L * (long double)t[k]);
     if ((long double)sim->L * bound * bound >= 9.0e18L)
       return fail(KPZ_EUNSUPPORTED, "sum of h^2 could overflow int64 at t=%lld for L=%lld", (long long)t[k], (long long)sim->L);
-    if (sim->path == KPZ_PATH_STREAM && bound >= 2147483647.0L)
+    if (sim->path != KPZ_PATH_ONCHIP && bound >= 2147483647.0L)
       return fail(KPZ_EUNSUPPORTED, "heights could overflow int32 at t=%lld", (long long)t[k]);
   }
   sim->rec_times.assign(t, t + nt);
@@ -591,6 +639,9 @@ int kpz_run(kpz_sim* sim, int64_t n_mcs) {
       fn<<<sim->S, block, 0, sim->stream>>>(D, A);
       KPZ_LAUNCH_CHECK("kpz_k1_kernel");
     }
+  } else if (sim->path == KPZ_PATH_BLOCKED) {
+    rc = k3t_run(sim, n_mcs);
+    if (rc) return rc;
   } else {
     rc = k3_run(sim, n_mcs);
     if (rc) return rc;

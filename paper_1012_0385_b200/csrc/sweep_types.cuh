@@ -39,6 +39,14 @@ struct KpzRunArgs {
   long long* rec_sum_h2;   // [nt][S]
 };
 
+// K3T (temporally blocked streamed sweep): D.E / D.O are the input ring, these the ping-pong output.
+struct K3TArgs {
+  uint32_t* Eout;
+  uint32_t* Oout;
+  long long t0;     // MCS already done
+  long long n_mcs;  // MCS of this chunk (<= 64: the window's end units absorb the contaminated sites)
+};
+
 // ---- two-lane model (lanes_k4.cuh, k4_lanes_jit.cuh) ---------------------------------------------------------------
 struct LanesDev {
   PhiloxKeys keys;

@@ -232,30 +232,45 @@ def test_k3_forced_on_small_rings(K, L, S):
     run_both_kpz(K, L, S, 0.75, 0.25, disorder=(0.2, 0.25, 0.3, 0.5), seed=5, times=[2, n], chunks=[n], path=2)
 
 
+@pytest.mark.parametrize("L,S", [(64, 2), (320, 3), (4096, 3), (256 * 30, 2), (256 * 31 + 64, 2), (65536 + 64, 2),
+                                 (1 << 18, 1)])
+def test_k3t_blocked_on_small_rings(K, L, S):
+    """Temporally blocked streamed path (windows of 32 units, 30 interior) against the oracle: rings shorter than a
+    window, exactly one window, one window plus a ragged unit, several windows; chunks of 32 MCS cut at record times."""
+    rng = np.random.default_rng(L + 1)
+    start = R.pack_sites((rng.random((S, L)) < 0.5).astype(np.uint8))
+    n = 75 if L < 100000 else 36
+    gpu, _ = run_both_kpz(K, L, S, 0.75, 0.25, seed=4, times=[1, 2, 33, n], chunks=[40, n - 40] if n > 40 else [n],
+                          start=start, path=3)
+    assert gpu.path == K.KPZ_PATH_BLOCKED
+    run_both_kpz(K, L, S, 0.9, 0.1, disorder=(0.2, 0.25, 0.3, 0.5), seed=5, times=[2, 34], chunks=[34], path=3)
+
+
 def test_k3_equals_k1_at_2p16(K):
     L, c = 1 << 16, workloads.CONFIGS[4]
     sims = []
-    for path in (1, 2):
+    for path in (1, 2, 3):
         g = K.KpzSim(L, 2, c["p"], c["q"], seed=c["seed"], path=path, max_records=8)
         g.set_record_times([1, 10, 100, 150])
         g.run(150)
         sims.append((K.words_to_numpy(g.lattice()), g.roughness()))
-    assert np.array_equal(sims[0][0], sims[1][0])
-    for k in ("sum_h", "sum_h2"):
-        assert np.array_equal(sims[0][1][k], sims[1][1][k])
+    for other in sims[1:]:
+        assert np.array_equal(sims[0][0], other[0])
+        for k in ("sum_h", "sum_h2"):
+            assert np.array_equal(sims[0][1][k], other[1][k])
 
 
 def test_config4_path_at_2p20_vs_oracle(K):
     c = workloads.CONFIGS[4]
     gpu, _ = run_both_kpz(K, 1 << 20, 1, c["p"], c["q"], seed=c["seed"], times=c["record_times"], chunks=[26])
-    assert gpu.path == K.KPZ_PATH_STREAM
+    assert gpu.path == K.KPZ_PATH_BLOCKED
 
 
 def test_config4_full_size_first_steps_and_invariants(K):
     c = workloads.CONFIGS[4]
     L = c["L"]
     gpu = K.KpzSim(L, 1, c["p"], c["q"], seed=c["seed"], max_records=8)
-    assert gpu.path == K.KPZ_PATH_STREAM
+    assert gpu.path == K.KPZ_PATH_BLOCKED
     times = [1, 2]
     gpu.set_record_times(times)
     gpu.run(2)

@@ -42,11 +42,15 @@ CONFIGS = {
             n_mcs=1000, record_times=_T20_1E3, seed=4),
     5: dict(name="config5_lanes_L16384_S256", kind="lanes", L=16384, S=256, p_a=1.0, p_b=1.0, rho0=0.3,
             turn_prob=0.05, turn_period=100, omega=0.1, n_mcs=100_000, record_times=_T50_1E5, seed=5),
-    # Auxiliary streamed runs: same kernel as config 4, dyadic rates (bandwidth-bound).
+    # Auxiliary streamed runs: dyadic rates, the pass-by-pass streamed kernel (path 2) forced, so
+    # that the sweep is bandwidth-bound: (i) ring in L2, (ii) ring beyond L2 (the HBM roofline case).
     "4-aux-i": dict(name="config4aux1_stream_L2p28_p075_q025", kind="kpz", L=1 << 28, S=1, p=0.75, q=0.25,
-                    disorder=None, n_mcs=1000, record_times=_T20_1E3, seed=4),
+                    disorder=None, n_mcs=1000, record_times=_T20_1E3, seed=4, path=2),
     "4-aux-ii": dict(name="config4aux2_stream_L2p32_p075_q025", kind="kpz", L=1 << 32, S=1, p=0.75, q=0.25,
-                     disorder=None, n_mcs=200, record_times=[1, 2, 4, 8, 16, 32, 64, 128, 200], seed=4),
+                     disorder=None, n_mcs=200, record_times=[1, 2, 4, 8, 16, 32, 64, 128, 200], seed=4, path=2),
+    # the same two rings on the default (temporally blocked) path
+    "4-aux-i-blocked": dict(name="config4aux1_blocked_L2p28_p075_q025", kind="kpz", L=1 << 28, S=1, p=0.75, q=0.25,
+                            disorder=None, n_mcs=1000, record_times=_T20_1E3, seed=4),
 }
 
 
