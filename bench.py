@@ -361,7 +361,7 @@ def run_cuda(args, cfg, cfg_key):
     # ---- CPU oracle on a bounded sample (one host core) -------------------------------------------------------
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        nsamp, nm = oracle_sample_shape(cfg, 150_000_000)      # ~15 s at ~1e7 site updates/s
+        nsamp, nm = oracle_sample_shape(cfg, 400_000_000)      # ~15 s at ~2.5e7 site updates/s
         v, dt = time_oracle(cfg, nsamp, nm)
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
                "sample": f"{nsamp} sample(s) x {nm} MCS of {cfg['name']} (of {cfg['S']} x {cfg['n_mcs']})"}

@@ -175,9 +175,10 @@ __device__ __forceinline__ void general_flips(uint32_t (&lt)[4], const uint32_t 
     }
   }
   if (NEAG < NPS) {
+    const unsigned alive = __activemask();  // the streamed pass kernel's last warp may be partly retired
 #pragma unroll 1
     for (int pl = NEAG; pl < NPS; pl += 2) {
-      if (!__any_sync(0xFFFFFFFFu, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u)) break;
+      if (!__any_sync(alive, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u)) break;
       const int pl1 = pl + 1 < 32 ? pl + 1 : 31;
       const uint4 v0 = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)pl << 22), K);
       const uint4 v1 = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)pl1 << 22), K);
@@ -235,11 +236,9 @@ struct Unit {
   int prv;
 };
 
-// frame 0 -> 1: P'[w] = P[w] >> 1 | next << 31
+// frame 0 -> 1: P'[w] = P[w] >> 1 | next << 31, h = word 0 of the next unit
 // (sh = 1; sh = 0 leaves P as it is: the branch-free sweep passes the offset itself)
-__device__ __forceinline__ void frame_up(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity,
-                                         uint32_t sh = 1u) {
-  const uint32_t h = unit_exchange(P[0], un.nxt, halo, parity);
+__device__ __forceinline__ void shift_up_words(uint32_t (&P)[4], int nw, uint32_t h, uint32_t sh) {
   if (!PARTIAL) {
     P[0] = __funnelshift_r(P[0], P[1], sh);
     P[1] = __funnelshift_r(P[1], P[2], sh);
@@ -248,17 +247,13 @@ __device__ __forceinline__ void frame_up(uint32_t (&P)[4], const Unit& un, uint3
   } else {
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
-      const uint32_t next = (w + 1 < un.nw) ? P[w + 1 < 4 ? w + 1 : 3] : h;
-      P[w] = (w < un.nw) ? __funnelshift_r(P[w], next, sh) : 0u;
+      const uint32_t next = (w + 1 < nw) ? P[w + 1 < 4 ? w + 1 : 3] : h;
+      P[w] = (w < nw) ? __funnelshift_r(P[w], next, sh) : 0u;
     }
   }
 }
-// frame 1 -> 0: P[w] = P'[w] << 1 | prev >> 31
-__device__ __forceinline__ void frame_down(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity,
-                                           uint32_t sh = 1u) {
-  uint32_t last = P[3];
-  if (PARTIAL) last = un.nw >= 4 ? P[3] : un.nw == 3 ? P[2] : un.nw == 2 ? P[1] : P[0];
-  const uint32_t h = unit_exchange(last, un.prv, halo, parity);
+// frame 1 -> 0: P[w] = P'[w] << 1 | prev >> 31, h = last valid word of the previous unit
+__device__ __forceinline__ void shift_down_words(uint32_t (&P)[4], int nw, uint32_t h, uint32_t sh) {
   if (!PARTIAL) {
     P[3] = __funnelshift_l(P[2], P[3], sh);
     P[2] = __funnelshift_l(P[1], P[2], sh);
@@ -268,9 +263,21 @@ __device__ __forceinline__ void frame_down(uint32_t (&P)[4], const Unit& un, uin
 #pragma unroll
     for (int w = 3; w >= 0; --w) {
       const uint32_t prev = (w > 0) ? P[w > 0 ? w - 1 : 0] : h;
-      P[w] = (w < un.nw) ? __funnelshift_l(prev, P[w], sh) : 0u;
+      P[w] = (w < nw) ? __funnelshift_l(prev, P[w], sh) : 0u;
     }
   }
+}
+__device__ __forceinline__ void frame_up(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity,
+                                         uint32_t sh = 1u) {
+  const uint32_t h = unit_exchange(P[0], un.nxt, halo, parity);
+  shift_up_words(P, un.nw, h, sh);
+}
+__device__ __forceinline__ void frame_down(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity,
+                                           uint32_t sh = 1u) {
+  uint32_t last = P[3];
+  if (PARTIAL) last = un.nw >= 4 ? P[3] : un.nw == 3 ? P[2] : un.nw == 2 ? P[1] : P[0];
+  const uint32_t h = unit_exchange(last, un.prv, halo, parity);
+  shift_down_words(P, un.nw, h, sh);
 }
 
 // Quenched tags in the frames the passes use them in.
@@ -493,7 +500,90 @@ __device__ __forceinline__ void mcs_step(Ctx& c, const Planes& Rc, Planes& Rn, c
 }  // namespace k1j
 }  // namespace kpz
 
-#ifndef K1J_TILE
+#if defined(K1J_STREAM)
+// ---- K3 pass kernel, specialised: one launch = one sub-lattice pass of a ring streamed through HBM (north_star (2)) --
+// Thread = one unit: 128-bit loads of its 4+4 words from the input buffer, the frame change (if this pass's offset
+// differs from the stored frame) with ONE extra word of the unmodified input (the halo), the same
+// folded pair logic as K1, 128-bit stores to the ping-pong partner.  The frame of the stored ring follows the offsets.
+extern "C" __global__ void __launch_bounds__(256)
+kpz_k3_pass_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::K3Pass A) {
+  using namespace kpz;
+  using namespace kpz::k1j;
+  const unsigned long long gid = (unsigned long long)blockIdx.x * 256ull + threadIdx.x;
+  if (gid >= (unsigned long long)D.S * U) return;
+  const int s = (int)(gid / U);
+  const int u = (int)(gid % U);
+  const int nw = PARTIAL ? min(4, PW - 4 * u) : 4;
+  const unsigned long long srow = (unsigned long long)s * PWp;
+  const unsigned long long row = srow + 4ull * u;
+  const uint32_t fin = A.fin[s];
+  const uint32_t o = A.fo ? A.fo[s] : 0u;
+  uint32_t P[4], Q[4];
+  {
+    const uint4 e = *reinterpret_cast<const uint4*>(A.Ein + row);
+    const uint4 q = *reinterpret_cast<const uint4*>(A.Oin + row);
+    P[0] = e.x; P[1] = e.y; P[2] = e.z; P[3] = e.w;
+    Q[0] = q.x; Q[1] = q.y; Q[2] = q.z; Q[3] = q.w;
+  }
+  const int nxt = (u + 1 >= U) ? 0 : u + 1;
+  if (fin != o) {
+    if (o) {
+      shift_up_words(P, nw, A.Ein[srow + 4ull * nxt], 1u);
+    } else {
+      const int prv = (u == 0) ? U - 1 : u - 1;
+      const int nwp = PARTIAL ? min(4, PW - 4 * prv) : 4;
+      shift_down_words(P, nw, A.Ein[srow + 4ull * prv + nwp - 1], 1u);
+    }
+  }
+  if (A.fo) {
+    uint32_t spa[4] = {0, 0, 0, 0}, sqb[4] = {0, 0, 0, 0};
+    if (DIS >= 1) {
+      const uint4 x = *reinterpret_cast<const uint4*>((o ? D.SPO : D.SPE) + row);
+      spa[0] = x.x; spa[1] = x.y; spa[2] = x.z; spa[3] = x.w;
+    }
+    if (DIS >= 2) {
+      const uint4 x = *reinterpret_cast<const uint4*>((o ? D.SQE : D.SQO) + row);
+      sqb[0] = x.x; sqb[1] = x.y; sqb[2] = x.z; sqb[3] = x.w;
+      if (o) shift_up_words(sqb, nw, D.SQE[srow + 4ull * nxt], 1u);
+    }
+    const uint32_t gs = (uint32_t)(D.first_sample + s);
+    const uint32_t tlo = (uint32_t)A.m, thi = (uint32_t)((unsigned long long)A.m >> 32);
+    uint32_t r[NPSA][4];
+#pragma unroll
+    for (int pl = 0; pl < NEAG; ++pl) {
+      const uint4 v = philox4x32_10((uint32_t)u, gs, tlo, ctr3(TAG_PAIR, (uint32_t)A.pass, (uint32_t)pl, thi), D.keys);
+      r[pl][0] = v.x; r[pl][1] = v.y; r[pl][2] = v.z; r[pl][3] = v.w;
+    }
+    const uint32_t M = 0u - o;
+    if constexpr (!GENERAL) {
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        const uint32_t a = lop3<0xCA>(M, Q[w], P[w]);
+        const uint32_t sel = select_word(a, spa[w], sqb[w], r, w);
+        const uint32_t np = lop3<0xD8>(P[w], Q[w], sel);
+        const uint32_t nq = lop3<0xE4>(P[w], Q[w], sel);
+        P[w] = np;
+        Q[w] = nq;
+      }
+    } else {
+      uint32_t a[4], x[4], lt[4];
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        a[w] = lop3<0xCA>(M, Q[w], P[w]);
+        x[w] = P[w] ^ Q[w];
+      }
+      general_flips(lt, x, a, spa, sqb, r, D.keys, (uint32_t)u, gs, tlo, ctr3(TAG_PAIR, (uint32_t)A.pass, 0u, thi));
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        P[w] ^= lt[w];
+        Q[w] ^= lt[w];
+      }
+    }
+  }
+  *reinterpret_cast<uint4*>(A.Eout + row) = make_uint4(P[0], P[1], P[2], P[3]);
+  *reinterpret_cast<uint4*>(A.Oout + row) = make_uint4(Q[0], Q[1], Q[2], Q[3]);
+}
+#elif !defined(K1J_TILE)
 // grid = S samples, block = NTHREADS; thread u = unit u (idle when u >= U, but it joins every barrier / shuffle).
 extern "C" __global__ void __launch_bounds__(kpz::k1j::NTHREADS)
 kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::KpzRunArgs A) {

@@ -260,7 +260,8 @@ K3Fn k3_pick_dis(int dis, int nps) {
   }
 }
 
-int k3_launch_pass(kpz_sim* sim, K3Fn fn, const unsigned char* fin, const unsigned char* fo, long long m, int pass) {
+int k3_launch_pass(kpz_sim* sim, K3Fn fn, void* jitfn, const unsigned char* fin, const unsigned char* fo, long long m,
+                   int pass) {
   KpzDev D = sim->dev;
   K3Pass A{};
   A.Ein = sim->E;
@@ -272,7 +273,12 @@ int k3_launch_pass(kpz_sim* sim, K3Fn fn, const unsigned char* fin, const unsign
   A.m = m;
   A.pass = pass;
   const size_t nunits = (size_t)D.S * D.U;
-  fn<<<(unsigned)((nunits + 255) / 256), 256, 0, sim->stream>>>(D, A);
+  if (jitfn) {
+    void* args[] = {(void*)&D, (void*)&A};
+    KPZ_CUDA_CHECK(cudaLaunchKernel(jitfn, dim3((unsigned)((nunits + 255) / 256)), dim3(256), args, 0, sim->stream));
+  } else {
+    fn<<<(unsigned)((nunits + 255) / 256), 256, 0, sim->stream>>>(D, A);
+  }
   KPZ_LAUNCH_CHECK("k3_pass_kernel");
   std::swap(sim->E, sim->E2);
   std::swap(sim->O, sim->O2);
@@ -308,6 +314,13 @@ int k3_run(kpz_sim* sim, int64_t n_mcs) {
   const bool partial = (D0.PW % 4) != 0;
   const int dis = sim->has_sq ? 2 : sim->has_sp ? 1 : 0;
   K3Fn fn = partial ? k3_pick_dis<true>(dis, D0.nplanes) : k3_pick_dis<false>(dis, D0.nplanes);
+  void* jitfn = nullptr;  // the same pass specialised on (L, thresholds) when run-time compilation is enabled
+  if (jit_enabled()) {
+    std::vector<std::string> defs = k1_jit_defines(D0, dis);
+    defs.push_back("K1J_STREAM=1");
+    int rcj = jit_get("k1_sweep_jit.cuh", "kpz_k3_pass_jit", defs, &jitfn);
+    if (rcj) return rcj;
+  }
   const int nt = (int)sim->rec_times.size();
   int ri = sim->nrec;
   const long long pass_begin = 2 * (long long)sim->t, pass_end = 2 * (long long)(sim->t + n_mcs);
@@ -328,13 +341,13 @@ int k3_run(kpz_sim* sim, int64_t n_mcs) {
       const long long gp = c0 + k;
       const long long m = gp >> 1;
       const int pass = (int)(gp & 1);
-      int rc = k3_launch_pass(sim, fn, sim->k3off + (size_t)fin_row * S, sim->k3off + (size_t)(k + 1) * S, m, pass);
+      int rc = k3_launch_pass(sim, fn, jitfn, sim->k3off + (size_t)fin_row * S, sim->k3off + (size_t)(k + 1) * S, m, pass);
       if (rc) return rc;
       fin_row = k + 1;
       frame_dirty = true;
       if (pass == 1 && ri < nt && sim->rec_times[ri] == m + 1) {
         // bring every sample to frame 0 (no update), then reduce
-        rc = k3_launch_pass(sim, fn, sim->k3off + (size_t)fin_row * S, nullptr, m, pass);
+        rc = k3_launch_pass(sim, fn, jitfn, sim->k3off + (size_t)fin_row * S, nullptr, m, pass);
         if (rc) return rc;
         // from now on the stored frame is 0: point fin at a zero row (row 0 rewritten to zero)
         k3_copy_row<<<grid_for(S), 256, 0, sim->stream>>>(sim->k3off, nullptr, S);
@@ -350,7 +363,7 @@ int k3_run(kpz_sim* sim, int64_t n_mcs) {
     if (fin_row == 0) frame_dirty = false;
   }
   if (frame_dirty) {
-    int rc = k3_launch_pass(sim, fn, prev_row, nullptr, 0, 0);
+    int rc = k3_launch_pass(sim, fn, jitfn, prev_row, nullptr, 0, 0);
     if (rc) return rc;
   }
   return KPZ_OK;

@@ -36,16 +36,6 @@ __global__ void k3_copy_row(unsigned char* dst, const unsigned char* src, int n)
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) dst[i] = src ? src[i] : 0;
 }
 
-struct K3Pass {
-  const uint32_t* Ein;
-  const uint32_t* Oin;
-  uint32_t* Eout;
-  uint32_t* Oout;
-  const unsigned char* fin;  // [S] frame of the input lattice
-  const unsigned char* fo;   // [S] offset of this pass = frame of the output; nullptr = "bring to frame 0, no update"
-  long long m;               // MCS index (time key)
-  int pass;
-};
 
 template <bool PARTIAL, int DIS, int NPS>
 __global__ void __launch_bounds__(256) k3_pass_kernel(const __grid_constant__ KpzDev D, const __grid_constant__ K3Pass A) {

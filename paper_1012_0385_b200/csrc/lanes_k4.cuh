@@ -117,7 +117,7 @@ __device__ __forceinline__ uint32_t lane_pass(uint32_t (&X)[8], int nwn, int o, 
 }
 
 template <bool SINGLE_WARP, bool PARTIAL>
-__global__ void lanes_k4_kernel(const __grid_constant__ LanesDev D, const __grid_constant__ LanesRunArgs R) {
+__global__ void __launch_bounds__(1024) lanes_k4_kernel(const __grid_constant__ LanesDev D, const __grid_constant__ LanesRunArgs R) {
   __shared__ uint32_t halo[SINGLE_WARP ? 1 : 2048];
   __shared__ unsigned long long red[SINGLE_WARP ? 1 : 4 * 32];
   const int s = blockIdx.x;

@@ -39,6 +39,18 @@ struct KpzRunArgs {
   long long* rec_sum_h2;   // [nt][S]
 };
 
+// K3 (pass-by-pass streamed sweep): one launch = one sub-lattice pass from (Ein, Oin) to (Eout, Oout).
+struct K3Pass {
+  const uint32_t* Ein;
+  const uint32_t* Oin;
+  uint32_t* Eout;
+  uint32_t* Oout;
+  const unsigned char* fin;  // [S] frame of the input lattice
+  const unsigned char* fo;   // [S] offset of this pass = frame of the output; nullptr = "bring to frame 0, no update"
+  long long m;               // MCS index (time key)
+  int pass;
+};
+
 // K3T (temporally blocked streamed sweep): D.E / D.O are the input ring, these the ping-pong output.
 struct K3TArgs {
   uint32_t* Eout;

@@ -403,3 +403,58 @@ def test_error_codes(K):
         g.set_disorder_masks(g.lattice())
     assert e.value.code == -1
     assert K.kernel_launches() > 0
+
+
+# ---------------------------------------------------------------------------------------------------------
+# every kernel variant behind the same ABI computes the same thing: statically compiled generic kernels
+# (KPZ_B200_JIT=0) and the tuning knobs of the run-time specialised ones
+# ---------------------------------------------------------------------------------------------------------
+
+class _env:
+    def __init__(self, **kv):
+        self.kv = kv
+
+    def __enter__(self):
+        import os
+        self.old = {k: os.environ.get(k) for k in self.kv}
+        os.environ.update({k: str(v) for k, v in self.kv.items()})
+
+    def __exit__(self, *a):
+        import os
+        for k, v in self.old.items():
+            if v is None:
+                os.environ.pop(k, None)
+            else:
+                os.environ[k] = v
+
+
+@pytest.mark.parametrize("env", [dict(KPZ_B200_JIT=0), dict(KPZ_B200_K1_VARIANT=0)])
+def test_k1_variants_against_oracle(K, env):
+    with _env(**env):
+        run_both_kpz(K, 8192 + 64, 3, 0.75, 0.25, seed=21, times=[1, 3, 20], chunks=[7, 13])
+        run_both_kpz(K, 16384, 2, 1.0, 0.0, disorder=(0.1, 0.5, 0.0, 0.0), seed=22, times=[20], chunks=[20])
+        run_both_kpz(K, 2048, 2, 0.8, 0.05, disorder=(0.3, 0.2, 0.3, 0.01), seed=23, times=[9], chunks=[9])
+
+
+def test_static_streamed_kernel_against_oracle(K):
+    with _env(KPZ_B200_JIT=0):
+        gpu, _ = run_both_kpz(K, 65536 + 64, 2, 0.9, 0.1, seed=24, times=[2, 9], chunks=[4, 5], path=2)
+        assert gpu.path == K.KPZ_PATH_STREAM
+        # without run-time compilation the default large-ring path is the pass-by-pass stream
+        g = K.KpzSim(1 << 19, 1, 0.5, 0.5, seed=1, max_records=1)
+        assert g.path == K.KPZ_PATH_STREAM
+        with pytest.raises(K.KpzError):
+            K.KpzSim(1 << 19, 1, 0.5, 0.5, seed=1, max_records=1, path=3)
+
+
+@pytest.mark.parametrize("env", [dict(KPZ_B200_JIT=0), dict(KPZ_B200_K4_TAIL=1), dict(KPZ_B200_K4_EAGER=1),
+                                 dict(KPZ_B200_K4_EAGER=7, KPZ_B200_K4_TAIL=1)])
+def test_k4_variants_against_oracle(K, env):
+    with _env(**env):
+        run_both_lanes(K, 8192 + 64, 2, 1.0, 1.0, 0.3, 0.05, 6, 0.1, seed=31, times=[1, 6, 13], chunks=[6, 7])
+        run_both_lanes(K, 2048, 2, 0.75, 0.5, 0.4, 0.3, 4, 0.3, seed=32, times=[9], chunks=[9])
+
+
+def test_k4_ring_beyond_the_specialised_kernel(K):
+    """L = 262144 per lane: more 128-site supergroups than a CTA has threads - the generic two-lane kernel runs."""
+    run_both_lanes(K, 262144, 1, 1.0, 1.0, 0.3, 0.05, 3, 0.1, seed=33, times=[3, 4], chunks=[4])

@@ -1,0 +1,62 @@
+"""The run-time specialised kernels (NVRTC, csrc/jit.cu) compile for sm_100a WITHOUT a GPU for every BASELINE.json
+configuration and for the edge shapes of each code path (no compute calls here): the LUT path (<= 3 selection
+inputs), the GENERAL path (tags + planes, non-dyadic rates), ragged rings, multi-warp rings, both offset modes, the
+streamed pass kernel, the temporally blocked window kernel and the two-lane kernel."""
+import pytest
+
+import workloads
+
+
+@pytest.fixture(scope="module")
+def K():
+    from paper_1012_0385_b200 import build
+    build.build()
+    import paper_1012_0385_b200 as pkg
+    pkg.load_library()
+    return pkg
+
+
+@pytest.mark.parametrize("key", [1, 2, 3, 4, "4-aux-i"])
+def test_kpz_configs_compile(K, key):
+    c = workloads.CONFIGS[key]
+    n = K.jit_check(c["L"], c["p"], c["q"], disorder=c["disorder"], path=c.get("path", 0))
+    if c.get("path", 0) == K.KPZ_PATH_STREAM:
+        assert n == 0          # kpz_jit_check reports the per-sample / blocked kernels only
+    else:
+        assert n > 10_000      # a real sm_100a cubin
+
+
+def test_config5_two_lane_compiles(K):
+    c = workloads.CONFIGS[5]
+    assert K.lanes_jit_check(c["L"], c["p_a"], c["p_b"], c["turn_prob"], c["turn_period"], c["omega"]) > 10_000
+
+
+@pytest.mark.parametrize("L,p,q,dis,mode,path", [
+    (64, 1.0, 0.0, None, 0, 1),                       # smallest ring, no plane
+    (320, 0.5, 0.5, None, 1, 1),                      # ragged unit, alternating offsets, 1 plane
+    (8192 + 64, 0.8, 0.0, None, 0, 1),                # 30-plane threshold: GENERAL path with a lazy tail, ragged
+    (16384, 0.75, 0.25, (0.5, 0.375, 0.5, 0.125), 0, 1),   # two tag classes + 3 planes: GENERAL, all planes eager
+    (1 << 18, 0.75, 0.25, None, 0, 1),                # 1024 threads per ring
+    (1 << 18, 0.9, 0.1, (0.1, 0.5, 0.0, 0.0), 0, 3),  # blocked window kernel with tags
+    (64, 0.75, 0.25, None, 1, 3),                     # ring shorter than a window
+])
+def test_edge_shapes_compile(K, L, p, q, dis, mode, path):
+    assert K.jit_check(L, p, q, disorder=dis, offset_mode=mode, path=path) > 10_000
+
+
+@pytest.mark.parametrize("L,pa,pb,turn,period,omega", [
+    (64, 1.0, 1.0, 0.05, 100, 0.1),
+    (64 * 5, 0.75, 0.5, 0.25, 0, 0.5),      # ragged, in-lane planes, turning points never redrawn
+    (131072, 1.0, 0.75, 0.05, 7, 1.0),      # largest ring of the specialised kernel
+])
+def test_two_lane_edge_shapes_compile(K, L, pa, pb, turn, period, omega):
+    assert K.lanes_jit_check(L, pa, pb, turn, period, omega) > 10_000
+
+
+def test_bad_arguments_are_refused_without_compiling(K):
+    with pytest.raises(K.KpzError):
+        K.jit_check(100, 0.5, 0.5)              # L not a multiple of 64
+    with pytest.raises(K.KpzError):
+        K.jit_check(64, 1.5, 0.5)
+    with pytest.raises(K.KpzError):
+        K.lanes_jit_check(64, 1.0, 1.0, 0.05, -1, 0.1)
