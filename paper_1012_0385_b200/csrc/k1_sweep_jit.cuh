@@ -20,6 +20,7 @@
 // = P shifted by one even site.  The lattice is in frame 0 at every MCS boundary.
 #pragma once
 #include "sweep_types.cuh"
+#include "height_lut.cuh"
 
 #ifndef K1J_VARIANT
 #define K1J_VARIANT 1  // 0: one code path per offset pair (4-way switch); 1: branch-free
@@ -345,51 +346,12 @@ __device__ __forceinline__ void pass_branchfree(uint32_t (&P)[4], uint32_t (&Q)[
 }
 
 // ---- K2 fused: heights h_x = inclusive prefix of (2n-1), exact sums per sample (a6, a7) -----------
-// 8 sites at a time through a 256-entry table in shared memory: index = 4 even-site bits | 4 odd-site bits << 4
-// (site order e0,o0,e1,o1,...); entry = (r8+8) | (s1+36)<<5 | s2<<12 with r_k the height after k sites relative to
-// the height before the byte, s1 = sum r_k, s2 = sum r_k^2.
-__device__ __forceinline__ uint32_t height_lut_entry(int idx) {
-  int r = 0, s1 = 0, s2 = 0;
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    r += 2 * ((idx >> k) & 1) - 1;
-    s1 += r;
-    s2 += r * r;
-    r += 2 * ((idx >> (4 + k)) & 1) - 1;
-    s1 += r;
-    s2 += r * r;
-  }
-  return (uint32_t)(r + 8) | ((uint32_t)(s1 + 36) << 5) | ((uint32_t)s2 << 12);
-}
-
-// Sums over this unit's sites of the heights relative to the site before the unit (|r| <= 256, s2 <= 2^24).
-__device__ __forceinline__ void unit_relative_sums(const uint32_t (&P)[4], const uint32_t (&Q)[4], int nw,
-                                                   const uint32_t* lut, int& r_out, int& s1_out, int& s2_out) {
-  int r = 0, s1 = 0, s2 = 0;
-#pragma unroll
-  for (int w = 0; w < 4; ++w) {
-    if (!PARTIAL || w < nw) {
-#pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const uint32_t idx = ((P[w] >> (4 * k)) & 15u) | (((Q[w] >> (4 * k)) & 15u) << 4);
-        const uint32_t v = lut[idx];
-        const int d = (int)(v & 31u) - 8, a1 = (int)((v >> 5) & 127u) - 36, a2 = (int)(v >> 12);
-        s1 += 8 * r + a1;
-        s2 += 8 * r * r + 2 * r * a1 + a2;
-        r += d;
-      }
-    }
-  }
-  r_out = r;
-  s1_out = s1;
-  s2_out = s2;
-}
-
+// 8 sites at a time through the byte table of height_lut.cuh.
 __device__ __forceinline__ void record_sums(const uint32_t (&P)[4], const uint32_t (&Q)[4], int nw,
                                             const uint32_t* lut, long long* scratch, long long* out_h,
                                             long long* out_h2) {
   int r = 0, s1 = 0, s2 = 0;
-  if (nw > 0) unit_relative_sums(P, Q, nw, lut, r, s1, s2);
+  if (nw > 0) unit_relative_sums_lut(P, Q, nw, lut, r, s1, s2);
   const int lane = threadIdx.x & 31;
   int incl = r;  // inclusive scan of the unit totals: the height before unit u is the sum over units < u
 #pragma unroll

@@ -8,6 +8,7 @@
 // pass).  The frame of the stored lattice follows the offsets: a pass with the same offset as the previous one
 // touches no neighbour at all.
 #pragma once
+#include "height_lut.cuh"
 #include "kpz_k1.cuh"
 
 namespace kpz {
@@ -171,6 +172,9 @@ __global__ void __launch_bounds__(256) k3_tile_sums(const uint32_t* E, const uin
                                                     unsigned long long* out_h2) {
   __shared__ int sm[8];
   __shared__ long long red[16];
+  __shared__ uint32_t lut[256];
+  lut[threadIdx.x] = height_lut_entry((int)threadIdx.x);
+  __syncthreads();
   const int s = blockIdx.x / ntiles, tile = blockIdx.x % ntiles;
   const int u = tile * 256 + threadIdx.x;
   int r = 0, s1 = 0, s2 = 0, nw = 0;
@@ -180,7 +184,7 @@ __global__ void __launch_bounds__(256) k3_tile_sums(const uint32_t* E, const uin
     const uint4 e = *reinterpret_cast<const uint4*>(E + row);
     const uint4 q = *reinterpret_cast<const uint4*>(O + row);
     const uint32_t P[4] = {e.x, e.y, e.z, e.w}, Q[4] = {q.x, q.y, q.z, q.w};
-    unit_relative_sums(P, Q, nw, r, s1, s2);
+    unit_relative_sums_lut(P, Q, nw, lut, r, s1, s2);
   }
   int total;
   const long long base = (long long)tile_base[(size_t)s * ntiles + tile] + block_exclusive_scan_256(r, sm, total);
