@@ -25,6 +25,13 @@
 #ifndef K1J_VARIANT
 #define K1J_VARIANT 1  // 0: one code path per offset pair (4-way switch); 1: branch-free
 #endif
+#ifndef K1J_REFRAME
+#ifdef K1J_TILE
+#define K1J_REFRAME 1  // merged frame changes: measured +5 % on the blocked stream (many warps per SM) ...
+#else
+#define K1J_REFRAME 0  // ... and -3 % / -9 % on the per-sample kernel (1.7 warps per SMSP), which keeps frame 0 per pass
+#endif
+#endif
 #ifndef K1J_EAGER
 #define K1J_EAGER 6  // GENERAL path: planes drawn one MCS ahead; deeper planes are evaluated lazily
 #endif
@@ -281,6 +288,32 @@ __device__ __forceinline__ void frame_down(uint32_t (&P)[4], const Unit& un, uin
   shift_down_words(P, un.nw, h, sh);
 }
 
+// Frame change `from` -> `to` (each 0 or 1, warp-uniform run-time values) with ONE neighbour exchange: every unit
+// publishes its first and its last valid word; the shift down by `from` uses the previous unit's last word, and the
+// shift up by `to` needs the next unit's first word AFTER that unit's own shift down - which is a function of words
+// this unit already holds (its own last word is the next unit's incoming word).
+__device__ __forceinline__ void reframe(uint32_t (&P)[4], const Unit& un, uint32_t from, uint32_t to, uint32_t* halo,
+                                        int& parity) {
+  uint32_t last = P[3];
+  if (PARTIAL) last = un.nw >= 4 ? P[3] : un.nw == 3 ? P[2] : un.nw == 2 ? P[1] : P[0];
+  uint32_t hn, hp;  // next unit's first word, previous unit's last word
+  if (SINGLE_WARP) {
+    hn = __shfl_sync(0xFFFFFFFFu, P[0], un.nxt);
+    hp = __shfl_sync(0xFFFFFFFFu, last, un.prv);
+  } else {
+    uint32_t* slot = halo + parity * (2 * NTHREADS);
+    slot[2 * threadIdx.x] = P[0];
+    slot[2 * threadIdx.x + 1] = last;
+    __syncthreads();
+    hn = slot[2 * un.nxt];
+    hp = slot[2 * un.prv + 1];
+    parity ^= 1;
+  }
+  hn = __funnelshift_l(last, hn, from);  // the next unit's first word after ITS shift down
+  shift_down_words(P, un.nw, hp, from);
+  shift_up_words(P, un.nw, hn, to);
+}
+
 // Quenched tags in the frames the passes use them in.
 struct Tags {
   uint32_t spa0[4];  // slow-p at even sites  (a side of frame 0)
@@ -303,16 +336,15 @@ __device__ __forceinline__ void mcs_logic(uint32_t (&P)[4], uint32_t (&Q)[4], co
   if (O1) frame_down(P, un, halo, parity);
 }
 
-// Branch-free form (K1J_VARIANT 1): the offset o of a pass is a run-time, warp-uniform value.  P goes to frame o by
-// a funnel shift by o bits, the a side is picked by a mask (P and Q enter the update symmetrically, so only the
-// rate selection needs to know which of them is a), and P returns to frame 0 by the opposite shift: the whole
-// MCS is one basic block, which the scheduler fills with the Philox rounds of the next MCS.
+// Branch-free form (K1J_VARIANT 1): the offset o of a pass is a run-time, warp-uniform value.  P is brought to frame
+// o by reframe() (funnel shifts by 0 or 1 bit), the a side is picked by a mask (P and Q enter the update
+// symmetrically, so only the rate selection needs to know which of them is a): the whole MCS is one basic block,
+// which the scheduler fills with the Philox rounds of the next MCS.  P must be in frame o on entry.
 __device__ __forceinline__ void pass_branchfree(uint32_t (&P)[4], uint32_t (&Q)[4], const Tags& G,
                                                 const uint32_t (&r)[NPSA][4], const Unit& un, uint32_t o,
                                                 uint32_t* halo, int& parity, const PhiloxKeys& K, uint32_t Gu,
                                                 uint32_t gs, uint32_t tlo, uint32_t c3) {
   const uint32_t M = 0u - o;  // all ones in frame 1
-  frame_up(P, un, halo, parity, o);
   if constexpr (!GENERAL) {
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
@@ -342,7 +374,6 @@ __device__ __forceinline__ void pass_branchfree(uint32_t (&P)[4], uint32_t (&Q)[
       Q[w] ^= lt[w];
     }
   }
-  frame_down(P, un, halo, parity, o);
 }
 
 // ---- K2 fused: heights h_x = inclusive prefix of (2n-1), exact sums per sample (a6, a7) -----------
@@ -419,6 +450,7 @@ struct Ctx {
   uint32_t G;    // supergroup index of this unit (Philox counter c0)
   int parity;
   uint32_t offbits;
+  uint32_t frame;  // frame P is in between MCS (branch-free sweep: the offset of the last pass; else 0)
 };
 
 // MCS m: draw the planes of MCS m+1 into Rn, then apply MCS m with the planes Rc drawn one step earlier.  Both sit
@@ -432,10 +464,24 @@ __device__ __forceinline__ void mcs_step(Ctx& c, const Planes& Rc, Planes& Rn, c
   } else if (K1J_VARIANT == 1 || GENERAL) {
     const uint32_t code = K1J_OFFSET_MODE == 1 ? 2u : (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
     draw_planes(Rn, K, c.G, c.gs, m + 1);
-    pass_branchfree(c.P, c.Q, c.tags, Rc.r[0], c.un, code & 1u, halo, c.parity, K, c.G, c.gs, tlo,
-                    ctr3(TAG_PAIR, 0u, 0u, thi));
-    pass_branchfree(c.P, c.Q, c.tags, Rc.r[1], c.un, code >> 1, halo, c.parity, K, c.G, c.gs, tlo,
-                    ctr3(TAG_PAIR, 1u, 0u, thi));
+    if (K1J_REFRAME) {  // one exchange per frame change, the frame is carried across MCS
+      reframe(c.P, c.un, c.frame, code & 1u, halo, c.parity);
+      pass_branchfree(c.P, c.Q, c.tags, Rc.r[0], c.un, code & 1u, halo, c.parity, K, c.G, c.gs, tlo,
+                      ctr3(TAG_PAIR, 0u, 0u, thi));
+      reframe(c.P, c.un, code & 1u, code >> 1, halo, c.parity);
+      pass_branchfree(c.P, c.Q, c.tags, Rc.r[1], c.un, code >> 1, halo, c.parity, K, c.G, c.gs, tlo,
+                      ctr3(TAG_PAIR, 1u, 0u, thi));
+      c.frame = code >> 1;
+    } else {  // frame 0 around every pass: shift up by o, pass, shift down by o
+      frame_up(c.P, c.un, halo, c.parity, code & 1u);
+      pass_branchfree(c.P, c.Q, c.tags, Rc.r[0], c.un, code & 1u, halo, c.parity, K, c.G, c.gs, tlo,
+                      ctr3(TAG_PAIR, 0u, 0u, thi));
+      frame_down(c.P, c.un, halo, c.parity, code & 1u);
+      frame_up(c.P, c.un, halo, c.parity, code >> 1);
+      pass_branchfree(c.P, c.Q, c.tags, Rc.r[1], c.un, code >> 1, halo, c.parity, K, c.G, c.gs, tlo,
+                      ctr3(TAG_PAIR, 1u, 0u, thi));
+      frame_down(c.P, c.un, halo, c.parity, code >> 1);
+    }
   } else {
     const uint32_t code = (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
     switch (code) {
@@ -551,7 +597,7 @@ extern "C" __global__ void __launch_bounds__(kpz::k1j::NTHREADS)
 kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::KpzRunArgs A) {
   using namespace kpz;
   using namespace kpz::k1j;
-  __shared__ uint32_t halo[SINGLE_WARP ? 1 : 2 * NTHREADS];
+  __shared__ uint32_t halo[SINGLE_WARP ? 1 : 4 * NTHREADS];
   __shared__ long long scratch[SINGLE_WARP ? 1 : 96];
   __shared__ uint32_t lut[256];
   for (int i = threadIdx.x; i < 256; i += NTHREADS) lut[i] = height_lut_entry(i);
@@ -568,6 +614,7 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   c.G = (uint32_t)u;
   c.parity = 0;
   c.offbits = 0;
+  c.frame = 0;
   const unsigned long long row = (unsigned long long)s * PWp + 4ull * (active ? u : 0);
 #pragma unroll
   for (int w = 0; w < 4; ++w) {
@@ -603,8 +650,15 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   Planes RA, RB;
   draw_planes(RA, D.keys, c.G, c.gs, m);
 
+  auto to_frame0 = [&]() {
+    if (c.frame) {  // warp- and CTA-uniform
+      reframe(c.P, c.un, c.frame, 0u, halo, c.parity);
+      c.frame = 0;
+    }
+  };
   auto after_mcs = [&]() {  // m has been advanced: t = m
     if (m == next_rec) {
+      to_frame0();
       record_sums(c.P, c.Q, c.un.nw, lut, scratch, A.rec_sum_h + (size_t)ri * D.S + s,
                   A.rec_sum_h2 + (size_t)ri * D.S + s);
       ++ri;
@@ -622,6 +676,7 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
     ++m;
     after_mcs();
   }
+  to_frame0();
 
   if (active) {
     *reinterpret_cast<uint4*>(D.E + row) = make_uint4(c.P[0], c.P[1], c.P[2], c.P[3]);
@@ -656,6 +711,7 @@ kpz_k3t_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__
   c.G = (uint32_t)g;
   c.parity = 0;
   c.offbits = 0;
+  c.frame = 0;
   const unsigned long long row = (unsigned long long)s * PWp + 4ull * g;
   {
     const uint4 e = *reinterpret_cast<const uint4*>(D.E + row);
@@ -692,6 +748,7 @@ kpz_k3t_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__
     ++m;
     if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
   }
+  if (c.frame) reframe(c.P, c.un, c.frame, 0u, nullptr, c.parity);
   if (lane >= 1 && lane <= TI && tile * TI + lane - 1 < U) {
     *reinterpret_cast<uint4*>(A.Eout + row) = make_uint4(c.P[0], c.P[1], c.P[2], c.P[3]);
     *reinterpret_cast<uint4*>(A.Oout + row) = make_uint4(c.Q[0], c.Q[1], c.Q[2], c.Q[3]);

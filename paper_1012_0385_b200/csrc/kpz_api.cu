@@ -193,6 +193,14 @@ std::vector<std::string> k1_jit_defines(const KpzDev& D, int dis) {
   d.push_back(buf);
   snprintf(buf, sizeof buf, "K1J_OFFSET_MODE=%d", D.offset_mode);
   d.push_back(buf);
+  if (const char* v = std::getenv("KPZ_B200_K1_REFRAME")) {  // tuning knob: merged frame changes (k1_sweep_jit.cuh)
+    snprintf(buf, sizeof buf, "K1J_REFRAME=%d", atoi(v));
+    d.push_back(buf);
+  }
+  if (const char* v = std::getenv("KPZ_B200_K1_EAGER")) {  // tuning knob: planes of the GENERAL path drawn one MCS ahead
+    snprintf(buf, sizeof buf, "K1J_EAGER=%d", atoi(v));
+    d.push_back(buf);
+  }
   if (const char* v = std::getenv("KPZ_B200_K1_VARIANT")) {  // tuning knob: code shape of the sweep (k1_sweep_jit.cuh)
     snprintf(buf, sizeof buf, "K1J_VARIANT=%d", atoi(v));
     d.push_back(buf);
