@@ -230,7 +230,8 @@ def run_cuda(args, cfg, cfg_key):
     if args.mcs is not None:
         cfg = workloads.truncated(cfg, n_mcs)
     su_step = workloads.site_updates(cfg)
-    sim = make_sim(pkg, cfg, first_sample=rank * cfg["S"])      # global sample indices: results independent of N
+    from paper_1012_0385_b200 import shard
+    sim = make_sim(pkg, cfg, first_sample=shard.weak_first_sample(cfg["S"], rank))   # global sample indices
     stream = torch.cuda.current_stream()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
