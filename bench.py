@@ -344,8 +344,11 @@ def run_cuda(args, cfg, cfg_key):
         n_launch = 2 * n_mcs
         bytes_launch = 2 * cfg["S"] * cfg["L"] / 8
         achieved = bytes_launch * n_launch / (ms_run * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": "k3_pass_kernel", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+        # dram__bytes_read.sum + dram__bytes_write.sum of one pass launch, from the ncu --set full capture summarised in
+        # profiles/r01_v2_summary.md (only taken at L=2^32; elsewhere unmeasured)
+        traffic = 536.878336e6 + 483.978496e6 if cfg["L"] == (1 << 32) and cfg["S"] == 1 else None
+        roof = {"bound": "hbm", "kernel": "kpz_k3_pass_jit", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"],
                 "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
     else:
         slots = ALU_SLOTS_PER_SU.get(cfg_key, ALU_SLOTS_PER_SU[2])
