@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — site-update throughput of the KPZ/ASEP hot path on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|5|4-aux-i|4-aux-ii|4-aux-i-blocked] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|5|4-aux-i|4-aux-ii|4-aux-i-blocked|paper-1024x30|paper-1024-fill|paper-qtasep-16384|paper-qssep-4096] [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: reset to the
 initial state (a1), run the configuration's full number of MCS with its record times (a2-a7 / a9), records left in
@@ -56,6 +56,12 @@ ALU_SLOTS_PER_SU = {
     "4-aux-i": (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,
     "4-aux-ii": (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,
     "4-aux-i-blocked": (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,
+    # paper parameter sets (p = 0.8: a 30-plane threshold, ~26 forward-active pairs per unit: log2(26)+1.33 planes;
+    # offsets alternate, so the frame changes twice per MCS)
+    "paper-1024x30": (2 * 6.0 * (34 + 12) + 2 * 4 * 3 + 8) / 256,
+    "paper-1024-fill": (2 * 6.0 * (34 + 12) + 2 * 4 * 3 + 8) / 256,
+    "paper-qtasep-16384": (2 * 6.0 * (34 + 12) + 2 * 4 * 3 + 8) / 256,
+    "paper-qssep-4096": (2 * 7.0 * (34 + 12) + 2 * 4 * 3 + 8) / 256,
 }
 ALU_SLOTS_PER_CLK_SMSP = 0.5
 # streamed sweep: one read + one write of the bit-packed ring per sub-lattice pass = 2 passes * 2 * 1/8 B
@@ -142,7 +148,7 @@ def _oracle_sim(cfg, nsamples, first_sample=0):
         return R.LanesRef(cfg["L"], nsamples, cfg["p_a"], cfg["p_b"], cfg["rho0"], cfg["turn_prob"], cfg["turn_period"],
                           cfg["omega"], seed=cfg["seed"], first_sample=first_sample)
     return R.KpzRef(cfg["L"], nsamples, cfg["p"], cfg["q"], disorder=cfg["disorder"], seed=cfg["seed"],
-                    first_sample=first_sample)
+                    first_sample=first_sample, offset_mode=cfg.get("offset_mode", 0))
 
 
 def oracle_sample_shape(cfg, target_su):
@@ -204,7 +210,8 @@ def make_sim(pkg, cfg, first_sample):
                            cfg["omega"], seed=cfg["seed"], first_sample=first_sample, max_records=nrec)
     else:
         sim = pkg.KpzSim(cfg["L"], cfg["S"], cfg["p"], cfg["q"], disorder=cfg["disorder"], seed=cfg["seed"],
-                         first_sample=first_sample, max_records=nrec, path=cfg.get("path", 0))
+                         first_sample=first_sample, max_records=nrec, path=cfg.get("path", 0),
+                         offset_mode=cfg.get("offset_mode", 0))
     sim.set_record_times(cfg["record_times"])
     return sim
 
@@ -372,7 +379,9 @@ def run_cuda(args, cfg, cfg_key):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
+        # only "paper-1024x30" is a workload the paper quotes a number for (another machine: context)
+        "vs_baseline": (value / cfg["paper_gsu"]) if (cfg.get("paper_gsu") and world == 1 and args.mcs is None) else None,
         "dtype": "u32", "data": "synthetic",
         "config": {"workload": cfg["name"], "config_key": str(cfg_key), "L": cfg["L"], "samples_per_gpu": cfg["S"],
                    "n_mcs": n_mcs, "records": len(cfg["record_times"]), "path": PATH_NAMES[path] if cfg["kind"] == "kpz" else "two-lane K4", "l2": "flushed between timed steps (256 MiB fill)",

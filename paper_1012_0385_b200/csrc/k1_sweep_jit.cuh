@@ -45,13 +45,17 @@ namespace k1j {
 constexpr int PW = K1J_PW;
 constexpr int PWp = (PW + 3) / 4 * 4;
 constexpr int U = PWp / 4;
+constexpr bool PARTIAL = (PW % 4) != 0;
 #ifdef K1J_TILE
 constexpr bool TILE = true;   // K3T: a warp sweeps a 32-unit window of a long ring (kpz_k3t_sweep_jit below)
 #else
 constexpr bool TILE = false;
 #endif
 constexpr bool SINGLE_WARP = TILE || U <= 32;
-constexpr bool PARTIAL = (PW % 4) != 0;
+// Small rings: a ring of U <= 16 units (L = 256 U sites, U a power of two) fills only U lanes, so a warp sweeps
+// SPW = 32 / U independent samples side by side; every per-sample quantity (offsets, frame, record sums) is then a
+// per-lane value and the shuffles run inside segments of U lanes.
+constexpr int SPW = (!TILE && !PARTIAL && U <= 16 && (U & (U - 1)) == 0) ? 32 / U : 1;
 constexpr int DIS = K1J_DIS;
 constexpr int NTHREADS = (U + 31) / 32 * 32;
 constexpr uint64_t T0 = K1J_T0, T1 = K1J_T1, T2 = K1J_T2, T3 = K1J_T3;
@@ -380,15 +384,17 @@ __device__ __forceinline__ void pass_branchfree(uint32_t (&P)[4], uint32_t (&Q)[
 // 8 sites at a time through the byte table of height_lut.cuh.
 __device__ __forceinline__ void record_sums(const uint32_t (&P)[4], const uint32_t (&Q)[4], int nw,
                                             const uint32_t* lut, long long* scratch, long long* out_h,
-                                            long long* out_h2) {
+                                            long long* out_h2, bool writer) {
   int r = 0, s1 = 0, s2 = 0;
   if (nw > 0) unit_relative_sums_lut(P, Q, nw, lut, r, s1, s2);
   const int lane = threadIdx.x & 31;
+  constexpr int SEG = SPW > 1 ? U : 32;  // lanes of one sample inside a warp
+  const int pos = lane & (SEG - 1);
   int incl = r;  // inclusive scan of the unit totals: the height before unit u is the sum over units < u
 #pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const int v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-    if (lane >= d) incl += v;
+  for (int d = 1; d < SEG; d <<= 1) {
+    const int v = __shfl_up_sync(0xFFFFFFFFu, incl, d, SEG);
+    if (pos >= d) incl += v;
   }
   long long base = (long long)(incl - r);
   if (!SINGLE_WARP) {
@@ -405,12 +411,12 @@ __device__ __forceinline__ void record_sums(const uint32_t (&P)[4], const uint32
   long long H = n * base + (long long)s1;
   long long H2 = n * base * base + 2LL * base * (long long)s1 + (long long)s2;
 #pragma unroll
-  for (int d = 16; d >= 1; d >>= 1) {
-    H += __shfl_down_sync(0xFFFFFFFFu, H, d);
-    H2 += __shfl_down_sync(0xFFFFFFFFu, H2, d);
+  for (int d = SEG / 2; d >= 1; d >>= 1) {
+    H += __shfl_down_sync(0xFFFFFFFFu, H, d, SEG);
+    H2 += __shfl_down_sync(0xFFFFFFFFu, H2, d, SEG);
   }
   if (SINGLE_WARP) {
-    if (lane == 0) {
+    if (pos == 0 && writer) {
       *out_h = H;
       *out_h2 = H2;
     }
@@ -461,10 +467,10 @@ __device__ __forceinline__ void mcs_step(Ctx& c, const Planes& Rc, Planes& Rn, c
   if (K1J_OFFSET_MODE == 1 && !GENERAL) {
     draw_planes(Rn, K, c.G, c.gs, m + 1);
     mcs_logic<0, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
-  } else if (K1J_VARIANT == 1 || GENERAL) {
+  } else if (K1J_VARIANT == 1 || GENERAL || SPW > 1) {
     const uint32_t code = K1J_OFFSET_MODE == 1 ? 2u : (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
     draw_planes(Rn, K, c.G, c.gs, m + 1);
-    if (K1J_REFRAME) {  // one exchange per frame change, the frame is carried across MCS
+    if (K1J_REFRAME && SPW == 1) {  // one exchange per frame change, the frame is carried across MCS
       reframe(c.P, c.un, c.frame, code & 1u, halo, c.parity);
       pass_branchfree(c.P, c.Q, c.tags, Rc.r[0], c.un, code & 1u, halo, c.parity, K, c.G, c.gs, tlo,
                       ctr3(TAG_PAIR, 0u, 0u, thi));
@@ -592,7 +598,8 @@ kpz_k3_pass_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ k
   *reinterpret_cast<uint4*>(A.Oout + row) = make_uint4(Q[0], Q[1], Q[2], Q[3]);
 }
 #elif !defined(K1J_TILE)
-// grid = S samples, block = NTHREADS; thread u = unit u (idle when u >= U, but it joins every barrier / shuffle).
+// grid = S samples (ceil(S / SPW) warps for small rings), block = NTHREADS; thread u = unit u (idle when u >= U, but it
+// joins every barrier / shuffle).
 extern "C" __global__ void __launch_bounds__(kpz::k1j::NTHREADS)
 kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::KpzRunArgs A) {
   using namespace kpz;
@@ -603,13 +610,16 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   for (int i = threadIdx.x; i < 256; i += NTHREADS) lut[i] = height_lut_entry(i);
   __syncthreads();
 
-  const int s = blockIdx.x;
-  const int u = threadIdx.x;
-  const bool active = u < U;
+  // SPW == 1: CTA = sample, thread = unit.  SPW > 1: CTA = one warp = SPW samples, lane = (sample, unit).
+  const int sub = SPW > 1 ? (int)threadIdx.x / U : 0;
+  const int s = SPW > 1 ? (int)blockIdx.x * SPW + sub : (int)blockIdx.x;
+  const int u = SPW > 1 ? (int)threadIdx.x % U : (int)threadIdx.x;
+  const int lane0 = SPW > 1 ? sub * U : 0;  // first lane of this sample
+  const bool active = u < U && s < D.S;
   Ctx c;
   c.un.nw = !active ? 0 : (PARTIAL ? min(4, PW - 4 * u) : 4);
-  c.un.nxt = (u + 1 >= U) ? 0 : u + 1;
-  c.un.prv = (u == 0) ? U - 1 : u - 1;
+  c.un.nxt = lane0 + ((u + 1 >= U) ? 0 : u + 1);
+  c.un.prv = lane0 + ((u == 0) ? U - 1 : u - 1);
   c.gs = (uint32_t)(D.first_sample + s);
   c.G = (uint32_t)u;
   c.parity = 0;
@@ -645,7 +655,18 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   long long next_rec = ri < A.nt ? A.rec_t[ri] : -1;
   const long long t_end = A.t0 + A.n_mcs;
   long long m = A.t0;
-  if (K1J_OFFSET_MODE == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+  auto draw_offsets = [&]() {
+    if (SPW == 1) {
+      c.offbits = draw_offsets16(D.keys, c.gs, m);
+    } else {
+#pragma unroll 1
+      for (int k = 0; k < SPW; ++k) {  // one ballot per sample of this warp; each lane keeps its own sample's
+        const uint32_t b = draw_offsets16(D.keys, (uint32_t)(D.first_sample + (int)blockIdx.x * SPW + k), m);
+        if (k == sub) c.offbits = b;
+      }
+    }
+  };
+  if (K1J_OFFSET_MODE == 0) draw_offsets();
 
   Planes RA, RB;
   draw_planes(RA, D.keys, c.G, c.gs, m);
@@ -660,11 +681,11 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
     if (m == next_rec) {
       to_frame0();
       record_sums(c.P, c.Q, c.un.nw, lut, scratch, A.rec_sum_h + (size_t)ri * D.S + s,
-                  A.rec_sum_h2 + (size_t)ri * D.S + s);
+                  A.rec_sum_h2 + (size_t)ri * D.S + s, active);
       ++ri;
       next_rec = ri < A.nt ? A.rec_t[ri] : -1;
     }
-    if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+    if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) draw_offsets();
   };
 
   while (m < t_end) {

@@ -653,7 +653,10 @@ int kpz_run(kpz_sim* sim, int64_t n_mcs) {
       rc = jit_get("k1_sweep_jit.cuh", "kpz_k1_sweep_jit", k1_jit_defines(D, dis), &kfn);
       if (rc) return rc;
       void* args[] = {(void*)&D, (void*)&A};
-      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(sim->S), dim3(block), args, 0, sim->stream));
+      // small rings (k1_sweep_jit.cuh, SPW): U <= 16 units, a power of two, no ragged unit -> 32/U samples per warp
+      const bool pack = D.U <= 16 && (D.U & (D.U - 1)) == 0 && !partial;
+      const int spw = pack ? 32 / D.U : 1;
+      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((sim->S + spw - 1) / spw), dim3(block), args, 0, sim->stream));
       KPZ_LAUNCH_CHECK("kpz_k1_sweep_jit");
     } else {
       K1Fn fn = k1_pick(single, partial, dis, D.nplanes);

@@ -458,3 +458,15 @@ def test_k4_variants_against_oracle(K, env):
 def test_k4_ring_beyond_the_specialised_kernel(K):
     """L = 262144 per lane: more 128-site supergroups than a CTA has threads - the generic two-lane kernel runs."""
     run_both_lanes(K, 262144, 1, 1.0, 1.0, 0.3, 0.05, 3, 0.1, seed=33, times=[3, 4], chunks=[4])
+
+
+@pytest.mark.parametrize("L,S", [(256, 33), (512, 17), (1024, 30), (2048, 5), (4096, 3)])
+def test_k1_small_rings_packed_per_warp(K, L, S):
+    """Rings of 1..16 units are swept 32/U samples per warp (k1_sweep_jit.cuh, SPW): sample counts that do not fill
+    the last warp, per-sample offsets / records / tags, the paper's rate p = 0.8 (lazy planes), both offset modes."""
+    rng = np.random.default_rng(L + S)
+    start = R.pack_sites((rng.random((S, L)) < 0.5).astype(np.uint8))
+    run_both_kpz(K, L, S, 0.75, 0.25, seed=41, times=[1, 2, 17, 40], chunks=[16, 24], start=start)
+    run_both_kpz(K, L, S, 0.8, 0.0, seed=42, times=[5, 33], chunks=[33])
+    run_both_kpz(K, L, S, 0.5, 0.5, disorder=(0.5, 0.1, 0.5, 0.1), seed=43, times=[9], chunks=[9], offset_mode=1)
+    run_both_kpz(K, L, S, 1.0, 0.0, disorder=(0.1, 0.5, 0.0, 0.0), seed=44, times=[20], chunks=[20], first_sample=7)

@@ -11,9 +11,23 @@ def test_record_time_rule_reproduces_frozen_lists():
     assert workloads.log_spaced_times(100_000, 50) == workloads.CONFIGS[5]["record_times"]
     assert workloads.log_spaced_times(1000, 20) == workloads.CONFIGS[4]["record_times"]
     assert workloads.CONFIGS[1]["record_times"] == [2 ** k for k in range(10)] + [1000]
-    for c in workloads.CONFIGS.values():
+    for key, c in workloads.CONFIGS.items():
         t = c["record_times"]
-        assert all(b > a for a, b in zip(t, t[1:])) and t[0] >= 1 and t[-1] == c["n_mcs"]
+        assert all(b > a for a, b in zip(t, t[1:])) and t[0] >= 1 and t[-1] <= c["n_mcs"]
+        if str(key).startswith("paper-"):
+            assert t == workloads.eq7_times(c["n_mcs"])     # Eq. 7
+        else:
+            assert t[-1] == c["n_mcs"]
+
+
+def test_eq7_sampling_times():
+    """t_0 = 30, t_{i+1} = 1.05 t_i; "260 data sampling events" up to 10^7 MCS - the integer rule
+    gives 270 (the first steps advance by 1 where 1.05 t rounds back to t)."""
+    t = workloads.eq7_times(10**7)
+    assert t[0] == 30 and t[1] == 31 and all(b > a for a, b in zip(t, t[1:]))
+    assert 255 <= len(t) <= 275
+    big = [x for x in t if x > 1000]
+    assert all(abs(b / a - 1.05) < 0.002 for a, b in zip(big, big[1:]))
 
 
 def test_configs_match_baseline_json_sizes():

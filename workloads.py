@@ -29,6 +29,16 @@ _T50_1E5 = [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 13, 17, 21, 27, 34, 43, 54, 69, 8
             24421, 30888, 39069, 49417, 62506, 79060, 100000]
 _T20_1E3 = [1, 2, 3, 4, 5, 6, 9, 13, 18, 26, 38, 55, 78, 113, 162, 234, 336, 483, 695, 1000]
 
+def eq7_times(T: int, t0: int = 30, factor: float = 1.05) -> list[int]:
+    """The paper's sampling times, Eq. 7: t_0 = 30, t_{i+1} = 1.05 t_i, made integer and strictly
+    increasing: t_{i+1} = max(t_i + 1, floor(1.05 t_i)); times beyond T are dropped."""
+    ts, t = [], t0
+    while t <= T:
+        ts.append(t)
+        t = max(t + 1, int(math.floor(t * factor)))
+    return ts
+
+
 # BASELINE.json `configs`[0..4]  (numbered 1..5 as in SURVEY.md §8(d)).
 CONFIGS = {
     1: dict(name="config1_kpz_L64_S16_p1", kind="kpz", L=64, S=16, p=1.0, q=0.0, disorder=None, n_mcs=1000,
@@ -48,6 +58,23 @@ CONFIGS = {
                     disorder=None, n_mcs=1000, record_times=_T20_1E3, seed=4, path=2),
     "4-aux-ii": dict(name="config4aux2_stream_L2p32_p075_q025", kind="kpz", L=1 << 32, S=1, p=0.75, q=0.25,
                      disorder=None, n_mcs=200, record_times=[1, 2, 4, 8, 16, 32, 64, 128, 200], seed=4, path=2),
+    # the paper's own parameter sets on the same kernels: TASEP p=0.8, q=0, strict
+    # even/odd alternation (offset_mode 1), Eq. 7 sampling.  "paper-1024x30" is the launch the paper times (30
+    # realisations of L=1024 to 10^6 MCS in 4.2 s on a Quadro FX 5800 = 7.3 GSU/s); "paper-1024-fill" is the same ring
+    # with enough realisations to fill a B200 (2 warps per SMSP, 8 rings per warp).
+    "paper-1024x30": dict(name="paper_tasep_L1024_S30_p08", kind="kpz", L=1024, S=30, p=0.8, q=0.0, disorder=None,
+                          n_mcs=1_000_000, record_times=eq7_times(1_000_000), seed=6, offset_mode=1,
+                          paper_gsu=30 * 1024 * 1e6 / 4.2 / 1e9),
+    "paper-1024-fill": dict(name="paper_tasep_L1024_S9472_p08", kind="kpz", L=1024, S=9472, p=0.8, q=0.0,
+                            disorder=None, n_mcs=10_000, record_times=eq7_times(10_000), seed=6, offset_mode=1),
+    # Q-TASEP (Eq. 8): Q = 0.5, slow sites hop with r p, r = 0.5 (the paper does not state r here)
+    "paper-qtasep-16384": dict(name="paper_qtasep_L16384_S512", kind="kpz", L=16384, S=512, p=0.8, q=0.0,
+                               disorder=(0.5, 0.4, 0.0, 0.0), n_mcs=10_000, record_times=eq7_times(10_000), seed=7,
+                               offset_mode=1),
+    # Q-SSEP: p = q with disorder r = 0.2 on both rates, L = 4096
+    "paper-qssep-4096": dict(name="paper_qssep_L4096_S2048", kind="kpz", L=4096, S=2048, p=0.5, q=0.5,
+                             disorder=(0.5, 0.1, 0.5, 0.1), n_mcs=10_000, record_times=eq7_times(10_000), seed=8,
+                             offset_mode=1),
     # the same two rings on the default (temporally blocked) path
     "4-aux-i-blocked": dict(name="config4aux1_blocked_L2p28_p075_q025", kind="kpz", L=1 << 28, S=1, p=0.75, q=0.25,
                             disorder=None, n_mcs=1000, record_times=_T20_1E3, seed=4),
