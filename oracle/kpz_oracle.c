@@ -16,7 +16,7 @@
  *   KPZ growth ................ effective beta in [0.26,0.36]
  *   two-lane .................. brute-force two-lane master equation, conservation, A-lane == KPZ ring at omega=0
  * PARITY UNPINNED (convention only, fixed by DESIGN.md, no external source): the layout of the uniforms
- * (6 bit-planes + one word per element, §R4), the counter packing / stream tags (§R4), the drawn-offset reading (§R1) beyond
+ * (8 bit-planes + one word per element, §R4), the counter packing / stream tags (§R4), the drawn-offset reading (§R1) beyond
  * its master-equation statistics, two-lane step order (§R12) and profile semantics (§R16).
  */
 #include "kpz_oracle.h"
@@ -75,11 +75,11 @@ int kpzref_philox_call(uint64_t seed, uint32_t tag, uint32_t sample, uint64_t ti
 }
 
 /* the 32-bit uniform of element e of a stream (tag, sample, time key, pass).
- *   - its top KPZREF_PLANE_BITS = 6 bits come from bit-planes: plane b = 0..5 supplies bit 31-b (plane 0 = most
+ *   - its top KPZREF_PLANE_BITS = 8 bits come from bit-planes: plane b = 0..7 supplies bit 31-b (plane 0 = most
  *     significant bit) as bit k = e&31 of word w = (e>>5)&3 of the call with c0 = G = e>>7, plane field b;
- *   - its low 26 bits are the top 26 bits of word 0 of the call with c0 = e itself and plane field 31.
+ *   - its low 24 bits are the top 24 bits of word 0 of the call with c0 = e itself and plane field 31.
  * Still a pure function of (seed, sample, mcs, pass, pair) as north_star asks. */
-#define KPZREF_PLANE_BITS 6u
+#define KPZREF_PLANE_BITS 8u
 #define KPZREF_DEEP_PLANE 31u
 int kpzref_uniform(uint64_t seed, uint32_t tag, uint32_t sample, uint64_t timekey, uint32_t pass,
                    uint64_t element, uint32_t* u) {
@@ -103,7 +103,7 @@ int kpzref_uniform(uint64_t seed, uint32_t tag, uint32_t sample, uint64_t timeke
 }
 
 /* The same uniforms for the first `count` (<= 128) elements of supergroup G at once: the definition
- * above evaluated for e = 128 G .. 128 G + count - 1 with the 6 plane calls made once (tests check
+ * above evaluated for e = 128 G .. 128 G + count - 1 with the 8 plane calls made once (tests check
  * the sweep against kpzref_uniform element by element). */
 static void uniform_block128(uint64_t seed, uint32_t tag, uint32_t sample, uint64_t timekey, uint32_t pass,
                              uint32_t G, int count, uint32_t u[128]) {
