@@ -15,8 +15,8 @@
  *   heights/W^2 ............... flat W^2=1/4, h_{L-1}=2N-L, definition on random lattices
  *   KPZ growth ................ effective beta in [0.26,0.36]
  *   two-lane .................. brute-force two-lane master equation, conservation, A-lane == KPZ ring at omega=0
- * PARITY UNPINNED (convention only, fixed by DESIGN.md, no external source): the layout of the uniforms
- * (8 bit-planes + one word per element, §R4), the counter packing / stream tags (§R4), the drawn-offset reading (§R1) beyond
+ * PARITY UNPINNED (convention only, fixed by DESIGN.md, no external source): the bit-plane layout of
+ * the uniforms (§R4), the counter packing / stream tags (§R4), the drawn-offset reading (§R1) beyond
  * its master-equation statistics, two-lane step order (§R12) and profile semantics (§R16).
  */
 #include "kpz_oracle.h"
@@ -74,51 +74,39 @@ int kpzref_philox_call(uint64_t seed, uint32_t tag, uint32_t sample, uint64_t ti
   return KPZREF_OK;
 }
 
-/* the 32-bit uniform of element e of a stream (tag, sample, time key, pass).
- *   - its top KPZREF_PLANE_BITS = 8 bits come from bit-planes: plane b = 0..7 supplies bit 31-b (plane 0 = most
- *     significant bit) as bit k = e&31 of word w = (e>>5)&3 of the call with c0 = G = e>>7, plane field b;
- *   - its low 24 bits are the top 24 bits of word 0 of the call with c0 = e itself and plane field 31.
- * Still a pure function of (seed, sample, mcs, pass, pair) as north_star asks. */
-#define KPZREF_PLANE_BITS 8u
-#define KPZREF_DEEP_PLANE 31u
+/* DESIGN §R4 (Appendix A-3): the 32-bit uniform of element e.  G = e>>7, word w = (e>>5)&3,
+ * bit k = e&31; plane b supplies bit 31-b (plane 0 = most significant bit). */
 int kpzref_uniform(uint64_t seed, uint32_t tag, uint32_t sample, uint64_t timekey, uint32_t pass,
                    uint64_t element, uint32_t* u) {
-  if (!u || (element >> 32) != 0) return KPZREF_EINVAL;
+  if (!u || (element >> 39) != 0) return KPZREF_EINVAL;
   uint32_t G = (uint32_t)(element >> 7);
   uint32_t w = (uint32_t)((element >> 5) & 3);
   uint32_t k = (uint32_t)(element & 31);
   uint32_t value = 0;
-  uint32_t words[4];
-  for (uint32_t plane = 0; plane < KPZREF_PLANE_BITS; ++plane) {
+  for (uint32_t plane = 0; plane < 32; ++plane) {
+    uint32_t words[4];
     int rc = kpzref_philox_call(seed, tag, sample, timekey, pass, plane, G, words);
     if (rc) return rc;
     uint32_t bit = (words[w] >> k) & 1u;
     value |= bit << (31 - plane);
   }
-  int rc = kpzref_philox_call(seed, tag, sample, timekey, pass, KPZREF_DEEP_PLANE, (uint32_t)element, words);
-  if (rc) return rc;
-  value |= words[0] >> KPZREF_PLANE_BITS;
   *u = value;
   return KPZREF_OK;
 }
 
 /* The same uniforms for the first `count` (<= 128) elements of supergroup G at once: the definition
- * above evaluated for e = 128 G .. 128 G + count - 1 with the 8 plane calls made once (tests check
+ * above evaluated for e = 128 G .. 128 G + count - 1 with the 32 Philox calls made once (tests check
  * the sweep against kpzref_uniform element by element). */
 static void uniform_block128(uint64_t seed, uint32_t tag, uint32_t sample, uint64_t timekey, uint32_t pass,
                              uint32_t G, int count, uint32_t u[128]) {
   memset(u, 0, 128 * sizeof(uint32_t));
-  uint32_t words[4];
-  for (uint32_t plane = 0; plane < KPZREF_PLANE_BITS; ++plane) {
+  for (uint32_t plane = 0; plane < 32; ++plane) {
+    uint32_t words[4];
     kpzref_philox_call(seed, tag, sample, timekey, pass, plane, G, words);
     for (int e = 0; e < count; ++e) {
       uint32_t bit = (words[e >> 5] >> (e & 31)) & 1u;
       u[e] |= bit << (31 - plane);
     }
-  }
-  for (int e = 0; e < count; ++e) {
-    kpzref_philox_call(seed, tag, sample, timekey, pass, KPZREF_DEEP_PLANE, (G << 7) + (uint32_t)e, words);
-    u[e] |= words[0] >> KPZREF_PLANE_BITS;
   }
 }
 
@@ -199,7 +187,7 @@ int kpzref_create(kpzref_sim** out, int64_t L, int32_t nsamples, double p, doubl
   *out = NULL;
   /* any even L >= 4 (pairs must tile the ring). */
   if (L < 4 || (L & 1) || nsamples < 1 || !valid_prob(p) || !valid_prob(q)) return KPZREF_EINVAL;
-  if (L > ((int64_t)1 << 32)) return KPZREF_EUNSUPPORTED; /* element indices are Philox counter words (§R4) */
+  if (L >= ((int64_t)1 << 38)) return KPZREF_EUNSUPPORTED;
   kpzref_disorder d = {0.0, p, 0.0, q};
   if (disorder) d = *disorder;
   if (!valid_prob(d.prob_slow_p) || !valid_prob(d.p_slow) || !valid_prob(d.prob_slow_q) || !valid_prob(d.q_slow))
