@@ -611,15 +611,20 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   __syncthreads();
 
   // SPW == 1: CTA = sample, thread = unit.  SPW > 1: CTA = one warp = SPW samples, lane = (sample, unit).
-  const int sub = SPW > 1 ? (int)threadIdx.x / U : 0;
-  const int s = SPW > 1 ? (int)blockIdx.x * SPW + sub : (int)blockIdx.x;
-  const int u = SPW > 1 ? (int)threadIdx.x % U : (int)threadIdx.x;
-  const int lane0 = SPW > 1 ? sub * U : 0;  // first lane of this sample
-  const bool active = u < U && s < D.S;
+  int sub = 0, s = (int)blockIdx.x, u = (int)threadIdx.x, lane0 = 0;  // lane0 = first lane of this sample
+  bool active = u < U;
+  if constexpr (SPW > 1) {
+    sub = (int)threadIdx.x / U;
+    s = (int)blockIdx.x * SPW + sub;
+    u = (int)threadIdx.x % U;
+    lane0 = sub * U;
+    active = s < D.S;
+  }
   Ctx c;
   c.un.nw = !active ? 0 : (PARTIAL ? min(4, PW - 4 * u) : 4);
   c.un.nxt = lane0 + ((u + 1 >= U) ? 0 : u + 1);
   c.un.prv = lane0 + ((u == 0) ? U - 1 : u - 1);
+  if (!SINGLE_WARP) asm volatile("" : "+r"(c.un.nxt), "+r"(c.un.prv));  // measured: +3.5 % on 2-warp rings, -5 % on 1-warp
   c.gs = (uint32_t)(D.first_sample + s);
   c.G = (uint32_t)u;
   c.parity = 0;
@@ -656,7 +661,7 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   const long long t_end = A.t0 + A.n_mcs;
   long long m = A.t0;
   auto draw_offsets = [&]() {
-    if (SPW == 1) {
+    if constexpr (SPW == 1) {
       c.offbits = draw_offsets16(D.keys, c.gs, m);
     } else {
 #pragma unroll 1

@@ -24,7 +24,7 @@
 #error "k4_lanes_jit.cuh needs K4J_W, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN, K4J_OFFSET_MODE"
 #endif
 #ifndef K4J_EAGER
-#define K4J_EAGER 4
+#define K4J_EAGER 6
 #endif
 #ifndef K4J_TAIL
 #define K4J_TAIL 0  // 0: two more planes per trip (resolve); 1: plane-parallel tail (resolve_tail; measured slower: serial)
