@@ -33,7 +33,14 @@
 #endif
 #endif
 #ifndef K1J_EAGER
-#define K1J_EAGER 6  // GENERAL path: planes drawn one MCS ahead; deeper planes are evaluated lazily
+#define K1J_EAGER 8  // GENERAL path: planes drawn one MCS ahead; deeper planes are evaluated lazily (6: -5 %, 10: -3 %)
+#endif
+#ifndef K1J_TRIP  // GENERAL path: planes per lazy trip
+#if defined(K1J_TILE) || defined(K1J_STREAM)
+#define K1J_TRIP 1  // many warps per SM: pipe-bound, never draw a plane that may not be needed (config 4: +5 %)
+#else
+#define K1J_TRIP 2  // 1.7 warps per SMSP: latency-bound, two independent calls per trip (p = 0.8 at L = 1024: +5 %)
+#endif
 #endif
 #ifndef K1J_PW
 #error "k1_sweep_jit.cuh needs K1J_PW, K1J_T0..3, K1J_DIS, K1J_OFFSET_MODE"
@@ -189,26 +196,26 @@ __device__ __forceinline__ void general_flips(uint32_t (&lt)[4], const uint32_t 
   if (NEAG < NPS) {
     const unsigned alive = __activemask();  // the streamed pass kernel's last warp may be partly retired
 #pragma unroll 1
-    for (int pl = NEAG; pl < NPS; pl += 2) {
+    for (int pl = NEAG; pl < NPS; pl += K1J_TRIP) {
       if (!__any_sync(alive, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u)) break;
-      const int pl1 = pl + 1 < 32 ? pl + 1 : 31;
-      const uint4 v0 = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)pl << 22), K);
-      const uint4 v1 = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)pl1 << 22), K);
-      const uint32_t R0[4] = {v0.x, v0.y, v0.z, v0.w};
-      const uint32_t R1[4] = {v1.x, v1.y, v1.z, v1.w};
-      const uint32_t s0 = 31 - pl, s1 = 31 - pl1;
-      const bool second = pl + 1 < NPS;
+      uint32_t R[K1J_TRIP][4];
 #pragma unroll
-      for (int w = 0; w < 4; ++w) {
-        uint32_t tb = class_mask(a[w], spa[w], sqb[w], (uint32_t)(T0 >> s0) & 1u, (uint32_t)(T1 >> s0) & 1u,
-                                 (uint32_t)(T2 >> s0) & 1u, (uint32_t)(T3 >> s0) & 1u);
-        lt[w] |= eq[w] & tb & ~R0[w];
-        eq[w] &= ~(R0[w] ^ tb);
-        if (second) {
-          tb = class_mask(a[w], spa[w], sqb[w], (uint32_t)(T0 >> s1) & 1u, (uint32_t)(T1 >> s1) & 1u,
-                          (uint32_t)(T2 >> s1) & 1u, (uint32_t)(T3 >> s1) & 1u);
-          lt[w] |= eq[w] & tb & ~R1[w];
-          eq[w] &= ~(R1[w] ^ tb);
+      for (int t = 0; t < K1J_TRIP; ++t) {  // independent calls: their rounds interleave
+        const int q = pl + t < 32 ? pl + t : 31;
+        const uint4 v = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)q << 22), K);
+        R[t][0] = v.x; R[t][1] = v.y; R[t][2] = v.z; R[t][3] = v.w;
+      }
+#pragma unroll
+      for (int t = 0; t < K1J_TRIP; ++t) {
+        if (pl + t < NPS) {
+          const uint32_t sh = 31 - (pl + t);
+#pragma unroll
+          for (int w = 0; w < 4; ++w) {
+            const uint32_t tb = class_mask(a[w], spa[w], sqb[w], (uint32_t)(T0 >> sh) & 1u, (uint32_t)(T1 >> sh) & 1u,
+                                           (uint32_t)(T2 >> sh) & 1u, (uint32_t)(T3 >> sh) & 1u);
+            lt[w] |= eq[w] & tb & ~R[t][w];
+            eq[w] &= ~(R[t][w] ^ tb);
+          }
         }
       }
     }
