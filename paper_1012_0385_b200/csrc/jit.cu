@@ -9,6 +9,7 @@
 #include <cuda_runtime.h>
 #include <nvrtc.h>
 
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <map>
@@ -56,8 +57,12 @@ int jit_compile(const char* source, const char* entry, const std::vector<std::st
     hnames.push_back(e.name);
     htexts.push_back(e.text);
   }
+  // name the program by its path at build time when that file still exists (ncu --import-source, -lineinfo)
+  std::string pname = std::string(kEmbeddedDir) + "/" + src->name;
+  if (FILE* f = std::fopen(pname.c_str(), "r")) std::fclose(f);
+  else pname = src->name;
   nvrtcProgram prog;
-  nvrtcResult r = nvrtcCreateProgram(&prog, src->text, src->name, (int)hnames.size(), htexts.data(), hnames.data());
+  nvrtcResult r = nvrtcCreateProgram(&prog, src->text, pname.c_str(), (int)hnames.size(), htexts.data(), hnames.data());
   if (r != NVRTC_SUCCESS) return fail(KPZ_ECUDA, "nvrtcCreateProgram: %s", nvrtcGetErrorString(r));
   std::vector<std::string> opts = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo", "-DKPZ_JIT=1"};
   for (const std::string& d : defines) opts.push_back("-D" + d);

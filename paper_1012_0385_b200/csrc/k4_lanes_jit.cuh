@@ -26,6 +26,9 @@
 #ifndef K4J_EAGER
 #define K4J_EAGER 6
 #endif
+#ifndef K4J_TRIP
+#define K4J_TRIP 2  // planes per lazy trip
+#endif
 #ifndef K4J_TAIL
 #define K4J_TAIL 0  // 0: two more planes per trip (resolve); 1: plane-parallel tail (resolve_tail; measured slower: serial)
 #endif
@@ -72,20 +75,24 @@ __device__ __forceinline__ void plane_step(uint32_t (&lt)[4], uint32_t (&eq)[4],
 }
 
 // Finish U < T for the still-undecided elements `eq` of supergroup G of stream c3 (tag | pass | time_hi), starting at
-// plane pl0.  Two planes per trip, trips are warp-uniform (a warp leaves when none of its lanes is undecided).
+// plane pl0.  K4J_TRIP planes per trip, trips are warp-uniform (a warp leaves when none of its lanes is undecided).
 template <uint64_t T>
 __device__ __forceinline__ void resolve(uint32_t (&lt)[4], uint32_t (&eq)[4], const PhiloxKeys& K, uint32_t G,
                                         uint32_t gs, uint32_t tlo, uint32_t c3, int pl0) {
   constexpr int NP = planes_of(T);
 #pragma unroll 1
-  for (int pl = pl0; pl < NP; pl += 2) {
+  for (int pl = pl0; pl < NP; pl += K4J_TRIP) {
     if (!__any_sync(FULL, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u)) break;
-    const uint4 v0 = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)pl << 22), K);
-    const uint4 v1 = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)(pl + 1 < 32 ? pl + 1 : 31) << 22), K);
-    const uint32_t R0[4] = {v0.x, v0.y, v0.z, v0.w};
-    const uint32_t R1[4] = {v1.x, v1.y, v1.z, v1.w};
-    plane_step<T>(lt, eq, R0, pl);
-    if (pl + 1 < NP) plane_step<T>(lt, eq, R1, pl + 1);
+    uint32_t R[K4J_TRIP][4];
+#pragma unroll
+    for (int t = 0; t < K4J_TRIP; ++t) {  // independent calls: their rounds interleave
+      const int q = pl + t < 32 ? pl + t : 31;
+      const uint4 v = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)q << 22), K);
+      R[t][0] = v.x; R[t][1] = v.y; R[t][2] = v.z; R[t][3] = v.w;
+    }
+#pragma unroll
+    for (int t = 0; t < K4J_TRIP; ++t)
+      if (pl + t < NP) plane_step<T>(lt, eq, R[t], pl + t);
   }
 }
 

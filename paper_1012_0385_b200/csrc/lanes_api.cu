@@ -90,6 +90,10 @@ std::vector<std::string> k4_jit_defines(const LanesDev& D) {
     snprintf(buf, sizeof buf, "K4J_EAGER=%d", atoi(v));
     d.push_back(buf);
   }
+  if (const char* v = std::getenv("KPZ_B200_K4_TRIP")) {  // tuning knob: planes per lazy trip
+    snprintf(buf, sizeof buf, "K4J_TRIP=%d", atoi(v));
+    d.push_back(buf);
+  }
   if (const char* v = std::getenv("KPZ_B200_K4_TAIL")) {  // tuning knob: 0 = plane pairs per trip, 1 = plane-parallel tail
     snprintf(buf, sizeof buf, "K4J_TAIL=%d", atoi(v));
     d.push_back(buf);
