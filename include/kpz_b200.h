@@ -84,6 +84,11 @@ int kpz_run(kpz_sim*, int64_t n_mcs);
 
 int kpz_time(const kpz_sim*, int64_t* t); /* MCS done so far (host value; no sync) */
 
+/* Checkpoint restore: continue from MCS count t (0 <= t < 2^54).  Every random number is a function of (seed,
+ * sample, MCS index, ...) (§R10), so the lattice (kpz_set_lattice), the disorder tags and t are the whole
+ * state.  Drops the record-time list and the captured records; host-side only (no sync). */
+int kpz_set_time(kpz_sim*, int64_t t);
+
 /* Back to the state right after kpz_create: flat lattice, disorder tags regenerated from the seed, t = 0,
  * captured records dropped (the record-time list is kept).  Enqueues the initialisation kernels; async. */
 int kpz_reset(kpz_sim*);
@@ -120,6 +125,8 @@ int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, doubl
 int lanes_set_record_times(lanes_sim*, const int64_t* t, int32_t nt);
 int lanes_run(lanes_sim*, int64_t n_mcs);
 int lanes_time(const lanes_sim*, int64_t* t);
+/* As kpz_set_time; restore lanes and turning-point mask with lanes_set_state.  Hop counters and profile keep going. */
+int lanes_set_time(lanes_sim*, int64_t t);
 int lanes_reset(lanes_sim*); /* as kpz_reset: initial occupations, epoch-0 turning points, zero counters; async */
 /* Occupations of lanes A, B and the current turning-point mask (device, natural layout, any may be NULL). Async. */
 int lanes_state(lanes_sim*, uint32_t* d_a, uint32_t* d_b, uint32_t* d_turn);

@@ -389,6 +389,16 @@ int kpzref_run_rsu(kpzref_sim* sim, int64_t n_mcs) {
   return KPZREF_OK;
 }
 
+/* Checkpoint restore: continue from MCS count t; with the lattice (kpzref_set_lattice) this is the whole
+ * state, because every random number is a function of (seed, sample, m, ...).  Drops the record list. */
+int kpzref_set_time(kpzref_sim* sim, int64_t t) {
+  if (!sim || t < 0 || ((uint64_t)t >> 54) != 0) return KPZREF_EINVAL;
+  int rc = kpzref_set_record_times(sim, NULL, 0);
+  if (rc) return rc;
+  sim->t = t;
+  return KPZREF_OK;
+}
+
 int kpzref_time(const kpzref_sim* sim, int64_t* t) {
   if (!sim || !t) return KPZREF_EINVAL;
   *t = sim->t;
@@ -678,6 +688,16 @@ int lanesref_run(lanesref_sim* sim, int64_t n_mcs) {
       sim->nrec++;
     }
   }
+  return KPZREF_OK;
+}
+
+/* As kpzref_set_time; the caller restores lanes and turning-point mask with lanesref_set_state.  Hop counters,
+ * profile counts and the snapshot count keep their values. */
+int lanesref_set_time(lanesref_sim* sim, int64_t t) {
+  if (!sim || t < 0 || ((uint64_t)t >> 54) != 0) return KPZREF_EINVAL;
+  int rc = lanesref_set_record_times(sim, NULL, 0);
+  if (rc) return rc;
+  sim->t = t;
   return KPZREF_OK;
 }
 

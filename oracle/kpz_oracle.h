@@ -80,6 +80,7 @@ int kpzref_set_record_times(kpzref_sim*, const int64_t* t, int32_t nt); /* stric
 int kpzref_run(kpzref_sim*, int64_t n_mcs);      /* two-sub-lattice SCA sweep, n_mcs Monte-Carlo steps */
 int kpzref_run_rsu(kpzref_sim*, int64_t n_mcs);  /* oracle-only: random-sequential updates */
 int kpzref_time(const kpzref_sim*, int64_t* t);
+int kpzref_set_time(kpzref_sim*, int64_t t); /* checkpoint restore: continue from MCS count t; drops the record list */
 int kpzref_lattice(kpzref_sim*, uint32_t* words);            /* [S][L/32 rounded up]; bit (i&31) of word i>>5 = n_i */
 int kpzref_set_lattice(kpzref_sim*, const uint32_t* words);
 int kpzref_disorder_masks(kpzref_sim*, uint32_t* slow_p, uint32_t* slow_q); /* same layout; either may be NULL */
@@ -97,6 +98,7 @@ int lanesref_create(lanesref_sim** out, int64_t L, int32_t nsamples, double p_a,
 int lanesref_set_record_times(lanesref_sim*, const int64_t* t, int32_t nt);
 int lanesref_run(lanesref_sim*, int64_t n_mcs);
 int lanesref_time(const lanesref_sim*, int64_t* t);
+int lanesref_set_time(lanesref_sim*, int64_t t);
 int lanesref_state(lanesref_sim*, uint32_t* a, uint32_t* b, uint32_t* turn); /* [S][L/32 rounded up], any may be NULL */
 int lanesref_set_state(lanesref_sim*, const uint32_t* a, const uint32_t* b, const uint32_t* turn); /* NULL = leave */
 int lanesref_currents(lanesref_sim*, int32_t* nt, int64_t* t, int64_t* j_a, int64_t* j_b, int64_t* n_a,

@@ -130,6 +130,9 @@ class KpzRef:
         _chk(lib().kpzref_time(self._h, C.byref(t)), "kpzref_time")
         return int(t.value)
 
+    def set_time(self, t):
+        _chk(lib().kpzref_set_time(self._h, C.c_int64(t)), "kpzref_set_time")
+
     def lattice(self):
         w = np.zeros((self.S, self.nw), dtype=np.uint32)
         _chk(lib().kpzref_lattice(self._h, _p(w, C.c_uint32)), "kpzref_lattice")
@@ -218,6 +221,9 @@ class LanesRef:
         t = C.c_int64()
         _chk(lib().lanesref_time(self._h, C.byref(t)), "lanesref_time")
         return int(t.value)
+
+    def set_time(self, t):
+        _chk(lib().lanesref_set_time(self._h, C.c_int64(t)), "lanesref_set_time")
 
     def state(self):
         a = np.zeros((self.S, self.nw), dtype=np.uint32)

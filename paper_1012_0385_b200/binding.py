@@ -46,6 +46,7 @@ SIGNATURES = {
     "kpz_set_record_times": (C.c_int, [_P, C.POINTER(C.c_int64), C.c_int32]),
     "kpz_run": (C.c_int, [_P, C.c_int64]),
     "kpz_time": (C.c_int, [_P, C.POINTER(C.c_int64)]),
+    "kpz_set_time": (C.c_int, [_P, C.c_int64]),
     "kpz_reset": (C.c_int, [_P]),
     "kpz_lattice": (C.c_int, [_P, _P]),
     "kpz_set_lattice": (C.c_int, [_P, _P]),
@@ -60,6 +61,7 @@ SIGNATURES = {
     "lanes_set_record_times": (C.c_int, [_P, C.POINTER(C.c_int64), C.c_int32]),
     "lanes_run": (C.c_int, [_P, C.c_int64]),
     "lanes_time": (C.c_int, [_P, C.POINTER(C.c_int64)]),
+    "lanes_set_time": (C.c_int, [_P, C.c_int64]),
     "lanes_reset": (C.c_int, [_P]),
     "lanes_state": (C.c_int, [_P, _P, _P, _P]),
     "lanes_set_state": (C.c_int, [_P, _P, _P, _P]),
@@ -187,6 +189,11 @@ class KpzSim:
         _chk(load_library().kpz_time(self._h, C.byref(t)), "kpz_time")
         return int(t.value)
 
+    def set_time(self, t):
+        """Checkpoint restore: continue from MCS count t (drops the record list)."""
+        _chk(load_library().kpz_set_time(self._h, int(t)), "kpz_set_time")
+        self._nt = 0
+
     def set_record_times(self, t):
         t = _times(t)
         self._nt = len(t)
@@ -277,6 +284,11 @@ class LanesSim:
         t = C.c_int64()
         _chk(load_library().lanes_time(self._h, C.byref(t)), "lanes_time")
         return int(t.value)
+
+    def set_time(self, t):
+        """Checkpoint restore: continue from MCS count t (drops the record list)."""
+        _chk(load_library().lanes_set_time(self._h, int(t)), "lanes_set_time")
+        self._nt = 0
 
     def set_record_times(self, t):
         t = _times(t)

@@ -609,6 +609,14 @@ int kpz_time(const kpz_sim* sim, int64_t* t) {
   return KPZ_OK;
 }
 
+int kpz_set_time(kpz_sim* sim, int64_t t) {
+  if (!sim || t < 0 || ((uint64_t)t >> 54) != 0) return fail(KPZ_EINVAL, "need 0 <= t < 2^54");
+  sim->t = t;
+  sim->rec_times.clear();
+  sim->nrec = 0;
+  return KPZ_OK;
+}
+
 int kpz_set_record_times(kpz_sim* sim, const int64_t* t, int32_t nt) {
   if (!sim || nt < 0 || (nt > 0 && !t)) return fail(KPZ_EINVAL, "bad record-time list");
   if (nt > sim->max_records) return fail(KPZ_ENOMEM, "%d record times but max_records=%d", nt, sim->max_records);

@@ -20,6 +20,7 @@ struct lanes_sim {
   long long* rec_t = nullptr;
   long long* rec = nullptr;  // [4][max_records][S] (plane stride = nt * S of the current list)
   int64_t t = 0;
+  int64_t nsnap = 0;  // profile snapshots taken (epoch ends passed by lanes_run)
   std::vector<int64_t> rec_times;
   int32_t nrec = 0;
   char* base = nullptr;   // workspace start
@@ -129,6 +130,7 @@ int lanes_reset(lanes_sim* sim) {
   int rc = lanes_init_state(sim);
   if (rc) return rc;
   sim->t = 0;
+  sim->nsnap = 0;
   sim->nrec = 0;
   return KPZ_OK;
 }
@@ -238,6 +240,14 @@ int lanes_time(const lanes_sim* sim, int64_t* t) {
   return KPZ_OK;
 }
 
+int lanes_set_time(lanes_sim* sim, int64_t t) {
+  if (!sim || t < 0 || ((uint64_t)t >> 54) != 0) return fail(KPZ_EINVAL, "need 0 <= t < 2^54");
+  sim->t = t;
+  sim->rec_times.clear();
+  sim->nrec = 0;
+  return KPZ_OK;
+}
+
 int lanes_set_record_times(lanes_sim* sim, const int64_t* t, int32_t nt) {
   if (!sim || nt < 0 || (nt > 0 && !t)) return fail(KPZ_EINVAL, "bad record-time list");
   if (nt > sim->max_records) return fail(KPZ_ENOMEM, "%d record times but max_records=%d", nt, sim->max_records);
@@ -284,6 +294,7 @@ int lanes_run(lanes_sim* sim, int64_t n_mcs) {
     else lanes_k4_kernel<false, false><<<sim->S, block, 0, sim->stream>>>(D, A);
   }
   KPZ_LAUNCH_CHECK("lanes_k4_kernel");
+  if (D.period > 0) sim->nsnap += (sim->t + n_mcs) / D.period - sim->t / D.period;
   sim->t += n_mcs;
   while (sim->nrec < nt && sim->rec_times[sim->nrec] <= sim->t) sim->nrec++;
   return KPZ_OK;
@@ -341,7 +352,7 @@ int lanes_profile(lanes_sim* sim, uint32_t* d_occ_a, uint32_t* d_occ_b, int64_t*
   if (d_occ_a) KPZ_CUDA_CHECK(cudaMemcpyAsync(d_occ_a, sim->dev.occA, bytes, cudaMemcpyDeviceToDevice, sim->stream));
   if (d_occ_b) KPZ_CUDA_CHECK(cudaMemcpyAsync(d_occ_b, sim->dev.occB, bytes, cudaMemcpyDeviceToDevice, sim->stream));
   KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
-  if (nsnap) *nsnap = sim->dev.period > 0 ? sim->t / sim->dev.period : 0;
+  if (nsnap) *nsnap = sim->nsnap;
   return KPZ_OK;
 }
 

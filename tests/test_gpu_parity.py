@@ -470,3 +470,68 @@ def test_k1_small_rings_packed_per_warp(K, L, S):
     run_both_kpz(K, L, S, 0.8, 0.0, seed=42, times=[5, 33], chunks=[33])
     run_both_kpz(K, L, S, 0.5, 0.5, disorder=(0.5, 0.1, 0.5, 0.1), seed=43, times=[9], chunks=[9], offset_mode=1)
     run_both_kpz(K, L, S, 1.0, 0.0, disorder=(0.1, 0.5, 0.0, 0.0), seed=44, times=[20], chunks=[20], first_sample=7)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# checkpoint restore and time keys beyond 32 bits (the paper runs t_max > 2^32)
+# ---------------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("path,L", [(1, 8192 + 64), (1, 1024), (2, 65536), (3, 65536)])
+def test_kpz_time_keys_beyond_32_bits(K, path, L):
+    """set_time moves both implementations to t = 2^32 - 7: the next MCS indices cross the 32-bit boundary of the
+    Philox time key (c2 wraps, c3 gains its first high bit) and a 16-MCS offset batch."""
+    t0, n = (1 << 32) - 7, 21
+    rng = np.random.default_rng(L)
+    start = R.pack_sites((rng.random((2, L)) < 0.5).astype(np.uint8))
+    ref = R.KpzRef(L, 2, 0.75, 0.25, seed=51)
+    gpu = K.KpzSim(L, 2, 0.75, 0.25, seed=51, path=path, max_records=2)
+    for sim, lat in ((ref, start), (gpu, K.words_from_numpy(start, "cuda"))):
+        sim.set_lattice(lat)
+        sim.set_time(t0)
+        sim.set_record_times([t0 + 3, t0 + n])
+        sim.run(n)
+    assert gpu.time == ref.time == t0 + n
+    assert np.array_equal(K.words_to_numpy(gpu.lattice()), ref.lattice())
+    g, r = gpu.roughness(), ref.roughness()
+    assert list(g["t"]) == list(r["t"]) == [t0 + 3, t0 + n]
+    assert np.array_equal(g["sum_h"], r["sum_h"]) and np.array_equal(g["sum_h2"], r["sum_h2"])
+    # the streams really changed with the high bit: the same run from t = 0 ends elsewhere
+    again = K.KpzSim(L, 2, 0.75, 0.25, seed=51, path=path, max_records=1)
+    again.set_lattice(K.words_from_numpy(start, "cuda"))
+    again.run(n)
+    assert not np.array_equal(K.words_to_numpy(again.lattice()), ref.lattice())
+
+
+def test_checkpoint_restore_reproduces_an_uninterrupted_run(K):
+    L, S, a, b = 4096 + 64, 3, 37, 29
+    full = K.KpzSim(L, S, 0.8, 0.1, disorder=(0.3, 0.2, 0.3, 0.05), seed=52, max_records=1)
+    full.run(a + b)
+    part = K.KpzSim(L, S, 0.8, 0.1, disorder=(0.3, 0.2, 0.3, 0.05), seed=52, max_records=1)
+    part.run(a)
+    saved = part.lattice().clone()
+    fresh = K.KpzSim(L, S, 0.8, 0.1, disorder=(0.3, 0.2, 0.3, 0.05), seed=52, max_records=1)
+    fresh.set_lattice(saved)
+    fresh.set_time(a)
+    fresh.run(b)
+    assert np.array_equal(K.words_to_numpy(fresh.lattice()), K.words_to_numpy(full.lattice()))
+
+
+def test_lanes_time_keys_beyond_32_bits(K):
+    """Two-lane model from t = 2^32 + 95 with period 100: crosses an epoch boundary (turning points redrawn with a
+    33-bit epoch-free time key, profile snapshot) right after the restore."""
+    t0, n, L = (1 << 32) + 95, 12, 4096
+    ref = R.LanesRef(L, 2, 1.0, 1.0, 0.3, 0.05, 100, 0.1, seed=53)
+    gpu = K.LanesSim(L, 2, 1.0, 1.0, 0.3, 0.05, 100, 0.1, seed=53, max_records=1)
+    for sim in (ref, gpu):
+        sim.set_time(t0)
+        sim.set_record_times([t0 + n])
+        sim.run(n)
+    for g, r in zip(gpu.state(), ref.state()):
+        assert np.array_equal(K.words_to_numpy(g), r)
+    gc, rc = gpu.currents(), ref.currents()
+    for k in ("j_a", "j_b", "n_a", "n_b"):
+        assert np.array_equal(gc[k], rc[k]), k
+    ga, gb, gn = gpu.profile()
+    ra, rb, rn = ref.profile()
+    assert gn == rn == 1
+    assert np.array_equal(K.words_to_numpy(ga), ra) and np.array_equal(K.words_to_numpy(gb), rb)

@@ -449,3 +449,25 @@ def test_kpz_growth_exponent_window():
     beta = 0.5 * slope
     assert 0.26 <= beta <= 0.36, beta
     assert np.all(np.diff(w2) > 0)                # roughening, no saturation yet (t << L^{3/2})
+
+
+def test_set_time_restores_a_checkpoint_exactly():
+    """lattice + t (+ quenched tags, regenerated from the seed) are the whole state."""
+    L, S, a, b = 192, 3, 23, 31
+    full = R.KpzRef(L, S, 0.8, 0.1, disorder=(0.3, 0.2, 0.3, 0.05), seed=61)
+    full.set_record_times([a + b])
+    full.run(a + b)
+    part = R.KpzRef(L, S, 0.8, 0.1, disorder=(0.3, 0.2, 0.3, 0.05), seed=61)
+    part.run(a)
+    fresh = R.KpzRef(L, S, 0.8, 0.1, disorder=(0.3, 0.2, 0.3, 0.05), seed=61)
+    fresh.set_lattice(part.lattice())
+    fresh.set_time(a)
+    fresh.set_record_times([a + b])
+    fresh.run(b)
+    assert fresh.time == a + b
+    assert np.array_equal(fresh.lattice(), full.lattice())
+    assert np.array_equal(fresh.roughness()["sum_h2"], full.roughness()["sum_h2"])
+    with pytest.raises(R.OracleError):
+        fresh.set_time(-1)
+    with pytest.raises(R.OracleError):
+        fresh.set_time(1 << 54)
