@@ -488,10 +488,13 @@ struct lanesref_sim {
   int32_t offset_mode;
   uint64_t seed;
   uint64_t T_pa, T_pb, T_turn, T_omega;
+  uint64_t T_w0;        /* crossing threshold at sites whose flag is 0 (0 for the turning-point model, §R13) */
+  int32_t independent;  /* 1: separate flags v_i for B->A, 0: one flag set for both directions */
   int64_t period;
   uint8_t* A;    /* [S][L] lane A occupation (particles hop right) */
   uint8_t* B;    /* [S][L] lane B occupation (particles hop left) */
-  uint8_t* turn; /* [S][L] turning-point flags of the current epoch */
+  uint8_t* turn; /* [S][L] flags u_i of the current epoch (turning points; A->B, and B->A unless independent) */
+  uint8_t* turn_v; /* [S][L] flags v_i for B->A when independent (else NULL) */
   int64_t t;
   int64_t* J_A;  /* [S] hops in lane A so far */
   int64_t* J_B;  /* [S] hops in lane B so far */
@@ -509,6 +512,7 @@ int lanesref_destroy(lanesref_sim* sim) {
   free(sim->A);
   free(sim->B);
   free(sim->turn);
+  free(sim->turn_v);
   free(sim->J_A);
   free(sim->J_B);
   free(sim->occ_A);
@@ -522,12 +526,25 @@ int lanesref_destroy(lanesref_sim* sim) {
   return KPZREF_OK;
 }
 
+/* DESIGN §R13 (turning-point model of configs[4]): crossing probability omega at flagged sites, 0 elsewhere, one
+ * flag set for both directions. */
 int lanesref_create(lanesref_sim** out, int64_t L, int32_t nsamples, double p_a, double p_b, double rho0,
                     double turn_prob, int64_t turn_period, double omega, uint64_t seed, const kpzref_options* opt) {
+  return lanesref_create_crossing(out, L, nsamples, p_a, p_b, rho0, turn_prob, omega, 0.0, 0, turn_period, seed, opt);
+}
+
+/* DESIGN §R18 (the paper's own two-lane model): every site can be crossed; the crossing probability
+ * is w_flagged where the site's flag is set and w_unflagged elsewhere ("the crossing probability is reduced from 0.8
+ * to 0.2" at flagged sites, flags set with probability 1/2); with independent = 1 the directions A->B and B->A have
+ * separate flag sets u_i (stream TURN) and v_i (stream TURN_V). */
+int lanesref_create_crossing(lanesref_sim** out, int64_t L, int32_t nsamples, double p_a, double p_b, double rho0,
+                             double turn_prob, double omega, double w_unflagged, int32_t independent,
+                             int64_t turn_period, uint64_t seed, const kpzref_options* opt) {
   if (!out) return KPZREF_EINVAL;
   *out = NULL;
   if (L < 4 || (L & 1) || nsamples < 1 || turn_period < 0) return KPZREF_EINVAL;
-  if (!valid_prob(p_a) || !valid_prob(p_b) || !valid_prob(rho0) || !valid_prob(turn_prob) || !valid_prob(omega))
+  if (!valid_prob(p_a) || !valid_prob(p_b) || !valid_prob(rho0) || !valid_prob(turn_prob) || !valid_prob(omega) ||
+      !valid_prob(w_unflagged) || (independent != 0 && independent != 1))
     return KPZREF_EINVAL;
   if (L >= ((int64_t)1 << 31)) return KPZREF_EUNSUPPORTED;
   kpzref_options o = {0, 0, 0};
@@ -545,15 +562,18 @@ int lanesref_create(lanesref_sim** out, int64_t L, int32_t nsamples, double p_a,
   kpzref_threshold(p_b, &sim->T_pb);
   kpzref_threshold(turn_prob, &sim->T_turn);
   kpzref_threshold(omega, &sim->T_omega);
+  kpzref_threshold(w_unflagged, &sim->T_w0);
+  sim->independent = independent;
   size_t cells = (size_t)nsamples * (size_t)L;
   sim->A = (uint8_t*)malloc(cells);
   sim->B = (uint8_t*)malloc(cells);
   sim->turn = (uint8_t*)malloc(cells);
+  if (independent) sim->turn_v = (uint8_t*)malloc(cells);
   sim->J_A = (int64_t*)calloc((size_t)nsamples, sizeof(int64_t));
   sim->J_B = (int64_t*)calloc((size_t)nsamples, sizeof(int64_t));
   sim->occ_A = (uint32_t*)calloc(cells, sizeof(uint32_t));
   sim->occ_B = (uint32_t*)calloc(cells, sizeof(uint32_t));
-  if (!sim->A || !sim->B || !sim->turn || !sim->J_A || !sim->J_B || !sim->occ_A || !sim->occ_B) {
+  if (!sim->A || !sim->B || !sim->turn || (independent && !sim->turn_v) || !sim->J_A || !sim->J_B || !sim->occ_A || !sim->occ_B) {
     lanesref_destroy(sim);
     return KPZREF_ENOMEM;
   }
@@ -566,6 +586,7 @@ int lanesref_create(lanesref_sim** out, int64_t L, int32_t nsamples, double p_a,
     bernoulli_sites(seed, KPZREF_TAG_INIT_B, gs, 0, T_rho, L, sim->B + (size_t)s * L);
     /* turning-point mask of epoch 0. */
     bernoulli_sites(seed, KPZREF_TAG_TURN, gs, 0, sim->T_turn, L, sim->turn + (size_t)s * L);
+    if (independent) bernoulli_sites(seed, KPZREF_TAG_TURN_V, gs, 0, sim->T_turn, L, sim->turn_v + (size_t)s * L);
   }
   *out = sim;
   return KPZREF_OK;
@@ -630,14 +651,16 @@ static void lanes_inlane_pass(lanesref_sim* sim, int32_t s, uint64_t m, uint32_t
 }
 
 /* Lane changes at turning points (§R13): from -> to at sites with turn = 1. */
-static void lanes_switch(lanesref_sim* sim, int32_t s, uint64_t m, uint32_t tag, uint8_t* from, uint8_t* to) {
+static void lanes_switch(lanesref_sim* sim, int32_t s, uint64_t m, uint32_t tag, uint8_t* from, uint8_t* to,
+                         const uint8_t* flags) {
   const int64_t L = sim->L;
-  const uint8_t* turn = sim->turn + (size_t)s * L;
+  const uint8_t* turn = flags + (size_t)s * L;
   uint32_t gs = (uint32_t)(sim->first_sample + s);
   uint32_t u[128];
   for (int64_t i = 0; i < L; ++i) {
     if ((i & 127) == 0) uniform_block128(sim->seed, tag, gs, m, 0, (uint32_t)(i >> 7), block_count(L, i), u);
-    if (turn[i] && from[i] == 1 && to[i] == 0 && accept(u[i & 127], sim->T_omega)) {
+    /* §R13 / §R18: threshold omega at flagged sites, w_unflagged (0 in the turning-point model) elsewhere */
+    if (from[i] == 1 && to[i] == 0 && accept(u[i & 127], turn[i] ? sim->T_omega : sim->T_w0)) {
       from[i] = 0;
       to[i] = 1;
     }
@@ -656,12 +679,18 @@ int lanesref_run(lanesref_sim* sim, int64_t n_mcs) {
       uint32_t gs = (uint32_t)(sim->first_sample + s);
       /* §R13: positions redrawn at the start of every epoch of `period` MCS (epoch 0 drawn at create). */
       if (sim->period > 0 && m > 0 && m % (uint64_t)sim->period == 0)
+      {
         bernoulli_sites(sim->seed, KPZREF_TAG_TURN, gs, m / (uint64_t)sim->period, sim->T_turn, L,
                         sim->turn + (size_t)s * L);
-      lanes_inlane_pass(sim, s, m, 0);                       /* PAPER.md:261 step 1 */
-      lanes_switch(sim, s, m, KPZREF_TAG_SWITCH_AB, A, B);   /* PAPER.md:262 step 2 */
-      lanes_inlane_pass(sim, s, m, 1);                       /* PAPER.md:263-264 steps 3,4 (closure = pair (L-1,0)) */
-      lanes_switch(sim, s, m, KPZREF_TAG_SWITCH_BA, B, A);   /* PAPER.md:265 step 5 */
+        if (sim->independent)
+          bernoulli_sites(sim->seed, KPZREF_TAG_TURN_V, gs, m / (uint64_t)sim->period, sim->T_turn, L,
+                          sim->turn_v + (size_t)s * L);
+      }
+      const uint8_t* fv = sim->independent ? sim->turn_v : sim->turn;
+      lanes_inlane_pass(sim, s, m, 0);                                  /* PAPER.md:261 step 1 */
+      lanes_switch(sim, s, m, KPZREF_TAG_SWITCH_AB, A, B, sim->turn);   /* PAPER.md:262 step 2, flags u_i */
+      lanes_inlane_pass(sim, s, m, 1);                                  /* PAPER.md:263-264 steps 3,4 (closure = pair (L-1,0)) */
+      lanes_switch(sim, s, m, KPZREF_TAG_SWITCH_BA, B, A, fv);          /* PAPER.md:265 step 5, flags v_i */
     }
     sim->t += 1;
     /* §R16: occupancy profile accumulated at the end of each turning-point epoch. */
@@ -725,6 +754,27 @@ int lanesref_set_state(lanesref_sim* sim, const uint32_t* a, const uint32_t* b, 
     if (a) unpack_bits(a + (size_t)s * nw, sim->L, sim->A + (size_t)s * sim->L);
     if (b) unpack_bits(b + (size_t)s * nw, sim->L, sim->B + (size_t)s * sim->L);
     if (turn) unpack_bits(turn + (size_t)s * nw, sim->L, sim->turn + (size_t)s * sim->L);
+  }
+  return KPZREF_OK;
+}
+
+int lanesref_flags(lanesref_sim* sim, uint32_t* u, uint32_t* v) {
+  if (!sim) return KPZREF_EINVAL;
+  int64_t nw = words_per_sample(sim->L);
+  const uint8_t* fv = sim->independent ? sim->turn_v : sim->turn;
+  for (int32_t s = 0; s < sim->S; ++s) {
+    if (u) pack_bits(sim->turn + (size_t)s * sim->L, sim->L, u + (size_t)s * nw);
+    if (v) pack_bits(fv + (size_t)s * sim->L, sim->L, v + (size_t)s * nw);
+  }
+  return KPZREF_OK;
+}
+
+int lanesref_set_flags(lanesref_sim* sim, const uint32_t* u, const uint32_t* v) {
+  if (!sim || (v && !sim->independent)) return KPZREF_EINVAL; /* one shared set: pass it as u */
+  int64_t nw = words_per_sample(sim->L);
+  for (int32_t s = 0; s < sim->S; ++s) {
+    if (u) unpack_bits(u + (size_t)s * nw, sim->L, sim->turn + (size_t)s * sim->L);
+    if (v) unpack_bits(v + (size_t)s * nw, sim->L, sim->turn_v + (size_t)s * sim->L);
   }
   return KPZREF_OK;
 }

@@ -39,7 +39,8 @@ enum {
   KPZREF_TAG_TURN = 7,      /* turning-point mask per epoch */
   KPZREF_TAG_SWITCH_AB = 8, /* A->B lane change uniforms */
   KPZREF_TAG_SWITCH_BA = 9, /* B->A lane change uniforms */
-  KPZREF_TAG_RSU = 10       /* oracle-only random-sequential mode */
+  KPZREF_TAG_RSU = 10,      /* oracle-only random-sequential mode */
+  KPZREF_TAG_TURN_V = 11    /* flags v_i of the B->A crossings when they are independent of u_i */
 };
 
 typedef struct {
@@ -95,6 +96,14 @@ int kpzref_destroy(kpzref_sim*);
 int lanesref_create(lanesref_sim** out, int64_t L, int32_t nsamples, double p_a, double p_b, double rho0,
                     double turn_prob, int64_t turn_period /* 0 = never redraw */, double omega, uint64_t seed,
                     const kpzref_options* opt);
+/* the paper's own two-lane model - crossing probability omega where the site's flag is set (flags
+ * Bernoulli(turn_prob)), w_unflagged elsewhere; independent = 1: separate flag sets for A->B and B->A. */
+int lanesref_create_crossing(lanesref_sim** out, int64_t L, int32_t nsamples, double p_a, double p_b, double rho0,
+                             double turn_prob, double omega, double w_unflagged, int32_t independent,
+                             int64_t turn_period, uint64_t seed, const kpzref_options* opt);
+/* Flag sets u (A->B) and v (B->A) of the current epoch, natural layout; v == u unless independent.  NULL = skip. */
+int lanesref_flags(lanesref_sim*, uint32_t* u, uint32_t* v);
+int lanesref_set_flags(lanesref_sim*, const uint32_t* u, const uint32_t* v);
 int lanesref_set_record_times(lanesref_sim*, const int64_t* t, int32_t nt);
 int lanesref_run(lanesref_sim*, int64_t n_mcs);
 int lanesref_time(const lanesref_sim*, int64_t* t);

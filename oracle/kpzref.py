@@ -14,7 +14,7 @@ from . import build as _build
 _lib = None
 
 TAGS = dict(PAIR=0, OFFSET=1, SLOW_P=2, SLOW_Q=3, INIT_A=4, INIT_B=5, PAIR_B=6, TURN=7, SWITCH_AB=8,
-            SWITCH_BA=9, RSU=10)
+            SWITCH_BA=9, RSU=10, TURN_V=11)
 
 
 class Disorder(C.Structure):
@@ -186,16 +186,37 @@ class LanesRef:
     """Oracle two-lane model ensemble (host memory)."""
 
     def __init__(self, L, nsamples, p_a, p_b, rho0, turn_prob, turn_period, omega, seed=0, first_sample=0,
-                 offset_mode=0):
+                 offset_mode=0, w_unflagged=None, independent=0):
+        """w_unflagged=None: the turning-point model (crossing only at flagged sites, one flag set, DESIGN §R13);
+        otherwise the paper's model (§R18): crossing probability omega at flagged sites, w_unflagged elsewhere."""
         self.L, self.S = int(L), int(nsamples)
         self.nw = (self.L + 31) // 32
         self._h = C.c_void_p()
         o = Options(int(first_sample), int(offset_mode), 0)
-        _chk(lib().lanesref_create(C.byref(self._h), C.c_int64(self.L), C.c_int32(self.S), C.c_double(p_a),
-                                   C.c_double(p_b), C.c_double(rho0), C.c_double(turn_prob),
-                                   C.c_int64(turn_period), C.c_double(omega), C.c_uint64(seed), C.byref(o)),
-             "lanesref_create")
+        if w_unflagged is None:
+            _chk(lib().lanesref_create(C.byref(self._h), C.c_int64(self.L), C.c_int32(self.S), C.c_double(p_a),
+                                       C.c_double(p_b), C.c_double(rho0), C.c_double(turn_prob),
+                                       C.c_int64(turn_period), C.c_double(omega), C.c_uint64(seed), C.byref(o)),
+                 "lanesref_create")
+        else:
+            _chk(lib().lanesref_create_crossing(C.byref(self._h), C.c_int64(self.L), C.c_int32(self.S),
+                                                C.c_double(p_a), C.c_double(p_b), C.c_double(rho0),
+                                                C.c_double(turn_prob), C.c_double(omega), C.c_double(w_unflagged),
+                                                C.c_int32(independent), C.c_int64(turn_period), C.c_uint64(seed),
+                                                C.byref(o)), "lanesref_create_crossing")
         self._nt = 0
+
+    def flags(self):
+        u = np.zeros((self.S, self.nw), dtype=np.uint32)
+        v = np.zeros((self.S, self.nw), dtype=np.uint32)
+        _chk(lib().lanesref_flags(self._h, _p(u, C.c_uint32), _p(v, C.c_uint32)), "lanesref_flags")
+        return u, v
+
+    def set_flags(self, u=None, v=None):
+        def prep(x):
+            return None if x is None else np.ascontiguousarray(x, dtype=np.uint32).reshape(self.S, self.nw)
+        u, v = prep(u), prep(v)
+        _chk(lib().lanesref_set_flags(self._h, _p(u, C.c_uint32), _p(v, C.c_uint32)), "lanesref_set_flags")
 
     def close(self):
         if self._h:

@@ -151,7 +151,8 @@ def lanes_pass(L, states, o, p_a, p_b):
     return T, ja, jb
 
 
-def lanes_switch(L, states, turn_mask, omega, a_to_b):
+def lanes_switch(L, states, turn_mask, omega, a_to_b, w_unflagged=0.0):
+    """Crossing probability omega at the sites of turn_mask, w_unflagged elsewhere (0: turning-point model)."""
     index = {s: k for k, s in enumerate(states)}
     n = len(states)
     T = np.zeros((n, n))
@@ -159,32 +160,32 @@ def lanes_switch(L, states, turn_mask, omega, a_to_b):
         A, B = s & ((1 << L) - 1), s >> L
         outcomes = [(s, 1.0)]
         for i in range(L):
-            if not (turn_mask >> i) & 1:
-                continue
+            w = omega if (turn_mask >> i) & 1 else w_unflagged
             src, dst = (A, B) if a_to_b else (B, A)
             if (src >> i) & 1 == 1 and (dst >> i) & 1 == 0:
                 flip = (1 << i) | (1 << (i + L))
                 nxt = []
                 for st, pr in outcomes:
-                    if omega > 0.0:
-                        nxt.append((st ^ flip, pr * omega))
-                    if omega < 1.0:
-                        nxt.append((st, pr * (1.0 - omega)))
+                    if w > 0.0:
+                        nxt.append((st ^ flip, pr * w))
+                    if w < 1.0:
+                        nxt.append((st, pr * (1.0 - w)))
                 outcomes = nxt
         for st, pr in outcomes:
             T[index[st], k] += pr
     return T
 
 
-def lanes_finite_time(L, start_state, turn_mask, p_a, p_b, omega, n_mcs, ab_first=True):
+def lanes_finite_time(L, start_state, turn_mask, p_a, p_b, omega, n_mcs, ab_first=True, w_unflagged=0.0,
+                      mask_v=None):
     """Exact distribution and expected J_A, J_B after n_mcs MCS (drawn offsets, fixed turn mask).
     ab_first=False swaps the two lane-change steps (an alternative reading used to show test power)."""
     NT = bin(start_state).count("1")
     states = lanes_states(L, NT)
     T0, ja0, jb0 = lanes_pass(L, states, 0, p_a, p_b)
     T1, ja1, jb1 = lanes_pass(L, states, 1, p_a, p_b)
-    SAB = lanes_switch(L, states, turn_mask, omega, True)
-    SBA = lanes_switch(L, states, turn_mask, omega, False)
+    SAB = lanes_switch(L, states, turn_mask, omega, True, w_unflagged)
+    SBA = lanes_switch(L, states, turn_mask if mask_v is None else mask_v, omega, False, w_unflagged)
     v = np.zeros(len(states))
     v[states.index(start_state)] = 1.0
     JA = JB = 0.0

@@ -178,3 +178,73 @@ def test_lanes_resume_and_first_sample_are_exact():
     solo.run(31)
     assert np.array_equal(solo.state()[0][0], one.state()[0][2])
     assert np.array_equal(solo.currents()["j_b"][:, 0], c1["j_b"][:, 2])
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the paper's own two-lane model - every site can be crossed, with probability
+# omega where its flag is set and w_unflagged elsewhere; separate flag sets u_i (A->B) and v_i (B->A)
+# ---------------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("p_a,p_b,w1,w0,mask_u,mask_v,start", [
+    (0.5, 0.5, 0.2, 0.8, 0b0101, 0b0011, (0b0011, 0b0100)),     # the paper's rates
+    (1.0, 0.75, 0.5, 0.25, 0b1000, 0b0110, (0b1001, 0b0010)),
+])
+def test_crossing_model_finite_time_master_equation(p_a, p_b, w1, w0, mask_u, mask_v, start):
+    """Exact distribution after 3 MCS on L=4 versus 30000 oracle samples: pins that unflagged sites cross with
+    w_unflagged, flagged ones with omega, and that A->B reads the flags u while B->A reads v."""
+    L, S, t = 4, 30000, 3
+    A0, B0 = start
+    states, v, JA, JB = ME.lanes_finite_time(L, A0 | (B0 << L), mask_u, p_a, p_b, w1, t, w_unflagged=w0, mask_v=mask_v)
+    sim = R.LanesRef(L, S, p_a, p_b, 0.5, 0.5, 0, w1, seed=202, w_unflagged=w0, independent=1)
+    ones = np.ones((S, 1), dtype=np.uint32)
+    sim.set_state(ones * A0, ones * B0)
+    sim.set_flags(ones * mask_u, ones * mask_v)
+    sim.run(t)
+    a, b, _ = sim.state()
+    codes = a[:, 0].astype(np.int64) | (b[:, 0].astype(np.int64) << L)
+    counts = np.array([(codes == s).sum() for s in states], dtype=np.float64)
+    keep = v * S >= 5
+    chi2 = ((counts[keep] - v[keep] * S) ** 2 / (v[keep] * S)).sum()
+    if v[~keep].sum() > 0:
+        chi2 += (counts[~keep].sum() - v[~keep].sum() * S) ** 2 / (v[~keep].sum() * S)
+    dof = int(keep.sum())
+    assert chi2 < dof + 5 * np.sqrt(2 * dof), (chi2, dof)
+    tot = sim.totals()
+    for got, exact in ((tot["j_a"], JA), (tot["j_b"], JB)):
+        assert abs(got.mean() - exact) < 5 * got.std(ddof=1) / np.sqrt(S) + 1e-12
+    # power: swapping the roles of u and v, or of the two crossing probabilities, is rejected
+    for alt in (dict(turn_mask=mask_v, mask_v=mask_u, omega=w1, w_unflagged=w0),
+                dict(turn_mask=mask_u, mask_v=mask_v, omega=w0, w_unflagged=w1)):
+        _, v_alt, _, _ = ME.lanes_finite_time(L, A0 | (B0 << L), alt["turn_mask"], p_a, p_b, alt["omega"], t,
+                                              w_unflagged=alt["w_unflagged"], mask_v=alt["mask_v"])
+        ok = v_alt * S >= 5
+        chi2_alt = ((counts[ok] - v_alt[ok] * S) ** 2 / (v_alt[ok] * S)).sum()
+        assert chi2_alt > 10 * dof, (chi2_alt, dof)
+
+
+def test_crossing_model_flags_conservation_and_reduction_to_the_turning_point_model():
+    L, S, seed = 512, 4, 77
+    sim = R.LanesRef(L, S, 0.5, 0.5, 0.5, 0.5, 0, 0.2, seed=seed, w_unflagged=0.8, independent=1)
+    u, v = [R.unpack_words(x, L) for x in sim.flags()]
+    assert not np.array_equal(u, v)
+    n = S * L
+    for f in (u, v):
+        assert abs(f.mean() - 0.5) < 5 * np.sqrt(0.25 / n)
+    for i in (0, 1, 129, L - 1):       # u from stream TURN, v from stream TURN_V, epoch 0
+        assert u[1, i] == (R.uniform(seed, R.TAGS["TURN"], 1, 0, 0, i) < R.threshold(0.5))
+        assert v[1, i] == (R.uniform(seed, R.TAGS["TURN_V"], 1, 0, 0, i) < R.threshold(0.5))
+    a0, b0, _ = sim.state()
+    n0 = R.unpack_words(a0, L).sum(axis=1) + R.unpack_words(b0, L).sum(axis=1)
+    sim.run(50)
+    a1, b1, _ = sim.state()
+    assert np.array_equal(R.unpack_words(a1, L).sum(axis=1) + R.unpack_words(b1, L).sum(axis=1), n0)
+    assert np.array_equal(R.unpack_words(sim.flags()[0], L), u)        # quenched: period 0
+    # w_unflagged = 0 with one shared flag set IS the turning-point model, bit for bit
+    x = R.LanesRef(L, S, 1.0, 1.0, 0.3, 0.05, 7, 0.1, seed=5)
+    y = R.LanesRef(L, S, 1.0, 1.0, 0.3, 0.05, 7, 0.1, seed=5, w_unflagged=0.0, independent=0)
+    x.run(30)
+    y.run(30)
+    for p, q in zip(x.state(), y.state()):
+        assert np.array_equal(p, q)
+    with pytest.raises(R.OracleError):
+        y.set_flags(None, np.zeros((S, L // 32), dtype=np.uint32))      # one shared set: there is no separate v
