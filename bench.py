@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — site-update throughput of the KPZ/ASEP hot path on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|5|4-aux-i|4-aux-ii|4-aux-i-blocked|paper-1024x30|paper-1024-fill|paper-qtasep-16384|paper-qssep-4096] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|5|4-aux-i|4-aux-ii|4-aux-i-blocked|paper-1024x30|paper-1024-fill|paper-qtasep-16384|paper-qssep-4096|paper-lanes-4096] [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: reset to the
 initial state (a1), run the configuration's full number of MCS with its record times (a2-a7 / a9), records left in
@@ -62,6 +62,9 @@ ALU_SLOTS_PER_SU = {
     "paper-1024-fill": (2 * 6.0 * (34 + 12) + 2 * 4 * 3 + 8) / 256,
     "paper-qtasep-16384": (2 * 6.0 * (34 + 12) + 2 * 4 * 3 + 8) / 256,
     "paper-qssep-4096": (2 * 7.0 * (34 + 12) + 2 * 4 * 3 + 8) / 256,
+    # paper two-lane model: per 128 sites of both lanes and MCS: in-lane p = 0.5 (1 plane per lane and pass, pair streams
+    # cover 256 sites per call: 2 lanes x 2 passes x 0.5 call) + crossings 2 steps x (log2(32 live)+1.33 planes) x (34+12)
+    "paper-lanes-4096": (2 * 34 + 2 * 6.33 * (34 + 12) + 2 * 2 * 4 * 5 + 2 * 4 * 4) / 256,
 }
 ALU_SLOTS_PER_CLK_SMSP = 0.5
 # streamed sweep: one read + one write of the bit-packed ring per sub-lattice pass = 2 passes * 2 * 1/8 B
@@ -146,7 +149,9 @@ def _oracle_sim(cfg, nsamples, first_sample=0):
     from oracle import kpzref as R  # test infrastructure: only the cpu_baseline / reference legs load it
     if cfg["kind"] == "lanes":
         return R.LanesRef(cfg["L"], nsamples, cfg["p_a"], cfg["p_b"], cfg["rho0"], cfg["turn_prob"], cfg["turn_period"],
-                          cfg["omega"], seed=cfg["seed"], first_sample=first_sample)
+                          cfg["omega"], seed=cfg["seed"], first_sample=first_sample,
+                          offset_mode=cfg.get("offset_mode", 0), w_unflagged=cfg.get("w_unflagged"),
+                          independent=cfg.get("independent", 0))
     return R.KpzRef(cfg["L"], nsamples, cfg["p"], cfg["q"], disorder=cfg["disorder"], seed=cfg["seed"],
                     first_sample=first_sample, offset_mode=cfg.get("offset_mode", 0))
 
@@ -207,7 +212,9 @@ def make_sim(pkg, cfg, first_sample):
     nrec = len(cfg["record_times"])
     if cfg["kind"] == "lanes":
         sim = pkg.LanesSim(cfg["L"], cfg["S"], cfg["p_a"], cfg["p_b"], cfg["rho0"], cfg["turn_prob"], cfg["turn_period"],
-                           cfg["omega"], seed=cfg["seed"], first_sample=first_sample, max_records=nrec)
+                           cfg["omega"], seed=cfg["seed"], first_sample=first_sample, max_records=nrec,
+                           offset_mode=cfg.get("offset_mode", 0), w_unflagged=cfg.get("w_unflagged"),
+                           independent=cfg.get("independent", 0))
     else:
         sim = pkg.KpzSim(cfg["L"], cfg["S"], cfg["p"], cfg["q"], disorder=cfg["disorder"], seed=cfg["seed"],
                          first_sample=first_sample, max_records=nrec, path=cfg.get("path", 0),

@@ -122,6 +122,25 @@ int lanes_workspace_bytes(int64_t L, int32_t nsamples, int32_t max_records, size
 int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, double p_b, double rho0, double turn_prob,
                  int64_t turn_period, double omega, uint64_t seed, const kpz_options* opt, int32_t max_records,
                  void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+/* The paper's own two-lane model: EVERY site can be crossed - with probability
+ * w_flagged where the site's flag is set and w_unflagged elsewhere (the paper: flags set with probability 1/2, crossing
+ * "reduced from 0.8 to 0.2" at flagged sites, in-lane p = 0.5, half filling).  independent = 1: the A->B crossings read
+ * the flags u_i, the B->A crossings their own set v_i; 0: one set for both.  Flags are redrawn every turn_period MCS
+ * (0 = quenched).  lanes_create is the case {turn_prob, omega, 0, 0}.  Runs on the run-time specialised kernel
+ * (L <= 131072); lanes_run returns KPZ_EUNSUPPORTED otherwise. */
+typedef struct {
+  double prob_flag;
+  double w_flagged;
+  double w_unflagged;
+  int32_t independent;
+} lanes_crossing;
+int lanes_create_crossing(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, double p_b, double rho0,
+                          const lanes_crossing* crossing, int64_t turn_period, uint64_t seed, const kpz_options* opt,
+                          int32_t max_records, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+/* Flag sets u (A->B) and v (B->A) of the current epoch (device, natural layout; NULL = skip; v = u unless
+ * independent, and lanes_set_flags then takes the one set as d_u).  Async. */
+int lanes_flags(lanes_sim*, uint32_t* d_u, uint32_t* d_v);
+int lanes_set_flags(lanes_sim*, const uint32_t* d_u, const uint32_t* d_v);
 int lanes_set_record_times(lanes_sim*, const int64_t* t, int32_t nt);
 int lanes_run(lanes_sim*, int64_t n_mcs);
 int lanes_time(const lanes_sim*, int64_t* t);
@@ -152,6 +171,8 @@ int kpz_jit_check(int64_t L, double p, double q, const kpz_disorder* disorder, c
                   size_t* cubin_bytes);
 int lanes_jit_check(int64_t L, double p_a, double p_b, double turn_prob, int64_t turn_period, double omega,
                     const kpz_options* opt, size_t* cubin_bytes); /* same for the two-lane kernel */
+int lanes_crossing_jit_check(int64_t L, double p_a, double p_b, const lanes_crossing* crossing, int64_t turn_period,
+                             const kpz_options* opt, size_t* cubin_bytes);
 
 #ifdef __cplusplus
 }

@@ -30,6 +30,11 @@ class Disorder(C.Structure):
                 ("q_slow", C.c_double)]
 
 
+class Crossing(C.Structure):
+    _fields_ = [("prob_flag", C.c_double), ("w_flagged", C.c_double), ("w_unflagged", C.c_double),
+                ("independent", C.c_int32)]
+
+
 class Options(C.Structure):
     _fields_ = [("first_sample", C.c_int32), ("offset_mode", C.c_int32), ("path", C.c_int32)]
 
@@ -58,6 +63,13 @@ SIGNATURES = {
     "lanes_workspace_bytes": (C.c_int, [C.c_int64, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]),
     "lanes_create": (C.c_int, [C.POINTER(_P), C.c_int64, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
                                C.c_int64, C.c_double, C.c_uint64, C.POINTER(Options), C.c_int32, _P, C.c_size_t, _P]),
+    "lanes_create_crossing": (C.c_int, [C.POINTER(_P), C.c_int64, C.c_int32, C.c_double, C.c_double, C.c_double,
+                                        C.POINTER(Crossing), C.c_int64, C.c_uint64, C.POINTER(Options), C.c_int32, _P,
+                                        C.c_size_t, _P]),
+    "lanes_flags": (C.c_int, [_P, _P, _P]),
+    "lanes_set_flags": (C.c_int, [_P, _P, _P]),
+    "lanes_crossing_jit_check": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.POINTER(Crossing), C.c_int64,
+                                           C.POINTER(Options), C.POINTER(C.c_size_t)]),
     "lanes_set_record_times": (C.c_int, [_P, C.POINTER(C.c_int64), C.c_int32]),
     "lanes_run": (C.c_int, [_P, C.c_int64]),
     "lanes_time": (C.c_int, [_P, C.POINTER(C.c_int64)]),
@@ -139,6 +151,17 @@ def lanes_jit_check(L, p_a, p_b, turn_prob, turn_period, omega, offset_mode=0) -
     n = C.c_size_t()
     _chk(load_library().lanes_jit_check(int(L), float(p_a), float(p_b), float(turn_prob), int(turn_period),
                                         float(omega), C.byref(o), C.byref(n)), "lanes_jit_check")
+    return int(n.value)
+
+
+def lanes_crossing_jit_check(L, p_a, p_b, prob_flag, w_flagged, w_unflagged, independent, turn_period,
+                             offset_mode=0) -> int:
+    """lanes_crossing_jit_check: compile (no GPU needed) the two-lane kernel of the site-wise crossing model."""
+    o = Options(0, int(offset_mode), 0)
+    c = Crossing(float(prob_flag), float(w_flagged), float(w_unflagged), int(independent))
+    n = C.c_size_t()
+    _chk(load_library().lanes_crossing_jit_check(int(L), float(p_a), float(p_b), C.byref(c), int(turn_period),
+                                                 C.byref(o), C.byref(n)), "lanes_crossing_jit_check")
     return int(n.value)
 
 
@@ -250,7 +273,9 @@ class LanesSim:
     """lanes_create / lanes_run / lanes_currents / lanes_profile on the current CUDA device and stream."""
 
     def __init__(self, L, nsamples, p_a, p_b, rho0, turn_prob, turn_period, omega, seed=0, first_sample=0,
-                 offset_mode=0, max_records=64, device=None):
+                 offset_mode=0, max_records=64, device=None, w_unflagged=None, independent=0):
+        """w_unflagged=None: lanes_create (turning-point model); otherwise lanes_create_crossing with
+        {prob_flag=turn_prob, w_flagged=omega, w_unflagged, independent} (the paper's own model)."""
         _require_cuda()
         lib = load_library()
         self.L, self.S = int(L), int(nsamples)
@@ -263,10 +288,25 @@ class LanesSim:
         self.workspace = torch.empty(nbytes.value + 256, dtype=torch.uint8, device=self.device)
         base = (self.workspace.data_ptr() + 255) // 256 * 256
         self._h = C.c_void_p()
-        _chk(lib.lanes_create(C.byref(self._h), self.L, self.S, float(p_a), float(p_b), float(rho0), float(turn_prob),
-                              int(turn_period), float(omega), int(seed), C.byref(self._o), self.max_records,
-                              C.c_void_p(base), nbytes.value, _stream_ptr()), "lanes_create")
+        if w_unflagged is None:
+            _chk(lib.lanes_create(C.byref(self._h), self.L, self.S, float(p_a), float(p_b), float(rho0),
+                                  float(turn_prob), int(turn_period), float(omega), int(seed), C.byref(self._o),
+                                  self.max_records, C.c_void_p(base), nbytes.value, _stream_ptr()), "lanes_create")
+        else:
+            c = Crossing(float(turn_prob), float(omega), float(w_unflagged), int(independent))
+            _chk(lib.lanes_create_crossing(C.byref(self._h), self.L, self.S, float(p_a), float(p_b), float(rho0),
+                                           C.byref(c), int(turn_period), int(seed), C.byref(self._o),
+                                           self.max_records, C.c_void_p(base), nbytes.value, _stream_ptr()),
+                 "lanes_create_crossing")
         self._nt = 0
+
+    def flags(self):
+        u, v = [torch.empty((self.S, self.nw), dtype=torch.int32, device=self.device) for _ in range(2)]
+        _chk(load_library().lanes_flags(self._h, _dptr(u), _dptr(v)), "lanes_flags")
+        return u, v
+
+    def set_flags(self, u=None, v=None):
+        _chk(load_library().lanes_set_flags(self._h, _dptr(u), _dptr(v)), "lanes_set_flags")
 
     def close(self):
         if getattr(self, "_h", None):

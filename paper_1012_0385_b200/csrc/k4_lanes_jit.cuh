@@ -16,12 +16,19 @@
 //     epoch ends by warp-transposed, coalesced red.global.add.
 //
 // Compile-time configuration (-D, set by lanes_api.cu): K4J_W = L/32, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN
-// (thresholds in [0, 2^32]), K4J_OFFSET_MODE, K4J_EAGER, K4J_TAIL.
+// (thresholds in [0, 2^32]), K4J_OFFSET_MODE, K4J_TW0 and K4J_INDEP (site-wise crossing model), K4J_EAGER,
+// K4J_TRIP, K4J_TAIL.
 #pragma once
 #include "sweep_types.cuh"
 
 #ifndef K4J_W
 #error "k4_lanes_jit.cuh needs K4J_W, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN, K4J_OFFSET_MODE"
+#endif
+#ifndef K4J_TW0
+#define K4J_TW0 0ull  // crossing threshold at unflagged sites: 0 = turning-point model, else §R18
+#endif
+#ifndef K4J_INDEP
+#define K4J_INDEP 0   // 1: the B->A crossings read their own flag set (D.V)
 #endif
 #ifndef K4J_EAGER
 #define K4J_EAGER 6
@@ -51,7 +58,9 @@ __host__ __device__ constexpr int planes_of(uint64_t T) {
   while (!((T >> z) & 1ull)) ++z;
   return 32 - z;
 }
-constexpr int NPW = planes_of(TOMEGA);
+constexpr uint64_t TW0 = K4J_TW0;
+constexpr bool CROSS = TW0 != 0;  // every site can be crossed: two rate classes, chosen by the site's flag
+constexpr int NPW = planes_of(TOMEGA) > planes_of(TW0) ? planes_of(TOMEGA) : planes_of(TW0);
 constexpr int EAGER = K4J_EAGER < NPW ? K4J_EAGER : NPW;
 constexpr int EAGERA = EAGER > 0 ? EAGER : 1;
 
@@ -281,23 +290,70 @@ __device__ __forceinline__ void draw_eager(Eager& E, const PhiloxKeys& K, const 
   }
 }
 
-// Lane changes at turning points: SRC -> DST where turn & SRC & ~DST and U < T(omega).
-__device__ __forceinline__ void lane_change(uint32_t (&SRC)[4], uint32_t (&DST)[4], const uint32_t (&T)[4],
+// Two rate classes: elements with flag F compare with T(omega) (bit b1 of this plane), the others with
+// T(w_unflagged) (bit b0).
+__device__ __forceinline__ void plane_step2(uint32_t (&lt)[4], uint32_t (&eq)[4], const uint32_t (&R)[4],
+                                            const uint32_t (&F)[4], uint32_t b1, uint32_t b0) {
+  const uint32_t B1 = 0u - b1, B0 = 0u - b0;
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    const uint32_t tb = (F[w] & B1) | (~F[w] & B0);
+    lt[w] |= eq[w] & tb & ~R[w];
+    eq[w] &= ~(R[w] ^ tb);
+  }
+}
+__host__ __device__ constexpr uint32_t tbit(uint64_t T, int pl) { return (uint32_t)((T >> (31 - pl)) & 1ull); }
+
+// Lane changes SRC -> DST where the source is occupied, the target empty and U < T(site) (§R18):
+// turning-point model: T = T(omega) at flagged sites F, no crossing elsewhere; site-wise crossing model: T(omega) at
+// flagged sites, T(w_unflagged) elsewhere.
+__device__ __forceinline__ void lane_change(uint32_t (&SRC)[4], uint32_t (&DST)[4], const uint32_t (&F)[4],
                                             const uint32_t (&r)[EAGERA][4], const PhiloxKeys& K, const Unit& un,
                                             uint32_t tag, uint32_t tlo, uint32_t thi) {
   uint32_t lt[4], eq[4];
+  if constexpr (!CROSS) {
 #pragma unroll
-  for (int w = 0; w < 4; ++w) {
-    const uint32_t live = lop3<0x20>(SRC[w], DST[w], T[w]);  // SRC & ~DST & T
-    lt[w] = (TOMEGA >= kOne) ? live : 0u;
-    eq[w] = (TOMEGA >= kOne || TOMEGA == 0) ? 0u : live;
-  }
-  if (TOMEGA > 0 && TOMEGA < kOne) {
+    for (int w = 0; w < 4; ++w) {
+      const uint32_t live = lop3<0x20>(SRC[w], DST[w], F[w]);  // SRC & ~DST & F
+      lt[w] = (TOMEGA >= kOne) ? live : 0u;
+      eq[w] = (TOMEGA >= kOne || TOMEGA == 0) ? 0u : live;
+    }
+    if (TOMEGA > 0 && TOMEGA < kOne) {
 #pragma unroll
-    for (int pl = 0; pl < EAGER; ++pl) plane_step<TOMEGA>(lt, eq, r[pl], pl);
+      for (int pl = 0; pl < EAGER; ++pl) plane_step<TOMEGA>(lt, eq, r[pl], pl);
+      if (EAGER < NPW) {
+        if (K4J_TAIL) resolve_tail<TOMEGA>(lt, eq, K, (uint32_t)(un.u & ~31), un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
+        else resolve<TOMEGA>(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
+      }
+    }
+  } else {
+    constexpr uint32_t AL1 = TOMEGA >= kOne ? ~0u : 0u, AL0 = TW0 >= kOne ? ~0u : 0u;          // always accepted
+    constexpr uint32_t PA1 = (TOMEGA > 0 && TOMEGA < kOne) ? ~0u : 0u, PA0 = TW0 < kOne ? ~0u : 0u;  // needs planes
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const uint32_t live = SRC[w] & ~DST[w];
+      lt[w] = live & ((F[w] & AL1) | (~F[w] & AL0));
+      eq[w] = live & ((F[w] & PA1) | (~F[w] & PA0));
+    }
+#pragma unroll
+    for (int pl = 0; pl < EAGER; ++pl) plane_step2(lt, eq, r[pl], F, tbit(TOMEGA, pl), tbit(TW0, pl));
     if (EAGER < NPW) {
-      if (K4J_TAIL) resolve_tail<TOMEGA>(lt, eq, K, (uint32_t)(un.u & ~31), un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
-      else resolve<TOMEGA>(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
+      const uint32_t c3 = ctr3(tag, 0, 0, thi);
+#pragma unroll 1
+      for (int pl = EAGER; pl < NPW; pl += K4J_TRIP) {
+        if (!__any_sync(FULL, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u)) break;
+        uint32_t R[K4J_TRIP][4];
+#pragma unroll
+        for (int t = 0; t < K4J_TRIP; ++t) {
+          const int q = pl + t < 32 ? pl + t : 31;
+          const uint4 v = philox4x32_10((uint32_t)un.u, un.gs, tlo, c3 | ((uint32_t)q << 22), K);
+          R[t][0] = v.x; R[t][1] = v.y; R[t][2] = v.z; R[t][3] = v.w;
+        }
+#pragma unroll
+        for (int t = 0; t < K4J_TRIP; ++t)
+          if (pl + t < NPW)
+            plane_step2(lt, eq, R[t], F, (uint32_t)(TOMEGA >> (31 - (pl + t))) & 1u, (uint32_t)(TW0 >> (31 - (pl + t))) & 1u);
+      }
     }
   }
 #pragma unroll
@@ -309,9 +365,9 @@ __device__ __forceinline__ void lane_change(uint32_t (&SRC)[4], uint32_t (&DST)[
 
 // Quenched-per-epoch turning-point mask of this thread's supergroup: all 128 sites are live.
 __device__ __forceinline__ void draw_turn(uint32_t (&T)[4], const PhiloxKeys& K, const Unit& un,
-                                          unsigned long long epoch) {
+                                          unsigned long long epoch, uint32_t tag) {
   const uint32_t live[4] = {FULL, FULL, FULL, FULL};
-  lazy_less<TTURN>(T, live, K, (uint32_t)un.u, un.gs, (uint32_t)epoch, ctr3(TAG_TURN, 0, 0, (uint32_t)(epoch >> 32)));
+  lazy_less<TTURN>(T, live, K, (uint32_t)un.u, un.gs, (uint32_t)epoch, ctr3(tag, 0, 0, (uint32_t)(epoch >> 32)));
 #pragma unroll
   for (int w = 0; w < 4; ++w) T[w] = (w < un.nwn) ? T[w] : 0u;
 }
@@ -362,6 +418,7 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
   int parity = 0;
 
   uint32_t A[4] = {0, 0, 0, 0}, B[4] = {0, 0, 0, 0}, T[4] = {0, 0, 0, 0};
+  uint32_t V[4] = {0, 0, 0, 0};  // flags of the B->A crossings when they are a set of their own (K4J_INDEP)
   if (active) {
     const uint4 a = *reinterpret_cast<const uint4*>(D.A + row);
     const uint4 b = *reinterpret_cast<const uint4*>(D.B + row);
@@ -369,6 +426,10 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
     A[0] = a.x; A[1] = a.y; A[2] = a.z; A[3] = a.w;
     B[0] = b.x; B[1] = b.y; B[2] = b.z; B[3] = b.w;
     T[0] = t.x; T[1] = t.y; T[2] = t.z; T[3] = t.w;
+    if (K4J_INDEP) {
+      const uint4 v = *reinterpret_cast<const uint4*>(D.V + row);
+      V[0] = v.x; V[1] = v.y; V[2] = v.z; V[3] = v.w;
+    }
   }
   unsigned long long jA = 0, jB = 0;
   int ri = R.rec_begin;
@@ -414,7 +475,10 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
   // One MCS m with the eager lane-change planes Ec drawn one step earlier; draws those of MCS m+1 into En.
   auto mcs = [&](const Eager& Ec, Eager& En) {
     const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
-    if (period > 0 && m > 0 && in_epoch == 0) draw_turn(T, D.keys, un, (unsigned long long)epoch);
+    if (period > 0 && m > 0 && in_epoch == 0) {
+      draw_turn(T, D.keys, un, (unsigned long long)epoch, TAG_TURN);
+      if (K4J_INDEP) draw_turn(V, D.keys, un, (unsigned long long)epoch, TAG_TURN_V);
+    }
     draw_eager(En, D.keys, un, m + 1);
 #pragma unroll
     for (int pass = 0; pass < 2; ++pass) {
@@ -460,7 +524,7 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
       }
       // lane changes at turning points: A->B after pass 0, B->A after pass 1
       if (pass == 0) lane_change(A, B, T, Ec.r[0], D.keys, un, TAG_SWITCH_AB, tlo, thi);
-      else lane_change(B, A, T, Ec.r[1], D.keys, un, TAG_SWITCH_BA, tlo, thi);
+      else lane_change(B, A, K4J_INDEP ? V : T, Ec.r[1], D.keys, un, TAG_SWITCH_BA, tlo, thi);
     }
     ++m;  // t = m from here on
     if (period > 0 && ++in_epoch == period) {
@@ -504,5 +568,6 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
     *reinterpret_cast<uint4*>(D.A + row) = make_uint4(A[0], A[1], A[2], A[3]);
     *reinterpret_cast<uint4*>(D.B + row) = make_uint4(B[0], B[1], B[2], B[3]);
     *reinterpret_cast<uint4*>(D.T + row) = make_uint4(T[0], T[1], T[2], T[3]);
+    if (K4J_INDEP) *reinterpret_cast<uint4*>(D.V + row) = make_uint4(V[0], V[1], V[2], V[3]);
   }
 }

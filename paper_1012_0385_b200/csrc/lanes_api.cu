@@ -31,7 +31,7 @@ struct lanes_sim {
 namespace {
 
 struct LLayout {
-  size_t off_A, off_B, off_T, off_JA, off_JB, off_occA, off_occB, off_rec_t, off_rec, total;
+  size_t off_A, off_B, off_T, off_V, off_JA, off_JB, off_occA, off_occB, off_rec_t, off_rec, total;
   int W, Wp, U;
 };
 
@@ -58,6 +58,7 @@ LLayout lanes_layout(int64_t L, int32_t S, int32_t max_records) {
   y.off_A = take(plane);
   y.off_B = take(plane);
   y.off_T = take(plane);
+  y.off_V = take(plane);
   y.off_JA = take((size_t)S * 8);
   y.off_JB = take((size_t)S * 8);
   y.off_occA = take((size_t)S * L * 4);
@@ -86,6 +87,10 @@ std::vector<std::string> k4_jit_defines(const LanesDev& D) {
   snprintf(buf, sizeof buf, "K4J_TTURN=0x%llxull", D.period > 0 ? T(D.t_turn) : 0ull);  // never redrawn without a period
   d.push_back(buf);
   snprintf(buf, sizeof buf, "K4J_OFFSET_MODE=%d", D.offset_mode);
+  d.push_back(buf);
+  snprintf(buf, sizeof buf, "K4J_TW0=0x%llxull", T(D.t_w0));
+  d.push_back(buf);
+  snprintf(buf, sizeof buf, "K4J_INDEP=%d", D.independent);
   d.push_back(buf);
   if (const char* v = std::getenv("KPZ_B200_K4_EAGER")) {  // tuning knob: lane-change planes drawn one MCS ahead
     snprintf(buf, sizeof buf, "K4J_EAGER=%d", atoi(v));
@@ -118,6 +123,10 @@ int lanes_init_state(lanes_sim* sim) {
   KPZ_LAUNCH_CHECK("k_site_mask_nat");
   k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_TURN, D.t_turn, 0, D.first_sample, D.S, D.W, D.Wp, D.T);
   KPZ_LAUNCH_CHECK("k_site_mask_nat");
+  if (D.independent) {
+    k_site_mask_nat<<<grid_for(ng, 128), 128, 0, sim->stream>>>(D.keys, TAG_TURN_V, D.t_turn, 0, D.first_sample, D.S, D.W, D.Wp, D.V);
+    KPZ_LAUNCH_CHECK("k_site_mask_nat");
+  }
   return KPZ_OK;
 }
 
@@ -146,13 +155,23 @@ int lanes_workspace_bytes(int64_t L, int32_t nsamples, int32_t max_records, size
 int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, double p_b, double rho0, double turn_prob,
                  int64_t turn_period, double omega, uint64_t seed, const kpz_options* opt, int32_t max_records,
                  void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  const lanes_crossing c{turn_prob, omega, 0.0, 0};  // turning-point model: no crossing at unflagged sites, one flag set
+  return lanes_create_crossing(out, L, nsamples, p_a, p_b, rho0, &c, turn_period, seed, opt, max_records, d_workspace,
+                               workspace_bytes, cuda_stream);
+}
+
+int lanes_create_crossing(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, double p_b, double rho0,
+                          const lanes_crossing* crossing, int64_t turn_period, uint64_t seed, const kpz_options* opt,
+                          int32_t max_records, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
   if (!out) return fail(KPZ_EINVAL, "out is NULL");
   *out = nullptr;
+  if (!crossing) return fail(KPZ_EINVAL, "crossing is NULL");
+  const double turn_prob = crossing->prob_flag, omega = crossing->w_flagged;
   int rc = lanes_validate(L, nsamples, max_records);
   if (rc) return rc;
   if (!valid_prob(p_a) || !valid_prob(p_b) || !valid_prob(rho0) || !valid_prob(turn_prob) || !valid_prob(omega) ||
-      turn_period < 0)
-    return fail(KPZ_EINVAL, "probabilities must lie in [0,1] and turn_period >= 0");
+      !valid_prob(crossing->w_unflagged) || turn_period < 0 || (crossing->independent != 0 && crossing->independent != 1))
+    return fail(KPZ_EINVAL, "probabilities must lie in [0,1], turn_period >= 0, independent in {0,1}");
   kpz_options o{0, 0, 0};
   if (opt) o = *opt;
   if (o.first_sample < 0 || (o.offset_mode != 0 && o.offset_mode != 1))
@@ -173,6 +192,8 @@ int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, doubl
   D.t_pb = make_thresh(p_b);
   D.t_turn = make_thresh(turn_prob);
   D.t_omega = make_thresh(omega);
+  D.t_w0 = make_thresh(crossing->w_unflagged);
+  D.independent = crossing->independent;
   D.np_a = planes_needed(D.t_pa);
   D.np_b = planes_needed(D.t_pb);
   D.np_w = planes_needed(D.t_omega);
@@ -186,6 +207,7 @@ int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, doubl
   D.A = (uint32_t*)(base + y.off_A);
   D.B = (uint32_t*)(base + y.off_B);
   D.T = (uint32_t*)(base + y.off_T);
+  D.V = D.independent ? (uint32_t*)(base + y.off_V) : D.T;
   D.JA = (unsigned long long*)(base + y.off_JA);
   D.JB = (unsigned long long*)(base + y.off_JB);
   D.occA = (uint32_t*)(base + y.off_occA);
@@ -207,17 +229,27 @@ int lanes_create(lanes_sim** out, int64_t L, int32_t nsamples, double p_a, doubl
 
 int lanes_jit_check(int64_t L, double p_a, double p_b, double turn_prob, int64_t turn_period, double omega,
                     const kpz_options* opt, size_t* cubin_bytes) {
-  if (!cubin_bytes) return fail(KPZ_EINVAL, "cubin_bytes is NULL");
+  const lanes_crossing c{turn_prob, omega, 0.0, 0};
+  return lanes_crossing_jit_check(L, p_a, p_b, &c, turn_period, opt, cubin_bytes);
+}
+
+int lanes_crossing_jit_check(int64_t L, double p_a, double p_b, const lanes_crossing* crossing, int64_t turn_period,
+                             const kpz_options* opt, size_t* cubin_bytes) {
+  if (!cubin_bytes || !crossing) return fail(KPZ_EINVAL, "NULL argument");
   *cubin_bytes = 0;
+  const double turn_prob = crossing->prob_flag, omega = crossing->w_flagged;
   int rc = lanes_validate(L, 1, 0);
   if (rc) return rc;
-  if (!valid_prob(p_a) || !valid_prob(p_b) || !valid_prob(turn_prob) || !valid_prob(omega) || turn_period < 0)
-    return fail(KPZ_EINVAL, "probabilities must lie in [0,1] and turn_period >= 0");
+  if (!valid_prob(p_a) || !valid_prob(p_b) || !valid_prob(turn_prob) || !valid_prob(omega) ||
+      !valid_prob(crossing->w_unflagged) || turn_period < 0 || (crossing->independent != 0 && crossing->independent != 1))
+    return fail(KPZ_EINVAL, "probabilities must lie in [0,1], turn_period >= 0, independent in {0,1}");
   LanesDev D{};
   D.t_pa = make_thresh(p_a);
   D.t_pb = make_thresh(p_b);
   D.t_turn = make_thresh(turn_prob);
   D.t_omega = make_thresh(omega);
+  D.t_w0 = make_thresh(crossing->w_unflagged);
+  D.independent = crossing->independent;
   D.offset_mode = opt ? opt->offset_mode : 0;
   D.W = (int)(L / 32);
   D.period = turn_period;
@@ -286,6 +318,9 @@ int lanes_run(lanes_sim* sim, int64_t n_mcs) {
     void* args[] = {(void*)&D, (void*)&A};
     const int block4 = ((D.W + 3) / 4 + 31) / 32 * 32;  // one thread per 128-site supergroup
     KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(sim->S), dim3(block4), args, 0, sim->stream));
+  } else if (D.independent || D.t_w0.value != 0 || D.t_w0.always) {
+    return fail(KPZ_EUNSUPPORTED, "the site-wise crossing model runs on the run-time specialised kernel only "
+                                  "(L <= 131072, KPZ_B200_JIT not 0)");
   } else if (single) {
     if (partial) lanes_k4_kernel<true, true><<<sim->S, block, 0, sim->stream>>>(D, A);
     else lanes_k4_kernel<true, false><<<sim->S, block, 0, sim->stream>>>(D, A);
@@ -321,6 +356,35 @@ int lanes_set_state(lanes_sim* sim, const uint32_t* d_a, const uint32_t* d_b, co
   const uint32_t* src[3] = {d_a, d_b, d_turn};
   uint32_t* dst[3] = {D.A, D.B, D.T};
   for (int k = 0; k < 3; ++k)
+    if (src[k]) {
+      k_copy_rows<<<grid_for(n), 256, 0, sim->stream>>>(src[k], D.S, D.W, D.W, D.Wp, dst[k]);
+      KPZ_LAUNCH_CHECK("k_copy_rows");
+    }
+  return KPZ_OK;
+}
+
+int lanes_flags(lanes_sim* sim, uint32_t* d_u, uint32_t* d_v) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  const LanesDev& D = sim->dev;
+  const size_t n = (size_t)D.S * D.W;
+  const uint32_t* src[2] = {D.T, D.V};
+  uint32_t* dst[2] = {d_u, d_v};
+  for (int k = 0; k < 2; ++k)
+    if (dst[k]) {
+      k_copy_rows<<<grid_for(n), 256, 0, sim->stream>>>(src[k], D.S, D.W, D.Wp, D.W, dst[k]);
+      KPZ_LAUNCH_CHECK("k_copy_rows");
+    }
+  return KPZ_OK;
+}
+
+int lanes_set_flags(lanes_sim* sim, const uint32_t* d_u, const uint32_t* d_v) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  const LanesDev& D = sim->dev;
+  if (d_v && !D.independent) return fail(KPZ_EINVAL, "one shared flag set: pass it as d_u");
+  const size_t n = (size_t)D.S * D.W;
+  const uint32_t* src[2] = {d_u, d_v};
+  uint32_t* dst[2] = {D.T, D.V};
+  for (int k = 0; k < 2; ++k)
     if (src[k]) {
       k_copy_rows<<<grid_for(n), 256, 0, sim->stream>>>(src[k], D.S, D.W, D.W, D.Wp, dst[k]);
       KPZ_LAUNCH_CHECK("k_copy_rows");

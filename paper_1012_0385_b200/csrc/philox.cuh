@@ -21,7 +21,8 @@ enum : uint32_t {
   TAG_PAIR_B = 6,
   TAG_TURN = 7,
   TAG_SWITCH_AB = 8,
-  TAG_SWITCH_BA = 9
+  TAG_SWITCH_BA = 9,
+  TAG_TURN_V = 11  // flags v_i of the B->A crossings when independent of u_i; 10 is oracle-only
 };
 
 // The ten round keys, precomputed on the host from the seed (the key schedule is a Weyl sequence, so the

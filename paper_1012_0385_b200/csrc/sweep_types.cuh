@@ -63,6 +63,8 @@ struct K3TArgs {
 struct LanesDev {
   PhiloxKeys keys;
   Thresh t_pa, t_pb, t_turn, t_omega;
+  Thresh t_w0;               // crossing threshold at unflagged sites (0 in the turning-point model)
+  int32_t independent;       // 1: B->A crossings read their own flag set V
   int32_t np_a, np_b, np_w;  // planes needed by the in-lane thresholds and by omega
   int32_t offset_mode;
   int32_t first_sample;
@@ -73,7 +75,8 @@ struct LanesDev {
   long long period;
   uint32_t* A;  // [S][Wp]
   uint32_t* B;
-  uint32_t* T;  // turning-point mask of the current epoch
+  uint32_t* T;  // flags of the current epoch (turning points; u_i of the A->B crossings)
+  uint32_t* V;  // flags v_i of the B->A crossings (== T unless independent)
   unsigned long long* JA;  // [S] hops so far
   unsigned long long* JB;
   uint32_t* occA;  // [S][L] epoch-end occupancy counts

@@ -297,19 +297,22 @@ def test_config4_full_size_first_steps_and_invariants(K):
 # ---------------------------------------------------------------------------------------------------------
 
 def run_both_lanes(K, L, S, p_a, p_b, rho0, turn_prob, period, omega, seed, times, chunks, first_sample=0,
-                   offset_mode=0):
+                   offset_mode=0, w_unflagged=None, independent=0):
     total = sum(chunks)
     times = [t for t in times if t <= total]
     ref = R.LanesRef(L, S, p_a, p_b, rho0, turn_prob, period, omega, seed=seed, first_sample=first_sample,
-                     offset_mode=offset_mode)
+                     offset_mode=offset_mode, w_unflagged=w_unflagged, independent=independent)
     gpu = K.LanesSim(L, S, p_a, p_b, rho0, turn_prob, period, omega, seed=seed, first_sample=first_sample,
-                     offset_mode=offset_mode, max_records=max(len(times), 1))
+                     offset_mode=offset_mode, max_records=max(len(times), 1), w_unflagged=w_unflagged,
+                     independent=independent)
     ref.set_record_times(times)
     gpu.set_record_times(times)
 
     def same_state(tag):
         for name, g, r in zip("AB T".replace(" ", ""), gpu.state(), ref.state()):
             assert np.array_equal(K.words_to_numpy(g), r), f"{name} differs {tag}"
+        for name, g, r in zip("uv", gpu.flags(), ref.flags()):
+            assert np.array_equal(K.words_to_numpy(g), r), f"flags {name} differ {tag}"
     same_state("initially")
     done = 0
     for n in chunks:
@@ -535,3 +538,43 @@ def test_lanes_time_keys_beyond_32_bits(K):
     ra, rb, rn = ref.profile()
     assert gn == rn == 1
     assert np.array_equal(K.words_to_numpy(ga), ra) and np.array_equal(K.words_to_numpy(gb), rb)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the paper's own two-lane model: site-wise crossing probabilities, separate flag sets u_i / v_i
+# ---------------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("L", [64, 320, 4096, 8192 + 64])
+def test_paper_two_lane_model_sizes(K, L):
+    """in-lane p = 0.5, half filling, flags with probability 1/2, crossing 0.2 at flagged sites and
+    0.8 elsewhere, u_i and v_i independent, quenched."""
+    run_both_lanes(K, L, 3, 0.5, 0.5, 0.5, 0.5, 0, 0.2, seed=L + 7, times=[1, 5, 17], chunks=[5, 12], w_unflagged=0.8,
+                   independent=1)
+
+
+@pytest.mark.parametrize("omega,w0,indep,period,tp", [(0.2, 0.8, 0, 0, 0.5), (0.25, 0.5, 1, 6, 0.3), (1.0, 0.1, 1, 4, 0.05),
+                                                     (0.0, 1.0, 1, 0, 0.5), (0.3, 0.0, 1, 5, 0.4)])
+def test_site_wise_crossing_rates(K, omega, w0, indep, period, tp):
+    run_both_lanes(K, 2048, 2, 0.75, 0.5, 0.45, tp, period, omega, seed=19, times=[2, 7, 8, 25], chunks=[25],
+                   w_unflagged=w0, independent=indep)
+    run_both_lanes(K, 2048, 2, 1.0, 1.0, 0.3, tp, period, omega, seed=20, times=[25], chunks=[25], offset_mode=1,
+                   w_unflagged=w0, independent=indep, first_sample=3)
+
+
+def test_crossing_model_flags_can_be_set_and_static_kernel_refuses(K):
+    L, S = 1024, 2
+    rng = np.random.default_rng(3)
+    u = R.pack_sites((rng.random((S, L)) < 0.3).astype(np.uint8))
+    v = R.pack_sites((rng.random((S, L)) < 0.7).astype(np.uint8))
+    ref = R.LanesRef(L, S, 0.5, 0.5, 0.5, 0.5, 0, 0.2, seed=4, w_unflagged=0.8, independent=1)
+    gpu = K.LanesSim(L, S, 0.5, 0.5, 0.5, 0.5, 0, 0.2, seed=4, w_unflagged=0.8, independent=1, max_records=1)
+    ref.set_flags(u, v)
+    gpu.set_flags(K.words_from_numpy(u, "cuda"), K.words_from_numpy(v, "cuda"))
+    ref.run(15)
+    gpu.run(15)
+    for g, r in zip(gpu.state()[:2], ref.state()[:2]):
+        assert np.array_equal(K.words_to_numpy(g), r)
+    with _env(KPZ_B200_JIT=0):
+        g2 = K.LanesSim(L, S, 0.5, 0.5, 0.5, 0.5, 0, 0.2, seed=4, w_unflagged=0.8, independent=1, max_records=1)
+        with pytest.raises(K.KpzError):
+            g2.run(1)

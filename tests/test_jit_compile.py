@@ -53,6 +53,11 @@ def test_two_lane_edge_shapes_compile(K, L, pa, pb, turn, period, omega):
     assert K.lanes_jit_check(L, pa, pb, turn, period, omega) > 10_000
 
 
+@pytest.mark.parametrize("L,indep,period", [(512, 1, 0), (4096, 1, 100), (131072, 0, 0)])
+def test_paper_two_lane_model_compiles(K, L, indep, period):
+    assert K.lanes_crossing_jit_check(L, 0.5, 0.5, 0.5, 0.2, 0.8, indep, period) > 10_000
+
+
 def test_bad_arguments_are_refused_without_compiling(K):
     with pytest.raises(K.KpzError):
         K.jit_check(100, 0.5, 0.5)              # L not a multiple of 64

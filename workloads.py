@@ -75,6 +75,11 @@ CONFIGS = {
     "paper-qssep-4096": dict(name="paper_qssep_L4096_S2048", kind="kpz", L=4096, S=2048, p=0.5, q=0.5,
                              disorder=(0.5, 0.1, 0.5, 0.1), n_mcs=10_000, record_times=eq7_times(10_000), seed=8,
                              offset_mode=1),
+    # the paper's own two-lane model: in-lane p = 0.5, half filling, every site crossed
+    # with 0.8 (0.2 at sites flagged with probability 1/2), separate quenched flags u_i, v_i, L = 4096, Eq. 7 sampling
+    "paper-lanes-4096": dict(name="paper_two_lane_L4096_S1024", kind="lanes", L=4096, S=1024, p_a=0.5, p_b=0.5, rho0=0.5,
+                             turn_prob=0.5, turn_period=0, omega=0.2, w_unflagged=0.8, independent=1, n_mcs=10_000,
+                             record_times=eq7_times(10_000), seed=9, offset_mode=1),
     # the same two rings on the default (temporally blocked) path
     "4-aux-i-blocked": dict(name="config4aux1_blocked_L2p28_p075_q025", kind="kpz", L=1 << 28, S=1, p=0.75, q=0.25,
                             disorder=None, n_mcs=1000, record_times=_T20_1E3, seed=4),
