@@ -95,9 +95,12 @@ __device__ __forceinline__ void resolve(uint32_t (&lt)[4], uint32_t (&eq)[4], co
     uint32_t R[K4J_TRIP][4];
 #pragma unroll
     for (int t = 0; t < K4J_TRIP; ++t) {  // independent calls: their rounds interleave
-      const int q = pl + t < 32 ? pl + t : 31;
-      const uint4 v = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)q << 22), K);
-      R[t][0] = v.x; R[t][1] = v.y; R[t][2] = v.z; R[t][3] = v.w;
+      if (pl + t < NP) {                   // (warp-uniform) never draw a plane T does not reach
+        const uint4 v = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)(pl + t) << 22), K);
+        R[t][0] = v.x; R[t][1] = v.y; R[t][2] = v.z; R[t][3] = v.w;
+      } else {
+        R[t][0] = R[t][1] = R[t][2] = R[t][3] = 0u;
+      }
     }
 #pragma unroll
     for (int t = 0; t < K4J_TRIP; ++t)

@@ -578,3 +578,62 @@ def test_crossing_model_flags_can_be_set_and_static_kernel_refuses(K):
         g2 = K.LanesSim(L, S, 0.5, 0.5, 0.5, 0.5, 0, 0.2, seed=4, w_unflagged=0.8, independent=1, max_records=1)
         with pytest.raises(K.KpzError):
             g2.run(1)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the launch configurations bench.py times, sampled: configs 3 and 5 at full ensemble size
+# ---------------------------------------------------------------------------------------------------------
+
+def test_config3_full_launch_sampled_against_solo_oracle_runs(K):
+    c = workloads.CONFIGS[3]
+    n, times = 120, [t for t in c["record_times"] if t <= 120]
+    gpu = K.KpzSim(c["L"], c["S"], c["p"], c["q"], disorder=c["disorder"], seed=c["seed"], max_records=len(times))
+    gpu.set_record_times(times)
+    gpu.run(n)
+    lat = K.words_to_numpy(gpu.lattice())
+    r = gpu.roughness()
+    for k in (0, 255, 511):
+        ref = R.KpzRef(c["L"], 1, c["p"], c["q"], disorder=c["disorder"], seed=c["seed"], first_sample=k)
+        ref.set_record_times(times)
+        ref.run(n)
+        assert np.array_equal(lat[k], ref.lattice()[0])
+        rr = ref.roughness()
+        assert np.array_equal(r["sum_h"][:, k], rr["sum_h"][:, 0]) and np.array_equal(r["sum_h2"][:, k], rr["sum_h2"][:, 0])
+    assert np.all(R.unpack_words(lat, c["L"]).sum(axis=1) == c["L"] // 2)      # conservation, every sample
+
+
+def test_config3_last_sample_long_run(K):
+    c = workloads.CONFIGS[3]
+    run_both_kpz(K, c["L"], 1, c["p"], c["q"], disorder=c["disorder"], seed=c["seed"], first_sample=c["S"] - 1,
+                 times=c["record_times"], chunks=[7000, 5068])        # through record time 12068
+
+
+def test_config5_full_launch_sampled_against_solo_oracle_runs(K):
+    c = workloads.CONFIGS[5]
+    n, times = 200, [t for t in c["record_times"] if t <= 200]
+    gpu = K.LanesSim(c["L"], c["S"], c["p_a"], c["p_b"], c["rho0"], c["turn_prob"], c["turn_period"], c["omega"],
+                     seed=c["seed"], max_records=len(times))
+    gpu.set_record_times(times)
+    gpu.run(n)
+    a, b, tn = [K.words_to_numpy(x) for x in gpu.state()]
+    cur = gpu.currents()
+    n0 = None
+    for k in (0, 128, 255):
+        ref = R.LanesRef(c["L"], 1, c["p_a"], c["p_b"], c["rho0"], c["turn_prob"], c["turn_period"], c["omega"],
+                         seed=c["seed"], first_sample=k)
+        ref.set_record_times(times)
+        ref.run(n)
+        ra, rb, rt = ref.state()
+        assert np.array_equal(a[k], ra[0]) and np.array_equal(b[k], rb[0]) and np.array_equal(tn[k], rt[0])
+        rc = ref.currents()
+        for key in ("j_a", "j_b", "n_a", "n_b"):
+            assert np.array_equal(cur[key][:, k], rc[key][:, 0]), key
+    # every sample: particles are conserved across the two lanes between the first and the last record
+    tot = cur["n_a"] + cur["n_b"]
+    assert np.all(tot[0] == tot[-1])
+
+
+def test_config5_last_sample_long_run(K):
+    c = workloads.CONFIGS[5]
+    run_both_lanes(K, c["L"], 1, c["p_a"], c["p_b"], c["rho0"], c["turn_prob"], c["turn_period"], c["omega"],
+                   c["seed"], c["record_times"], [2330, 617], first_sample=c["S"] - 1)      # through record time 2947
