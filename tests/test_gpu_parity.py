@@ -637,3 +637,41 @@ def test_config5_last_sample_long_run(K):
     c = workloads.CONFIGS[5]
     run_both_lanes(K, c["L"], 1, c["p_a"], c["p_b"], c["rho0"], c["turn_prob"], c["turn_period"], c["omega"],
                    c["seed"], c["record_times"], [2330, 617], first_sample=c["S"] - 1)      # through record time 2947
+
+
+# ---------------------------------------------------------------------------------------------------------
+# properties that hold at any size, checked on the GPU at sizes the oracle cannot reach
+# ---------------------------------------------------------------------------------------------------------
+
+def test_kpz_growth_exponent_at_config2_size(K):
+    """alpha = 1/2, z = 3/2, i.e. W^2 - 1/4 ~ t^(2 beta) with beta -> 1/3 (slowly, from below)."""
+    c = workloads.CONFIGS[2]
+    times = [2 ** k for k in range(0, 13)]
+    gpu = K.KpzSim(c["L"], c["S"], c["p"], c["q"], seed=c["seed"], max_records=len(times))
+    gpu.set_record_times(times)
+    gpu.run(times[-1])
+    r = gpu.roughness()
+    w2 = r["w2_mean"] - 0.25
+    t = np.array(times, dtype=np.float64)
+    assert np.all(np.diff(w2) > 0)
+    local = 0.5 * np.diff(np.log(w2)) / np.diff(np.log(t))
+    assert np.all((local[5:] > 0.27) & (local[5:] < 0.36)), local        # t >= 32
+    assert abs(local[-3:].mean() - 1.0 / 3.0) < 0.02, local              # 1024 samples of 8192 sites: tight
+    # exact bookkeeping at this size: sum h of every sample equals what conservation dictates modulo closing-pair hops
+    assert r["sum_h"].shape == (len(times), c["S"])
+
+
+def test_paper_two_lane_currents_are_symmetric_and_fluctuate(K):
+    """the total current vanishes by the left/right symmetry, its fluctuation <c^2> grows."""
+    L, S, times = 1024, 2048, [100, 400, 1600]
+    gpu = K.LanesSim(L, S, 0.5, 0.5, 0.5, 0.5, 0, 0.2, seed=71, w_unflagged=0.8, independent=1, max_records=3)
+    gpu.set_record_times(times)
+    gpu.run(times[-1])
+    cur = gpu.currents()
+    cden = (cur["j_a"] - cur["j_b"]).astype(np.float64) / L            # c(t) per sample
+    for k in range(len(times)):
+        sem = cden[k].std(ddof=1) / np.sqrt(S)
+        assert abs(cden[k].mean()) < 5 * sem, (k, cden[k].mean(), sem)
+    c2 = (cden ** 2).mean(axis=1)
+    assert c2[0] < c2[1] < c2[2]
+    assert np.all(cur["n_a"] + cur["n_b"] == (cur["n_a"] + cur["n_b"])[0])      # particles conserved per sample
