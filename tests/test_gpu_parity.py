@@ -675,3 +675,24 @@ def test_paper_two_lane_currents_are_symmetric_and_fluctuate(K):
     c2 = (cden ** 2).mean(axis=1)
     assert c2[0] < c2[1] < c2[2]
     assert np.all(cur["n_a"] + cur["n_b"] == (cur["n_a"] + cur["n_b"])[0])      # particles conserved per sample
+
+
+def test_kpz_finite_size_collapse_at_reduced_scale(K):
+    """PAPER.md:139-145 (Fig. 3) at reduced scale: W^2 - 1/4 of L = 512, 1024, 2048 collapses with the 1+1D KPZ
+    exponents alpha = 1/2, z = 3/2 - and does not with the Q-TASEP pair alpha = 1, z = 1."""
+    from paper_1012_0385_b200 import analysis as A
+    times = [2 ** k for k in range(4, 16)]
+    curves = []
+    for L in (512, 1024, 2048):
+        gpu = K.KpzSim(L, 1024, 0.75, 0.25, seed=81, max_records=len(times))
+        gpu.set_record_times(times)
+        gpu.run(times[-1])
+        r = gpu.roughness()
+        curves.append((L, times, A.w2_mean(L, r["sum_h"], r["sum_h2"])))
+    good = A.collapse_spread(curves, 0.5, 1.5)
+    bad = A.collapse_spread(curves, 1.0, 1.0)
+    assert good < 0.12, (good, bad)
+    assert bad > 4 * good, (good, bad)
+    # the smallest ring has saturated (t >> L^(3/2) = 11585): its width stopped growing, W^2_sat ~ L/12 * O(1)
+    w_small = curves[0][2]
+    assert abs(w_small[-1] / w_small[-2] - 1.0) < 0.08
