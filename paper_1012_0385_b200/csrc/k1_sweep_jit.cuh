@@ -32,8 +32,19 @@
 #define K1J_REFRAME 0  // ... and -3 % / -9 % on the per-sample kernel (1.7 warps per SMSP), which keeps frame 0 per pass
 #endif
 #endif
-#ifndef K1J_EAGER
-#define K1J_EAGER 8  // GENERAL path: planes drawn one MCS ahead; deeper planes are evaluated lazily (6: -5 %, 10: -3 %)
+#ifndef K1J_EAGER  // GENERAL path: planes drawn unconditionally; deeper planes are evaluated lazily
+#ifdef K1J_TILE
+#define K1J_EAGER 12  // blocked stream, planes drawn right before use: a warp needs ~12 planes anyway (8: -9 %, 16: -16 %)
+#else
+#define K1J_EAGER 8   // drawn one MCS ahead (6: -5 %, 10: -3 %)
+#endif
+#endif
+#ifndef K1J_AHEAD  // 1: the planes of MCS m+1 are drawn while MCS m runs (two register sets); 0 (blocked stream only):
+#ifdef K1J_TILE    // drawn right before use - fewer registers, more resident warps (config 4: +3.6 %)
+#define K1J_AHEAD 0
+#else
+#define K1J_AHEAD 1
+#endif
 #endif
 #ifndef K1J_TRIP  // GENERAL path: planes per lazy trip
 #if defined(K1J_TILE) || defined(K1J_STREAM)
@@ -472,11 +483,11 @@ __device__ __forceinline__ void mcs_step(Ctx& c, const Planes& Rc, Planes& Rn, c
                                          uint32_t* halo) {
   const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
   if (K1J_OFFSET_MODE == 1 && !GENERAL) {
-    draw_planes(Rn, K, c.G, c.gs, m + 1);
+    if (K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
     mcs_logic<0, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
   } else if (K1J_VARIANT == 1 || GENERAL || SPW > 1) {
     const uint32_t code = K1J_OFFSET_MODE == 1 ? 2u : (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
-    draw_planes(Rn, K, c.G, c.gs, m + 1);
+    if (K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
     if (K1J_REFRAME && SPW == 1) {  // one exchange per frame change, the frame is carried across MCS
       reframe(c.P, c.un, c.frame, code & 1u, halo, c.parity);
       pass_branchfree(c.P, c.Q, c.tags, Rc.r[0], c.un, code & 1u, halo, c.parity, K, c.G, c.gs, tlo,
@@ -499,19 +510,19 @@ __device__ __forceinline__ void mcs_step(Ctx& c, const Planes& Rc, Planes& Rn, c
     const uint32_t code = (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
     switch (code) {
       case 0:
-        draw_planes(Rn, K, c.G, c.gs, m + 1);
+        if (K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
         mcs_logic<0, 0>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
         break;
       case 1:
-        draw_planes(Rn, K, c.G, c.gs, m + 1);
+        if (K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
         mcs_logic<1, 0>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
         break;
       case 2:
-        draw_planes(Rn, K, c.G, c.gs, m + 1);
+        if (K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
         mcs_logic<0, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
         break;
       default:
-        draw_planes(Rn, K, c.G, c.gs, m + 1);
+        if (K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
         mcs_logic<1, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
         break;
     }
@@ -770,16 +781,27 @@ kpz_k3t_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__
   const long long t_end = A.t0 + A.n_mcs;
   long long m = A.t0;
   if (K1J_OFFSET_MODE == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
-  Planes RA, RB;
-  draw_planes(RA, D.keys, c.G, c.gs, m);
-  while (m < t_end) {
-    mcs_step(c, RA, RB, D.keys, m, nullptr);
-    ++m;
-    if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
-    if (m >= t_end) break;
-    mcs_step(c, RB, RA, D.keys, m, nullptr);
-    ++m;
-    if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+  if (K1J_AHEAD) {
+    Planes RA, RB;
+    draw_planes(RA, D.keys, c.G, c.gs, m);
+    while (m < t_end) {
+      mcs_step(c, RA, RB, D.keys, m, nullptr);
+      ++m;
+      if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+      if (m >= t_end) break;
+      mcs_step(c, RB, RA, D.keys, m, nullptr);
+      ++m;
+      if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+    }
+  } else {
+    Planes RA;
+#pragma unroll 1
+    while (m < t_end) {
+      draw_planes(RA, D.keys, c.G, c.gs, m);
+      mcs_step(c, RA, RA, D.keys, m, nullptr);
+      ++m;
+      if (K1J_OFFSET_MODE == 0 && ((int)m & 15) == 0) c.offbits = draw_offsets16(D.keys, c.gs, m);
+    }
   }
   if (c.frame) reframe(c.P, c.un, c.frame, 0u, nullptr, c.parity);
   if (lane >= 1 && lane <= TI && tile * TI + lane - 1 < U) {

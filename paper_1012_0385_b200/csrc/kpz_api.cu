@@ -201,6 +201,10 @@ std::vector<std::string> k1_jit_defines(const KpzDev& D, int dis) {
     snprintf(buf, sizeof buf, "K1J_EAGER=%d", atoi(v));
     d.push_back(buf);
   }
+  if (const char* v = std::getenv("KPZ_B200_K1_AHEAD")) {  // tuning knob (blocked stream): 0 = planes drawn right before use
+    snprintf(buf, sizeof buf, "K1J_AHEAD=%d", atoi(v));
+    d.push_back(buf);
+  }
   if (const char* v = std::getenv("KPZ_B200_K1_TRIP")) {  // tuning knob: planes per lazy trip of the GENERAL path
     snprintf(buf, sizeof buf, "K1J_TRIP=%d", atoi(v));
     d.push_back(buf);
