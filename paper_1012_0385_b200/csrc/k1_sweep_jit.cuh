@@ -46,6 +46,9 @@
 #define K1J_AHEAD 1
 #endif
 #endif
+#if !defined(K1J_TILE) && K1J_AHEAD == 0
+#error "K1J_AHEAD = 0 is implemented by the blocked-stream kernel only"
+#endif
 #ifndef K1J_TRIP  // GENERAL path: planes per lazy trip
 #if defined(K1J_TILE) || defined(K1J_STREAM)
 #define K1J_TRIP 1  // many warps per SM: pipe-bound, never draw a plane that may not be needed (config 4: +5 %)

@@ -201,10 +201,6 @@ std::vector<std::string> k1_jit_defines(const KpzDev& D, int dis) {
     snprintf(buf, sizeof buf, "K1J_EAGER=%d", atoi(v));
     d.push_back(buf);
   }
-  if (const char* v = std::getenv("KPZ_B200_K1_AHEAD")) {  // tuning knob (blocked stream): 0 = planes drawn right before use
-    snprintf(buf, sizeof buf, "K1J_AHEAD=%d", atoi(v));
-    d.push_back(buf);
-  }
   if (const char* v = std::getenv("KPZ_B200_K1_TRIP")) {  // tuning knob: planes per lazy trip of the GENERAL path
     snprintf(buf, sizeof buf, "K1J_TRIP=%d", atoi(v));
     d.push_back(buf);
@@ -393,6 +389,9 @@ int k3t_run(kpz_sim* sim, int64_t n_mcs) {
   const int dis = sim->has_sq ? 2 : sim->has_sp ? 1 : 0;
   std::vector<std::string> defs = k1_jit_defines(sim->dev, dis);
   defs.push_back("K1J_TILE=1");
+  if (const char* v = std::getenv("KPZ_B200_K1_AHEAD")) {  // tuning knob (blocked stream only): 1 = planes drawn one MCS ahead
+    defs.push_back(std::string("K1J_AHEAD=") + (atoi(v) ? "1" : "0"));
+  }
   void* kfn = nullptr;
   int rc = jit_get("k1_sweep_jit.cuh", "kpz_k3t_sweep_jit", defs, &kfn);
   if (rc) return rc;
