@@ -17,7 +17,8 @@
  *   two-lane .................. brute-force two-lane master equation, conservation, A-lane == KPZ ring at omega=0
  * PARITY UNPINNED (convention only, fixed by DESIGN.md, no external source): the bit-plane layout of
  * the uniforms (§R4), the counter packing / stream tags (§R4), the drawn-offset reading (§R1) beyond
- * its master-equation statistics, two-lane step order (§R12) and profile semantics (§R16).
+ * its master-equation statistics, two-lane step order (§R12), profile semantics (§R16), and for the site-wise
+ * crossing model (§R18) the "once per run" reading of the flag redraw and the TURN_V stream tag.
  */
 #include "kpz_oracle.h"
 
