@@ -696,3 +696,48 @@ def test_kpz_finite_size_collapse_at_reduced_scale(K):
     # the smallest ring has saturated (t >> L^(3/2) = 11585): its width stopped growing, W^2_sat ~ L/12 * O(1)
     w_small = curves[0][2]
     assert abs(w_small[-1] / w_small[-2] - 1.0) < 0.08
+
+
+# ---------------------------------------------------------------------------------------------------------
+# seeded random differential test: parameters nobody picked by hand
+# ---------------------------------------------------------------------------------------------------------
+
+_DYADIC = [0.0, 0.125, 0.25, 0.375, 0.5, 0.75, 1.0]
+
+
+def _rand_prob(rng):
+    return float(rng.choice(_DYADIC)) if rng.random() < 0.5 else float(np.round(rng.random(), 3))
+
+
+@pytest.mark.parametrize("case", range(36))
+def test_random_kpz_configurations(K, case):
+    rng = np.random.default_rng(1000 + case)
+    L = 64 * int(rng.choice([1, 2, 3, 4, 5, 8, 16, 31, 32, 33, 64, 65, 100, 128, 200]))
+    S = int(rng.integers(1, 6))
+    p, q = _rand_prob(rng), _rand_prob(rng)
+    dis = None
+    if rng.random() < 0.5:
+        dis = (float(np.round(rng.random(), 2)), _rand_prob(rng), float(np.round(rng.random(), 2)) * (rng.random() < 0.6),
+               _rand_prob(rng))
+    path = int(rng.choice([0, 1, 2, 3]))
+    mode = int(rng.random() < 0.3)
+    n1, n2 = int(rng.integers(1, 40)), int(rng.integers(1, 40))
+    times = sorted(set(int(x) for x in rng.integers(1, n1 + n2 + 1, size=3)))
+    start = None
+    if rng.random() < 0.5:
+        start = R.pack_sites((rng.random((S, L)) < rng.random()).astype(np.uint8))
+    run_both_kpz(K, L, S, p, q, disorder=dis, seed=int(rng.integers(0, 2**40)), first_sample=int(rng.integers(0, 50)),
+                 offset_mode=mode, path=path, times=times, chunks=[n1, n2], start=start)
+
+
+@pytest.mark.parametrize("case", range(18))
+def test_random_two_lane_configurations(K, case):
+    rng = np.random.default_rng(2000 + case)
+    L = 64 * int(rng.choice([1, 2, 3, 4, 5, 8, 16, 33, 64, 100]))
+    S = int(rng.integers(1, 4))
+    crossing = rng.random() < 0.5
+    run_both_lanes(K, L, S, _rand_prob(rng), _rand_prob(rng), float(np.round(rng.random(), 2)),
+                   float(np.round(rng.random(), 2)), int(rng.choice([0, 1, 3, 7, 10])), _rand_prob(rng),
+                   seed=int(rng.integers(0, 2**40)), times=[1, 5, 19], chunks=[int(rng.integers(1, 12)), int(rng.integers(1, 12))],
+                   first_sample=int(rng.integers(0, 9)), offset_mode=int(rng.random() < 0.3),
+                   w_unflagged=_rand_prob(rng) if crossing else None, independent=int(rng.random() < 0.5) if crossing else 0)
