@@ -48,6 +48,9 @@ constexpr int U = (W + 3) / 4;
 constexpr bool SINGLE_WARP = U <= 32;
 constexpr bool PARTIAL = (W % 4) != 0;
 constexpr int NTHREADS = (U + 31) / 32 * 32;
+// Small rings (the paper's L = 512 ... 2048): U <= 16 supergroups fill only U lanes, so a warp sweeps SPW = 32 / U
+// independent samples side by side; offsets and record sums become per-lane values (segments of U lanes).
+constexpr int SPW = (!PARTIAL && U <= 16 && (U & (U - 1)) == 0) ? 32 / U : 1;
 constexpr uint64_t TPA = K4J_TPA, TPB = K4J_TPB, TOMEGA = K4J_TOMEGA, TTURN = K4J_TTURN;
 constexpr uint64_t kOne = 1ull << 32;
 constexpr uint32_t FULL = 0xFFFFFFFFu;
@@ -113,9 +116,9 @@ __device__ __forceinline__ void resolve(uint32_t (&lt)[4], uint32_t (&eq)[4], co
 // (lane l draws plane pl0 + l), a ballot per undecided element assembles the rest of its uniform, and one integer
 // comparison with the rest of T finishes it: one Philox call of the warp per undecided supergroup instead of two
 // per pair of planes.  Same result as resolve<T>() by construction (U < T with an equal prefix <=> suffix(U) <
-// suffix(T)).  `u0` = supergroup index of lane 0 of this warp.
+// suffix(T)).
 template <uint64_t T>
-__device__ __forceinline__ void resolve_tail(uint32_t (&lt)[4], uint32_t (&eq)[4], const PhiloxKeys& K, uint32_t u0,
+__device__ __forceinline__ void resolve_tail(uint32_t (&lt)[4], uint32_t (&eq)[4], const PhiloxKeys& K, uint32_t G,
                                              uint32_t gs, uint32_t tlo, uint32_t c3, int pl0) {
   const int lane = threadIdx.x & 31;
   const uint32_t t_suffix = (uint32_t)T & (pl0 > 0 ? (0xFFFFFFFFu >> pl0) : 0xFFFFFFFFu);
@@ -124,7 +127,8 @@ __device__ __forceinline__ void resolve_tail(uint32_t (&lt)[4], uint32_t (&eq)[4
     const int src = __ffs(todo) - 1;
     todo &= todo - 1;
     const int pl = pl0 + lane;
-    const uint4 v = philox4x32_10(u0 + (uint32_t)src, gs, tlo, c3 | ((uint32_t)(pl < 32 ? pl : 31) << 22), K);
+    const uint32_t Gs = __shfl_sync(FULL, G, src), gss = __shfl_sync(FULL, gs, src);  // the owner's supergroup, sample
+    const uint4 v = philox4x32_10(Gs, gss, tlo, c3 | ((uint32_t)(pl < 32 ? pl : 31) << 22), K);
     const uint32_t R[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
@@ -325,7 +329,7 @@ __device__ __forceinline__ void lane_change(uint32_t (&SRC)[4], uint32_t (&DST)[
 #pragma unroll
       for (int pl = 0; pl < EAGER; ++pl) plane_step<TOMEGA>(lt, eq, r[pl], pl);
       if (EAGER < NPW) {
-        if (K4J_TAIL) resolve_tail<TOMEGA>(lt, eq, K, (uint32_t)(un.u & ~31), un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
+        if (K4J_TAIL) resolve_tail<TOMEGA>(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
         else resolve<TOMEGA>(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
       }
     }
@@ -377,16 +381,21 @@ __device__ __forceinline__ void draw_turn(uint32_t (&T)[4], const PhiloxKeys& K,
 
 // Epoch-end occupancy profile: occ[site] += bit.  The warp transposes its 32 x 4 words so that lane l
 // adds the bits of sites 32 j + l: every red.global.add of the warp covers 128 consecutive bytes.
-__device__ __forceinline__ void add_profile(const uint32_t (&X)[4], uint32_t* occ_sample) {
+__device__ __forceinline__ void add_profile(const uint32_t (&X)[4], uint32_t* occ, int S) {
   const int lane = threadIdx.x & 31;
-  const int warp_base = (threadIdx.x & ~31) * 128;  // first site of this warp
 #pragma unroll 1
   for (int t = 0; t < 32; ++t) {
+    // source lane t of this warp holds supergroup g of sample smp
+    const int thr = (int)(threadIdx.x & ~31u) + t;
+    const int smp = SPW > 1 ? (int)blockIdx.x * SPW + thr / U : (int)blockIdx.x;
+    const int g = SPW > 1 ? thr % U : thr;
+    const bool ok = smp < S && g < U;
+    uint32_t* dst = occ + (size_t)smp * (32 * W) + 128 * g;
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
       const uint32_t v = __shfl_sync(FULL, X[w], t);
-      const int site = warp_base + 128 * t + 32 * w + lane;
-      if (((v >> lane) & 1u) && site < 32 * W) atomicAdd(occ_sample + site, 1u);
+      const int site = 128 * g + 32 * w + lane;
+      if (ok && ((v >> lane) & 1u) && site < 32 * W) atomicAdd(dst + 32 * w + lane, 1u);
     }
   }
 }
@@ -408,14 +417,22 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
   using namespace kpz::k4j;
   __shared__ uint32_t halo[SINGLE_WARP ? 1 : 2 * NTHREADS];
   __shared__ unsigned long long red[SINGLE_WARP ? 1 : 4 * 32];
-  const int s = blockIdx.x;
+  // SPW == 1: CTA = sample, thread = supergroup.  SPW > 1: CTA = one warp = SPW samples, lane = (sample, supergroup).
+  int sub = 0, s = (int)blockIdx.x, lane0 = 0;
   const int lane = threadIdx.x & 31;
   Unit un;
   un.u = threadIdx.x;
-  const bool active = un.u < U;
+  bool active = un.u < U;
+  if constexpr (SPW > 1) {
+    sub = (int)threadIdx.x / U;
+    s = (int)blockIdx.x * SPW + sub;
+    un.u = (int)threadIdx.x % U;
+    lane0 = sub * U;
+    active = s < D.S;
+  }
   un.nwn = !active ? 0 : (PARTIAL ? min(4, W - 4 * un.u) : 4);
-  un.nxt = (un.u + 1 >= U) ? 0 : un.u + 1;
-  un.prv = (un.u == 0) ? U - 1 : un.u - 1;
+  un.nxt = lane0 + ((un.u + 1 >= U) ? 0 : un.u + 1);
+  un.prv = lane0 + ((un.u == 0) ? U - 1 : un.u - 1);
   un.gs = (uint32_t)(D.first_sample + s);
   const unsigned long long row = (unsigned long long)s * D.Wp + 4ull * (active ? un.u : 0);
   int parity = 0;
@@ -444,7 +461,18 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
   long long epoch = period > 0 ? m / period : 0;
   long long in_epoch = period > 0 ? m - epoch * period : 0;  // m mod period
   uint32_t offbits = 0;
-  if (K4J_OFFSET_MODE == 0) offbits = draw_offsets16(D.keys, un.gs, m);
+  auto draw_offsets = [&]() {
+    if constexpr (SPW == 1) {
+      offbits = draw_offsets16(D.keys, un.gs, m);
+    } else {
+#pragma unroll 1
+      for (int k = 0; k < SPW; ++k) {  // one ballot per sample of this warp; each lane keeps its own sample's
+        const uint32_t b = draw_offsets16(D.keys, (uint32_t)(D.first_sample + (int)blockIdx.x * SPW + k), m);
+        if (k == sub) offbits = b;
+      }
+    }
+  };
+  if (K4J_OFFSET_MODE == 0) draw_offsets();
 
   auto block_sum4 = [&](unsigned long long v0, unsigned long long v1, unsigned long long v2, unsigned long long v3,
                         unsigned long long (&out)[4]) {
@@ -452,10 +480,10 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
 #pragma unroll
     for (int k = 0; k < 4; ++k)
 #pragma unroll
-      for (int d = 16; d >= 1; d >>= 1) v[k] += __shfl_down_sync(FULL, v[k], d);
+      for (int d = (SPW > 1 ? U : 32) / 2; d >= 1; d >>= 1) v[k] += __shfl_down_sync(FULL, v[k], d, SPW > 1 ? U : 32);
     if (SINGLE_WARP) {
 #pragma unroll
-      for (int k = 0; k < 4; ++k) out[k] = v[k];  // valid in lane 0
+      for (int k = 0; k < 4; ++k) out[k] = v[k];  // valid in the first lane of each sample
     } else {
       const int warp = threadIdx.x >> 5;
       __syncthreads();
@@ -492,7 +520,7 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
         // rate 1 in both lanes (config 5): the hop over a thread boundary is decided by old bits alone,
         // so both sides compute it from ONE exchange: first bits go to the previous thread, last bits to the next
         uint32_t nx = 0, in = 0;
-        if (o) {
+        if (SPW > 1 || o) {  // (per-lane offsets when a warp holds several samples: every lane joins the shuffle)
           uint32_t lastA = A[3], lastB = B[3];
           if (PARTIAL) {
             lastA = un.nwn >= 4 ? A[3] : A[1];
@@ -501,9 +529,9 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
           const uint32_t mine = (A[0] & 1u) | ((B[0] & 1u) << 1) | ((lastA >> 31) << 2) | ((lastB >> 31) << 3);
           uint32_t vn, vp;
           unit_exchange2(mine, un.nxt, un.prv, vn, vp, halo, parity);
-          nx = active ? (vn & 3u) : 0u;  // idle threads hold all-zero words and must not see a neighbour bit
+          nx = (active && o) ? (vn & 3u) : 0u;  // idle threads hold all-zero words and must not see a neighbour bit
           // lane A: particle on the previous thread's last site, hole on my first; lane B: the other way round
-          in = active ? (((vp >> 2) & ~A[0] & 1u) | ((~(vp >> 3) & B[0] & 1u) << 1)) : 0u;
+          in = (active && o) ? (((vp >> 2) & ~A[0] & 1u) | ((~(vp >> 3) & B[0] & 1u) << 1)) : 0u;
         }
         lane_pass<true, TPA>(A, un, o, nx & 1u, D.keys, TAG_PAIR, tlo, c3t, jA);
         lane_pass<false, TPB>(B, un, o, nx >> 1, D.keys, TAG_PAIR_B, tlo, c3t, jB);
@@ -511,13 +539,13 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
         B[0] ^= in >> 1;
       } else {
         uint32_t nx = 0;
-        if (o) {
+        if (SPW > 1 || o) {
           nx = unit_exchange((A[0] & 1u) | ((B[0] & 1u) << 1), un.nxt, halo, parity);
-          if (!active) nx = 0;
+          if (!active || !o) nx = 0;
         }
         const uint32_t cA = lane_pass<true, TPA>(A, un, o, nx & 1u, D.keys, TAG_PAIR, tlo, c3t, jA);
         const uint32_t cB = lane_pass<false, TPB>(B, un, o, nx >> 1, D.keys, TAG_PAIR_B, tlo, c3t, jB);
-        if (o) {
+        if (SPW > 1 || o) {  // the carries are zero in an offset-0 pass
           const uint32_t in = unit_exchange(cA | (cB << 1), un.prv, halo, parity);
           if (active) {
             A[0] ^= in & 1u;
@@ -533,14 +561,14 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
     if (period > 0 && ++in_epoch == period) {
       in_epoch = 0;
       ++epoch;
-      add_profile(A, D.occA + (size_t)s * 32 * W);  // occupancy profile at epoch ends
-      add_profile(B, D.occB + (size_t)s * 32 * W);
+      add_profile(A, D.occA, D.S);  // occupancy profile at epoch ends
+      add_profile(B, D.occB, D.S);
     }
     if (m == next_rec) {
       unsigned long long tot[4];
       block_sum4(jA, jB, (unsigned long long)(__popc(A[0]) + __popc(A[1]) + __popc(A[2]) + __popc(A[3])),
                  (unsigned long long)(__popc(B[0]) + __popc(B[1]) + __popc(B[2]) + __popc(B[3])), tot);
-      if (threadIdx.x == 0) {
+      if (SPW > 1 ? (un.u == 0 && active) : threadIdx.x == 0) {
         const size_t cell = (size_t)ri * D.S + s, plane = (size_t)R.nt * D.S;
         R.rec[cell] = (long long)(D.JA[s] + tot[0]);
         R.rec[plane + cell] = (long long)(D.JB[s] + tot[1]);
@@ -550,7 +578,7 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
       ++ri;
       next_rec = ri < R.nt ? R.rec_t[ri] : -1;
     }
-    if (K4J_OFFSET_MODE == 0 && ((int)m & 15) == 0) offbits = draw_offsets16(D.keys, un.gs, m);
+    if (K4J_OFFSET_MODE == 0 && ((int)m & 15) == 0) draw_offsets();
   };
 
   while (m < t_end) {
@@ -562,7 +590,7 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
   {
     unsigned long long tot[4];
     block_sum4(jA, jB, 0, 0, tot);
-    if (threadIdx.x == 0) {
+    if (SPW > 1 ? (un.u == 0 && active) : threadIdx.x == 0) {
       D.JA[s] += tot[0];
       D.JB[s] += tot[1];
     }

@@ -316,8 +316,12 @@ int lanes_run(lanes_sim* sim, int64_t n_mcs) {
     int rc = jit_get("k4_lanes_jit.cuh", "lanes_k4_sweep_jit", k4_jit_defines(D), &kfn);
     if (rc) return rc;
     void* args[] = {(void*)&D, (void*)&A};
-    const int block4 = ((D.W + 3) / 4 + 31) / 32 * 32;  // one thread per 128-site supergroup
-    KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(sim->S), dim3(block4), args, 0, sim->stream));
+    const int U4 = (D.W + 3) / 4;                      // one thread per 128-site supergroup
+    const int block4 = (U4 + 31) / 32 * 32;
+    // small rings (k4_lanes_jit.cuh, SPW): U4 <= 16 supergroups, a power of two, no ragged word -> 32/U4 samples per warp
+    const bool pack = (D.W % 4) == 0 && U4 <= 16 && (U4 & (U4 - 1)) == 0;
+    const int spw = pack ? 32 / U4 : 1;
+    KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((sim->S + spw - 1) / spw), dim3(block4), args, 0, sim->stream));
   } else if (D.independent || D.t_w0.value != 0 || D.t_w0.always) {
     return fail(KPZ_EUNSUPPORTED, "the site-wise crossing model runs on the run-time specialised kernel only "
                                   "(L <= 131072, KPZ_B200_JIT not 0)");
