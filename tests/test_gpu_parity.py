@@ -741,3 +741,14 @@ def test_random_two_lane_configurations(K, case):
                    seed=int(rng.integers(0, 2**40)), times=[1, 5, 19], chunks=[int(rng.integers(1, 12)), int(rng.integers(1, 12))],
                    first_sample=int(rng.integers(0, 9)), offset_mode=int(rng.random() < 0.3),
                    w_unflagged=_rand_prob(rng) if crossing else None, independent=int(rng.random() < 0.5) if crossing else 0)
+
+
+@pytest.mark.parametrize("L,S", [(512, 37), (1024, 9), (2048, 5)])
+def test_two_lane_small_rings_packed_per_warp(K, L, S):
+    """Rings of 4 ... 16 supergroups are swept 32/U samples per warp (k4_lanes_jit.cuh, SPW): sample counts that do
+    not fill the last warp, per-sample offsets / hop counters / records / profile snapshots, both models."""
+    run_both_lanes(K, L, S, 1.0, 1.0, 0.3, 0.05, 5, 0.1, seed=L + 1, times=[1, 5, 11, 23], chunks=[11, 12],
+                   first_sample=3)
+    run_both_lanes(K, L, S, 0.5, 0.5, 0.5, 0.5, 4, 0.2, seed=L + 2, times=[7, 16], chunks=[16], w_unflagged=0.8,
+                   independent=1)
+    run_both_lanes(K, L, S, 0.75, 0.5, 0.4, 0.3, 0, 0.3, seed=L + 3, times=[9], chunks=[9], offset_mode=1)
