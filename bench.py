@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — site-update throughput of the KPZ/ASEP hot path on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|5|4-aux-i|4-aux-ii|4-aux-i-blocked|paper-1024x30|paper-1024-fill|paper-qtasep-16384|paper-qssep-4096|paper-lanes-4096] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|5|2-fill|3-fill|4-aux-i|4-aux-ii|4-aux-i-blocked|paper-1024x30|paper-1024-fill|paper-qtasep-16384|paper-qssep-4096|paper-lanes-4096] [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: reset to the
 initial state (a1), run the configuration's full number of MCS with its record times (a2-a7 / a9), records left in
@@ -53,6 +53,8 @@ ALU_SLOTS_PER_SU = {
     3: (2 * 1 * 34 + 2 * 4 * 3 + 4) / 256,          # 1 plane (slow sites only)
     4: (2 * 7.33 * (34 + 12) + 2 * 4 * 3 + 4) / 256,  # 32-plane thresholds: log2(64)+1.33 planes per unit and pass
     5: (2 * 2.0 * 34 + 2 * 2 * 4 * 5 + 2 * 4 * 4) / 256,  # two-lane: lane changes dominate
+    "2-fill": (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,
+    "3-fill": (2 * 1 * 34 + 2 * 4 * 3 + 4) / 256,
     "4-aux-i": (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,
     "4-aux-ii": (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,
     "4-aux-i-blocked": (2 * 2 * 34 + 2 * 4 * 3 + 4) / 256,

@@ -52,6 +52,13 @@ CONFIGS = {
             n_mcs=1000, record_times=_T20_1E3, seed=4),
     5: dict(name="config5_lanes_L16384_S256", kind="lanes", L=16384, S=256, p_a=1.0, p_b=1.0, rho0=0.3,
             turn_prob=0.05, turn_period=100, omega=0.1, n_mcs=100_000, record_times=_T50_1E5, seed=5),
+    # Configs 2 and 3 with sample counts that fill a B200's warp slots evenly (592 SMSPs x 2 resp. 4 warps): the
+    # BASELINE.json counts (1024 one-warp rings, 512 two-warp rings) leave 13.5 % of the second slots empty.
+    "2-fill": dict(name="config2_shape_S1184", kind="kpz", L=8192, S=1184, p=0.75, q=0.25, disorder=None,
+                   n_mcs=10_000, record_times=_T40_1E4, seed=2),
+    "3-fill": dict(name="config3_shape_S1184", kind="kpz", L=16384, S=1184, p=1.0, q=0.0,
+                   disorder=(0.1, 0.5, 0.0, 0.0), n_mcs=20_000, record_times=[t for t in _T50_1E5 if t <= 20_000] + [20_000],
+                   seed=3),
     # Auxiliary streamed runs: dyadic rates, the pass-by-pass streamed kernel (path 2) forced, so
     # that the sweep is bandwidth-bound: (i) ring in L2, (ii) ring beyond L2 (the HBM roofline case).
     "4-aux-i": dict(name="config4aux1_stream_L2p28_p075_q025", kind="kpz", L=1 << 28, S=1, p=0.75, q=0.25,
