@@ -13,7 +13,7 @@
 //   K1J_T0..K1J_T3    thresholds T(p), T(p_slow), T(q), T(q_slow) as integers in [0, 2^32]
 //   K1J_DIS           0 no disorder tags, 1 slow-p tags, 2 slow-p and slow-q tags
 //   K1J_OFFSET_MODE   0 drawn offsets, 1 alternating
-//   K1J_VARIANT       code shape of the drawn-offset sweep (see pass_branchfree)
+//   K1J_VARIANT       code shape of the drawn-offset sweep (see below and pass_branchfree)
 //
 // Layout on chip: as K1 v1 (kpz_k1.cuh): thread = one unit = 128 pairs = one Philox supergroup, 4 even-site words
 // P[4] and 4 odd-site words Q[4] in registers; frame 0 pairs (P,Q) = sites (2k,2k+1), frame 1 pairs (Q,P') with P'
@@ -22,8 +22,12 @@
 #include "sweep_types.cuh"
 #include "height_lut.cuh"
 
-#ifndef K1J_VARIANT
-#define K1J_VARIANT 1  // 0: one code path per offset pair (4-way switch); 1: branch-free
+#ifndef K1J_VARIANT  // code shape of the drawn-offset sweep on the LUT path:
+#ifdef K1J_TILE      //   0: one code path per offset pair (4-way switch) with the Philox rounds repeated inside each;
+#define K1J_VARIANT 2  // 1: branch-free (roles by mask, shifts by the offset): one basic block per MCS, most slots;
+#else                //   2: 4-way switch after the Philox rounds: fewest alu slots, no overlap inside a warp.
+#define K1J_VARIANT 1  // Measured: per-sample kernel (1.7 warps per SMSP) 1 >> 0, 2 (config 2: 19.3 / 17.4 / 16.0
+#endif               // TSU/s); blocked stream (many warps hide the latency) 2 > 1 (20.8 vs 19.4 TSU/s).
 #endif
 #ifndef K1J_REFRAME
 #ifdef K1J_TILE
@@ -511,21 +515,23 @@ __device__ __forceinline__ void mcs_step(Ctx& c, const Planes& Rc, Planes& Rn, c
     }
   } else {
     const uint32_t code = (c.offbits >> (2 * ((int)m & 15))) & 3u;  // o0 | o1 << 1
+    constexpr bool INSIDE = K1J_VARIANT == 0;  // variant 0: the Philox rounds are repeated inside every code path;
+    if (!INSIDE && K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);  // variant 2: drawn once, before the switch
     switch (code) {
       case 0:
-        if (K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
+        if (INSIDE && K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
         mcs_logic<0, 0>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
         break;
       case 1:
-        if (K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
+        if (INSIDE && K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
         mcs_logic<1, 0>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
         break;
       case 2:
-        if (K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
+        if (INSIDE && K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
         mcs_logic<0, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
         break;
       default:
-        if (K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
+        if (INSIDE && K1J_AHEAD) draw_planes(Rn, K, c.G, c.gs, m + 1);
         mcs_logic<1, 1>(c.P, c.Q, c.tags, Rc, c.un, halo, c.parity);
         break;
     }
