@@ -65,3 +65,12 @@ def test_bad_arguments_are_refused_without_compiling(K):
         K.jit_check(64, 1.5, 0.5)
     with pytest.raises(K.KpzError):
         K.lanes_jit_check(64, 1.0, 1.0, 0.05, -1, 0.1)
+
+
+@pytest.mark.parametrize("variant", ["0", "1", "2"])
+def test_every_code_shape_of_the_sweep_compiles(K, variant, monkeypatch):
+    """K1J_VARIANT: 4-way switch with the Philox rounds inside, branch-free, 4-way switch after the Philox rounds."""
+    monkeypatch.setenv("KPZ_B200_K1_VARIANT", variant)
+    assert K.jit_check(8192, 0.75, 0.25) > 10_000
+    assert K.jit_check(16384, 1.0, 0.0, disorder=(0.1, 0.5, 0.0, 0.0)) > 10_000
+    assert K.jit_check(1 << 20, 0.75, 0.25, path=3) > 10_000
