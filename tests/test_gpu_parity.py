@@ -431,7 +431,8 @@ class _env:
                 os.environ[k] = v
 
 
-@pytest.mark.parametrize("env", [dict(KPZ_B200_JIT=0), dict(KPZ_B200_K1_VARIANT=0)])
+@pytest.mark.parametrize("env", [dict(KPZ_B200_JIT=0), dict(KPZ_B200_K1_VARIANT=0), dict(KPZ_B200_K1_VARIANT=2),
+                                 dict(KPZ_B200_K1_REFRAME=1), dict(KPZ_B200_K1_EAGER=3, KPZ_B200_K1_TRIP=3)])
 def test_k1_variants_against_oracle(K, env):
     with _env(**env):
         run_both_kpz(K, 8192 + 64, 3, 0.75, 0.25, seed=21, times=[1, 3, 20], chunks=[7, 13])
