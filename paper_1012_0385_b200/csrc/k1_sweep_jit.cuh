@@ -1,12 +1,14 @@
 // k1_sweep_jit.cuh — K1 v2: the on-chip per-sample sweep specialised at run time (NVRTC, see jit.cu) on the
 // ring size and on the four acceptance thresholds (north_star (1),(3)).
 //
-// Why specialise.  The sweep is integer work on two pipes: Philox needs 20 IMAD.WIDE per call (fmaheavy pipe,
-// measured 0.25 warp-instr/clk/SMSP on B200) and 20 LOP3 (alu pipe, 0.5/clk); the pair logic is LOP3 only.  With
-// thresholds known at compile time the lazy MSB-first comparison U < T folds into a fixed boolean
-// function of the few bit-planes T needs, so the logic costs ~4 LOP3 per 32 pairs instead of ~15, the plane count
-// is a constant, and the Philox calls of the NEXT MCS (counter-based, state-independent) are issued in the same
-// basic block as the logic of the current one: the kernel runs at the IMAD.WIDE rate of the Philox rounds.
+// Why specialise.  The sweep is integer work bound by alu-pipe slots (LOP3 / SHF and - because it
+// also takes an alu slot - IMAD.WIDE issue at 0.5 warp-instr/clk/SMSP; a Philox call is 20 IMAD.WIDE + 20 LOP3).  With
+// the thresholds known at compile time the lazy MSB-first comparison U < T folds into a fixed boolean
+// function of the few bit-planes T needs, so the pair logic costs 3-4 LOP3 per 32 pairs instead of ~15, the plane count
+// is a constant, and the Philox calls of the NEXT MCS (counter-based, state-independent) are issued in the same basic
+// block as the logic of the current one.  One source, three entry points: kpz_k1_sweep_jit (a CTA per sample, the whole
+// run on chip), kpz_k3t_sweep_jit (K1J_TILE: 32-unit windows of a long ring, 32 MCS per trip through HBM) and
+// kpz_k3_pass_jit (K1J_STREAM: one sub-lattice pass per launch).
 //
 // Compile-time configuration (all -D macros, set by jit.cu):
 //   K1J_PW            pair-words (64-site groups) per sample = L/64
