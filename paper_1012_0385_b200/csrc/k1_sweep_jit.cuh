@@ -193,31 +193,76 @@ __host__ __device__ constexpr uint32_t tbit(uint64_t T, int pl) { return (uint32
 __host__ __device__ constexpr uint32_t is_always(uint64_t T) { return T >= kOne ? 1u : 0u; }
 __host__ __device__ constexpr uint32_t is_partial(uint64_t T) { return (T > 0 && T < kOne) ? 1u : 0u; }
 
+// MSB-first comparison of ONE rate class against its constant threshold T: eq = pairs of the class whose prefix still
+// equals T's, lt |= pairs decided "U < T".  A plane whose T bit is 0 costs one LOP3 per word, a 1 bit two; once T has no
+// bit left below, an equal prefix can no longer become "less" and the class drops out.
+template <uint64_t T>
+__device__ __forceinline__ void class_planes_eager(uint32_t (&lt)[4], uint32_t (&eq)[4], const uint32_t (&r)[NPSA][4]) {
+  if constexpr (T > 0 && T < kOne) {
+#pragma unroll
+    for (int pl = 0; pl < NEAG; ++pl) {
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        if (pl >= planes_of(T)) {
+          eq[w] = 0u;
+        } else if (tbit(T, pl)) {
+          lt[w] |= eq[w] & ~r[pl][w];
+          eq[w] &= r[pl][w];
+        } else {
+          eq[w] &= ~r[pl][w];
+        }
+      }
+    }
+  }
+}
+template <uint64_t T>
+__device__ __forceinline__ void class_plane_lazy(uint32_t (&lt)[4], uint32_t (&eq)[4], const uint32_t (&R)[4], int pl) {
+  if constexpr (T > 0 && T < kOne) {
+    if (pl >= planes_of(T)) {  // warp-uniform
+#pragma unroll
+      for (int w = 0; w < 4; ++w) eq[w] = 0u;
+    } else {
+      const uint32_t tb = 0u - ((uint32_t)(T >> (31 - pl)) & 1u);
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        lt[w] |= eq[w] & tb & ~R[w];
+        eq[w] &= ~(R[w] ^ tb);
+      }
+    }
+  }
+}
+
 // flips of the 32 pairs of each word of one pass: x = active pairs, a = side holding the particle's departure site.
+// The pairs are split into their rate classes (0 = p, 1 = p_slow, 2 = q, 3 = q_slow) once; every class then compares
+// against its own constant threshold.
 __device__ __forceinline__ void general_flips(uint32_t (&lt)[4], const uint32_t (&x)[4], const uint32_t (&a)[4],
                                               const uint32_t (&spa)[4], const uint32_t (&sqb)[4],
                                               const uint32_t (&r)[NPSA][4], const PhiloxKeys& K, uint32_t G, uint32_t gs,
                                               uint32_t tlo, uint32_t c3) {
-  uint32_t eq[4];
+  uint32_t e0[4], e1[4], e2[4], e3[4];
 #pragma unroll
   for (int w = 0; w < 4; ++w) {
-    lt[w] = x[w] & class_mask(a[w], spa[w], sqb[w], is_always(T0), is_always(T1), is_always(T2), is_always(T3));
-    eq[w] = x[w] & class_mask(a[w], spa[w], sqb[w], is_partial(T0), is_partial(T1), is_partial(T2), is_partial(T3));
+    const uint32_t xp = x[w] & a[w], xq = x[w] & ~a[w];
+    const uint32_t m0 = DIS >= 1 ? (xp & ~spa[w]) : xp, m1 = DIS >= 1 ? (xp & spa[w]) : 0u;
+    const uint32_t m2 = DIS >= 2 ? (xq & ~sqb[w]) : xq, m3 = DIS >= 2 ? (xq & sqb[w]) : 0u;
+    lt[w] = (is_always(T0) ? m0 : 0u) | (is_always(T1) ? m1 : 0u) | (is_always(T2) ? m2 : 0u) | (is_always(T3) ? m3 : 0u);
+    e0[w] = is_partial(T0) ? m0 : 0u;
+    e1[w] = is_partial(T1) ? m1 : 0u;
+    e2[w] = is_partial(T2) ? m2 : 0u;
+    e3[w] = is_partial(T3) ? m3 : 0u;
   }
-#pragma unroll
-  for (int pl = 0; pl < NEAG; ++pl) {
-#pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      const uint32_t tb = class_mask(a[w], spa[w], sqb[w], tbit(T0, pl), tbit(T1, pl), tbit(T2, pl), tbit(T3, pl));
-      lt[w] |= eq[w] & tb & ~r[pl][w];
-      eq[w] &= ~(r[pl][w] ^ tb);
-    }
-  }
+  class_planes_eager<T0>(lt, e0, r);
+  if (DIS >= 1) class_planes_eager<T1>(lt, e1, r);
+  class_planes_eager<T2>(lt, e2, r);
+  if (DIS >= 2) class_planes_eager<T3>(lt, e3, r);
   if (NEAG < NPS) {
     const unsigned alive = __activemask();  // the streamed pass kernel's last warp may be partly retired
 #pragma unroll 1
     for (int pl = NEAG; pl < NPS; pl += K1J_TRIP) {
-      if (!__any_sync(alive, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u)) break;
+      uint32_t any = 0u;
+#pragma unroll
+      for (int w = 0; w < 4; ++w) any |= e0[w] | e1[w] | e2[w] | e3[w];
+      if (!__any_sync(alive, any != 0u)) break;
       uint32_t R[K1J_TRIP][4];
 #pragma unroll
       for (int t = 0; t < K1J_TRIP; ++t) {  // independent calls: their rounds interleave
@@ -228,14 +273,10 @@ __device__ __forceinline__ void general_flips(uint32_t (&lt)[4], const uint32_t 
 #pragma unroll
       for (int t = 0; t < K1J_TRIP; ++t) {
         if (pl + t < NPS) {
-          const uint32_t sh = 31 - (pl + t);
-#pragma unroll
-          for (int w = 0; w < 4; ++w) {
-            const uint32_t tb = class_mask(a[w], spa[w], sqb[w], (uint32_t)(T0 >> sh) & 1u, (uint32_t)(T1 >> sh) & 1u,
-                                           (uint32_t)(T2 >> sh) & 1u, (uint32_t)(T3 >> sh) & 1u);
-            lt[w] |= eq[w] & tb & ~R[t][w];
-            eq[w] &= ~(R[t][w] ^ tb);
-          }
+          class_plane_lazy<T0>(lt, e0, R[t], pl + t);
+          if (DIS >= 1) class_plane_lazy<T1>(lt, e1, R[t], pl + t);
+          class_plane_lazy<T2>(lt, e2, R[t], pl + t);
+          if (DIS >= 2) class_plane_lazy<T3>(lt, e3, R[t], pl + t);
         }
       }
     }
