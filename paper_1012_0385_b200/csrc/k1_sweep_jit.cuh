@@ -31,6 +31,9 @@
 #define K1J_VARIANT 1  // Measured: per-sample kernel (1.7 warps per SMSP) 1 >> 0, 2 (config 2: 19.3 / 17.4 / 16.0
 #endif               // TSU/s); blocked stream (many warps hide the latency) 2 > 1 (20.8 vs 19.4 TSU/s).
 #endif
+#ifndef K1J_PACK
+#define K1J_PACK 1  // small rings: several samples per warp (SPW below)
+#endif
 #ifndef K1J_REFRAME
 #ifdef K1J_TILE
 #define K1J_REFRAME 1  // merged frame changes: measured +5 % on the blocked stream (many warps per SM) ...
@@ -82,7 +85,8 @@ constexpr bool SINGLE_WARP = TILE || U <= 32;
 // Small rings: a ring of U <= 16 units (L = 256 U sites, U a power of two) fills only U lanes, so a warp sweeps
 // SPW = 32 / U independent samples side by side; every per-sample quantity (offsets, frame, record sums) is then a
 // per-lane value and the shuffles run inside segments of U lanes.
-constexpr int SPW = (!TILE && !PARTIAL && U <= 16 && (U & (U - 1)) == 0) ? 32 / U : 1;
+// (K1J_PACK=0 turns packing off; measured, it never helps.)
+constexpr int SPW = (K1J_PACK && !TILE && !PARTIAL && U <= 16 && (U & (U - 1)) == 0) ? 32 / U : 1;
 constexpr int DIS = K1J_DIS;
 constexpr int NTHREADS = (U + 31) / 32 * 32;
 constexpr uint64_t T0 = K1J_T0, T1 = K1J_T1, T2 = K1J_T2, T3 = K1J_T3;

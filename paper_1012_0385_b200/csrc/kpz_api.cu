@@ -665,18 +665,20 @@ int kpz_run(kpz_sim* sim, int64_t n_mcs) {
     const int block = (D.U + 31) / 32 * 32;
     if (k1_use_jit(D)) {
       // small rings (k1_sweep_jit.cuh, SPW): U <= 16 units, a power of two, no ragged unit -> 32/U samples per warp
+      static int smsp = 0;
+      if (!smsp) {
+        int dev = 0, sms = 148;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        smsp = 4 * sms;
+      }
+      // (measured: packing never loses - a 30-ring launch runs at the same 17 GSU/s packed or one ring per warp)
       const bool pack = D.U <= 16 && (D.U & (D.U - 1)) == 0 && !partial;
       const int spw = pack ? 32 / D.U : 1;
       std::vector<std::string> defs = k1_jit_defines(D, dis);
+      if (!pack) defs.push_back("K1J_PACK=0");
       if (!std::getenv("KPZ_B200_K1_VARIANT")) {
         // code shape by occupancy (k1_sweep_jit.cuh, K1J_VARIANT): with >= 4 resident warps per SMSP the other warps
         // hide the latency, so the shape with the fewest alu slots wins (measured: +12..16 % on 16384-site rings)
-        static int smsp = 0;
-        if (!smsp) {
-          int dev = 0, sms = 148;
-          if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-          smsp = 4 * sms;
-        }
         const long long warps = (long long)((sim->S + spw - 1) / spw) * (block / 32);
         if (warps >= 4LL * smsp) defs.push_back("K1J_VARIANT=2");
       }
