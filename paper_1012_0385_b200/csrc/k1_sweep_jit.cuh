@@ -184,15 +184,7 @@ __device__ __forceinline__ uint32_t select_word(uint32_t a, uint32_t spa, uint32
   return lop3<sel_lut()>(in[0], in[1], in[2]);
 }
 
-// GENERAL path.  Elements whose rate class c (0 = p, 1 = p_slow, 2 = q, 3 = q_slow) has bit b_c set; the b_c are
-// compile-time constants for the eager planes and warp-uniform values in the lazy loop.
-__device__ __forceinline__ uint32_t class_mask(uint32_t a, uint32_t spa, uint32_t sqb, uint32_t b0, uint32_t b1,
-                                               uint32_t b2, uint32_t b3) {
-  const uint32_t B0 = 0u - b0, B1 = 0u - b1, B2 = 0u - b2, B3 = 0u - b3;
-  const uint32_t mp = DIS >= 1 ? ((spa & B1) | (~spa & B0)) : B0;
-  const uint32_t mq = DIS >= 2 ? ((sqb & B3) | (~sqb & B2)) : B2;
-  return (a & mp) | (~a & mq);
-}
+// GENERAL path helpers.
 __host__ __device__ constexpr uint32_t tbit(uint64_t T, int pl) { return (uint32_t)((T >> (31 - pl)) & 1ull); }
 __host__ __device__ constexpr uint32_t is_always(uint64_t T) { return T >= kOne ? 1u : 0u; }
 __host__ __device__ constexpr uint32_t is_partial(uint64_t T) { return (T > 0 && T < kOne) ? 1u : 0u; }
