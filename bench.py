@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — site-update throughput of the KPZ/ASEP hot path on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|5|2-fill|3-fill|4-aux-i|4-aux-ii|4-aux-i-blocked|paper-1024x30|paper-1024-fill|paper-qtasep-16384|paper-qssep-4096|paper-lanes-4096] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|5|2-fill|3-fill|4-aux-i|4-aux-ii|4-aux-i-blocked|paper-1024x30|paper-1024-fill|paper-qtasep-16384|paper-qssep-4096|paper-lanes-4096|paper-scan-512…32768] [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: reset to the
 initial state (a1), run the configuration's full number of MCS with its record times (a2-a7 / a9), records left in

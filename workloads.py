@@ -87,10 +87,24 @@ CONFIGS = {
     "paper-lanes-4096": dict(name="paper_two_lane_L4096_S1024", kind="lanes", L=4096, S=1024, p_a=0.5, p_b=0.5, rho0=0.5,
                              turn_prob=0.5, turn_period=0, omega=0.2, w_unflagged=0.8, independent=1, n_mcs=10_000,
                              record_times=eq7_times(10_000), seed=9, offset_mode=1),
+    # PAPER.md:235-239 (Sect. 2.4, Fig. 8a): "running the simulations up to t_max = 10^5 MCs for 560 realizations" of
+    # the TASEP for 512 <= L <= 32K; the paper reports T ~ L^0.9 on a Tesla C2070.  Keys "paper-scan-512" ... "-32768"
+    # are added below (`_add_scan`).
     # the same two rings on the default (temporally blocked) path
     "4-aux-i-blocked": dict(name="config4aux1_blocked_L2p28_p075_q025", kind="kpz", L=1 << 28, S=1, p=0.75, q=0.25,
                             disorder=None, n_mcs=1000, record_times=_T20_1E3, seed=4),
 }
+
+
+def _add_scan() -> None:
+    for k in range(9, 16):
+        L = 1 << k
+        CONFIGS[f"paper-scan-{L}"] = dict(name=f"paper_scan_tasep_L{L}_S560_p08", kind="kpz", L=L, S=560, p=0.8, q=0.0,
+                                          disorder=None, n_mcs=100_000, record_times=eq7_times(100_000), seed=10,
+                                          offset_mode=1)
+
+
+_add_scan()
 
 
 def site_updates(cfg: dict, n_mcs: int | None = None, nsamples: int | None = None) -> int:
