@@ -603,6 +603,31 @@ def test_config3_full_launch_sampled_against_solo_oracle_runs(K):
     assert np.all(R.unpack_words(lat, c["L"]).sum(axis=1) == c["L"] // 2)      # conservation, every sample
 
 
+@pytest.mark.parametrize("key,n", [("paper-scan-512", 150), ("paper-scan-32768", 40), ("paper-1024x30", 150),
+                                   ("paper-qtasep-16384", 60), ("paper-qssep-4096", 100)])
+def test_paper_workloads_full_launch_sampled_against_solo_oracle_runs(K, key, n):
+    """The paper's own parameter sets in the launch configuration bench.py times
+    (all samples, even/odd alternation, Eq. 7 sampling), shortened; first, middle and last sample against solo oracle
+    runs: lattice words and every record."""
+    c = workloads.CONFIGS[key]
+    times = [t for t in c["record_times"] if t <= n]
+    gpu = K.KpzSim(c["L"], c["S"], c["p"], c["q"], disorder=c["disorder"], seed=c["seed"], max_records=len(times),
+                   offset_mode=c["offset_mode"])
+    gpu.set_record_times(times)
+    gpu.run(n)
+    lat = K.words_to_numpy(gpu.lattice())
+    r = gpu.roughness()
+    for k in (0, c["S"] // 2 + 1, c["S"] - 1):
+        ref = R.KpzRef(c["L"], 1, c["p"], c["q"], disorder=c["disorder"], seed=c["seed"], first_sample=k,
+                       offset_mode=c["offset_mode"])
+        ref.set_record_times(times)
+        ref.run(n)
+        assert np.array_equal(lat[k], ref.lattice()[0])
+        rr = ref.roughness()
+        assert np.array_equal(r["sum_h"][:, k], rr["sum_h"][:, 0]) and np.array_equal(r["sum_h2"][:, k], rr["sum_h2"][:, 0])
+    assert np.all(R.unpack_words(lat, c["L"]).sum(axis=1) == c["L"] // 2)      # conservation, every sample
+
+
 def test_config3_last_sample_long_run(K):
     c = workloads.CONFIGS[3]
     run_both_kpz(K, c["L"], 1, c["p"], c["q"], disorder=c["disorder"], seed=c["seed"], first_sample=c["S"] - 1,
