@@ -352,6 +352,10 @@ def run_cuda(args, cfg, cfg_key):
         return 0
 
     # ---- roofline of the dominant kernel -------------------------------------------------------------------
+    # dram__bytes_read.sum + dram__bytes_write.sum of one K1 launch from the ncu --set full captures summarised in
+    # profiles/r01_v2_summary.md (taken on 1000-MCS launches: an on-chip launch reads the packed lattice once, S*L/8
+    # bytes, and writes its results from L2, whatever its length); other configurations: not captured per launch
+    NCU_DRAM_BYTES_PER_LAUNCH = {2: 1.085184e6, 3: 2.132224e6}
     peaks = measured_peaks()
     path = sim.path if cfg["kind"] == "kpz" else 1
     ms_run = ms_run_total / args.steps
@@ -373,7 +377,7 @@ def run_cuda(args, cfg, cfg_key):
         kname = {1: "kpz_k1_sweep_jit", 3: "kpz_k3t_sweep_jit"}.get(path, "kpz_k1_sweep_jit") if cfg["kind"] == "kpz" \
             else "lanes_k4_sweep_jit"
         roof = {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "Tslot/s",
-                "frac": achieved / peak, "traffic": None,
+                "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg_key),
                 "peak_source": f"148 SM x 4 SMSP x 0.5 alu-pipe warp-instr/clk (measured) x 32 lanes x "
                                f"{peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max clock)",
                 "algorithmic_slots_per_site_update": slots}
