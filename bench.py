@@ -1,25 +1,34 @@
 #!/usr/bin/env python
 """bench.py — site-update throughput of the KPZ/ASEP hot path on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|5|2-fill|3-fill|4-aux-i|4-aux-ii|4-aux-i-blocked|paper-1024x30|paper-1024-fill|paper-qtasep-16384|paper-qssep-4096|paper-lanes-4096|paper-scan-512…32768] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1|2|3|4|5|4-aux-i|4-aux-ii|2-fill|3-fill|paper-...]
+                    [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: reset to the
 initial state (a1), run the configuration's full number of MCS with its record times (a2-a7 / a9), records left in
-device memory.  The default workload is BASELINE.json `configs[1]` (config 2: KPZ ring L=8192, 1024 samples,
-p=0.75/q=0.25, 10^4 MCS, 40 record times), the configuration the metric is quoted on.
+device memory.
+
+Default (`--config all`): BASELINE.json's `metric` names no configuration, so the headline (top-level `value`,
+`ms_per_step`, `config.workload`, `roofline`, `cpu_baseline`, `e2e`, `clocks`) is the LARGEST single-GPU configuration,
+config 3 (512 rings x 16384 sites x 10^5 MCS = 8.39e11 site updates), and the same line carries one full sub-record
+per other BASELINE configuration (1, 2, 4, 5) and for the two auxiliary streamed runs of SURVEY §8(d) (4-aux-i: L=2^28
+ring in L2; 4-aux-ii: L=2^32, the HBM roofline case) under `"per_config"`, each timed with its own K steps after W
+warm-up steps.  `--config X` runs one workload only.
 
 value      site updates / s (GSU/s) of the whole job, device-timed (CUDA events on the launching stream), inputs
            resident in HBM when the timed region starts.
 e2e        same metric through the C ABI with HOST buffers: pinned initial lattice -> device, kpz_set_lattice,
            kpz_run, kpz_roughness (records -> host) and the final lattice -> pinned host, all inside the timed region.
-roofline   the dominant kernel against the bound DESIGN.md §6 derives for it.
+roofline   the dominant kernel against the bound DESIGN.md §6 derives for it: `frac` = ALGORITHMIC slots (or bytes) per
+           second / peak.  `traffic` and `measured` (ncu pipe / issue utilisation of the same launch shape) are read from
+           the committed capture table profiles/ncu_counters.csv (`traffic_source` names the row's capture) or are null.
 cpu_baseline  the oracle (oracle/, as it stands) on one host core over a bounded sample of the same workload.
 
-N > 1 (torchrun): every rank runs the same workload on its own samples (first_sample = rank * S): weak scaling, no
+N > 1 (torchrun): every rank runs the same workloads on its own samples (first_sample = rank * S): weak scaling, no
 collective on the data path; time = max over ranks.
 
 --impl reference times the CPU oracle (there is no reference implementation to install: /root/reference holds only
-the paper's text).
+the paper's text) on the headline workload (or on --config X).
 """
 from __future__ import annotations
 
@@ -43,7 +52,6 @@ UNIT = "GSU/s"
 # ---------------------------------------------------------------------------------------------------------------
 # roofline model: algorithmic cost per site-update of the dominant kernel of each workload
 # ---------------------------------------------------------------------------------------------------------------
-SM_COUNT = 148
 # alu-pipe slots per site update of the on-chip / blocked sweeps and the two-lane kernel: one slot =
 # one LOP3 / SHF / IMAD.WIDE lane-instruction; the pipe takes 0.5 warp-instructions per clock and SMSP (measured).
 #   Philox call = 34 slots per 128 elements and plane; pair logic 3 LOP3 per 32 pairs and pass; 4 SHF per MCS.
@@ -68,6 +76,11 @@ ALU_SLOTS_PER_SU = {
     # cover 256 sites per call: 2 lanes x 2 passes x 0.5 call) + crossings 2 steps x (log2(32 live)+1.33 planes) x (34+12)
     "paper-lanes-4096": (2 * 34 + 2 * 6.33 * (34 + 12) + 2 * 2 * 4 * 5 + 2 * 4 * 4) / 256,
 }
+for _L in (512, 1024, 2048, 4096, 8192, 16384, 32768):   # the paper's size scan: same rates and schedule as paper-1024x30
+    ALU_SLOTS_PER_SU[f"paper-scan-{_L}"] = ALU_SLOTS_PER_SU["paper-1024x30"]
+# default run: the headline first, then the other BASELINE configs and the auxiliary streamed runs of SURVEY §8(d)
+HEADLINE = 3
+DEFAULT_SET = [3, 1, 2, 4, 5, "4-aux-i", "4-aux-ii"]
 ALU_SLOTS_PER_CLK_SMSP = 0.5
 # streamed sweep: one read + one write of the bit-packed ring per sub-lattice pass = 2 passes * 2 * 1/8 B
 STREAM_BYTES_PER_SU = 0.5
@@ -84,6 +97,20 @@ def measured_peaks():
         except Exception:
             pass
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def ncu_counters(cfg_key):
+    """Row of profiles/ncu_counters.csv for this workload (written from `ncu --set full` captures of one launch of the
+    dominant kernel in the launch shape bench.py times; the row names its capture), or None."""
+    path = os.path.join(ROOT, "profiles", "ncu_counters.csv")
+    if not os.path.exists(path):
+        return None
+    import csv
+    with open(path) as f:
+        for row in csv.DictReader(r for r in f if not r.startswith("#")):
+            if row.get("config_key") == str(cfg_key):
+                return row
+    return None
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -225,31 +252,61 @@ def make_sim(pkg, cfg, first_sample):
     return sim
 
 
-def run_cuda(args, cfg, cfg_key):
-    import torch
-    import torch.distributed as dist
+class Ctx:
+    """Process-wide state of the CUDA arm: device, ranks, the L2-flush buffer."""
 
-    import paper_1012_0385_b200 as pkg
+    def __init__(self):
+        import torch
+        import torch.distributed as dist
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-    pkg.load_library()
+        import paper_1012_0385_b200 as pkg
 
+        self.torch, self.dist, self.pkg = torch, dist, pkg
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        if not torch.cuda.is_available():
+            raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+        torch.cuda.set_device(self.local_rank)
+        self.dev = torch.device("cuda", self.local_rank)
+        if self.world > 1:
+            dist.init_process_group("nccl", device_id=self.dev)
+        pkg.load_library()
+        self.sm_count = int(torch.cuda.get_device_properties(self.dev).multi_processor_count)
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=self.dev)   # > 126 MB L2
+        self.peaks = measured_peaks()
+
+    def barrier(self):
+        self.torch.cuda.synchronize()
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def max_over_ranks(self, values):
+        t = self.torch.tensor(list(values), dtype=self.torch.float64, device=self.dev)
+        if self.world > 1:
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return [float(x) for x in t]
+
+    def close(self):
+        if self.world > 1:
+            self.dist.destroy_process_group()
+
+
+def bench_one(ctx, args, cfg_key, with_cpu):
+    """K timed steps of one workload after W warm-up steps; returns the record of that workload (on every rank)."""
+    torch, pkg = ctx.torch, ctx.pkg
+    cfg = dict(workloads.CONFIGS[cfg_key])
     n_mcs = cfg["n_mcs"] if args.mcs is None else args.mcs
     if args.mcs is not None:
         cfg = workloads.truncated(cfg, n_mcs)
+    if args.samples is not None:
+        cfg["S"] = args.samples
     su_step = workloads.site_updates(cfg)
     from paper_1012_0385_b200 import shard
-    sim = make_sim(pkg, cfg, first_sample=shard.weak_first_sample(cfg["S"], rank))   # global sample indices
+    sim = make_sim(pkg, cfg, first_sample=shard.weak_first_sample(cfg["S"], ctx.rank))   # global sample indices
     stream = torch.cuda.current_stream()
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    world = ctx.world
 
     def step(ev=None):
         if ev:
@@ -261,46 +318,62 @@ def run_cuda(args, cfg, cfg_key):
         if ev:
             ev[2].record(stream)
 
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
     for _ in range(args.warmup):
-        flush.fill_(1)
+        ctx.flush.fill_(1)
         step()
-    barrier()
+    ctx.barrier()
 
-    sampler = ClockSampler(local_rank)
+    sampler = ClockSampler(ctx.local_rank)
     events = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
     launches0 = pkg.kernel_launches()
     sampler.start()
     wall0 = time.perf_counter()
     for k in range(args.steps):
-        flush.fill_(k & 0xFF)          # L2 flush between timed iterations (outside the events)
+        ctx.flush.fill_(k & 0xFF)          # L2 flush between timed iterations (outside the events)
         step(events[k])
-    barrier()
+    ctx.barrier()
     wall = time.perf_counter() - wall0
     clocks = sampler.stop()
     launches = pkg.kernel_launches() - launches0
     t_step = [e[0].elapsed_time(e[2]) for e in events]       # ms, reset + run
     t_run = [e[1].elapsed_time(e[2]) for e in events]        # ms, kpz_run / lanes_run only
-    t_total = torch.tensor([sum(t_step), sum(t_run)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t_total, op=dist.ReduceOp.MAX)
-    ms_total, ms_run_total = float(t_total[0]), float(t_total[1])
+    ms_total, ms_run_total = ctx.max_over_ranks([sum(t_step), sum(t_run)])
     value = world * su_step * args.steps / (ms_total * 1e-3) / 1e9
+    e2e = time_e2e(ctx, args, cfg, sim, n_mcs, su_step)
+    path = sim.path if cfg["kind"] == "kpz" else 1
+    ms_run = ms_run_total / args.steps
+    roof = roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run)
+    cpu = None
+    if with_cpu and ctx.rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nsamp, nm = oracle_sample_shape(cfg, args.cpu_su)
+        v, dt = time_oracle(cfg, nsamp, nm)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
+               "sample": f"{nsamp} sample(s) x {nm} MCS of {cfg['name']} (of {cfg['S']} x {cfg['n_mcs']})"}
+    sim.close()
+    return {
+        "value": value, "unit": UNIT, "ms_per_step": ms_total / args.steps, "ms_run_per_step": ms_run,
+        # only "paper-1024x30" is a workload the paper quotes a number for (BASELINE.md; another machine: context)
+        "vs_baseline": (value / cfg["paper_gsu"]) if (cfg.get("paper_gsu") and world == 1 and args.mcs is None
+                                                      and args.samples is None) else None,
+        "config": {"workload": cfg["name"], "config_key": str(cfg_key), "L": cfg["L"], "samples_per_gpu": cfg["S"],
+                   "n_mcs": n_mcs, "records": len(cfg["record_times"]),
+                   "path": PATH_NAMES[path] if cfg["kind"] == "kpz" else "two-lane K4",
+                   "l2": "flushed between timed steps (256 MiB fill)", "parallelism": f"samples x{world}"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
+        "wall_s_timed_region": wall,
+    }
 
-    # ---- e2e: host buffers through the C ABI ------------------------------------------------------------------
-    e2e = None
+
+def time_e2e(ctx, args, cfg, sim, n_mcs, su_step):
+    """The same metric end to end through the public API with HOST buffers inside the timed region."""
+    torch = ctx.torch
     if cfg["kind"] == "kpz":
-        nw = cfg["L"] // 32
         import numpy as np
+        nw = cfg["L"] // 32
         h_in = torch.from_numpy(np.full((cfg["S"], nw), 0xAAAAAAAA, dtype=np.uint32).view(np.int32)).pin_memory()
         h_out = torch.empty((cfg["S"], nw), dtype=torch.int32).pin_memory()
-        d_in = torch.empty((cfg["S"], nw), dtype=torch.int32, device=dev)
-        d_out = torch.empty((cfg["S"], nw), dtype=torch.int32, device=dev)
+        d_in = torch.empty((cfg["S"], nw), dtype=torch.int32, device=ctx.dev)
+        d_out = torch.empty((cfg["S"], nw), dtype=torch.int32, device=ctx.dev)
 
         def e2e_step():
             sim.reset()
@@ -312,99 +385,106 @@ def run_cuda(args, cfg, cfg_key):
             return sim.roughness()        # syncs; records -> host
 
         e2e_step()
-        barrier()
+        ctx.barrier()
         t0 = time.perf_counter()
         for _ in range(args.steps):
             rec = e2e_step()
-        barrier()
-        dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ctx.barrier()
+        dt, = ctx.max_over_ranks([time.perf_counter() - t0])
         rec_bytes = int(rec["sum_h"].nbytes + rec["sum_h2"].nbytes)
-        e2e = {"value": world * su_step * args.steps / float(tt[0]) / 1e9, "unit": UNIT,
-               "h2d_bytes_per_step": int(h_in.numel() * 4), "d2h_bytes_per_step": int(h_out.numel() * 4) + rec_bytes}
-    else:
-        def e2e_step():
-            sim.reset()
-            sim.run(n_mcs)
-            a, b, _ = sim.state()
-            ha, hb = a.cpu(), b.cpu()
-            return sim.currents(), ha, hb
+        return {"value": ctx.world * su_step * args.steps / dt / 1e9, "unit": UNIT,
+                "h2d_bytes_per_step": int(h_in.numel() * 4), "d2h_bytes_per_step": int(h_out.numel() * 4) + rec_bytes}
 
-        e2e_step()
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.steps):
-            cur, ha, hb = e2e_step()
-        barrier()
-        dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * su_step * args.steps / float(tt[0]) / 1e9, "unit": UNIT, "h2d_bytes_per_step": 0,
-               "d2h_bytes_per_step": int(ha.numel() * 4 + hb.numel() * 4 + 4 * cur["j_a"].nbytes),
-               "note": "the two-lane initial state is generated on the device from the seed; no host input exists"}
+    def e2e_step():
+        sim.reset()
+        sim.run(n_mcs)
+        a, b, _ = sim.state()
+        ha, hb = a.cpu(), b.cpu()
+        return sim.currents(), ha, hb
 
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return 0
+    e2e_step()
+    ctx.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        cur, ha, hb = e2e_step()
+    ctx.barrier()
+    dt, = ctx.max_over_ranks([time.perf_counter() - t0])
+    return {"value": ctx.world * su_step * args.steps / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": 0,
+            "d2h_bytes_per_step": int(ha.numel() * 4 + hb.numel() * 4 + 4 * cur["j_a"].nbytes),
+            "note": "the two-lane initial state is generated on the device from the seed; no host input exists"}
 
-    # ---- roofline of the dominant kernel -------------------------------------------------------------------
-    # dram__bytes_read.sum + dram__bytes_write.sum of one K1 launch from the ncu --set full captures summarised in
-    # profiles/r01_v2_summary.md (taken on 1000-MCS launches: an on-chip launch reads the packed lattice once, S*L/8
-    # bytes, and writes its results from L2, whatever its length); other configurations: not captured per launch
-    NCU_DRAM_BYTES_PER_LAUNCH = {2: 1.085184e6, 3: 2.132224e6}
-    peaks = measured_peaks()
-    path = sim.path if cfg["kind"] == "kpz" else 1
-    ms_run = ms_run_total / args.steps
+
+def roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run):
+    """The dominant kernel against its bound.  `achieved` uses the ALGORITHMIC slots / bytes of the method
+    and the device time of kpz_run / lanes_run measured in this run; `traffic` and `measured` come from the committed ncu
+    capture table (one launch of the same kernel and launch shape), never from this run."""
+    peaks = ctx.peaks
+    row = ncu_counters(cfg_key)
+
+    def num(name):
+        try:
+            return float(row[name]) if row and row.get(name) not in (None, "") else None
+        except ValueError:
+            return None
+
+    traffic = None
+    if row and num("dram_bytes_read") is not None and num("dram_bytes_write") is not None:
+        traffic = num("dram_bytes_read") + num("dram_bytes_write")
+    measured = None
+    if row:
+        measured = {k: num(k) for k in ("issue_active_pct", "pipe_alu_pct", "pipe_fmaheavy_pct", "warps_active_per_smsp")
+                    if num(k) is not None} or None
+    src = (f"profiles/ncu_counters.csv row {cfg_key}: {row.get('capture', '')}" if row else None)
     if path == 2:
         # streamed sweep: 2*n_mcs pass kernels per run; per launch one read + one write of the ring
         n_launch = 2 * n_mcs
         bytes_launch = 2 * cfg["S"] * cfg["L"] / 8
         achieved = bytes_launch * n_launch / (ms_run * 1e-3) / 1e9
-        # dram__bytes_read.sum + dram__bytes_write.sum of one pass launch, from the ncu --set full capture summarised in
-        # profiles/r01_v2_summary.md (only taken at L=2^32; elsewhere unmeasured)
-        traffic = 536.878336e6 + 483.978496e6 if cfg["L"] == (1 << 32) and cfg["S"] == 1 else None
-        roof = {"bound": "hbm", "kernel": "kpz_k3_pass_jit", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"],
-                "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
-    else:
-        slots = ALU_SLOTS_PER_SU.get(cfg_key, ALU_SLOTS_PER_SU[2])
-        peak = SM_COUNT * 4 * ALU_SLOTS_PER_CLK_SMSP * 32 * peaks["sm_max_mhz"] * 1e6 / 1e12   # T lane-slots/s
-        achieved = slots * su_step / (ms_run * 1e-3) / 1e12
-        kname = {1: "kpz_k1_sweep_jit", 3: "kpz_k3t_sweep_jit"}.get(path, "kpz_k1_sweep_jit") if cfg["kind"] == "kpz" \
-            else "lanes_k4_sweep_jit"
-        roof = {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "Tslot/s",
-                "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg_key),
-                "peak_source": f"148 SM x 4 SMSP x 0.5 alu-pipe warp-instr/clk (measured) x 32 lanes x "
-                               f"{peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max clock)",
-                "algorithmic_slots_per_site_update": slots}
+        return {"bound": "hbm", "kernel": "kpz_k3_pass_jit", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "traffic_source": src, "measured": measured,
+                "peak_source": peaks["source"], "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
+    slots = ALU_SLOTS_PER_SU.get(cfg_key)
+    kname = {1: "kpz_k1_sweep_jit", 3: "kpz_k3t_sweep_jit"}.get(path, "kpz_k1_sweep_jit") if cfg["kind"] == "kpz" \
+        else "lanes_k4_sweep_jit"
+    if slots is None:
+        return {"bound": "alu", "kernel": kname, "achieved": None, "peak": None, "unit": "Tslot/s", "frac": None,
+                "traffic": traffic, "reason": f"no algorithmic slot count is modelled for workload key {cfg_key!r}"}
+    peak = ctx.sm_count * 4 * ALU_SLOTS_PER_CLK_SMSP * 32 * peaks["sm_max_mhz"] * 1e6 / 1e12   # T lane-slots/s
+    achieved = slots * su_step / (ms_run * 1e-3) / 1e12
+    return {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "Tslot/s",
+            "frac": achieved / peak, "traffic": traffic, "traffic_source": src, "measured": measured,
+            "frac_definition": "algorithmic alu-pipe slots of the method (DESIGN.md 6.1) per second / alu-pipe slot peak; "
+                               "`measured` holds the ncu pipe / issue utilisation of the same kernel",
+            "peak_source": f"{ctx.sm_count} SM (queried) x 4 SMSP x 0.5 alu-pipe warp-instr/clk (measured, "
+                           f"profiles/r01_pipe_rates.md) x 32 lanes x {peaks['sm_max_mhz']:.0f} MHz "
+                           f"({peaks['source']} max clock)",
+            "algorithmic_slots_per_site_update": slots}
 
-    # ---- CPU oracle on a bounded sample (one host core) -------------------------------------------------------
-    cpu = None
-    if world == 1 and not args.no_cpu_baseline:
-        nsamp, nm = oracle_sample_shape(cfg, 400_000_000)      # ~15 s at ~2.5e7 site updates/s
-        v, dt = time_oracle(cfg, nsamp, nm)
-        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
-               "sample": f"{nsamp} sample(s) x {nm} MCS of {cfg['name']} (of {cfg['S']} x {cfg['n_mcs']})"}
 
+def run_cuda(args, keys):
+    ctx = Ctx()
+    records = {}
+    for i, key in enumerate(keys):
+        records[str(key)] = bench_one(ctx, args, key, with_cpu=True)
+    if ctx.rank != 0:
+        ctx.close()
+        return 0
+    head = records[str(keys[0])]
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
-        # only "paper-1024x30" is a workload the paper quotes a number for (BASELINE.md; another machine: context)
-        "vs_baseline": (value / cfg["paper_gsu"]) if (cfg.get("paper_gsu") and world == 1 and args.mcs is None) else None,
-        "dtype": "u32", "data": "synthetic",
-        "config": {"workload": cfg["name"], "config_key": str(cfg_key), "L": cfg["L"], "samples_per_gpu": cfg["S"],
-                   "n_mcs": n_mcs, "records": len(cfg["record_times"]), "path": PATH_NAMES[path] if cfg["kind"] == "kpz" else "two-lane K4", "l2": "flushed between timed steps (256 MiB fill)",
-                   "parallelism": f"samples x{world}"},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
-        "ms_run_per_step": ms_run, "wall_s_timed_region": wall,
+        "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": ctx.world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": head["vs_baseline"], "dtype": "u32", "data": "synthetic", "config": head["config"],
+        "clocks": head["clocks"], "e2e": head["e2e"],
+        "gpu_launches": int(sum(r["gpu_launches"] for r in records.values())),
+        "roofline": head["roofline"], "cpu_baseline": head["cpu_baseline"], "ms_run_per_step": head["ms_run_per_step"],
+        "wall_s_timed_region": head["wall_s_timed_region"], "sm_count": ctx.sm_count,
     }
+    if len(keys) > 1:
+        line["per_config"] = records
+        line["headline"] = (f"config {keys[0]}: BASELINE.json's metric names no configuration, so the top-level keys are "
+                            f"the largest single-GPU configuration; every other workload is a full sub-record in per_config")
     print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    ctx.close()
     return 0
 
 
@@ -414,15 +494,23 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--config", default="2")
+    ap.add_argument("--config", default="all")
     ap.add_argument("--mcs", type=int, default=None, help="truncate the run to this many MCS (diagnostics only)")
+    ap.add_argument("--samples", type=int, default=None, help="override the sample count (diagnostics only)")
+    ap.add_argument("--debug-config", default=None, help="kpz_debug_config string (kernel tuning knobs; diagnostics only)")
+    ap.add_argument("--cpu-su", type=int, default=250_000_000, help="site updates of the cpu_baseline sample per workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
-    key = int(args.config) if args.config.isdigit() else args.config
-    cfg = dict(workloads.CONFIGS[key])
+    if args.config == "all":
+        keys = list(DEFAULT_SET)
+    else:
+        keys = [int(k) if k.isdigit() else k for k in args.config.split(",")]
     if args.impl == "reference":
-        return run_reference(args, cfg, key)
-    return run_cuda(args, cfg, key)
+        return run_reference(args, dict(workloads.CONFIGS[keys[0]]), keys[0])
+    if args.debug_config:
+        import paper_1012_0385_b200 as pkg
+        pkg.debug_config(args.debug_config)
+    return run_cuda(args, keys)
 
 
 if __name__ == "__main__":

@@ -1,7 +1,7 @@
-"""Build and run csrc/pipe_microbench.cu: the B200 issue rates behind the alu-pipe slot roofline.
+"""Build and run bench_micro/pipe_microbench.cu: the B200 issue rates behind the alu-pipe slot roofline.
 
-    python -m paper_1012_0385_b200.microbench            # needs a GPU; prints cycles per step for every instruction mix
-    python -m paper_1012_0385_b200.microbench --build    # compile only (no GPU needed)
+    python bench_micro/microbench.py            # needs a GPU; prints cycles per step for every instruction mix
+    python bench_micro/microbench.py --build    # compile only (no GPU needed)
 """
 from __future__ import annotations
 
@@ -10,7 +10,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "csrc", "pipe_microbench.cu")
+SRC = os.path.join(HERE, "pipe_microbench.cu")
 EXE = os.path.join(HERE, "pipe_microbench")
 
 

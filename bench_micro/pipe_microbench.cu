@@ -1,6 +1,6 @@
 // pipe_microbench.cu — measures the B200 issue rates the sweep's roofline is built on.
 //
-// Stand-alone program (built and run by `python -m paper_1012_0385_b200.microbench`): for each instruction class of
+// Stand-alone program (built and run by `python bench_micro/microbench.py`): for each instruction class of
 // the sweep (LOP3, SHF, IMAD.WIDE, IMAD.lo, IMAD.HI, POPC, SHFL) and for mixes of IMAD.WIDE with n LOP3, every SMSP
 // runs W warps with 4 independent chains per thread; it prints the cycles one "step" (NA instructions of class A + NB
 // of class B) takes per SMSP.  Findings the kernels rely on: LOP3/SHF/IMAD.lo 2 clk, IMAD.WIDE 4 clk alone, and

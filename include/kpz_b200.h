@@ -82,7 +82,9 @@ int kpz_set_record_times(kpz_sim*, const int64_t* t, int32_t nt);
  * run(a); run(b) is bit-identical to run(a+b). */
 int kpz_run(kpz_sim*, int64_t n_mcs);
 
-int kpz_time(const kpz_sim*, int64_t* t); /* MCS done so far (host value; no sync) */
+/* MCS done so far: "when all sites are updated once the time (t) is incremented by one Monte Carlo step"
+ * (DESIGN §R10).  Host value; no sync. */
+int kpz_time(const kpz_sim*, int64_t* t);
 
 /* Checkpoint restore: continue from MCS count t (0 <= t < 2^54).  Every random number is a function of (seed,
  * sample, MCS index, ...) (§R10), so the lattice (kpz_set_lattice), the disorder tags and t are the whole
@@ -93,7 +95,11 @@ int kpz_set_time(kpz_sim*, int64_t t);
  * captured records dropped (the record-time list is kept).  Enqueues the initialisation kernels; async. */
 int kpz_reset(kpz_sim*);
 
-/* Copy the occupation bits out / in (device buffers, natural layout, nsamples * L/32 words).  Async. */
+/* Copy the occupation bits out / in (device buffers, natural layout, nsamples * L/32 words).  Async.
+ * The overflow guard of the exact sums (|h| <= 1 + 8 t from the flat start) cannot know how rough a lattice
+ * handed in here is: on rings long enough for sum h^2 to leave int64 (L^3 >= 9e18) kpz_set_lattice also measures
+ * max |h| on the device, and the next kpz_set_record_times / kpz_run reads it back (one 4-byte copy, syncs once) and
+ * refuses record times with KPZ_EUNSUPPORTED as it would after kpz_create. */
 int kpz_lattice(kpz_sim*, uint32_t* d_words);
 int kpz_set_lattice(kpz_sim*, const uint32_t* d_words);
 /* Quenched disorder tags, same layout; either pointer may be NULL.  Async. */
@@ -109,6 +115,8 @@ int kpz_heights(kpz_sim*, int32_t sample, int32_t* d_h);
  * (L*sum_h2 - sum_h^2)/L^2.  Any output pointer may be NULL. */
 int kpz_roughness(kpz_sim*, int32_t* nt, int64_t* t, int64_t* sum_h, int64_t* sum_h2, double* w2_mean);
 
+/* Frees the host-side handle only ("device memory is touched at the start and the end of a time loop", PAPER.md:91:
+ * the state lives in the caller's workspace, which the caller frees).  Pending work on the stream is not waited for. */
 int kpz_destroy(kpz_sim*);
 
 /* ---- two-lane opposite-direction model -------------------------------------------------- */
@@ -141,9 +149,14 @@ int lanes_create_crossing(lanes_sim** out, int64_t L, int32_t nsamples, double p
  * independent, and lanes_set_flags then takes the one set as d_u).  Async. */
 int lanes_flags(lanes_sim*, uint32_t* d_u, uint32_t* d_v);
 int lanes_set_flags(lanes_sim*, const uint32_t* d_u, const uint32_t* d_v);
+/* Record times of the currents, "sampling ... done in the same way as in case of ASEP simulations (7)" (PAPER.md:275,
+ * 134): as kpz_set_record_times. */
 int lanes_set_record_times(lanes_sim*, const int64_t* t, int32_t nt);
+/* Advance by n_mcs sweeps of the five-part sequence of PAPER.md:259-265: in-lane pass of both lanes,
+ * A->B changes, second in-lane pass with the ring closure, B->A changes; hop counters, records and the
+ * epoch-end profile (§R16) are updated in the kernel.  Asynchronous; run(a); run(b) == run(a+b). */
 int lanes_run(lanes_sim*, int64_t n_mcs);
-int lanes_time(const lanes_sim*, int64_t* t);
+int lanes_time(const lanes_sim*, int64_t* t); /* sweeps done so far; host value */
 /* As kpz_set_time; restore lanes and turning-point mask with lanes_set_state.  Hop counters and profile keep going. */
 int lanes_set_time(lanes_sim*, int64_t t);
 int lanes_reset(lanes_sim*); /* as kpz_reset: initial occupations, epoch-0 turning points, zero counters; async */
@@ -154,17 +167,31 @@ int lanes_set_state(lanes_sim*, const uint32_t* d_a, const uint32_t* d_b, const 
 int lanes_currents(lanes_sim*, int32_t* nt, int64_t* t, int64_t* j_a, int64_t* j_b, int64_t* n_a, int64_t* n_b);
 /* Epoch-end occupancy counts [nsamples][L] per lane (device, uint32) and the snapshot count. SYNCS. */
 int lanes_profile(lanes_sim*, uint32_t* d_occ_a, uint32_t* d_occ_b, int64_t* nsnap);
-int lanes_destroy(lanes_sim*);
+int lanes_destroy(lanes_sim*); /* as kpz_destroy: host-side handle only */
 
 /* ---- diagnostics ------------------------------------------------------------------------------------------ */
+/* Text of an error code.  The paper's programs report nothing of the kind; this serves the "no exception or abort
+ * crosses the ABI" rule of SURVEY §8(b). */
 const char* kpz_strerror(int code);
 const char* kpz_last_error(void);        /* thread-local detail of the last failing call */
 int64_t kpz_kernel_launches(void);       /* kernels launched by this library in this process so far */
 /* Which kernel family a handle's kpz_run uses: 1 = on-chip per-sample (K1), 2 = streamed (K3), 3 = blocked (K3T). */
 int kpz_path(const kpz_sim*, int32_t* path);
 
+/* Test and tuning hook, not part of the paper's problem statement: a ';'-separated list of NAME=VALUE items that
+ * replaces the process-wide debug configuration (NULL or "" restores the defaults).  "jit=0" selects the statically
+ * compiled generic kernels instead of the run-time specialised ones; "K1J_<X>=v" / "K4J_<X>=v" are appended as
+ * definitions to every later run-time compilation of the KPZ / two-lane sweep kernels (the knobs documented at the top
+ * of csrc/k1_sweep_jit.cuh and csrc/k4_lanes_jit.cuh).  Every setting computes the same results (tests/ check that);
+ * kpz_run / lanes_run read no environment variable.  KPZ_EINVAL for anything else. */
+int kpz_debug_config(const char* spec);
+/* Writes every kernel image compiled by this process so far (kpz_run, lanes_run, *_jit_check) to
+ * <dir>/<entry>_<n>.cubin with its definition list in <dir>/<entry>_<n>.txt, for `cuobjdump -sass` (the instruction
+ * census behind DESIGN §6.1).  count (may be NULL) receives the number of images.  Host-side only. */
+int kpz_debug_dump_cubins(const char* dir, int32_t* count);
+
 /* The on-chip sweep kernel is specialised at run time (NVRTC) on the ring size and the acceptance thresholds
- * (DESIGN §5); the environment variable KPZ_B200_JIT=0 selects the statically compiled generic kernels instead.
+ * (DESIGN §5); kpz_debug_config("jit=0") selects the statically compiled generic kernels instead.
  * kpz_jit_check compiles - without loading, so it needs no GPU - the kernel kpz_run would use for these parameters
  * and returns the size of its sm_100a cubin (0 when that configuration runs on a statically compiled kernel). */
 int kpz_jit_check(int64_t L, double p, double q, const kpz_disorder* disorder, const kpz_options* opt,

@@ -84,6 +84,8 @@ SIGNATURES = {
     "kpz_last_error": (C.c_char_p, []),
     "kpz_kernel_launches": (C.c_int64, []),
     "kpz_path": (C.c_int, [_P, C.POINTER(C.c_int32)]),
+    "kpz_debug_config": (C.c_int, [C.c_char_p]),
+    "kpz_debug_dump_cubins": (C.c_int, [C.c_char_p, C.POINTER(C.c_int32)]),
     "kpz_jit_check": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.POINTER(Disorder), C.POINTER(Options),
                                 C.POINTER(C.c_size_t)]),
     "lanes_jit_check": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int64, C.c_double,
@@ -133,6 +135,29 @@ def _times(t):
 
 def kernel_launches() -> int:
     return int(load_library().kpz_kernel_launches())
+
+
+class debug_config:
+    """kpz_debug_config: test / tuning hook ("jit=0", "K1J_VARIANT=2;K1J_EAGER=3", ...).  Usable as a plain call or as a
+    context manager that restores the defaults on exit."""
+
+    def __init__(self, spec: str | None = None):
+        _chk(load_library().kpz_debug_config((spec or "").encode()), "kpz_debug_config")
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        _chk(load_library().kpz_debug_config(b""), "kpz_debug_config")
+        return False
+
+
+def debug_dump_cubins(directory: str) -> int:
+    """kpz_debug_dump_cubins: every kernel image compiled by this process so far -> <directory>/<entry>_<n>.cubin."""
+    os.makedirs(directory, exist_ok=True)
+    n = C.c_int32(0)
+    _chk(load_library().kpz_debug_dump_cubins(directory.encode(), C.byref(n)), "kpz_debug_dump_cubins")
+    return int(n.value)
 
 
 def jit_check(L, p, q, disorder=None, offset_mode=0, path=KPZ_PATH_AUTO) -> int:

@@ -9,6 +9,7 @@
 #include <cuda_runtime.h>
 #include <nvrtc.h>
 
+#include <cctype>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -35,6 +36,13 @@ struct Entry {
 };
 std::mutex g_mu;
 std::map<std::string, Entry> g_cache;
+// every image compiled by this process, loaded or not (kpz_debug_dump_cubins): entry -> (definitions, cubin)
+struct Compiled {
+  std::string entry, defines;
+  std::vector<char> cubin;
+};
+std::mutex g_compiled_mu;
+std::vector<Compiled> g_compiled;
 
 const Embedded* find_source(const char* name) {
   for (const Embedded& e : kEmbedded)
@@ -43,9 +51,63 @@ const Embedded* find_source(const char* name) {
 }
 }  // namespace
 
+namespace {
+std::mutex g_dbg_mu;
+bool g_jit_on = true;
+std::vector<std::string> g_dbg_defs;
+}  // namespace
+
 bool jit_enabled() {
-  const char* e = std::getenv("KPZ_B200_JIT");
-  return !(e && e[0] == '0');
+  std::lock_guard<std::mutex> lock(g_dbg_mu);
+  return g_jit_on;
+}
+
+int debug_config(const char* spec) {
+  std::vector<std::string> defs;
+  bool jit_on = true;
+  std::string s = spec ? spec : "";
+  size_t pos = 0;
+  while (pos <= s.size()) {
+    size_t end = s.find(';', pos);
+    if (end == std::string::npos) end = s.size();
+    std::string tok = s.substr(pos, end - pos);
+    pos = end + 1;
+    while (!tok.empty() && tok.front() == ' ') tok.erase(tok.begin());
+    while (!tok.empty() && tok.back() == ' ') tok.pop_back();
+    if (tok.empty()) continue;
+    const size_t eq = tok.find('=');
+    if (eq == std::string::npos || eq == 0 || eq + 1 >= tok.size())
+      return fail(KPZ_EINVAL, "debug config: '%s' is not NAME=VALUE", tok.c_str());
+    for (char c : tok)
+      if (!(std::isalnum((unsigned char)c) || c == '_' || c == '=' || c == '-'))
+        return fail(KPZ_EINVAL, "debug config: bad character in '%s'", tok.c_str());
+    if (tok.compare(0, eq, "jit") == 0) {
+      jit_on = tok[eq + 1] != '0';
+    } else if (tok.compare(0, 4, "K1J_") == 0 || tok.compare(0, 4, "K4J_") == 0) {
+      defs.push_back(tok);
+    } else {
+      return fail(KPZ_EINVAL, "debug config: unknown name in '%s' (jit, K1J_*, K4J_*)", tok.c_str());
+    }
+  }
+  std::lock_guard<std::mutex> lock(g_dbg_mu);
+  g_jit_on = jit_on;
+  g_dbg_defs.swap(defs);
+  return KPZ_OK;
+}
+
+void debug_defines(const char* prefix, std::vector<std::string>* out) {
+  std::lock_guard<std::mutex> lock(g_dbg_mu);
+  const size_t n = std::strlen(prefix);
+  for (const std::string& d : g_dbg_defs)
+    if (d.compare(0, n, prefix) == 0) out->push_back(d);
+}
+
+bool debug_has(const char* name) {
+  std::lock_guard<std::mutex> lock(g_dbg_mu);
+  const size_t n = std::strlen(name);
+  for (const std::string& d : g_dbg_defs)
+    if (d.size() > n && d.compare(0, n, name) == 0 && d[n] == '=') return true;
+  return false;
 }
 
 int jit_compile(const char* source, const char* entry, const std::vector<std::string>& defines,
@@ -88,6 +150,34 @@ int jit_compile(const char* source, const char* entry, const std::vector<std::st
   r = nvrtcGetCUBIN(prog, cubin->data());
   nvrtcDestroyProgram(&prog);
   if (r != NVRTC_SUCCESS) return fail(KPZ_ECUDA, "nvrtcGetCUBIN: %s", nvrtcGetErrorString(r));
+  {
+    std::string dl;
+    for (const std::string& d : defines) dl += "-D" + d + "\n";
+    std::lock_guard<std::mutex> lock(g_compiled_mu);
+    bool seen = false;
+    for (const Compiled& c : g_compiled) seen = seen || (c.entry == entry && c.defines == dl);
+    if (!seen) g_compiled.push_back(Compiled{entry, dl, *cubin});
+  }
+  return KPZ_OK;
+}
+
+int dump_cubins(const char* dir, int* count) {
+  if (!dir) return fail(KPZ_EINVAL, "dir is NULL");
+  std::lock_guard<std::mutex> lock(g_compiled_mu);
+  int n = 0;
+  for (const Compiled& c : g_compiled) {
+    const std::string base = std::string(dir) + "/" + c.entry + "_" + std::to_string(n);
+    FILE* f = std::fopen((base + ".cubin").c_str(), "wb");
+    if (!f) return fail(KPZ_EINVAL, "cannot write %s.cubin", base.c_str());
+    std::fwrite(c.cubin.data(), 1, c.cubin.size(), f);
+    std::fclose(f);
+    f = std::fopen((base + ".txt").c_str(), "w");
+    if (!f) return fail(KPZ_EINVAL, "cannot write %s.txt", base.c_str());
+    std::fputs(c.defines.c_str(), f);
+    std::fclose(f);
+    ++n;
+  }
+  if (count) *count = n;
   return KPZ_OK;
 }
 

@@ -69,6 +69,10 @@ struct kpz_sim {
   int frame = 0;  // K3: frame of the stored lattice (always 0 between calls)
   std::vector<int64_t> rec_times;
   int32_t nrec = 0;  // records captured (times <= t)
+  // overflow guard of the exact sums: |h| <= min(L, h0 + 8 (t - t_h0)); flat start: h0 = 1, t_h0 = 0
+  int64_t h0 = 1, t_h0 = 0;
+  bool h0_pending = false;  // h0 is being measured on the device (kpz_set_lattice on a ring long enough to overflow)
+  bool guard_checked = true;  // the current record-time list has been checked against the current (h0, t_h0)
 };
 
 namespace {
@@ -91,7 +95,7 @@ int choose_path(int64_t L, const kpz_options* opt, int* path) {
   if (want != KPZ_PATH_ONCHIP && want != KPZ_PATH_STREAM && want != KPZ_PATH_BLOCKED)
     return fail(KPZ_EINVAL, "options.path must be 0, 1, 2 or 3");
   if (want == KPZ_PATH_BLOCKED && !jit_enabled())
-    return fail(KPZ_EUNSUPPORTED, "the blocked streamed path is compiled at run time (KPZ_B200_JIT=0 disables it)");
+    return fail(KPZ_EUNSUPPORTED, "the blocked streamed path is compiled at run time (kpz_debug_config(\"jit=0\") disables it)");
   *path = want;
   return KPZ_OK;
 }
@@ -193,22 +197,7 @@ std::vector<std::string> k1_jit_defines(const KpzDev& D, int dis) {
   d.push_back(buf);
   snprintf(buf, sizeof buf, "K1J_OFFSET_MODE=%d", D.offset_mode);
   d.push_back(buf);
-  if (const char* v = std::getenv("KPZ_B200_K1_REFRAME")) {  // tuning knob: merged frame changes (k1_sweep_jit.cuh)
-    snprintf(buf, sizeof buf, "K1J_REFRAME=%d", atoi(v));
-    d.push_back(buf);
-  }
-  if (const char* v = std::getenv("KPZ_B200_K1_EAGER")) {  // tuning knob: planes of the GENERAL path drawn one MCS ahead
-    snprintf(buf, sizeof buf, "K1J_EAGER=%d", atoi(v));
-    d.push_back(buf);
-  }
-  if (const char* v = std::getenv("KPZ_B200_K1_TRIP")) {  // tuning knob: planes per lazy trip of the GENERAL path
-    snprintf(buf, sizeof buf, "K1J_TRIP=%d", atoi(v));
-    d.push_back(buf);
-  }
-  if (const char* v = std::getenv("KPZ_B200_K1_VARIANT")) {  // tuning knob: code shape of the sweep (k1_sweep_jit.cuh)
-    snprintf(buf, sizeof buf, "K1J_VARIANT=%d", atoi(v));
-    d.push_back(buf);
-  }
+  debug_defines("K1J_", &d);  // kpz_debug_config: tests and tuning only (the run reads no environment)
   return d;
 }
 
@@ -389,9 +378,6 @@ int k3t_run(kpz_sim* sim, int64_t n_mcs) {
   const int dis = sim->has_sq ? 2 : sim->has_sp ? 1 : 0;
   std::vector<std::string> defs = k1_jit_defines(sim->dev, dis);
   defs.push_back("K1J_TILE=1");
-  if (const char* v = std::getenv("KPZ_B200_K1_AHEAD")) {  // tuning knob (blocked stream only): 1 = planes drawn one MCS ahead
-    defs.push_back(std::string("K1J_AHEAD=") + (atoi(v) ? "1" : "0"));
-  }
   void* kfn = nullptr;
   int rc = jit_get("k1_sweep_jit.cuh", "kpz_k3t_sweep_jit", defs, &kfn);
   if (rc) return rc;
@@ -427,6 +413,57 @@ int k3t_run(kpz_sim* sim, int64_t n_mcs) {
   return KPZ_OK;
 }
 
+// ---- overflow guard ------------------------------------------------------------------------------
+// A pass moves h_x by at most 2 through its own pair and 2 more through the closing pair: |h| grows by <= 8 per MCS.
+int guard_record_times(kpz_sim* sim, const int64_t* t, int32_t nt) {
+  if (sim->h0_pending) {  // measured by kpz_set_lattice: max |height in front of a unit| + 256
+    int v = 0;
+    KPZ_CUDA_CHECK(cudaMemcpyAsync(&v, sim->scratch + sim->dev.PW + 16, sizeof(int), cudaMemcpyDeviceToHost, sim->stream));
+    KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
+    sim->h0 = (int64_t)v + 256;
+    sim->h0_pending = false;
+  }
+  for (int32_t k = 0; k < nt; ++k) {
+    if (t[k] <= sim->t) continue;  // already captured
+    const long double bound = std::min<long double>((long double)sim->L,
+                                                    (long double)sim->h0 + 8.0L * (long double)(t[k] - sim->t_h0));
+    if ((long double)sim->L * bound * bound >= 9.0e18L)
+      return fail(KPZ_EUNSUPPORTED, "sum of h^2 could overflow int64 at t=%lld for L=%lld", (long long)t[k], (long long)sim->L);
+    if (sim->path != KPZ_PATH_ONCHIP && bound >= 2147483647.0L)
+      return fail(KPZ_EUNSUPPORTED, "heights could overflow int32 at t=%lld", (long long)t[k]);
+  }
+  sim->guard_checked = true;
+  return KPZ_OK;
+}
+
+// A lattice handed in by the caller can be as rough as |h| = L/2: measure it when that could matter.
+int measure_h0(kpz_sim* sim) {
+  const KpzDev& D = sim->dev;
+  sim->t_h0 = sim->t;
+  sim->guard_checked = false;
+  const long double Lh = (long double)sim->L;
+  if (Lh * Lh * Lh < 9.0e18L && (sim->path == KPZ_PATH_ONCHIP || Lh < 2147483647.0L)) {
+    sim->h0 = sim->L;  // the trivial bound |h| <= L never overflows on this ring
+    sim->h0_pending = false;
+    return KPZ_OK;
+  }
+  // streamed / blocked rings only reach this point (an on-chip ring has L <= 262144): their tile scan gives the height
+  // in front of every 256-site unit
+  int* slot = sim->scratch + D.PW + 16;  // beyond the PW ints kpz_heights uses
+  const int nt = sim->ntiles;
+  const bool partial = (D.PW % 4) != 0;
+  KPZ_CUDA_CHECK(cudaMemsetAsync(slot, 0, sizeof(int), sim->stream));
+  if (partial) k3_tile_totals<true><<<D.S * nt, 256, 0, sim->stream>>>(sim->E, sim->O, D.S, D.U, D.PW, D.PWp, nt, sim->tiles);
+  else k3_tile_totals<false><<<D.S * nt, 256, 0, sim->stream>>>(sim->E, sim->O, D.S, D.U, D.PW, D.PWp, nt, sim->tiles);
+  KPZ_LAUNCH_CHECK("k3_tile_totals");
+  k3_scan_tiles<<<D.S, 1024, 0, sim->stream>>>(sim->tiles, nt);
+  KPZ_LAUNCH_CHECK("k3_scan_tiles");
+  k3_tile_absmax<<<D.S * nt, 256, 0, sim->stream>>>(sim->E, sim->O, D.U, D.PW, D.PWp, nt, sim->tiles, slot);
+  KPZ_LAUNCH_CHECK("k3_tile_absmax");
+  sim->h0_pending = true;
+  return KPZ_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -443,6 +480,14 @@ const char* kpz_strerror(int code) {
 }
 const char* kpz_last_error(void) { return kpz::g_err; }
 int64_t kpz_kernel_launches(void) { return (int64_t)kpz::g_launches.load(); }
+
+int kpz_debug_config(const char* spec) { return kpz::debug_config(spec); }
+int kpz_debug_dump_cubins(const char* dir, int32_t* count) {
+  int n = 0;
+  const int rc = kpz::dump_cubins(dir, &n);
+  if (count) *count = n;
+  return rc;
+}
 
 int kpz_workspace_bytes(int64_t L, int32_t nsamples, const kpz_disorder* disorder, const kpz_options* opt,
                         int32_t max_records, size_t* bytes) {
@@ -597,6 +642,10 @@ int kpz_reset(kpz_sim* sim) {
   sim->t = 0;
   sim->nrec = 0;
   sim->frame = 0;
+  sim->h0 = 1;
+  sim->t_h0 = 0;
+  sim->h0_pending = false;
+  sim->guard_checked = false;
   return KPZ_OK;
 }
 
@@ -614,6 +663,10 @@ int kpz_time(const kpz_sim* sim, int64_t* t) {
 
 int kpz_set_time(kpz_sim* sim, int64_t t) {
   if (!sim || t < 0 || ((uint64_t)t >> 54) != 0) return fail(KPZ_EINVAL, "need 0 <= t < 2^54");
+  if (!sim->h0_pending) {  // the lattice is as rough as it was a moment ago; only the clock moves
+    sim->h0 = std::min<int64_t>(sim->L, sim->h0 + 8 * std::max<int64_t>(sim->t - sim->t_h0, 0));
+  }
+  sim->t_h0 = t;
   sim->t = t;
   sim->rec_times.clear();
   sim->nrec = 0;
@@ -626,13 +679,9 @@ int kpz_set_record_times(kpz_sim* sim, const int64_t* t, int32_t nt) {
   for (int32_t k = 0; k < nt; ++k) {
     if (t[k] < 1 || (k == 0 ? t[k] <= sim->t : t[k] <= t[k - 1]))
       return fail(KPZ_EINVAL, "record times must be strictly increasing and later than the current time");
-    // |h| <= min(L, 1 + 8 t); refuse when L * bound^2 could overflow int64
-    const long double bound = std::min<long double>((long double)sim->L, 1.0L + 8.0L * (long double)t[k]);
-    if ((long double)sim->L * bound * bound >= 9.0e18L)
-      return fail(KPZ_EUNSUPPORTED, "sum of h^2 could overflow int64 at t=%lld for L=%lld", (long long)t[k], (long long)sim->L);
-    if (sim->path != KPZ_PATH_ONCHIP && bound >= 2147483647.0L)
-      return fail(KPZ_EUNSUPPORTED, "heights could overflow int32 at t=%lld", (long long)t[k]);
   }
+  // |h| <= min(L, h0 + 8 (t - t0)); refuse when L * bound^2 could overflow int64
+  if (int rc = guard_record_times(sim, t, nt)) return rc;
   sim->rec_times.assign(t, t + nt);
   sim->nrec = 0;
   if (nt > 0) {
@@ -649,6 +698,10 @@ int kpz_run(kpz_sim* sim, int64_t n_mcs) {
   if (((uint64_t)(sim->t + n_mcs) >> 54) != 0) return fail(KPZ_EUNSUPPORTED, "time beyond 2^54 MCS");
   const int32_t nt = (int32_t)sim->rec_times.size();
   int rc = KPZ_OK;
+  if (!sim->guard_checked) {  // the lattice was replaced after the record times were listed
+    rc = guard_record_times(sim, sim->rec_times.data(), nt);
+    if (rc) return rc;
+  }
   if (sim->path == KPZ_PATH_ONCHIP) {
     KpzRunArgs A{};
     A.t0 = sim->t;
@@ -676,7 +729,7 @@ int kpz_run(kpz_sim* sim, int64_t n_mcs) {
       const int spw = pack ? 32 / D.U : 1;
       std::vector<std::string> defs = k1_jit_defines(D, dis);
       if (!pack) defs.push_back("K1J_PACK=0");
-      if (!std::getenv("KPZ_B200_K1_VARIANT")) {
+      if (!debug_has("K1J_VARIANT")) {
         // code shape by occupancy (k1_sweep_jit.cuh, K1J_VARIANT): with >= 4 resident warps per SMSP the other warps
         // hide the latency, so the shape with the fewest alu slots wins (measured: +12..16 % on 16384-site rings)
         const long long warps = (long long)((sim->S + spw - 1) / spw) * (block / 32);
@@ -718,7 +771,7 @@ int kpz_set_lattice(kpz_sim* sim, const uint32_t* d_words) {
   const KpzDev& D = sim->dev;
   k_nat_to_eo<<<grid_for((size_t)D.S * D.PW), 256, 0, sim->stream>>>(d_words, D.S, D.PW, D.PWp, sim->E, sim->O);
   KPZ_LAUNCH_CHECK("k_nat_to_eo");
-  return KPZ_OK;
+  return measure_h0(sim);
 }
 
 int kpz_disorder_masks(kpz_sim* sim, uint32_t* d_slow_p, uint32_t* d_slow_q) {

@@ -166,6 +166,30 @@ __global__ void k3_scan_tiles(int* tile_tot, int ntiles) {
   }
 }
 
+// max over the units of |height before the unit| (the overflow guard after kpz_set_lattice): inside a unit
+// the height moves by at most 256 more.
+__global__ void __launch_bounds__(256) k3_tile_absmax(const uint32_t* E, const uint32_t* O, int U, int PW, int PWp,
+                                                      int ntiles, const int* tile_base, int* out) {
+  __shared__ int sm[8];
+  const int s = blockIdx.x / ntiles, tile = blockIdx.x % ntiles;
+  const int u = tile * 256 + threadIdx.x;
+  int r = 0;
+  if (u < U) {
+    const int nw = min(4, PW - 4 * u);
+    const size_t row = (size_t)s * PWp + 4 * (size_t)u;
+    const uint4 e = *reinterpret_cast<const uint4*>(E + row);
+    const uint4 q = *reinterpret_cast<const uint4*>(O + row);
+    r = 2 * (__popc(e.x) + __popc(e.y) + __popc(e.z) + __popc(e.w) + __popc(q.x) + __popc(q.y) + __popc(q.z) + __popc(q.w)) -
+        64 * nw;  // pad words are zero
+  }
+  int total;
+  const int base = tile_base[(size_t)s * ntiles + tile] + block_exclusive_scan_256(r, sm, total);
+  int m = u < U ? abs(base) : 0;
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) m = max(m, __shfl_xor_sync(0xFFFFFFFFu, m, d));
+  if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
+}
+
 template <bool PARTIAL>
 __global__ void __launch_bounds__(256) k3_tile_sums(const uint32_t* E, const uint32_t* O, int S, int U, int PW, int PWp,
                                                     int ntiles, const int* tile_base, unsigned long long* out_h,

@@ -92,18 +92,7 @@ std::vector<std::string> k4_jit_defines(const LanesDev& D) {
   d.push_back(buf);
   snprintf(buf, sizeof buf, "K4J_INDEP=%d", D.independent);
   d.push_back(buf);
-  if (const char* v = std::getenv("KPZ_B200_K4_EAGER")) {  // tuning knob: lane-change planes drawn one MCS ahead
-    snprintf(buf, sizeof buf, "K4J_EAGER=%d", atoi(v));
-    d.push_back(buf);
-  }
-  if (const char* v = std::getenv("KPZ_B200_K4_TRIP")) {  // tuning knob: planes per lazy trip
-    snprintf(buf, sizeof buf, "K4J_TRIP=%d", atoi(v));
-    d.push_back(buf);
-  }
-  if (const char* v = std::getenv("KPZ_B200_K4_TAIL")) {  // tuning knob: 0 = plane pairs per trip, 1 = plane-parallel tail
-    snprintf(buf, sizeof buf, "K4J_TAIL=%d", atoi(v));
-    d.push_back(buf);
-  }
+  debug_defines("K4J_", &d);  // kpz_debug_config: tests and tuning only (the run reads no environment)
   return d;
 }
 

@@ -408,40 +408,51 @@ def test_error_codes(K):
     assert K.kernel_launches() > 0
 
 
+def test_overflow_guard_measures_a_lattice_handed_in(K):
+    """the guard of the exact sums assumes |h| <= 1 + 8 t from the flat start.  A lattice handed in through
+    kpz_set_lattice can be as rough as |h| = L/2: on a ring long enough for sum h^2 to leave int64 the library measures it
+    on the device and refuses the record times at the next run - a flat lattice handed in the same way still runs."""
+    L = 1 << 22                                  # L * (L/2)^2 = 2^64
+    g = K.KpzSim(L, 1, 0.5, 0.5, seed=1, max_records=2)
+    g.set_record_times([2])                      # fine from the flat start
+    step = np.zeros((1, L // 32), dtype=np.uint32)
+    step[0, :L // 64] = 0xFFFFFFFF               # all particles in the first half: h climbs to L/2
+    g.set_lattice(K.words_from_numpy(step, g.device))
+    with pytest.raises(K.KpzError) as e:
+        g.run(2)
+    assert e.value.code == -2
+    with pytest.raises(K.KpzError) as e:
+        g.set_record_times([1])
+    assert e.value.code == -2
+    flat = np.full((1, L // 32), 0xAAAAAAAA, dtype=np.uint32)
+    g.set_lattice(K.words_from_numpy(flat, g.device))
+    g.set_record_times([2])
+    g.run(2)
+    r = g.roughness()
+    ref = R.KpzRef(L, 1, 0.5, 0.5, seed=1)
+    ref.set_record_times([2])
+    ref.run(2)
+    rr = ref.roughness()
+    assert np.array_equal(r["sum_h"], rr["sum_h"]) and np.array_equal(r["sum_h2"], rr["sum_h2"])
+    g.reset()                                    # back to the flat-start bound
+    g.run(2)
+
+
 # ---------------------------------------------------------------------------------------------------------
 # every kernel variant behind the same ABI computes the same thing: statically compiled generic kernels
-# (KPZ_B200_JIT=0) and the tuning knobs of the run-time specialised ones
+# (kpz_debug_config("jit=0")) and the tuning knobs of the run-time specialised ones
 # ---------------------------------------------------------------------------------------------------------
 
-class _env:
-    def __init__(self, **kv):
-        self.kv = kv
-
-    def __enter__(self):
-        import os
-        self.old = {k: os.environ.get(k) for k in self.kv}
-        os.environ.update({k: str(v) for k, v in self.kv.items()})
-
-    def __exit__(self, *a):
-        import os
-        for k, v in self.old.items():
-            if v is None:
-                os.environ.pop(k, None)
-            else:
-                os.environ[k] = v
-
-
-@pytest.mark.parametrize("env", [dict(KPZ_B200_JIT=0), dict(KPZ_B200_K1_VARIANT=0), dict(KPZ_B200_K1_VARIANT=2),
-                                 dict(KPZ_B200_K1_REFRAME=1), dict(KPZ_B200_K1_EAGER=3, KPZ_B200_K1_TRIP=3)])
-def test_k1_variants_against_oracle(K, env):
-    with _env(**env):
+@pytest.mark.parametrize("cfg", ["jit=0", "K1J_VARIANT=0", "K1J_VARIANT=2", "K1J_REFRAME=1", "K1J_EAGER=3;K1J_TRIP=3"])
+def test_k1_variants_against_oracle(K, cfg):
+    with K.debug_config(cfg):
         run_both_kpz(K, 8192 + 64, 3, 0.75, 0.25, seed=21, times=[1, 3, 20], chunks=[7, 13])
         run_both_kpz(K, 16384, 2, 1.0, 0.0, disorder=(0.1, 0.5, 0.0, 0.0), seed=22, times=[20], chunks=[20])
         run_both_kpz(K, 2048, 2, 0.8, 0.05, disorder=(0.3, 0.2, 0.3, 0.01), seed=23, times=[9], chunks=[9])
 
 
 def test_static_streamed_kernel_against_oracle(K):
-    with _env(KPZ_B200_JIT=0):
+    with K.debug_config("jit=0"):
         gpu, _ = run_both_kpz(K, 65536 + 64, 2, 0.9, 0.1, seed=24, times=[2, 9], chunks=[4, 5], path=2)
         assert gpu.path == K.KPZ_PATH_STREAM
         # without run-time compilation the default large-ring path is the pass-by-pass stream
@@ -451,10 +462,9 @@ def test_static_streamed_kernel_against_oracle(K):
             K.KpzSim(1 << 19, 1, 0.5, 0.5, seed=1, max_records=1, path=3)
 
 
-@pytest.mark.parametrize("env", [dict(KPZ_B200_JIT=0), dict(KPZ_B200_K4_TAIL=1), dict(KPZ_B200_K4_EAGER=1),
-                                 dict(KPZ_B200_K4_EAGER=7, KPZ_B200_K4_TAIL=1)])
-def test_k4_variants_against_oracle(K, env):
-    with _env(**env):
+@pytest.mark.parametrize("cfg", ["jit=0", "K4J_TAIL=1", "K4J_EAGER=1", "K4J_EAGER=7;K4J_TAIL=1"])
+def test_k4_variants_against_oracle(K, cfg):
+    with K.debug_config(cfg):
         run_both_lanes(K, 8192 + 64, 2, 1.0, 1.0, 0.3, 0.05, 6, 0.1, seed=31, times=[1, 6, 13], chunks=[6, 7])
         run_both_lanes(K, 2048, 2, 0.75, 0.5, 0.4, 0.3, 4, 0.3, seed=32, times=[9], chunks=[9])
 
@@ -575,7 +585,7 @@ def test_crossing_model_flags_can_be_set_and_static_kernel_refuses(K):
     gpu.run(15)
     for g, r in zip(gpu.state()[:2], ref.state()[:2]):
         assert np.array_equal(K.words_to_numpy(g), r)
-    with _env(KPZ_B200_JIT=0):
+    with K.debug_config("jit=0"):
         g2 = K.LanesSim(L, S, 0.5, 0.5, 0.5, 0.5, 0, 0.2, seed=4, w_unflagged=0.8, independent=1, max_records=1)
         with pytest.raises(K.KpzError):
             g2.run(1)

@@ -68,9 +68,31 @@ def test_bad_arguments_are_refused_without_compiling(K):
 
 
 @pytest.mark.parametrize("variant", ["0", "1", "2"])
-def test_every_code_shape_of_the_sweep_compiles(K, variant, monkeypatch):
+def test_every_code_shape_of_the_sweep_compiles(K, variant):
     """K1J_VARIANT: 4-way switch with the Philox rounds inside, branch-free, 4-way switch after the Philox rounds."""
-    monkeypatch.setenv("KPZ_B200_K1_VARIANT", variant)
+    with K.debug_config("K1J_VARIANT=" + variant):
+        assert K.jit_check(8192, 0.75, 0.25) > 10_000
+        assert K.jit_check(16384, 1.0, 0.0, disorder=(0.1, 0.5, 0.0, 0.0)) > 10_000
+        assert K.jit_check(1 << 20, 0.75, 0.25, path=3) > 10_000
+
+
+def test_debug_config_is_validated_and_restored(K):
+    with pytest.raises(K.KpzError):
+        K.debug_config("FOO=1")
+    with pytest.raises(K.KpzError):
+        K.debug_config("K1J_VARIANT")
+    with pytest.raises(K.KpzError):
+        K.debug_config("K1J_X=1 -DY")
+    with K.debug_config("jit=0"):
+        assert K.jit_check(8192, 0.75, 0.25) == 0          # statically compiled kernel: nothing to specialise
     assert K.jit_check(8192, 0.75, 0.25) > 10_000
-    assert K.jit_check(16384, 1.0, 0.0, disorder=(0.1, 0.5, 0.0, 0.0)) > 10_000
-    assert K.jit_check(1 << 20, 0.75, 0.25, path=3) > 10_000
+
+
+def test_compiled_images_can_be_dumped(K, tmp_path):
+    K.jit_check(8192, 0.75, 0.25)
+    n = K.debug_dump_cubins(str(tmp_path))
+    assert n >= 1
+    names = sorted(p.name for p in tmp_path.iterdir())
+    assert any(x.startswith("kpz_k1_sweep_jit_") and x.endswith(".cubin") for x in names)
+    txt = next(p for p in tmp_path.iterdir() if p.name.startswith("kpz_k1_sweep_jit_") and p.suffix == ".txt")
+    assert "-DK1J_PW=128" in txt.read_text()
