@@ -308,7 +308,8 @@ def _oracle_current(row, mode, S, burn, n_mcs, seed):
 
 
 @pytest.mark.parametrize("idx,mode", [(1, "drawn"), (1, "alternating"), (3, "drawn"), (2, "drawn"),
-                                      (7, "drawn"), (7, "alternating"), (1, "rsu"), (3, "rsu")])
+                                      (7, "drawn"), (7, "alternating"), (1, "rsu"), (3, "rsu"),
+                                      (6, "drawn"), (6, "alternating"), (6, "rsu")])  # row 6: p=0.9, q=0.1 (32 planes)
 def test_oracle_stationary_current_matches_master_equation(idx, mode):
     row = _golden_currents()[idx]
     if mode == "alternating" and row["slow"] >= 0:
@@ -371,6 +372,49 @@ def test_finite_time_distribution_with_slow_sites_chi2():
     assert chi2(v_alt2)[0] > 20 * dof
     _, v_swapped, _, _ = ME.kpz_finite_time(L, N, qs, ps, flat, t, "drawn")
     assert chi2(v_swapped)[0] > 20 * dof
+
+
+@pytest.mark.parametrize("p,q,p_slow,q_slow", [(0.3, 0.6, 0.9, 0.1), (0.9, 0.1, 0.8, 1.0 / 3.0)])
+def test_finite_time_distribution_non_dyadic_rates_chi2(p, q, p_slow, q_slow):
+    """As above with rates whose thresholds use all 32 bit-planes (0.3 -> 0x4CCCCCCC, 0.6 -> 0x99999999, 0.9, 0.1, 0.8,
+    1/3): the acceptance comparison has to be right beyond the two leading planes.  Power: the
+    same histogram rejects the distribution for rates rounded to their 2 leading bits."""
+    L, N, S, t = 8, 4, 60000, 2
+    sp_site, sq_site = 2, 5
+    flat = sum(1 << i for i in range(1, L, 2))
+    ps, qs = [p] * L, [q] * L
+    ps[sp_site], qs[sq_site] = p_slow, q_slow
+    states, v, fwd, bwd = ME.kpz_finite_time(L, N, ps, qs, flat, t, "drawn")
+    sim = R.KpzRef(L, S, p, q, disorder=(0.0, p_slow, 0.0, q_slow), seed=78)
+    mp = np.zeros((S, L), dtype=np.uint8)
+    mq = np.zeros((S, L), dtype=np.uint8)
+    mp[:, sp_site] = 1
+    mq[:, sq_site] = 1
+    sim.set_disorder_masks(R.pack_sites(mp), R.pack_sites(mq))
+    sim.run(t)
+    codes = sim.lattice()[:, 0].astype(np.int64)
+    counts = np.array([(codes == s).sum() for s in states], dtype=np.float64)
+    assert counts.sum() == S
+
+    def chi2(prob):
+        keep = prob * S >= 5
+        c = ((counts[keep] - prob[keep] * S) ** 2 / (prob[keep] * S)).sum()
+        rest_exp = prob[~keep].sum() * S
+        if rest_exp > 0:
+            c += (counts[~keep].sum() - rest_exp) ** 2 / rest_exp
+        return c, int(keep.sum())
+
+    c, dof = chi2(v)
+    assert c < dof + 5 * np.sqrt(2 * dof), (c, dof)
+    f, b = sim.hops()
+    assert abs(f.mean() - fwd) < 5 * f.std(ddof=1) / np.sqrt(S)
+    assert abs(b.mean() - bwd) < 5 * b.std(ddof=1) / np.sqrt(S)
+    trunc = lambda x: np.floor(x * 4) / 4                        # what a comparison of the 2 leading planes would give
+    _, v2, _, _ = ME.kpz_finite_time(L, N, [trunc(x) for x in ps], [trunc(x) for x in qs], flat, t, "drawn")
+    assert chi2(v2)[0] > 20 * dof
+    trunc4 = lambda x: np.floor(x * 16) / 16                     # ... of the 4 leading planes
+    _, v4, _, _ = ME.kpz_finite_time(L, N, [trunc4(x) for x in ps], [trunc4(x) for x in qs], flat, t, "drawn")
+    assert chi2(v4)[0] > dof + 8 * np.sqrt(2 * dof)
 
 
 def test_stationary_width_matches_master_equation():

@@ -94,6 +94,7 @@ def test_lane_b_hops_left_lane_a_hops_right():
     (0.5, 0.5, 0.8, 0b0101, (0b0011, 0b0100)),
     (1.0, 1.0, 0.1, 0b0010, (0b1001, 0b0001)),
     (0.75, 0.25, 0.5, 0b1111, (0b0001, 0b0110)),
+    (0.3, 0.6, 0.1, 0b1111, (0b0101, 0b0010)),      # every threshold uses all 32 bit-planes (omega = 0.1 as in config 5)
 ])
 def test_finite_time_two_lane_master_equation(p_a, p_b, omega, turn_mask, start):
     """Exact distribution and expected hop counts after 3 MCS on L=4 versus the oracle's histogram over 30000

@@ -5,6 +5,10 @@
   DESIGN.md §R3-R4 documents (convention — "parity unpinned" by any external source), assembled here
   from the KAT-pinned block function only.
 * Statistical sanity of the streams (uniformity, fair offsets, independence of streams).
+* "Is it still a fair 32-bit uniform": every one of the 32 bits of kpzref_uniform is fair and the bits are pairwise
+  uncorrelated over 2^17 elements, U/2^32 passes a Kolmogorov-Smirnov test, acceptance frequencies of non-dyadic
+  thresholds hold to 3 decimal places, and the nested-threshold property [U < 2^(32-k)] <=> "planes 0..k-1 are all zero"
+  ties the plane ORDER to the sweep's acceptance rule (a zeroed, duplicated or swapped plane fails one of them).
 """
 import os
 
@@ -116,3 +120,66 @@ def test_uniforms_are_uniform_and_streams_differ():
     assert not np.array_equal(u0, u1) and not np.array_equal(u0, u2)
     for a, b in ((u0, u1), (u0, u2)):
         assert abs(np.corrcoef(a, b)[0, 1]) < 5 / np.sqrt(n)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# the uniform as a whole: all 32 planes (earlier pins only had power on planes 0-2)
+# ------------------------------------------------------------------------------------------------------------------
+
+_N_BITS = 1 << 17
+
+
+@pytest.fixture(scope="module")
+def uniforms():
+    """U32 of 2^17 consecutive elements of three streams (PAIR pass 0, PAIR pass 1 at another time, SWITCH_AB)."""
+    out = {}
+    for name, (tag, tk, ps) in {"pair0": (R.TAGS["PAIR"], 7, 0), "pair1": (R.TAGS["PAIR"], (1 << 33) + 5, 1),
+                                "switch": (R.TAGS["SWITCH_AB"], 123456, 0)}.items():
+        out[name] = np.array([R.uniform(2024, tag, 3, tk, ps, e) for e in range(_N_BITS)], dtype=np.uint64)
+    return out
+
+
+@pytest.mark.parametrize("stream", ["pair0", "pair1", "switch"])
+def test_every_bit_of_the_uniform_is_fair_and_bits_are_uncorrelated(uniforms, stream):
+    u = uniforms[stream]
+    n = len(u)
+    bits = ((u[:, None] >> np.arange(32, dtype=np.uint64)[None, :]) & 1).astype(np.float64)      # [n][32]
+    mean = bits.mean(axis=0)
+    assert np.all(np.abs(mean - 0.5) < 5 * 0.5 / np.sqrt(n)), mean       # a stuck plane fails here
+    c = np.corrcoef(bits.T)
+    off = c[~np.eye(32, dtype=bool)]
+    assert np.all(np.abs(off) < 5.5 / np.sqrt(n)), np.abs(off).max()     # a duplicated plane has correlation 1
+    # neighbouring ELEMENTS are independent too (bit b of element e vs bit b of element e+1, e+32, e+128)
+    for lag in (1, 32, 128):
+        x, y = bits[:-lag], bits[lag:]
+        r = ((x - 0.5) * (y - 0.5)).mean(axis=0) * 4
+        assert np.all(np.abs(r) < 5 / np.sqrt(n - lag)), (lag, np.abs(r).max())
+
+
+@pytest.mark.parametrize("stream", ["pair0", "pair1", "switch"])
+def test_uniform_passes_kolmogorov_smirnov_and_hits_non_dyadic_thresholds(uniforms, stream):
+    from scipy import stats
+    u = uniforms[stream]
+    n = len(u)
+    x = (u.astype(np.float64) + 0.5) / 2.0**32
+    assert stats.kstest(x, "uniform").pvalue > 1e-4
+    # low 16 bits on their own (planes 16-31): a KS test of the high bits cannot see them
+    lo = ((u & np.uint64(0xFFFF)).astype(np.float64) + 0.5) / 65536.0
+    assert stats.kstest(lo, "uniform").pvalue > 1e-4
+    for prob in (0.9, 0.1, 0.8, 0.3, 0.6, 0.05, 1.0 / 3.0):
+        T = R.threshold(prob)
+        f = (u < np.uint64(T)).mean()
+        assert abs(f - T / 2.0**32) < 5 * np.sqrt(prob * (1 - prob) / n), (prob, f)
+
+
+def test_plane_order_is_msb_first_through_the_acceptance_rule():
+    """[U < 2^(32-k)] holds exactly when planes 0..k-1 of the element are all zero: plane b carries bit 31-b.  The
+    left side is the acceptance rule of the sweep applied to kpzref_uniform, the right side comes from the
+    KAT-pinned block function plane by plane; any permutation of the planes breaks the equivalence for some k."""
+    seed, tag, sample, tk, ps = 99, R.TAGS["PAIR"], 1, 31, 0
+    for element in (0, 5, 37, 127, 128, 1000, 4097):
+        G, w, k = element >> 7, (element >> 5) & 3, element & 31
+        plane_bits = [(R.philox_call(seed, tag, sample, tk, ps, b, G)[w] >> k) & 1 for b in range(32)]
+        u = R.uniform(seed, tag, sample, tk, ps, element)
+        for kk in range(1, 33):
+            assert (u < (1 << (32 - kk))) == (not any(plane_bits[:kk]))
