@@ -26,11 +26,13 @@ __device__ __forceinline__ uint32_t height_lut_entry(int idx) {
 
 // Sums over the 64*nw sites of one unit (even-site words P, odd-site words Q, frame 0) of the heights relative to the
 // site before the unit: r = total slope, s1 = sum, s2 = sum of squares (|r| <= 256, s2 <= 2^24: int32 is exact).
-__device__ __forceinline__ void unit_relative_sums_lut(const uint32_t (&P)[4], const uint32_t (&Q)[4], int nw,
+// (N = 4 words per thread, or 8 when a thread of the on-chip sweep holds two units: |r| <= 512, s2 <= 2^27.)
+template <int N>
+__device__ __forceinline__ void unit_relative_sums_lut(const uint32_t (&P)[N], const uint32_t (&Q)[N], int nw,
                                                        const uint32_t* lut, int& r_out, int& s1_out, int& s2_out) {
   int r = 0, s1 = 0, s2 = 0;
 #pragma unroll
-  for (int w = 0; w < 4; ++w) {
+  for (int w = 0; w < N; ++w) {
     if (w < nw) {
 #pragma unroll
       for (int k = 0; k < 8; ++k) {

@@ -110,6 +110,14 @@ bool debug_has(const char* name) {
   return false;
 }
 
+int debug_int(const char* name, int dflt) {
+  std::lock_guard<std::mutex> lock(g_dbg_mu);
+  const size_t n = std::strlen(name);
+  for (const std::string& d : g_dbg_defs)
+    if (d.size() > n && d.compare(0, n, name) == 0 && d[n] == '=') return std::atoi(d.c_str() + n + 1);
+  return dflt;
+}
+
 int jit_compile(const char* source, const char* entry, const std::vector<std::string>& defines,
                 std::vector<char>* cubin, std::string* log) {
   const Embedded* src = find_source(source);

@@ -15,6 +15,8 @@ int debug_config(const char* spec);
 void debug_defines(const char* prefix, std::vector<std::string>* defs);
 // True when the debug configuration defines NAME (whatever its value).
 bool debug_has(const char* name);
+// Integer value of NAME in the debug configuration, or dflt.
+int debug_int(const char* name, int dflt);
 
 // Compile `entry` (an extern "C" __global__ function) of the embedded source file `source` for sm_100a with the
 // given NAME=VALUE definitions.  Needs no GPU.  Returns KPZ_OK and the cubin, or an error code (text in

@@ -65,6 +65,12 @@
 #define K1J_TRIP 2  // 1.7 warps per SMSP: latency-bound, two independent calls per trip (p = 0.8 at L = 1024: +5 %)
 #endif
 #endif
+#ifndef K1J_UPT   // units (Philox supergroups of 256 sites) per thread of the per-sample kernel.  2: a ring of 64 units is
+#define K1J_UPT 1  // ONE warp - no __syncthreads, no shared-memory halo, two independent units of pair logic per thread
+#endif             // (L = 16384: see DESIGN §5); rings whose unit count is even and not ragged only.
+#if (defined(K1J_TILE) || defined(K1J_STREAM)) && K1J_UPT != 1
+#error "K1J_UPT > 1 is implemented by the per-sample kernel only"
+#endif
 #ifndef K1J_PW
 #error "k1_sweep_jit.cuh needs K1J_PW, K1J_T0..3, K1J_DIS, K1J_OFFSET_MODE"
 #endif
@@ -74,21 +80,25 @@ namespace k1j {
 
 constexpr int PW = K1J_PW;
 constexpr int PWp = (PW + 3) / 4 * 4;
-constexpr int U = PWp / 4;
+constexpr int U = PWp / 4;                 // units (Philox supergroups) per sample
+constexpr int UPT = K1J_UPT;               // units per thread
+constexpr int NW = 4 * UPT;                // pair-words per thread
+constexpr int UT = (U + UPT - 1) / UPT;    // threads per sample
 constexpr bool PARTIAL = (PW % 4) != 0;
+static_assert(UPT == 1 || (!PARTIAL && U % UPT == 0), "several units per thread: whole units, evenly divided");
 #ifdef K1J_TILE
 constexpr bool TILE = true;   // K3T: a warp sweeps a 32-unit window of a long ring (kpz_k3t_sweep_jit below)
 #else
 constexpr bool TILE = false;
 #endif
-constexpr bool SINGLE_WARP = TILE || U <= 32;
+constexpr bool SINGLE_WARP = TILE || UT <= 32;
 // Small rings: a ring of U <= 16 units (L = 256 U sites, U a power of two) fills only U lanes, so a warp sweeps
 // SPW = 32 / U independent samples side by side; every per-sample quantity (offsets, frame, record sums) is then a
 // per-lane value and the shuffles run inside segments of U lanes.
 // (K1J_PACK=0 turns packing off; measured, it never helps.)
-constexpr int SPW = (K1J_PACK && !TILE && !PARTIAL && U <= 16 && (U & (U - 1)) == 0) ? 32 / U : 1;
+constexpr int SPW = (K1J_PACK && !TILE && !PARTIAL && UT <= 16 && (UT & (UT - 1)) == 0) ? 32 / UT : 1;
 constexpr int DIS = K1J_DIS;
-constexpr int NTHREADS = (U + 31) / 32 * 32;
+constexpr int NTHREADS = (UT + 31) / 32 * 32;
 constexpr uint64_t T0 = K1J_T0, T1 = K1J_T1, T2 = K1J_T2, T3 = K1J_T3;
 constexpr uint64_t kOne = 1ull << 32;
 
@@ -113,7 +123,7 @@ constexpr int NPSA = NEAG > 0 ? NEAG : 1;  // array extent
 
 // The eagerly drawn random bit-planes of one MCS of one unit: r[pass][plane][word].
 struct Planes {
-  uint32_t r[2][NPSA][4];
+  uint32_t r[2][NPSA][NW];
 };
 
 __device__ __forceinline__ void draw_planes(Planes& R, const PhiloxKeys& K, uint32_t G, uint32_t gs, long long m) {
@@ -122,11 +132,14 @@ __device__ __forceinline__ void draw_planes(Planes& R, const PhiloxKeys& K, uint
   for (int pass = 0; pass < 2; ++pass) {
 #pragma unroll
     for (int pl = 0; pl < NEAG; ++pl) {
-      const uint4 v = philox4x32_10(G, gs, tlo, ctr3(TAG_PAIR, (uint32_t)pass, (uint32_t)pl, thi), K);
-      R.r[pass][pl][0] = v.x;
-      R.r[pass][pl][1] = v.y;
-      R.r[pass][pl][2] = v.z;
-      R.r[pass][pl][3] = v.w;
+#pragma unroll
+      for (int j = 0; j < UPT; ++j) {  // G = the thread's first supergroup
+        const uint4 v = philox4x32_10(G + j, gs, tlo, ctr3(TAG_PAIR, (uint32_t)pass, (uint32_t)pl, thi), K);
+        R.r[pass][pl][4 * j + 0] = v.x;
+        R.r[pass][pl][4 * j + 1] = v.y;
+        R.r[pass][pl][4 * j + 2] = v.z;
+        R.r[pass][pl][4 * j + 3] = v.w;
+      }
     }
   }
 }
@@ -173,7 +186,7 @@ __host__ __device__ constexpr int sel_lut() {
 }
 
 // sel for one word (LUT path only): a = departure side of a forward hop; spa / sqb = the tags of the pair's a / b site.
-__device__ __forceinline__ uint32_t select_word(uint32_t a, uint32_t spa, uint32_t sqb, const uint32_t (&r)[NPSA][4],
+__device__ __forceinline__ uint32_t select_word(uint32_t a, uint32_t spa, uint32_t sqb, const uint32_t (&r)[NPSA][NW],
                                                 int w) {
   uint32_t in[3] = {a, 0u, 0u};
   int k = 1;
@@ -193,12 +206,12 @@ __host__ __device__ constexpr uint32_t is_partial(uint64_t T) { return (T > 0 &&
 // equals T's, lt |= pairs decided "U < T".  A plane whose T bit is 0 costs one LOP3 per word, a 1 bit two; once T has no
 // bit left below, an equal prefix can no longer become "less" and the class drops out.
 template <uint64_t T>
-__device__ __forceinline__ void class_planes_eager(uint32_t (&lt)[4], uint32_t (&eq)[4], const uint32_t (&r)[NPSA][4]) {
+__device__ __forceinline__ void class_planes_eager(uint32_t (&lt)[NW], uint32_t (&eq)[NW], const uint32_t (&r)[NPSA][NW]) {
   if constexpr (T > 0 && T < kOne) {
 #pragma unroll
     for (int pl = 0; pl < NEAG; ++pl) {
 #pragma unroll
-      for (int w = 0; w < 4; ++w) {
+      for (int w = 0; w < NW; ++w) {
         if (pl >= planes_of(T)) {
           eq[w] = 0u;
         } else if (tbit(T, pl)) {
@@ -212,15 +225,15 @@ __device__ __forceinline__ void class_planes_eager(uint32_t (&lt)[4], uint32_t (
   }
 }
 template <uint64_t T>
-__device__ __forceinline__ void class_plane_lazy(uint32_t (&lt)[4], uint32_t (&eq)[4], const uint32_t (&R)[4], int pl) {
+__device__ __forceinline__ void class_plane_lazy(uint32_t (&lt)[NW], uint32_t (&eq)[NW], const uint32_t (&R)[NW], int pl) {
   if constexpr (T > 0 && T < kOne) {
     if (pl >= planes_of(T)) {  // warp-uniform
 #pragma unroll
-      for (int w = 0; w < 4; ++w) eq[w] = 0u;
+      for (int w = 0; w < NW; ++w) eq[w] = 0u;
     } else {
       const uint32_t tb = 0u - ((uint32_t)(T >> (31 - pl)) & 1u);
 #pragma unroll
-      for (int w = 0; w < 4; ++w) {
+      for (int w = 0; w < NW; ++w) {
         lt[w] |= eq[w] & tb & ~R[w];
         eq[w] &= ~(R[w] ^ tb);
       }
@@ -231,13 +244,13 @@ __device__ __forceinline__ void class_plane_lazy(uint32_t (&lt)[4], uint32_t (&e
 // flips of the 32 pairs of each word of one pass: x = active pairs, a = side holding the particle's departure site.
 // The pairs are split into their rate classes (0 = p, 1 = p_slow, 2 = q, 3 = q_slow) once; every class then compares
 // against its own constant threshold.
-__device__ __forceinline__ void general_flips(uint32_t (&lt)[4], const uint32_t (&x)[4], const uint32_t (&a)[4],
-                                              const uint32_t (&spa)[4], const uint32_t (&sqb)[4],
-                                              const uint32_t (&r)[NPSA][4], const PhiloxKeys& K, uint32_t G, uint32_t gs,
+__device__ __forceinline__ void general_flips(uint32_t (&lt)[NW], const uint32_t (&x)[NW], const uint32_t (&a)[NW],
+                                              const uint32_t (&spa)[NW], const uint32_t (&sqb)[NW],
+                                              const uint32_t (&r)[NPSA][NW], const PhiloxKeys& K, uint32_t G, uint32_t gs,
                                               uint32_t tlo, uint32_t c3) {
-  uint32_t e0[4], e1[4], e2[4], e3[4];
+  uint32_t e0[NW], e1[NW], e2[NW], e3[NW];
 #pragma unroll
-  for (int w = 0; w < 4; ++w) {
+  for (int w = 0; w < NW; ++w) {
     const uint32_t xp = x[w] & a[w], xq = x[w] & ~a[w];
     const uint32_t m0 = DIS >= 1 ? (xp & ~spa[w]) : xp, m1 = DIS >= 1 ? (xp & spa[w]) : 0u;
     const uint32_t m2 = DIS >= 2 ? (xq & ~sqb[w]) : xq, m3 = DIS >= 2 ? (xq & sqb[w]) : 0u;
@@ -257,14 +270,17 @@ __device__ __forceinline__ void general_flips(uint32_t (&lt)[4], const uint32_t 
     for (int pl = NEAG; pl < NPS; pl += K1J_TRIP) {
       uint32_t any = 0u;
 #pragma unroll
-      for (int w = 0; w < 4; ++w) any |= e0[w] | e1[w] | e2[w] | e3[w];
+      for (int w = 0; w < NW; ++w) any |= e0[w] | e1[w] | e2[w] | e3[w];
       if (!__any_sync(alive, any != 0u)) break;
-      uint32_t R[K1J_TRIP][4];
+      uint32_t R[K1J_TRIP][NW];
 #pragma unroll
       for (int t = 0; t < K1J_TRIP; ++t) {  // independent calls: their rounds interleave
         const int q = pl + t < 32 ? pl + t : 31;
-        const uint4 v = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)q << 22), K);
-        R[t][0] = v.x; R[t][1] = v.y; R[t][2] = v.z; R[t][3] = v.w;
+#pragma unroll
+        for (int j = 0; j < UPT; ++j) {
+          const uint4 v = philox4x32_10(G + j, gs, tlo, c3 | ((uint32_t)q << 22), K);
+          R[t][4 * j + 0] = v.x; R[t][4 * j + 1] = v.y; R[t][4 * j + 2] = v.z; R[t][4 * j + 3] = v.w;
+        }
       }
 #pragma unroll
       for (int t = 0; t < K1J_TRIP; ++t) {
@@ -280,10 +296,10 @@ __device__ __forceinline__ void general_flips(uint32_t (&lt)[4], const uint32_t 
 }
 
 // One sub-lattice pass with the roles known at compile time (§R3).
-__device__ __forceinline__ void pass_logic(uint32_t (&a)[4], uint32_t (&b)[4], const uint32_t (&spa)[4],
-                                           const uint32_t (&sqb)[4], const uint32_t (&r)[NPSA][4]) {
+__device__ __forceinline__ void pass_logic(uint32_t (&a)[NW], uint32_t (&b)[NW], const uint32_t (&spa)[NW],
+                                           const uint32_t (&sqb)[NW], const uint32_t (&r)[NPSA][NW]) {
 #pragma unroll
-  for (int w = 0; w < 4; ++w) {
+  for (int w = 0; w < NW; ++w) {
     const uint32_t sel = select_word(a[w], spa[w], sqb[w], r, w);
     const uint32_t na = lop3<0xD8>(a[w], b[w], sel);  // a ^ ((a ^ b) & sel)
     const uint32_t nb = lop3<0xE4>(a[w], b[w], sel);  // b ^ ((a ^ b) & sel)
@@ -307,19 +323,18 @@ __device__ __forceinline__ uint32_t unit_exchange(uint32_t mine, int src, uint32
 }
 
 struct Unit {
-  int nw;   // valid words of this unit (4, fewer in the last unit of a ragged ring, 0 for an idle lane)
-  int nxt;  // unit holding the next 256 sites (ring closure: the last unit's successor is unit 0)
+  int nw;   // valid words of this thread (NW, fewer in the last unit of a ragged ring, 0 for an idle lane)
+  int nxt;  // thread holding the next sites (ring closure: the last unit's successor is unit 0)
   int prv;
 };
 
 // frame 0 -> 1: P'[w] = P[w] >> 1 | next << 31, h = word 0 of the next unit
 // (sh = 1; sh = 0 leaves P as it is: the branch-free sweep passes the offset itself)
-__device__ __forceinline__ void shift_up_words(uint32_t (&P)[4], int nw, uint32_t h, uint32_t sh) {
+__device__ __forceinline__ void shift_up_words(uint32_t (&P)[NW], int nw, uint32_t h, uint32_t sh) {
   if (!PARTIAL) {
-    P[0] = __funnelshift_r(P[0], P[1], sh);
-    P[1] = __funnelshift_r(P[1], P[2], sh);
-    P[2] = __funnelshift_r(P[2], P[3], sh);
-    P[3] = __funnelshift_r(P[3], h, sh);
+#pragma unroll
+    for (int w = 0; w < NW - 1; ++w) P[w] = __funnelshift_r(P[w], P[w + 1], sh);
+    P[NW - 1] = __funnelshift_r(P[NW - 1], h, sh);
   } else {
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
@@ -329,11 +344,10 @@ __device__ __forceinline__ void shift_up_words(uint32_t (&P)[4], int nw, uint32_
   }
 }
 // frame 1 -> 0: P[w] = P'[w] << 1 | prev >> 31, h = last valid word of the previous unit
-__device__ __forceinline__ void shift_down_words(uint32_t (&P)[4], int nw, uint32_t h, uint32_t sh) {
+__device__ __forceinline__ void shift_down_words(uint32_t (&P)[NW], int nw, uint32_t h, uint32_t sh) {
   if (!PARTIAL) {
-    P[3] = __funnelshift_l(P[2], P[3], sh);
-    P[2] = __funnelshift_l(P[1], P[2], sh);
-    P[1] = __funnelshift_l(P[0], P[1], sh);
+#pragma unroll
+    for (int w = NW - 1; w > 0; --w) P[w] = __funnelshift_l(P[w - 1], P[w], sh);
     P[0] = __funnelshift_l(h, P[0], sh);
   } else {
 #pragma unroll
@@ -343,14 +357,14 @@ __device__ __forceinline__ void shift_down_words(uint32_t (&P)[4], int nw, uint3
     }
   }
 }
-__device__ __forceinline__ void frame_up(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity,
+__device__ __forceinline__ void frame_up(uint32_t (&P)[NW], const Unit& un, uint32_t* halo, int& parity,
                                          uint32_t sh = 1u) {
   const uint32_t h = unit_exchange(P[0], un.nxt, halo, parity);
   shift_up_words(P, un.nw, h, sh);
 }
-__device__ __forceinline__ void frame_down(uint32_t (&P)[4], const Unit& un, uint32_t* halo, int& parity,
+__device__ __forceinline__ void frame_down(uint32_t (&P)[NW], const Unit& un, uint32_t* halo, int& parity,
                                            uint32_t sh = 1u) {
-  uint32_t last = P[3];
+  uint32_t last = P[NW - 1];
   if (PARTIAL) last = un.nw >= 4 ? P[3] : un.nw == 3 ? P[2] : un.nw == 2 ? P[1] : P[0];
   const uint32_t h = unit_exchange(last, un.prv, halo, parity);
   shift_down_words(P, un.nw, h, sh);
@@ -360,9 +374,9 @@ __device__ __forceinline__ void frame_down(uint32_t (&P)[4], const Unit& un, uin
 // publishes its first and its last valid word; the shift down by `from` uses the previous unit's last word, and the
 // shift up by `to` needs the next unit's first word AFTER that unit's own shift down - which is a function of words
 // this unit already holds (its own last word is the next unit's incoming word).
-__device__ __forceinline__ void reframe(uint32_t (&P)[4], const Unit& un, uint32_t from, uint32_t to, uint32_t* halo,
+__device__ __forceinline__ void reframe(uint32_t (&P)[NW], const Unit& un, uint32_t from, uint32_t to, uint32_t* halo,
                                         int& parity) {
-  uint32_t last = P[3];
+  uint32_t last = P[NW - 1];
   if (PARTIAL) last = un.nw >= 4 ? P[3] : un.nw == 3 ? P[2] : un.nw == 2 ? P[1] : P[0];
   uint32_t hn, hp;  // next unit's first word, previous unit's last word
   if (SINGLE_WARP) {
@@ -384,15 +398,15 @@ __device__ __forceinline__ void reframe(uint32_t (&P)[4], const Unit& un, uint32
 
 // Quenched tags in the frames the passes use them in.
 struct Tags {
-  uint32_t spa0[4];  // slow-p at even sites  (a side of frame 0)
-  uint32_t spa1[4];  // slow-p at odd sites   (a side of frame 1)
-  uint32_t sqb0[4];  // slow-q at odd sites   (b side of frame 0)
-  uint32_t sqb1[4];  // slow-q at even sites, shifted to frame 1 (b side of frame 1)
+  uint32_t spa0[NW];  // slow-p at even sites  (a side of frame 0)
+  uint32_t spa1[NW];  // slow-p at odd sites   (a side of frame 1)
+  uint32_t sqb0[NW];  // slow-q at odd sites   (b side of frame 0)
+  uint32_t sqb1[NW];  // slow-q at even sites, shifted to frame 1 (b side of frame 1)
 };
 
 // One MCS with the offsets (O0, O1) of its two passes known at compile time; frame 0 on entry and exit.
 template <int O0, int O1>
-__device__ __forceinline__ void mcs_logic(uint32_t (&P)[4], uint32_t (&Q)[4], const Tags& G, const Planes& R,
+__device__ __forceinline__ void mcs_logic(uint32_t (&P)[NW], uint32_t (&Q)[NW], const Tags& G, const Planes& R,
                                           const Unit& un, uint32_t* halo, int& parity) {
   if (O0) frame_up(P, un, halo, parity);
   if (O0) pass_logic(Q, P, G.spa1, G.sqb1, R.r[0]);
@@ -408,14 +422,14 @@ __device__ __forceinline__ void mcs_logic(uint32_t (&P)[4], uint32_t (&Q)[4], co
 // o by reframe() (funnel shifts by 0 or 1 bit), the a side is picked by a mask (P and Q enter the update
 // symmetrically, so only the rate selection needs to know which of them is a): the whole MCS is one basic block,
 // which the scheduler fills with the Philox rounds of the next MCS.  P must be in frame o on entry.
-__device__ __forceinline__ void pass_branchfree(uint32_t (&P)[4], uint32_t (&Q)[4], const Tags& G,
-                                                const uint32_t (&r)[NPSA][4], const Unit& un, uint32_t o,
+__device__ __forceinline__ void pass_branchfree(uint32_t (&P)[NW], uint32_t (&Q)[NW], const Tags& G,
+                                                const uint32_t (&r)[NPSA][NW], const Unit& un, uint32_t o,
                                                 uint32_t* halo, int& parity, const PhiloxKeys& K, uint32_t Gu,
                                                 uint32_t gs, uint32_t tlo, uint32_t c3) {
   const uint32_t M = 0u - o;  // all ones in frame 1
   if constexpr (!GENERAL) {
 #pragma unroll
-    for (int w = 0; w < 4; ++w) {
+    for (int w = 0; w < NW; ++w) {
       const uint32_t a = lop3<0xCA>(M, Q[w], P[w]);  // frame 1: a = odd site (Q); frame 0: a = even site (P)
       uint32_t spa = 0u, sqb = 0u;
       if (DIS >= 1) spa = lop3<0xCA>(M, G.spa1[w], G.spa0[w]);
@@ -427,9 +441,9 @@ __device__ __forceinline__ void pass_branchfree(uint32_t (&P)[4], uint32_t (&Q)[
       Q[w] = nq;
     }
   } else {
-    uint32_t a[4], x[4], spa[4], sqb[4], lt[4];
+    uint32_t a[NW], x[NW], spa[NW], sqb[NW], lt[NW];
 #pragma unroll
-    for (int w = 0; w < 4; ++w) {
+    for (int w = 0; w < NW; ++w) {
       a[w] = lop3<0xCA>(M, Q[w], P[w]);
       x[w] = P[w] ^ Q[w];
       spa[w] = DIS >= 1 ? lop3<0xCA>(M, G.spa1[w], G.spa0[w]) : 0u;
@@ -437,7 +451,7 @@ __device__ __forceinline__ void pass_branchfree(uint32_t (&P)[4], uint32_t (&Q)[
     }
     general_flips(lt, x, a, spa, sqb, r, K, Gu, gs, tlo, c3);
 #pragma unroll
-    for (int w = 0; w < 4; ++w) {
+    for (int w = 0; w < NW; ++w) {
       P[w] ^= lt[w];
       Q[w] ^= lt[w];
     }
@@ -446,13 +460,13 @@ __device__ __forceinline__ void pass_branchfree(uint32_t (&P)[4], uint32_t (&Q)[
 
 // ---- K2 fused: heights h_x = inclusive prefix of (2n-1), exact sums per sample (a6, a7) -----------
 // 8 sites at a time through the byte table of height_lut.cuh.
-__device__ __forceinline__ void record_sums(const uint32_t (&P)[4], const uint32_t (&Q)[4], int nw,
+__device__ __forceinline__ void record_sums(const uint32_t (&P)[NW], const uint32_t (&Q)[NW], int nw,
                                             const uint32_t* lut, long long* scratch, long long* out_h,
                                             long long* out_h2, bool writer) {
   int r = 0, s1 = 0, s2 = 0;
-  if (nw > 0) unit_relative_sums_lut(P, Q, nw, lut, r, s1, s2);
+  if (nw > 0) unit_relative_sums_lut<NW>(P, Q, nw, lut, r, s1, s2);
   const int lane = threadIdx.x & 31;
-  constexpr int SEG = SPW > 1 ? U : 32;  // lanes of one sample inside a warp
+  constexpr int SEG = SPW > 1 ? UT : 32;  // lanes of one sample inside a warp
   const int pos = lane & (SEG - 1);
   int incl = r;  // inclusive scan of the unit totals: the height before unit u is the sum over units < u
 #pragma unroll
@@ -513,11 +527,11 @@ __device__ __forceinline__ uint32_t draw_offsets16(const PhiloxKeys& K, uint32_t
 }
 
 struct Ctx {
-  uint32_t P[4], Q[4];
+  uint32_t P[NW], Q[NW];
   Tags tags;
   Unit un;
   uint32_t gs;   // global sample index (Philox counter c1)
-  uint32_t G;    // supergroup index of this unit (Philox counter c0)
+  uint32_t G;    // supergroup index of this thread's first unit (Philox counter c0)
   int parity;
   uint32_t offbits;
   uint32_t frame;  // frame P is in between MCS (branch-free sweep: the offset of the last pass; else 0)
@@ -664,8 +678,8 @@ kpz_k3_pass_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ k
   *reinterpret_cast<uint4*>(A.Oout + row) = make_uint4(Q[0], Q[1], Q[2], Q[3]);
 }
 #elif !defined(K1J_TILE)
-// grid = S samples (ceil(S / SPW) warps for small rings), block = NTHREADS; thread u = unit u (idle when u >= U, but it
-// joins every barrier / shuffle).
+// grid = S samples (ceil(S / SPW) warps for small rings), block = NTHREADS; thread u = units UPT u .. UPT u + UPT - 1
+// (idle when u >= UT, but it joins every barrier / shuffle).
 extern "C" __global__ void __launch_bounds__(kpz::k1j::NTHREADS)
 kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::KpzRunArgs A) {
   using namespace kpz;
@@ -676,48 +690,49 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   for (int i = threadIdx.x; i < 256; i += NTHREADS) lut[i] = height_lut_entry(i);
   __syncthreads();
 
-  // SPW == 1: CTA = sample, thread = unit.  SPW > 1: CTA = one warp = SPW samples, lane = (sample, unit).
+  // SPW == 1: CTA = sample, thread = UPT units.  SPW > 1: CTA = one warp = SPW samples, lane = (sample, units).
   int sub = 0, s = (int)blockIdx.x, u = (int)threadIdx.x, lane0 = 0;  // lane0 = first lane of this sample
-  bool active = u < U;
+  bool active = u < UT;
   if constexpr (SPW > 1) {
-    sub = (int)threadIdx.x / U;
+    sub = (int)threadIdx.x / UT;
     s = (int)blockIdx.x * SPW + sub;
-    u = (int)threadIdx.x % U;
-    lane0 = sub * U;
+    u = (int)threadIdx.x % UT;
+    lane0 = sub * UT;
     active = s < D.S;
   }
   Ctx c;
-  c.un.nw = !active ? 0 : (PARTIAL ? min(4, PW - 4 * u) : 4);
-  c.un.nxt = lane0 + ((u + 1 >= U) ? 0 : u + 1);
-  c.un.prv = lane0 + ((u == 0) ? U - 1 : u - 1);
+  c.un.nw = !active ? 0 : (PARTIAL ? min(4, PW - 4 * u) : NW);
+  c.un.nxt = lane0 + ((u + 1 >= UT) ? 0 : u + 1);
+  c.un.prv = lane0 + ((u == 0) ? UT - 1 : u - 1);
   if (!SINGLE_WARP) asm volatile("" : "+r"(c.un.nxt), "+r"(c.un.prv));  // measured: +3.5 % on 2-warp rings, -5 % on 1-warp
   c.gs = (uint32_t)(D.first_sample + s);
-  c.G = (uint32_t)u;
+  c.G = (uint32_t)(UPT * u);
   c.parity = 0;
   c.offbits = 0;
   c.frame = 0;
-  const unsigned long long row = (unsigned long long)s * PWp + 4ull * (active ? u : 0);
+  const unsigned long long row = (unsigned long long)s * PWp + (unsigned long long)NW * (active ? u : 0);
 #pragma unroll
-  for (int w = 0; w < 4; ++w) {
+  for (int w = 0; w < NW; ++w) {
     c.P[w] = c.Q[w] = 0u;
     c.tags.spa0[w] = c.tags.spa1[w] = c.tags.sqb0[w] = c.tags.sqb1[w] = 0u;
   }
+  auto load_words = [&](uint32_t(&dst)[NW], const uint32_t* src) {
+#pragma unroll
+    for (int j = 0; j < UPT; ++j) {
+      const uint4 v = *reinterpret_cast<const uint4*>(src + row + 4 * j);
+      dst[4 * j + 0] = v.x; dst[4 * j + 1] = v.y; dst[4 * j + 2] = v.z; dst[4 * j + 3] = v.w;
+    }
+  };
   if (active) {
-    const uint4 e = *reinterpret_cast<const uint4*>(D.E + row);
-    const uint4 o = *reinterpret_cast<const uint4*>(D.O + row);
-    c.P[0] = e.x; c.P[1] = e.y; c.P[2] = e.z; c.P[3] = e.w;
-    c.Q[0] = o.x; c.Q[1] = o.y; c.Q[2] = o.z; c.Q[3] = o.w;
+    load_words(c.P, D.E);
+    load_words(c.Q, D.O);
     if (DIS >= 1) {
-      const uint4 x = *reinterpret_cast<const uint4*>(D.SPE + row);
-      const uint4 y = *reinterpret_cast<const uint4*>(D.SPO + row);
-      c.tags.spa0[0] = x.x; c.tags.spa0[1] = x.y; c.tags.spa0[2] = x.z; c.tags.spa0[3] = x.w;
-      c.tags.spa1[0] = y.x; c.tags.spa1[1] = y.y; c.tags.spa1[2] = y.z; c.tags.spa1[3] = y.w;
+      load_words(c.tags.spa0, D.SPE);
+      load_words(c.tags.spa1, D.SPO);
     }
     if (DIS >= 2) {
-      const uint4 x = *reinterpret_cast<const uint4*>(D.SQO + row);
-      const uint4 y = *reinterpret_cast<const uint4*>(D.SQE + row);
-      c.tags.sqb0[0] = x.x; c.tags.sqb0[1] = x.y; c.tags.sqb0[2] = x.z; c.tags.sqb0[3] = x.w;
-      c.tags.sqb1[0] = y.x; c.tags.sqb1[1] = y.y; c.tags.sqb1[2] = y.z; c.tags.sqb1[3] = y.w;
+      load_words(c.tags.sqb0, D.SQO);
+      load_words(c.tags.sqb1, D.SQE);
     }
   }
   if (DIS >= 2) frame_up(c.tags.sqb1, c.un, halo, c.parity);  // b side of frame 1 = the NEXT even site
@@ -771,8 +786,11 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   to_frame0();
 
   if (active) {
-    *reinterpret_cast<uint4*>(D.E + row) = make_uint4(c.P[0], c.P[1], c.P[2], c.P[3]);
-    *reinterpret_cast<uint4*>(D.O + row) = make_uint4(c.Q[0], c.Q[1], c.Q[2], c.Q[3]);
+#pragma unroll
+    for (int j = 0; j < UPT; ++j) {
+      *reinterpret_cast<uint4*>(D.E + row + 4 * j) = make_uint4(c.P[4 * j], c.P[4 * j + 1], c.P[4 * j + 2], c.P[4 * j + 3]);
+      *reinterpret_cast<uint4*>(D.O + row + 4 * j) = make_uint4(c.Q[4 * j], c.Q[4 * j + 1], c.Q[4 * j + 2], c.Q[4 * j + 3]);
+    }
   }
 }
 #else  // K1J_TILE

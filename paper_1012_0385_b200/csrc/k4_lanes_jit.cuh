@@ -9,15 +9,21 @@
 //   * in-lane hops are word-local bit logic: with sh = (X >> 1 | next word << 31), lane A (right) hops where
 //     X & ~sh & pairmask(o), lane B (left) where ~X & sh & pairmask(o); offset 1 needs bit 0 of the next thread's
 //     word 0 and sends one carry bit back (ring closure = wrap-around of that exchange);
-//   * lane changes: live = turn & source & ~target; U < T(omega) is evaluated MSB-first over bit-planes: the first
-//     K4J_EAGER planes of both lane-change steps of MCS m+1 are drawn while MCS m is processed (counter-based, state
-//     independent), deeper planes only while some live site of the warp is still undecided, two planes per trip;
+//   * lane changes: live = turn & source & ~target; U < T(omega) is evaluated MSB-first over bit-planes.  The live sites
+//     are sparse (config 5: 1.3 per supergroup), so after every plane fewer lanes of a warp still hold an undecided
+//     site (74 %, 49 %, 29 %, 15 %, ... of them).  The first K4J_EAGER planes of both lane-change steps of MCS m+1 are
+//     drawn while MCS m is processed (counter-based, state independent; default 1: three lanes in four need plane 0
+//     anyway).  Deeper planes are drawn by a PACKED trip (resolve_packed): when n <= 16 lanes are undecided the idle
+//     lanes draw the following planes of the SAME supergroups - s = 2, 4 (K4J_SMAX) consecutive planes per trip,
+//     handed back through a per-warp shared-memory slot - so a trip of the warp advances the comparison by s planes
+//     instead of one.  Same result as plane-by-plane evaluation (the comparison steps run in plane order).
+//     Measured planes drawn per lane-change step: see profiles/;
 //   * hop counters by POPC of two merged hop words (hops of one pass sit on one bit parity), occupancy profile at
 //     epoch ends by warp-transposed, coalesced red.global.add.
 //
 // Compile-time configuration (-D, set by lanes_api.cu): K4J_W = L/32, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN
 // (thresholds in [0, 2^32]), K4J_OFFSET_MODE, K4J_TW0 and K4J_INDEP (site-wise crossing model), K4J_EAGER,
-// K4J_TRIP, K4J_TAIL.
+// K4J_SMAX, K4J_TRIP.
 #pragma once
 #include "sweep_types.cuh"
 
@@ -31,13 +37,16 @@
 #define K4J_INDEP 0   // 1: the B->A crossings read their own flag set (D.V)
 #endif
 #ifndef K4J_EAGER
-#define K4J_EAGER 6
+#define K4J_EAGER 1  // lane-change planes drawn one MCS ahead
+#endif
+#ifndef K4J_SMAX
+#define K4J_SMAX 4   // packed trips: at most this many consecutive planes per trip (1 = plane by plane; a power of two)
 #endif
 #ifndef K4J_TRIP
-#define K4J_TRIP 2  // planes per lazy trip
+#define K4J_TRIP 2  // planes per trip of the unpacked loop (turning-point redraw, in-lane rates < 1 with K4J_SMAX = 1)
 #endif
-#ifndef K4J_TAIL
-#define K4J_TAIL 0  // 0: two more planes per trip (resolve); 1: plane-parallel tail (resolve_tail; measured slower: serial)
+#if K4J_SMAX != 1 && K4J_SMAX != 2 && K4J_SMAX != 4 && K4J_SMAX != 8 && K4J_SMAX != 16 && K4J_SMAX != 32
+#error "K4J_SMAX must be a power of two in [1, 32]"
 #endif
 
 namespace kpz {
@@ -78,7 +87,7 @@ __device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
 // U < T, eq = prefix still equal to T's.
 template <uint64_t T>
 __device__ __forceinline__ void plane_step(uint32_t (&lt)[4], uint32_t (&eq)[4], const uint32_t (&R)[4], int pl) {
-  const uint32_t tb = 0u - (uint32_t)((T >> (31 - pl)) & 1ull);
+  const uint32_t tb = 0u - (((uint32_t)T >> (31 - pl)) & 1u);  // callers: 0 < T < 2^32
 #pragma unroll
   for (int w = 0; w < 4; ++w) {
     lt[w] |= eq[w] & tb & ~R[w];
@@ -111,41 +120,63 @@ __device__ __forceinline__ void resolve(uint32_t (&lt)[4], uint32_t (&eq)[4], co
   }
 }
 
-// Plane-parallel tail: after the eager planes only a few elements of a warp are still undecided (live * 2^-EAGER).
-// For each lane that still holds one, the WHOLE warp draws the remaining planes of that lane's supergroup at once
-// (lane l draws plane pl0 + l), a ballot per undecided element assembles the rest of its uniform, and one integer
-// comparison with the rest of T finishes it: one Philox call of the warp per undecided supergroup instead of two
-// per pair of planes.  Same result as resolve<T>() by construction (U < T with an equal prefix <=> suffix(U) <
-// suffix(T)).
-template <uint64_t T>
-__device__ __forceinline__ void resolve_tail(uint32_t (&lt)[4], uint32_t (&eq)[4], const PhiloxKeys& K, uint32_t G,
-                                             uint32_t gs, uint32_t tlo, uint32_t c3, int pl0) {
+// Per-warp exchange area of the packed trips.
+struct PackSmem {
+  uint4 plane[32];         // plane[j] = the 128 bits lane j drew
+  unsigned char owner[32];  // owner[r] = lane of the r-th undecided supergroup of the warp
+};
+
+// Finish the comparison for the undecided elements of every lane of the warp, starting at plane pl0 (< NP planes in
+// all).  Each trip: n = lanes still undecided.  While n > 16 (or K4J_SMAX = 1) every lane draws the next plane of its
+// own supergroup.  Once n <= 32 / s the 32 lanes are dealt out as (undecided supergroup i, plane pl + t), i < 32 / s,
+// t < s: lane j draws plane pl + (j / npad) of the supergroup owned by the (j mod npad)-th undecided lane, every lane
+// parks its 128 bits in shared memory, and an owner then applies planes pl .. pl + s - 1 IN ORDER - the comparison is
+// the plane-by-plane one, only the drawing is spread over the idle lanes.  step(lt, eq, R, pl) is one MSB-first step.
+template <class Step>
+__device__ __forceinline__ void resolve_packed(uint32_t (&lt)[4], uint32_t (&eq)[4], const PhiloxKeys& K, uint32_t G,
+                                               uint32_t gs, uint32_t tlo, uint32_t c3, int pl0, int NP, PackSmem* xs,
+                                               Step step) {
   const int lane = threadIdx.x & 31;
-  const uint32_t t_suffix = (uint32_t)T & (pl0 > 0 ? (0xFFFFFFFFu >> pl0) : 0xFFFFFFFFu);
-  uint32_t todo = __ballot_sync(FULL, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u);
-  while (todo) {
-    const int src = __ffs(todo) - 1;
-    todo &= todo - 1;
-    const int pl = pl0 + lane;
-    const uint32_t Gs = __shfl_sync(FULL, G, src), gss = __shfl_sync(FULL, gs, src);  // the owner's supergroup, sample
-    const uint4 v = philox4x32_10(Gs, gss, tlo, c3 | ((uint32_t)(pl < 32 ? pl : 31) << 22), K);
-    const uint32_t R[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      uint32_t e = __shfl_sync(FULL, eq[w], src);  // the owner's undecided elements of word w (warp-uniform)
-      uint32_t acc = 0u;
-      while (e) {
-        const int k = __ffs(e) - 1;
-        e &= e - 1;
-        // bit l of the ballot = plane pl0 + l of this element's uniform = bit 31 - pl0 - l of U
-        const uint32_t planes = __ballot_sync(FULL, ((R[w] >> k) & 1u) != 0u && pl < 32);
-        const uint32_t u_suffix = __brev(planes) >> pl0;
-        acc |= (u_suffix < t_suffix ? 1u : 0u) << k;
+  int pl = pl0;
+#pragma unroll 1
+  while (pl < NP) {  // warp-uniform
+    const bool und = (eq[0] | eq[1] | eq[2] | eq[3]) != 0u;
+    const uint32_t mask = __ballot_sync(FULL, und);
+    if (!mask) break;
+    const int n = __popc(mask);
+    int lg = 0;  // log2 of the planes of this trip
+    if (K4J_SMAX >= 2 && n <= 16) lg = 1;
+    if (K4J_SMAX >= 4 && n <= 8) lg = 2;
+    if (K4J_SMAX >= 8 && n <= 4) lg = 3;
+    if (K4J_SMAX >= 16 && n <= 2) lg = 4;
+    if (K4J_SMAX >= 32 && n <= 1) lg = 5;
+    if (lg == 0) {
+      const uint4 v = philox4x32_10(G, gs, tlo, c3 | ((uint32_t)pl << 22), K);
+      const uint32_t R[4] = {v.x, v.y, v.z, v.w};
+      step(lt, eq, R, pl);
+      pl += 1;
+    } else {
+      const int npad = 32 >> lg;
+      const int rank = __popc(mask & ((1u << lane) - 1u));
+      if (und) xs->owner[rank] = (unsigned char)lane;
+      __syncwarp();
+      const int i = lane & (npad - 1), t = lane >> (5 - lg);
+      const int src = i < n ? (int)xs->owner[i] : lane;  // spare lanes redraw a plane of their own: never read
+      const uint32_t Gs = __shfl_sync(FULL, G, src), gss = __shfl_sync(FULL, gs, src);
+      const int q = pl + t < 32 ? pl + t : 31;
+      xs->plane[lane] = philox4x32_10(Gs, gss, tlo, c3 | ((uint32_t)q << 22), K);
+      __syncwarp();
+      const int mine = rank & (npad - 1);  // decided lanes read somebody's planes: eq = 0 makes the step a no-op
+#pragma unroll 1
+      for (int tt = 0; tt < (1 << lg); ++tt) {
+        if (pl + tt < NP) {  // warp-uniform
+          const uint4 v = xs->plane[mine + tt * npad];
+          const uint32_t R[4] = {v.x, v.y, v.z, v.w};
+          step(lt, eq, R, pl + tt);
+        }
       }
-      if (lane == src) {
-        lt[w] |= acc;
-        eq[w] = 0u;
-      }
+      __syncwarp();  // the slots are rewritten by the next trip
+      pl += 1 << lg;
     }
   }
 }
@@ -161,6 +192,20 @@ __device__ __forceinline__ void lazy_less(uint32_t (&lt)[4], const uint32_t (&li
     eq[w] = (T >= kOne || T == 0) ? 0u : live[w];
   }
   if (T > 0 && T < kOne) resolve<T>(lt, eq, K, G, gs, tlo, c3, 0);
+}
+// Same through packed trips (every lane of the warp must call it).
+template <uint64_t T>
+__device__ __forceinline__ void lazy_less_packed(uint32_t (&lt)[4], const uint32_t (&live)[4], const PhiloxKeys& K,
+                                                 uint32_t G, uint32_t gs, uint32_t tlo, uint32_t c3, PackSmem* xs) {
+  uint32_t eq[4];
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    lt[w] = (T >= kOne) ? live[w] : 0u;
+    eq[w] = (T >= kOne || T == 0) ? 0u : live[w];
+  }
+  if (T > 0 && T < kOne)
+    resolve_packed(lt, eq, K, G, gs, tlo, c3, 0, planes_of(T), xs,
+                   [](uint32_t (&l)[4], uint32_t (&e)[4], const uint32_t (&R)[4], int pl) { plane_step<T>(l, e, R, pl); });
 }
 
 // ---- bit gathers between site order and pair order ------------------------------------------------------------------
@@ -224,7 +269,7 @@ struct Unit {
 template <bool RIGHT, uint64_t TP>
 __device__ __forceinline__ uint32_t lane_pass(uint32_t (&X)[4], const Unit& un, uint32_t o, uint32_t next0,
                                               const PhiloxKeys& K, uint32_t tag, uint32_t tlo, uint32_t c3time,
-                                              unsigned long long& hops) {
+                                              unsigned long long& hops, PackSmem* xs) {
   uint32_t hop[4];
   const uint32_t amask = o ? 0xAAAAAAAAu : 0x55555555u;
 #pragma unroll
@@ -243,7 +288,7 @@ __device__ __forceinline__ uint32_t lane_pass(uint32_t (&X)[4], const Unit& un, 
     const bool hi = (un.u & 1) != 0;
     uint32_t live[4] = {hi ? 0u : lv0, hi ? 0u : lv1, hi ? lv0 : 0u, hi ? lv1 : 0u};
     uint32_t acc[4];
-    lazy_less<TP>(acc, live, K, (uint32_t)(un.u >> 1), un.gs, tlo, ctr3(tag, 0, 0, 0) | c3time);
+    lazy_less_packed<TP>(acc, live, K, (uint32_t)(un.u >> 1), un.gs, tlo, ctr3(tag, 0, 0, 0) | c3time, xs);
     const uint32_t a0 = hi ? acc[2] : acc[0], a1 = hi ? acc[3] : acc[1];
     hop[0] = spread_even(a0) << o;
     hop[1] = spread_even(a0 >> 16) << o;
@@ -316,7 +361,7 @@ __host__ __device__ constexpr uint32_t tbit(uint64_t T, int pl) { return (uint32
 // flagged sites, T(w_unflagged) elsewhere.
 __device__ __forceinline__ void lane_change(uint32_t (&SRC)[4], uint32_t (&DST)[4], const uint32_t (&F)[4],
                                             const uint32_t (&r)[EAGERA][4], const PhiloxKeys& K, const Unit& un,
-                                            uint32_t tag, uint32_t tlo, uint32_t thi) {
+                                            uint32_t tag, uint32_t tlo, uint32_t thi, PackSmem* xs) {
   uint32_t lt[4], eq[4];
   if constexpr (!CROSS) {
 #pragma unroll
@@ -328,10 +373,11 @@ __device__ __forceinline__ void lane_change(uint32_t (&SRC)[4], uint32_t (&DST)[
     if (TOMEGA > 0 && TOMEGA < kOne) {
 #pragma unroll
       for (int pl = 0; pl < EAGER; ++pl) plane_step<TOMEGA>(lt, eq, r[pl], pl);
-      if (EAGER < NPW) {
-        if (K4J_TAIL) resolve_tail<TOMEGA>(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
-        else resolve<TOMEGA>(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER);
-      }
+      if (EAGER < NPW)
+        resolve_packed(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER, NPW, xs,
+                       [](uint32_t (&l)[4], uint32_t (&e)[4], const uint32_t (&R)[4], int pl) {
+                         plane_step<TOMEGA>(l, e, R, pl);
+                       });
     }
   } else {
     constexpr uint32_t AL1 = TOMEGA >= kOne ? ~0u : 0u, AL0 = TW0 >= kOne ? ~0u : 0u;          // always accepted
@@ -344,24 +390,12 @@ __device__ __forceinline__ void lane_change(uint32_t (&SRC)[4], uint32_t (&DST)[
     }
 #pragma unroll
     for (int pl = 0; pl < EAGER; ++pl) plane_step2(lt, eq, r[pl], F, tbit(TOMEGA, pl), tbit(TW0, pl));
-    if (EAGER < NPW) {
-      const uint32_t c3 = ctr3(tag, 0, 0, thi);
-#pragma unroll 1
-      for (int pl = EAGER; pl < NPW; pl += K4J_TRIP) {
-        if (!__any_sync(FULL, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u)) break;
-        uint32_t R[K4J_TRIP][4];
-#pragma unroll
-        for (int t = 0; t < K4J_TRIP; ++t) {
-          const int q = pl + t < 32 ? pl + t : 31;
-          const uint4 v = philox4x32_10((uint32_t)un.u, un.gs, tlo, c3 | ((uint32_t)q << 22), K);
-          R[t][0] = v.x; R[t][1] = v.y; R[t][2] = v.z; R[t][3] = v.w;
-        }
-#pragma unroll
-        for (int t = 0; t < K4J_TRIP; ++t)
-          if (pl + t < NPW)
-            plane_step2(lt, eq, R[t], F, (uint32_t)(TOMEGA >> (31 - (pl + t))) & 1u, (uint32_t)(TW0 >> (31 - (pl + t))) & 1u);
-      }
-    }
+    if (EAGER < NPW)
+      resolve_packed(lt, eq, K, (uint32_t)un.u, un.gs, tlo, ctr3(tag, 0, 0, thi), EAGER, NPW, xs,
+                     [&F](uint32_t (&l)[4], uint32_t (&e)[4], const uint32_t (&R)[4], int pl) {
+                       plane_step2(l, e, R, F, ((uint32_t)TOMEGA >> (31 - pl)) & (TOMEGA < kOne ? 1u : 0u),
+                                   ((uint32_t)TW0 >> (31 - pl)) & (TW0 < kOne ? 1u : 0u));
+                     });
   }
 #pragma unroll
   for (int w = 0; w < 4; ++w) {
@@ -417,6 +451,8 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
   using namespace kpz::k4j;
   __shared__ uint32_t halo[SINGLE_WARP ? 1 : 2 * NTHREADS];
   __shared__ unsigned long long red[SINGLE_WARP ? 1 : 4 * 32];
+  __shared__ PackSmem pack[NTHREADS / 32];
+  PackSmem* const xs = pack + (threadIdx.x >> 5);
   // SPW == 1: CTA = sample, thread = supergroup.  SPW > 1: CTA = one warp = SPW samples, lane = (sample, supergroup).
   int sub = 0, s = (int)blockIdx.x, lane0 = 0;
   const int lane = threadIdx.x & 31;
@@ -533,8 +569,8 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
           // lane A: particle on the previous thread's last site, hole on my first; lane B: the other way round
           in = (active && o) ? (((vp >> 2) & ~A[0] & 1u) | ((~(vp >> 3) & B[0] & 1u) << 1)) : 0u;
         }
-        lane_pass<true, TPA>(A, un, o, nx & 1u, D.keys, TAG_PAIR, tlo, c3t, jA);
-        lane_pass<false, TPB>(B, un, o, nx >> 1, D.keys, TAG_PAIR_B, tlo, c3t, jB);
+        lane_pass<true, TPA>(A, un, o, nx & 1u, D.keys, TAG_PAIR, tlo, c3t, jA, xs);
+        lane_pass<false, TPB>(B, un, o, nx >> 1, D.keys, TAG_PAIR_B, tlo, c3t, jB, xs);
         A[0] ^= in & 1u;
         B[0] ^= in >> 1;
       } else {
@@ -543,8 +579,8 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
           nx = unit_exchange((A[0] & 1u) | ((B[0] & 1u) << 1), un.nxt, halo, parity);
           if (!active || !o) nx = 0;
         }
-        const uint32_t cA = lane_pass<true, TPA>(A, un, o, nx & 1u, D.keys, TAG_PAIR, tlo, c3t, jA);
-        const uint32_t cB = lane_pass<false, TPB>(B, un, o, nx >> 1, D.keys, TAG_PAIR_B, tlo, c3t, jB);
+        const uint32_t cA = lane_pass<true, TPA>(A, un, o, nx & 1u, D.keys, TAG_PAIR, tlo, c3t, jA, xs);
+        const uint32_t cB = lane_pass<false, TPB>(B, un, o, nx >> 1, D.keys, TAG_PAIR_B, tlo, c3t, jB, xs);
         if (SPW > 1 || o) {  // the carries are zero in an offset-0 pass
           const uint32_t in = unit_exchange(cA | (cB << 1), un.prv, halo, parity);
           if (active) {
@@ -554,8 +590,8 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
         }
       }
       // lane changes at turning points: A->B after pass 0, B->A after pass 1
-      if (pass == 0) lane_change(A, B, T, Ec.r[0], D.keys, un, TAG_SWITCH_AB, tlo, thi);
-      else lane_change(B, A, K4J_INDEP ? V : T, Ec.r[1], D.keys, un, TAG_SWITCH_BA, tlo, thi);
+      if (pass == 0) lane_change(A, B, T, Ec.r[0], D.keys, un, TAG_SWITCH_AB, tlo, thi, xs);
+      else lane_change(B, A, K4J_INDEP ? V : T, Ec.r[1], D.keys, un, TAG_SWITCH_BA, tlo, thi, xs);
     }
     ++m;  // t = m from here on
     if (period > 0 && ++in_epoch == period) {

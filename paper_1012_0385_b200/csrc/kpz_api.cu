@@ -203,6 +203,54 @@ std::vector<std::string> k1_jit_defines(const KpzDev& D, int dis) {
 
 bool k1_use_jit(const KpzDev&) { return jit_enabled(); }
 
+// The streamed kernels keep one unit per thread whatever the debug configuration says.
+void drop_define(std::vector<std::string>* defs, const char* name) {
+  const std::string key = std::string(name) + "=";
+  defs->erase(std::remove_if(defs->begin(), defs->end(),
+                             [&](const std::string& d) { return d.compare(0, key.size(), key) == 0; }),
+              defs->end());
+}
+
+// Launch shape of the per-sample kernel (k1_sweep_jit.cuh): definitions, block size, samples per warp.
+struct K1Shape {
+  std::vector<std::string> defs;
+  int block = 32, spw = 1, upt = 1;
+};
+K1Shape k1_shape(const KpzDev& D, int S, int dis) {
+  static int smsp = 0;
+  if (!smsp) {
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    smsp = 4 * sms;
+  }
+  K1Shape sh;
+  const bool partial = (D.PW % 4) != 0;
+  // units per thread (K1J_UPT): a ring of 64 or more units gives every thread two of them - half the warps, no
+  // barrier at all for L = 16384, two independent chains of pair logic per thread
+  sh.upt = debug_int("K1J_UPT", (!partial && D.U >= 64 && D.U % 2 == 0) ? 2 : 1);
+  if (partial || D.U % sh.upt != 0) sh.upt = 1;
+  const int UT = D.U / sh.upt;
+  sh.block = (UT + 31) / 32 * 32;
+  // small rings (SPW): UT <= 16 threads, a power of two, no ragged unit -> 32/UT samples per warp
+  // (measured: packing never loses - a 30-ring launch runs at the same 17 GSU/s packed or one ring per warp)
+  const bool pack = UT <= 16 && (UT & (UT - 1)) == 0 && !partial;
+  sh.spw = pack ? 32 / UT : 1;
+  sh.defs = k1_jit_defines(D, dis);
+  char buf[32];
+  if (!debug_has("K1J_UPT")) {
+    snprintf(buf, sizeof buf, "K1J_UPT=%d", sh.upt);
+    sh.defs.push_back(buf);
+  }
+  if (!pack) sh.defs.push_back("K1J_PACK=0");
+  if (!debug_has("K1J_VARIANT")) {
+    // code shape by occupancy (k1_sweep_jit.cuh, K1J_VARIANT): with >= 4 resident warps per SMSP the other warps
+    // hide the latency, so the shape with the fewest alu slots wins (measured: +12..16 % on 16384-site rings)
+    const long long warps = (long long)((S + sh.spw - 1) / sh.spw) * (sh.block / 32);
+    if (warps >= 4LL * smsp) sh.defs.push_back("K1J_VARIANT=2");
+  }
+  return sh;
+}
+
 void refresh_planes(kpz_sim* sim) {
   int np = std::max(planes_needed(sim->dev.thr[0]), planes_needed(sim->dev.thr[2]));
   if (sim->has_sp) np = std::max(np, planes_needed(sim->dev.thr[1]));
@@ -318,6 +366,7 @@ int k3_run(kpz_sim* sim, int64_t n_mcs) {
   void* jitfn = nullptr;  // the same pass specialised on (L, thresholds) when run-time compilation is enabled
   if (jit_enabled()) {
     std::vector<std::string> defs = k1_jit_defines(D0, dis);
+    drop_define(&defs, "K1J_UPT");
     defs.push_back("K1J_STREAM=1");
     int rcj = jit_get("k1_sweep_jit.cuh", "kpz_k3_pass_jit", defs, &jitfn);
     if (rcj) return rcj;
@@ -377,6 +426,7 @@ constexpr long long kK3TChunk = 32;
 int k3t_run(kpz_sim* sim, int64_t n_mcs) {
   const int dis = sim->has_sq ? 2 : sim->has_sp ? 1 : 0;
   std::vector<std::string> defs = k1_jit_defines(sim->dev, dis);
+  drop_define(&defs, "K1J_UPT");
   defs.push_back("K1J_TILE=1");
   void* kfn = nullptr;
   int rc = jit_get("k1_sweep_jit.cuh", "kpz_k3t_sweep_jit", defs, &kfn);
@@ -618,8 +668,14 @@ int kpz_jit_check(int64_t L, double p, double q, const kpz_disorder* disorder, c
   refresh_planes(&tmp);
   if (!k1_use_jit(D)) return KPZ_OK;
   std::vector<char> cubin;
-  std::vector<std::string> defs = k1_jit_defines(D, tmp.has_sq ? 2 : tmp.has_sp ? 1 : 0);
-  if (path == KPZ_PATH_BLOCKED) defs.push_back("K1J_TILE=1");
+  D.PWp = (D.PW + 3) / 4 * 4;
+  D.U = D.PWp / 4;
+  const int dis_c = tmp.has_sq ? 2 : tmp.has_sp ? 1 : 0;
+  std::vector<std::string> defs = path == KPZ_PATH_BLOCKED ? k1_jit_defines(D, dis_c) : k1_shape(D, 1, dis_c).defs;
+  if (path == KPZ_PATH_BLOCKED) {
+    drop_define(&defs, "K1J_UPT");
+    defs.push_back("K1J_TILE=1");
+  }
   rc = jit_compile("k1_sweep_jit.cuh", path == KPZ_PATH_BLOCKED ? "kpz_k3t_sweep_jit" : "kpz_k1_sweep_jit", defs, &cubin,
                    nullptr);
   if (rc) return rc;
@@ -717,29 +773,12 @@ int kpz_run(kpz_sim* sim, int64_t n_mcs) {
     const int dis = sim->has_sq ? 2 : sim->has_sp ? 1 : 0;
     const int block = (D.U + 31) / 32 * 32;
     if (k1_use_jit(D)) {
-      // small rings (k1_sweep_jit.cuh, SPW): U <= 16 units, a power of two, no ragged unit -> 32/U samples per warp
-      static int smsp = 0;
-      if (!smsp) {
-        int dev = 0, sms = 148;
-        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        smsp = 4 * sms;
-      }
-      // (measured: packing never loses - a 30-ring launch runs at the same 17 GSU/s packed or one ring per warp)
-      const bool pack = D.U <= 16 && (D.U & (D.U - 1)) == 0 && !partial;
-      const int spw = pack ? 32 / D.U : 1;
-      std::vector<std::string> defs = k1_jit_defines(D, dis);
-      if (!pack) defs.push_back("K1J_PACK=0");
-      if (!debug_has("K1J_VARIANT")) {
-        // code shape by occupancy (k1_sweep_jit.cuh, K1J_VARIANT): with >= 4 resident warps per SMSP the other warps
-        // hide the latency, so the shape with the fewest alu slots wins (measured: +12..16 % on 16384-site rings)
-        const long long warps = (long long)((sim->S + spw - 1) / spw) * (block / 32);
-        if (warps >= 4LL * smsp) defs.push_back("K1J_VARIANT=2");
-      }
+      K1Shape sh = k1_shape(D, sim->S, dis);
       void* kfn = nullptr;
-      rc = jit_get("k1_sweep_jit.cuh", "kpz_k1_sweep_jit", defs, &kfn);
+      rc = jit_get("k1_sweep_jit.cuh", "kpz_k1_sweep_jit", sh.defs, &kfn);
       if (rc) return rc;
       void* args[] = {(void*)&D, (void*)&A};
-      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((sim->S + spw - 1) / spw), dim3(block), args, 0, sim->stream));
+      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((sim->S + sh.spw - 1) / sh.spw), dim3(sh.block), args, 0, sim->stream));
       KPZ_LAUNCH_CHECK("kpz_k1_sweep_jit");
     } else {
       K1Fn fn = k1_pick(single, partial, dis, D.nplanes);

@@ -462,7 +462,7 @@ def test_static_streamed_kernel_against_oracle(K):
             K.KpzSim(1 << 19, 1, 0.5, 0.5, seed=1, max_records=1, path=3)
 
 
-@pytest.mark.parametrize("cfg", ["jit=0", "K4J_TAIL=1", "K4J_EAGER=1", "K4J_EAGER=7;K4J_TAIL=1"])
+@pytest.mark.parametrize("cfg", ["jit=0", "K4J_SMAX=1", "K4J_EAGER=0;K4J_SMAX=32", "K4J_EAGER=7;K4J_SMAX=2", "K4J_EAGER=3;K4J_SMAX=8"])
 def test_k4_variants_against_oracle(K, cfg):
     with K.debug_config(cfg):
         run_both_lanes(K, 8192 + 64, 2, 1.0, 1.0, 0.3, 0.05, 6, 0.1, seed=31, times=[1, 6, 13], chunks=[6, 7])
