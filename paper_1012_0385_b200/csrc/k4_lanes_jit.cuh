@@ -9,21 +9,26 @@
 //   * in-lane hops are word-local bit logic: with sh = (X >> 1 | next word << 31), lane A (right) hops where
 //     X & ~sh & pairmask(o), lane B (left) where ~X & sh & pairmask(o); offset 1 needs bit 0 of the next thread's
 //     word 0 and sends one carry bit back (ring closure = wrap-around of that exchange);
-//   * lane changes: live = turn & source & ~target; U < T(omega) is evaluated MSB-first over bit-planes.  The live sites
-//     are sparse (config 5: 1.3 per supergroup), so after every plane fewer lanes of a warp still hold an undecided
-//     site (74 %, 49 %, 29 %, 15 %, ... of them).  The first K4J_EAGER planes of both lane-change steps of MCS m+1 are
-//     drawn while MCS m is processed (counter-based, state independent; default 1: three lanes in four need plane 0
-//     anyway).  Deeper planes are drawn by a PACKED trip (resolve_packed): when n <= 16 lanes are undecided the idle
-//     lanes draw the following planes of the SAME supergroups - s = 2, 4 (K4J_SMAX) consecutive planes per trip,
-//     handed back through a per-warp shared-memory slot - so a trip of the warp advances the comparison by s planes
-//     instead of one.  Same result as plane-by-plane evaluation (the comparison steps run in plane order).
-//     Measured planes drawn per lane-change step: see profiles/;
+//   * lane changes (K4J_PRE = 1, default): whether a site WOULD let a particle change lane in step st of MCS m - "is a
+//     turning point and U(SWITCH_st, m, site) < T(omega)" - does not depend on the occupations.  So every warp computes
+//     these acceptance masks for its 32 supergroups for a CHUNK of MCS ahead (precompute_chunk) and parks them in shared
+//     memory; the sweep itself then only ANDs them with "source occupied, target empty".  This takes the lazy MSB-first
+//     comparison - a chain of dependent Philox calls - off the latency-critical, barrier-coupled path of the sweep
+//     (measured: with ~1.7 warps per SMSP every dependent trip cost ~400 clk) and turns it into throughput work with
+//     full SIMT efficiency: all lanes draw the first K4J_DIRECT planes of their items, items that are still undecided
+//     go to a per-warp queue, and every further trip of the warp pops 32 queued (supergroup, MCS, step, plane) entries
+//     - whatever items they belong to - draws their planes, and pushes back those still undecided.  No lane ever idles
+//     while another waits for a deeper plane.  Candidates are the ~6 turning points of a supergroup (4.0 planes per
+//     supergroup and step on average) instead of the ~1.3 live ones (1.8 planes), but the warp draws 5.3 planes per
+//     32 supergroups where the SIMT-lazy loop over live sites drew 8.8.  Results are identical: the comparison of one
+//     element still runs plane by plane, MSB first.
+//     K4J_PRE = 0 keeps the live-site evaluation inside the sweep (K4J_EAGER planes drawn one MCS ahead, resolve_packed);
 //   * hop counters by POPC of two merged hop words (hops of one pass sit on one bit parity), occupancy profile at
 //     epoch ends by warp-transposed, coalesced red.global.add.
 //
 // Compile-time configuration (-D, set by lanes_api.cu): K4J_W = L/32, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN
 // (thresholds in [0, 2^32]), K4J_OFFSET_MODE, K4J_TW0 and K4J_INDEP (site-wise crossing model), K4J_EAGER,
-// K4J_SMAX, K4J_TRIP.
+// K4J_SMAX, K4J_TRIP, K4J_PRE, K4J_CHUNK, K4J_DIRECT.
 #pragma once
 #include "sweep_types.cuh"
 
@@ -36,11 +41,20 @@
 #ifndef K4J_INDEP
 #define K4J_INDEP 0   // 1: the B->A crossings read their own flag set (D.V)
 #endif
+#ifndef K4J_PRE
+#define K4J_PRE 1    // 1: lane-change acceptance masks precomputed per chunk of MCS (see above); 0: evaluated in the sweep
+#endif
+#ifndef K4J_CHUNK
+#define K4J_CHUNK 16  // MCS per precomputed chunk (lanes_api.cu sizes the dynamic shared memory with the same number)
+#endif
+#ifndef K4J_DIRECT
+#define K4J_DIRECT 4  // planes every lane draws for each of its items before undecided items go to the queue
+#endif
 #ifndef K4J_EAGER
-#define K4J_EAGER 1  // lane-change planes drawn one MCS ahead
+#define K4J_EAGER 6  // K4J_PRE = 0: lane-change planes drawn one MCS ahead
 #endif
 #ifndef K4J_SMAX
-#define K4J_SMAX 4   // packed trips: at most this many consecutive planes per trip (1 = plane by plane; a power of two)
+#define K4J_SMAX 1   // packed trips: at most this many consecutive planes per trip (1 = plane by plane; a power of two)
 #endif
 #ifndef K4J_TRIP
 #define K4J_TRIP 2  // planes per trip of the unpacked loop (turning-point redraw, in-lane rates < 1 with K4J_SMAX = 1)
@@ -356,6 +370,145 @@ __device__ __forceinline__ void plane_step2(uint32_t (&lt)[4], uint32_t (&eq)[4]
 }
 __host__ __device__ constexpr uint32_t tbit(uint64_t T, int pl) { return (uint32_t)((T >> (31 - pl)) & 1ull); }
 
+// ---- precomputed lane-change acceptance (K4J_PRE) ---------------------------------------------------------------------
+constexpr int CHUNK = K4J_CHUNK;
+constexpr int DIRECT = K4J_DIRECT < NPW ? K4J_DIRECT : NPW;
+constexpr int QCAP = 128;  // queue entries per warp (a power of two >= 32 + 64 + 32)
+static_assert(CHUNK >= 1 && CHUNK <= 256, "K4J_CHUNK: the chunk index has 8 bits in a queue entry");
+
+// Per-warp shared memory of the precompute.
+struct WarpSmem {
+  uint4 acc[CHUNK][2][32];  // acc[k][st][lane]: sites of the lane's supergroup that accept a lane change in step st of
+                            //   MCS m0 + k (st 0: A->B, 1: B->A) - candidates only (turning points / every site)
+  uint4 qeq[QCAP];          // queue of undecided items: their elements whose prefix still equals the threshold's ...
+  uint32_t qid[QCAP];       //   ... and lane | k << 5 | st << 13 | next plane << 14
+  uint4 flag[2][32];        // site-wise crossing model: the flag words of every lane for step 0 / 1 (rate class per site)
+};
+
+__host__ __device__ constexpr uint32_t dyn_tbit(uint64_t T, int pl) {
+  return (T > 0 && T < kOne) ? (((uint32_t)T >> (31 - pl)) & 1u) : 0u;
+}
+// One MSB-first comparison step of a lane-change item with plane pl; F = flag words (rate class per site, CROSS only).
+__device__ __forceinline__ void change_step(uint32_t (&lt)[4], uint32_t (&eq)[4], const uint32_t (&R)[4],
+                                            const uint32_t (&F)[4], int pl) {
+  if constexpr (!CROSS) plane_step<TOMEGA>(lt, eq, R, pl);
+  else plane_step2(lt, eq, R, F, dyn_tbit(TOMEGA, pl), dyn_tbit(TW0, pl));
+}
+// Candidates of one item: lt = accepted whatever U is, eq = needs planes.  F = flags of the step, nwn = valid words.
+__device__ __forceinline__ void change_init(uint32_t (&lt)[4], uint32_t (&eq)[4], const uint32_t (&F)[4], int nwn) {
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    if constexpr (!CROSS) {
+      lt[w] = (TOMEGA >= kOne) ? F[w] : 0u;
+      eq[w] = (TOMEGA > 0 && TOMEGA < kOne) ? F[w] : 0u;
+    } else {
+      constexpr uint32_t AL1 = TOMEGA >= kOne ? ~0u : 0u, AL0 = TW0 >= kOne ? ~0u : 0u;
+      constexpr uint32_t PA1 = (TOMEGA > 0 && TOMEGA < kOne) ? ~0u : 0u, PA0 = (TW0 > 0 && TW0 < kOne) ? ~0u : 0u;
+      const uint32_t valid = w < nwn ? FULL : 0u;
+      lt[w] = valid & ((F[w] & AL1) | (~F[w] & AL0));
+      eq[w] = valid & ((F[w] & PA1) | (~F[w] & PA0));
+    }
+  }
+}
+
+struct Queue {
+  uint32_t head, tail;  // warp-uniform
+};
+
+// Append the lanes' undecided items (und) to the queue.
+__device__ __forceinline__ void queue_push(WarpSmem* ws, Queue& q, bool und, const uint32_t (&eq)[4], uint32_t id) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t mask = __ballot_sync(FULL, und);
+  if (und) {
+    const uint32_t j = (q.tail + (uint32_t)__popc(mask & ((1u << lane) - 1u))) & (QCAP - 1);
+    ws->qeq[j] = make_uint4(eq[0], eq[1], eq[2], eq[3]);
+    ws->qid[j] = id;
+  }
+  q.tail += (uint32_t)__popc(mask);
+}
+
+// One trip of the warp over up to 32 queued entries: each lane draws the next plane of ITS entry (whatever lane, MCS
+// and step that entry belongs to), applies it, ORs newly accepted sites into the entry's mask and queues the entry
+// again while it is undecided.  Entries are unique per (lane, k, st), so the read-modify-write of acc needs no atomic.
+__device__ __forceinline__ void queue_trip(WarpSmem* ws, Queue& q, const PhiloxKeys& K, uint32_t G, uint32_t gs,
+                                           long long m0) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t nv = q.tail - q.head < 32u ? q.tail - q.head : 32u;
+  const bool valid = (uint32_t)lane < nv;
+  const uint32_t j = (q.head + (uint32_t)lane) & (QCAP - 1);
+  const uint32_t id = valid ? ws->qid[j] : 0u;
+  const uint4 e = ws->qeq[j];
+  q.head += nv;
+  const int le = (int)(id & 31u), k = (int)((id >> 5) & 255u), st = (int)((id >> 13) & 1u), pl = (int)(id >> 14);
+  const uint32_t Gs = __shfl_sync(FULL, G, le), gss = __shfl_sync(FULL, gs, le);
+  const unsigned long long mm = (unsigned long long)(m0 + k);
+  const uint4 v = philox4x32_10(Gs, gss, (uint32_t)mm,
+                                ctr3(st ? TAG_SWITCH_BA : TAG_SWITCH_AB, 0, (uint32_t)pl, (uint32_t)(mm >> 32)), K);
+  const uint32_t R[4] = {v.x, v.y, v.z, v.w};
+  uint32_t F[4] = {0u, 0u, 0u, 0u};
+  if constexpr (CROSS) {
+    const uint4 f = ws->flag[st][le];
+    F[0] = f.x; F[1] = f.y; F[2] = f.z; F[3] = f.w;
+  }
+  uint32_t lt[4] = {0u, 0u, 0u, 0u};
+  uint32_t eq[4] = {valid ? e.x : 0u, valid ? e.y : 0u, valid ? e.z : 0u, valid ? e.w : 0u};
+  change_step(lt, eq, R, F, pl);
+  if ((lt[0] | lt[1] | lt[2] | lt[3]) != 0u) {
+    uint4 a = ws->acc[k][st][le];
+    a.x |= lt[0]; a.y |= lt[1]; a.z |= lt[2]; a.w |= lt[3];
+    ws->acc[k][st][le] = a;
+  }
+  __syncwarp();  // the popped slots may be reused by the pushes below
+  queue_push(ws, q, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u && pl + 1 < NPW, eq, id + (1u << 14));
+  __syncwarp();
+}
+
+// Acceptance masks of this warp's supergroups for MCS m0 .. m0 + n - 1 (n <= CHUNK), both lane-change steps.
+// F0 / F1 = the lane's flag words of step 0 / 1 (turning points; u_i / v_i), fixed over the chunk.
+__device__ __forceinline__ void precompute_chunk(WarpSmem* ws, const PhiloxKeys& K, const Unit& un, const uint32_t (&F0)[4],
+                                                 const uint32_t (&F1)[4], long long m0, int n) {
+  const int lane = threadIdx.x & 31;
+  if constexpr (CROSS) {
+    ws->flag[0][lane] = make_uint4(F0[0], F0[1], F0[2], F0[3]);
+    ws->flag[1][lane] = make_uint4(F1[0], F1[1], F1[2], F1[3]);
+  }
+  __syncwarp();
+  Queue q{0u, 0u};
+#pragma unroll 1
+  for (int k = 0; k < n; ++k) {
+    const unsigned long long mm = (unsigned long long)(m0 + k);
+    const uint32_t tlo = (uint32_t)mm, thi = (uint32_t)(mm >> 32);
+    uint32_t lt0[4], eq0[4], lt1[4], eq1[4];
+    change_init(lt0, eq0, F0, un.nwn);
+    change_init(lt1, eq1, F1, un.nwn);
+    if (NPW > 0) {
+      uint32_t R0[DIRECT > 0 ? DIRECT : 1][4], R1[DIRECT > 0 ? DIRECT : 1][4];
+#pragma unroll
+      for (int pl = 0; pl < DIRECT; ++pl) {  // 2 * DIRECT independent calls: their rounds interleave
+        const uint4 a = philox4x32_10((uint32_t)un.u, un.gs, tlo, ctr3(TAG_SWITCH_AB, 0, (uint32_t)pl, thi), K);
+        const uint4 b = philox4x32_10((uint32_t)un.u, un.gs, tlo, ctr3(TAG_SWITCH_BA, 0, (uint32_t)pl, thi), K);
+        R0[pl][0] = a.x; R0[pl][1] = a.y; R0[pl][2] = a.z; R0[pl][3] = a.w;
+        R1[pl][0] = b.x; R1[pl][1] = b.y; R1[pl][2] = b.z; R1[pl][3] = b.w;
+      }
+#pragma unroll
+      for (int pl = 0; pl < DIRECT; ++pl) {
+        change_step(lt0, eq0, R0[pl], F0, pl);
+        change_step(lt1, eq1, R1[pl], F1, pl);
+      }
+    }
+    ws->acc[k][0][lane] = make_uint4(lt0[0], lt0[1], lt0[2], lt0[3]);
+    ws->acc[k][1][lane] = make_uint4(lt1[0], lt1[1], lt1[2], lt1[3]);
+    __syncwarp();
+    const uint32_t id = (uint32_t)lane | ((uint32_t)k << 5) | ((uint32_t)DIRECT << 14);
+    queue_push(ws, q, DIRECT < NPW && (eq0[0] | eq0[1] | eq0[2] | eq0[3]) != 0u, eq0, id);
+    queue_push(ws, q, DIRECT < NPW && (eq1[0] | eq1[1] | eq1[2] | eq1[3]) != 0u, eq1, id | (1u << 13));
+    __syncwarp();
+    while (q.tail - q.head >= 32u) queue_trip(ws, q, K, (uint32_t)un.u, un.gs, m0);
+  }
+  while (q.tail != q.head) queue_trip(ws, q, K, (uint32_t)un.u, un.gs, m0);
+  __syncwarp();
+}
+
 // Lane changes SRC -> DST where the source is occupied, the target empty and U < T(site) (§R18):
 // turning-point model: T = T(omega) at flagged sites F, no crossing elsewhere; site-wise crossing model: T(omega) at
 // flagged sites, T(w_unflagged) elsewhere.
@@ -401,6 +554,17 @@ __device__ __forceinline__ void lane_change(uint32_t (&SRC)[4], uint32_t (&DST)[
   for (int w = 0; w < 4; ++w) {
     SRC[w] ^= lt[w];
     DST[w] ^= lt[w];
+  }
+}
+
+// The same with the acceptance mask precomputed (K4J_PRE): acc = candidate sites whose uniform is below their threshold.
+__device__ __forceinline__ void lane_change_pre(uint32_t (&SRC)[4], uint32_t (&DST)[4], const uint4 acc) {
+  const uint32_t a[4] = {acc.x, acc.y, acc.z, acc.w};
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    const uint32_t mv = lop3<0x20>(SRC[w], DST[w], a[w]);  // SRC & ~DST & acc
+    SRC[w] ^= mv;
+    DST[w] ^= mv;
   }
 }
 
@@ -453,6 +617,8 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
   __shared__ unsigned long long red[SINGLE_WARP ? 1 : 4 * 32];
   __shared__ PackSmem pack[NTHREADS / 32];
   PackSmem* const xs = pack + (threadIdx.x >> 5);
+  extern __shared__ __align__(16) unsigned char k4_dyn_smem[];  // K4J_PRE: NTHREADS / 32 WarpSmem (lanes_api.cu sizes it)
+  WarpSmem* const ws = reinterpret_cast<WarpSmem*>(k4_dyn_smem) + (threadIdx.x >> 5);
   // SPW == 1: CTA = sample, thread = supergroup.  SPW > 1: CTA = one warp = SPW samples, lane = (sample, supergroup).
   int sub = 0, s = (int)blockIdx.x, lane0 = 0;
   const int lane = threadIdx.x & 31;
@@ -537,16 +703,23 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
   };
 
   Eager EA, EB;
-  draw_eager(EA, D.keys, un, m);
+  if (!K4J_PRE) draw_eager(EA, D.keys, un, m);
 
-  // One MCS m with the eager lane-change planes Ec drawn one step earlier; draws those of MCS m+1 into En.
-  auto mcs = [&](const Eager& Ec, Eager& En) {
-    const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
+  auto redraw_flags = [&]() {  // a new epoch starts at MCS m
     if (period > 0 && m > 0 && in_epoch == 0) {
       draw_turn(T, D.keys, un, (unsigned long long)epoch, TAG_TURN);
       if (K4J_INDEP) draw_turn(V, D.keys, un, (unsigned long long)epoch, TAG_TURN_V);
     }
-    draw_eager(En, D.keys, un, m + 1);
+  };
+
+  // One MCS m.  K4J_PRE: the lane-change acceptance masks are entry kc of the precomputed chunk.  Otherwise: with the
+  // eager lane-change planes Ec drawn one step earlier; draws those of MCS m+1 into En.
+  auto mcs = [&](const Eager& Ec, Eager& En, int kc) {
+    const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
+    if (!K4J_PRE) {
+      redraw_flags();
+      draw_eager(En, D.keys, un, m + 1);
+    }
 #pragma unroll
     for (int pass = 0; pass < 2; ++pass) {
       const uint32_t o = K4J_OFFSET_MODE ? (uint32_t)pass : ((offbits >> (2 * ((int)m & 15) + pass)) & 1u);
@@ -590,8 +763,13 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
         }
       }
       // lane changes at turning points: A->B after pass 0, B->A after pass 1
-      if (pass == 0) lane_change(A, B, T, Ec.r[0], D.keys, un, TAG_SWITCH_AB, tlo, thi, xs);
-      else lane_change(B, A, K4J_INDEP ? V : T, Ec.r[1], D.keys, un, TAG_SWITCH_BA, tlo, thi, xs);
+      if (K4J_PRE) {
+        if (pass == 0) lane_change_pre(A, B, ws->acc[kc][0][lane]);
+        else lane_change_pre(B, A, ws->acc[kc][1][lane]);
+      } else {
+        if (pass == 0) lane_change(A, B, T, Ec.r[0], D.keys, un, TAG_SWITCH_AB, tlo, thi, xs);
+        else lane_change(B, A, K4J_INDEP ? V : T, Ec.r[1], D.keys, un, TAG_SWITCH_BA, tlo, thi, xs);
+      }
     }
     ++m;  // t = m from here on
     if (period > 0 && ++in_epoch == period) {
@@ -617,10 +795,20 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
     if (K4J_OFFSET_MODE == 0 && ((int)m & 15) == 0) draw_offsets();
   };
 
-  while (m < t_end) {
-    mcs(EA, EB);
-    if (m >= t_end) break;
-    mcs(EB, EA);
+  if (K4J_PRE) {
+    while (m < t_end) {  // chunks end at epoch ends: the flags are fixed over a chunk
+      long long n = t_end - m < (long long)CHUNK ? t_end - m : (long long)CHUNK;
+      if (period > 0 && period - in_epoch < n) n = period - in_epoch;
+      redraw_flags();
+      precompute_chunk(ws, D.keys, un, T, K4J_INDEP ? V : T, m, (int)n);
+      for (int kc = 0; kc < (int)n; ++kc) mcs(EA, EA, kc);
+    }
+  } else {
+    while (m < t_end) {
+      mcs(EA, EB, 0);
+      if (m >= t_end) break;
+      mcs(EB, EA, 0);
+    }
   }
 
   {

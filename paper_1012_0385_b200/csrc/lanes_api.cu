@@ -72,6 +72,13 @@ LLayout lanes_layout(int64_t L, int32_t S, int32_t max_records) {
 // ---- K4 v2: kernel specialised at run time on (L, thresholds, offset mode) — k4_lanes_jit.cuh ---------------------
 bool k4_use_jit(const LanesDev& D) { return jit_enabled() && (D.W + 3) / 4 <= 1024; }
 
+// MCS per precomputed chunk: as many as keep the CTA's shared memory near 100 KB (two CTAs per SM), at most 16.
+int k4_chunk(const LanesDev& D) {
+  const int nwarps = ((D.W + 3) / 4 + 31) / 32;
+  const int per_warp = 100 * 1024 / nwarps - (128 * 16 + 128 * 4 + 1024);
+  return std::max(1, std::min(16, per_warp / 1024));
+}
+
 std::vector<std::string> k4_jit_defines(const LanesDev& D) {
   auto T = [](const Thresh& t) -> unsigned long long { return t.always ? (1ull << 32) : (unsigned long long)t.value; };
   char buf[64];
@@ -93,7 +100,20 @@ std::vector<std::string> k4_jit_defines(const LanesDev& D) {
   snprintf(buf, sizeof buf, "K4J_INDEP=%d", D.independent);
   d.push_back(buf);
   debug_defines("K4J_", &d);  // kpz_debug_config: tests and tuning only (the run reads no environment)
+  if (!debug_has("K4J_CHUNK")) {
+    snprintf(buf, sizeof buf, "K4J_CHUNK=%d", k4_chunk(D));
+    d.push_back(buf);
+  }
   return d;
+}
+
+// Dynamic shared memory of the kernel: one WarpSmem (k4_lanes_jit.cuh) per warp when the lane-change acceptance is
+// precomputed: acc[CHUNK][2][32] uint4 + a 128-entry queue (uint4 + uint32) + flag[2][32] uint4.
+size_t k4_smem_bytes(const LanesDev& D) {
+  if (!debug_int("K4J_PRE", 1)) return 0;
+  const int nwarps = ((D.W + 3) / 4 + 31) / 32;
+  const int chunk = debug_int("K4J_CHUNK", k4_chunk(D));
+  return (size_t)nwarps * ((size_t)chunk * 1024 + 128 * 16 + 128 * 4 + 1024);
 }
 
 int grid_for(size_t n, int block = 256) {
@@ -310,7 +330,10 @@ int lanes_run(lanes_sim* sim, int64_t n_mcs) {
     // small rings (k4_lanes_jit.cuh, SPW): U4 <= 16 supergroups, a power of two, no ragged word -> 32/U4 samples per warp
     const bool pack = (D.W % 4) == 0 && U4 <= 16 && (U4 & (U4 - 1)) == 0;
     const int spw = pack ? 32 / U4 : 1;
-    KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((sim->S + spw - 1) / spw), dim3(block4), args, 0, sim->stream));
+    const size_t smem = k4_smem_bytes(D);
+    if (smem > 48 * 1024)
+      KPZ_CUDA_CHECK(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((sim->S + spw - 1) / spw), dim3(block4), args, smem, sim->stream));
   } else if (D.independent || D.t_w0.value != 0 || D.t_w0.always) {
     return fail(KPZ_EUNSUPPORTED, "the site-wise crossing model runs on the run-time specialised kernel only "
                                   "(L <= 131072, KPZ_B200_JIT not 0)");

@@ -266,30 +266,30 @@ def test_config4_path_at_2p20_vs_oracle(K):
     assert gpu.path == K.KPZ_PATH_BLOCKED
 
 
-def test_config4_full_size_first_steps_and_invariants(K):
+def test_config4_full_size_invariants(K):
+    """Properties that hold at any size, at L = 2^28 on the default path (the comparison with the oracle at this size -
+    32 MCS on the blocked path, 4 MCS pass by pass - is tests/test_gpu_full_size.py)."""
     c = workloads.CONFIGS[4]
     L = c["L"]
     gpu = K.KpzSim(L, 1, c["p"], c["q"], seed=c["seed"], max_records=8)
     assert gpu.path == K.KPZ_PATH_BLOCKED
-    times = [1, 2]
-    gpu.set_record_times(times)
-    gpu.run(2)
-    ref = R.KpzRef(L, 1, c["p"], c["q"], seed=c["seed"])
-    ref.set_record_times(times)
-    ref.run(2)
-    assert np.array_equal(K.words_to_numpy(gpu.lattice()), ref.lattice())
-    gr, rr = gpu.roughness(), ref.roughness()
-    assert np.array_equal(gr["sum_h"], rr["sum_h"]) and np.array_equal(gr["sum_h2"], rr["sum_h2"])
-    # longer run at full size: properties that hold at any size
     gpu.set_record_times([20])
-    gpu.run(18)
-    lat = gpu.lattice()
+    gpu.run(20)
     h = gpu.heights(0)
     assert int(h[-1].item()) == 0                                  # h_{L-1} = 2N - L = 0 at half filling
     r = gpu.roughness()
     assert r["sum_h"][0, 0] == int(h.sum(dtype=torch.int64).item())
     assert r["sum_h2"][0, 0] == int((h.to(torch.int64) ** 2).sum().item())
-    del lat
+
+
+def test_k3_run_across_its_offset_chunks(K):
+    """The pass-by-pass driver draws offsets for 4096 passes (2048 MCS) at a time (kpz_api.cu, kK3ChunkPasses): one
+    kpz_run of 4300 MCS crosses two chunk boundaries, with records right before, on and after the first one and a
+    record on the second (the carried frame row / restaged row 0 were never exercised)."""
+    gpu, r = run_both_kpz(K, 320, 3, 0.75, 0.25, seed=61, path=2, times=[5, 2047, 2048, 2049, 4096, 4300], chunks=[4300])
+    assert gpu.path == K.KPZ_PATH_STREAM
+    run_both_kpz(K, 64 * 5, 2, 0.9, 0.1, disorder=(0.2, 0.3, 0.1, 0.05), seed=62, path=2, times=[2048, 2100],
+                 chunks=[2047, 53])                 # a run that ends one MCS before the boundary, then crosses it
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -443,7 +443,8 @@ def test_overflow_guard_measures_a_lattice_handed_in(K):
 # (kpz_debug_config("jit=0")) and the tuning knobs of the run-time specialised ones
 # ---------------------------------------------------------------------------------------------------------
 
-@pytest.mark.parametrize("cfg", ["jit=0", "K1J_VARIANT=0", "K1J_VARIANT=2", "K1J_REFRAME=1", "K1J_EAGER=3;K1J_TRIP=3"])
+@pytest.mark.parametrize("cfg", ["jit=0", "K1J_VARIANT=0", "K1J_VARIANT=2", "K1J_REFRAME=1", "K1J_EAGER=3;K1J_TRIP=3",
+                                 "K1J_UPT=1", "K1J_UPT=2", "K1J_UPT=2;K1J_VARIANT=2", "K1J_UPT=2;K1J_REFRAME=1"])
 def test_k1_variants_against_oracle(K, cfg):
     with K.debug_config(cfg):
         run_both_kpz(K, 8192 + 64, 3, 0.75, 0.25, seed=21, times=[1, 3, 20], chunks=[7, 13])
@@ -462,7 +463,9 @@ def test_static_streamed_kernel_against_oracle(K):
             K.KpzSim(1 << 19, 1, 0.5, 0.5, seed=1, max_records=1, path=3)
 
 
-@pytest.mark.parametrize("cfg", ["jit=0", "K4J_SMAX=1", "K4J_EAGER=0;K4J_SMAX=32", "K4J_EAGER=7;K4J_SMAX=2", "K4J_EAGER=3;K4J_SMAX=8"])
+@pytest.mark.parametrize("cfg", ["jit=0", "K4J_PRE=0", "K4J_PRE=0;K4J_EAGER=0;K4J_SMAX=32", "K4J_PRE=0;K4J_EAGER=7;K4J_SMAX=2",
+                                 "K4J_PRE=0;K4J_EAGER=3;K4J_SMAX=8", "K4J_CHUNK=3;K4J_DIRECT=1", "K4J_CHUNK=1;K4J_DIRECT=0",
+                                 "K4J_CHUNK=7;K4J_DIRECT=9"])
 def test_k4_variants_against_oracle(K, cfg):
     with K.debug_config(cfg):
         run_both_lanes(K, 8192 + 64, 2, 1.0, 1.0, 0.3, 0.05, 6, 0.1, seed=31, times=[1, 6, 13], chunks=[6, 7])
@@ -638,12 +641,6 @@ def test_paper_workloads_full_launch_sampled_against_solo_oracle_runs(K, key, n)
     assert np.all(R.unpack_words(lat, c["L"]).sum(axis=1) == c["L"] // 2)      # conservation, every sample
 
 
-def test_config3_last_sample_long_run(K):
-    c = workloads.CONFIGS[3]
-    run_both_kpz(K, c["L"], 1, c["p"], c["q"], disorder=c["disorder"], seed=c["seed"], first_sample=c["S"] - 1,
-                 times=c["record_times"], chunks=[7000, 5068])        # through record time 12068
-
-
 def test_config5_full_launch_sampled_against_solo_oracle_runs(K):
     c = workloads.CONFIGS[5]
     n, times = 200, [t for t in c["record_times"] if t <= 200]
@@ -667,12 +664,6 @@ def test_config5_full_launch_sampled_against_solo_oracle_runs(K):
     # every sample: particles are conserved across the two lanes between the first and the last record
     tot = cur["n_a"] + cur["n_b"]
     assert np.all(tot[0] == tot[-1])
-
-
-def test_config5_last_sample_long_run(K):
-    c = workloads.CONFIGS[5]
-    run_both_lanes(K, c["L"], 1, c["p_a"], c["p_b"], c["rho0"], c["turn_prob"], c["turn_period"], c["omega"],
-                   c["seed"], c["record_times"], [2330, 617], first_sample=c["S"] - 1)      # through record time 2947
 
 
 # ---------------------------------------------------------------------------------------------------------
