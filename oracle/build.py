@@ -1,6 +1,9 @@
 """Build the CPU oracle (test infrastructure) into oracle/libkpz_oracle.so with gcc.
 
-Usage:  python -m oracle.build      (also called by __graft_entry__.build and by oracle/kpzref.py on demand)
+Usage:  python -m oracle.build               (also called by __graft_entry__.build and by oracle/kpzref.py on demand)
+        python -m oracle.build --sanitize    same library with -fsanitize=address,undefined (-O1 -g): run the oracle pins
+                                             under it with LD_PRELOAD=$(gcc -print-file-name=libasan.so), then rebuild
+                                             with --force (profiles/r02_sanitizers.md holds the commands and the result)
 """
 from __future__ import annotations
 
@@ -21,14 +24,15 @@ def needs_build() -> bool:
     return any(os.path.getmtime(f) > t for f in (SRC, HDR))
 
 
-def build(force: bool = False) -> str:
-    if force or needs_build():
+def build(force: bool = False, sanitize: bool = False) -> str:
+    if force or sanitize or needs_build():
         tmp = LIB + f".tmp{os.getpid()}"
-        cmd = ["gcc", "-std=c11", "-O3", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, SRC, "-lm"]
+        opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"] if sanitize else ["-O3"]
+        cmd = ["gcc", "-std=c11", *opt, "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, SRC, "-lm"]
         subprocess.run(cmd, check=True, cwd=HERE)
         os.replace(tmp, LIB)
     return LIB
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv))
+    print(build(force="--force" in sys.argv, sanitize="--sanitize" in sys.argv))

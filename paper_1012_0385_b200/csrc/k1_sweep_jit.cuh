@@ -71,6 +71,9 @@
 #if (defined(K1J_TILE) || defined(K1J_STREAM)) && K1J_UPT != 1
 #error "K1J_UPT > 1 is implemented by the per-sample kernel only"
 #endif
+#ifndef K1J_HALOCHECK  // debug (compute-sanitizer's racecheck is closed on the GPU pool): every word published through
+#define K1J_HALOCHECK 0  // the shared-memory halo carries the number of its exchange; a reader that finds another number
+#endif                   // - a slot not yet written, or already overwritten by a later exchange - counts an error
 #ifndef K1J_PW
 #error "k1_sweep_jit.cuh needs K1J_PW, K1J_T0..3, K1J_DIS, K1J_OFFSET_MODE"
 #endif
@@ -309,15 +312,27 @@ __device__ __forceinline__ void pass_logic(uint32_t (&a)[NW], uint32_t (&b)[NW],
 }
 
 // ---- neighbour word exchange (a5): the value held by unit `src` of this sample ---------------------------------
+// `parity` counts the exchanges of the CTA; the slot set alternates with it, so that a warp that runs ahead writes the
+// set nobody reads any more (one barrier per exchange).
+#if K1J_HALOCHECK
+__device__ unsigned int* g_halo_check;  // = KpzRunArgs.check
+#endif
+constexpr int HALO_WORDS = (K1J_HALOCHECK ? 8 : 4) * NTHREADS;  // [2 sets][2 words per thread] (+ the same for the tags)
 __device__ __forceinline__ uint32_t unit_exchange(uint32_t mine, int src, uint32_t* halo, int& parity) {
   if (SINGLE_WARP) {
     return __shfl_sync(0xFFFFFFFFu, mine, src);
   } else {
-    uint32_t* slot = halo + parity * NTHREADS;
+    uint32_t* slot = halo + (parity & 1) * NTHREADS;
     slot[threadIdx.x] = mine;
+#if K1J_HALOCHECK
+    slot[4 * NTHREADS + threadIdx.x] = (uint32_t)parity;
+#endif
     __syncthreads();
     const uint32_t v = slot[src];
-    parity ^= 1;
+#if K1J_HALOCHECK
+    if (slot[4 * NTHREADS + src] != (uint32_t)parity) atomicAdd(g_halo_check, 1u);
+#endif
+    parity += 1;
     return v;
   }
 }
@@ -383,13 +398,20 @@ __device__ __forceinline__ void reframe(uint32_t (&P)[NW], const Unit& un, uint3
     hn = __shfl_sync(0xFFFFFFFFu, P[0], un.nxt);
     hp = __shfl_sync(0xFFFFFFFFu, last, un.prv);
   } else {
-    uint32_t* slot = halo + parity * (2 * NTHREADS);
+    uint32_t* slot = halo + (parity & 1) * (2 * NTHREADS);
     slot[2 * threadIdx.x] = P[0];
     slot[2 * threadIdx.x + 1] = last;
+#if K1J_HALOCHECK
+    slot[4 * NTHREADS + 2 * threadIdx.x] = (uint32_t)parity;
+#endif
     __syncthreads();
     hn = slot[2 * un.nxt];
     hp = slot[2 * un.prv + 1];
-    parity ^= 1;
+#if K1J_HALOCHECK
+    if (slot[4 * NTHREADS + 2 * un.nxt] != (uint32_t)parity || slot[4 * NTHREADS + 2 * un.prv] != (uint32_t)parity)
+      atomicAdd(g_halo_check, 1u);
+#endif
+    parity += 1;
   }
   hn = __funnelshift_l(last, hn, from);  // the next unit's first word after ITS shift down
   shift_down_words(P, un.nw, hp, from);
@@ -684,10 +706,13 @@ extern "C" __global__ void __launch_bounds__(kpz::k1j::NTHREADS)
 kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::KpzRunArgs A) {
   using namespace kpz;
   using namespace kpz::k1j;
-  __shared__ uint32_t halo[SINGLE_WARP ? 1 : 4 * NTHREADS];
+  __shared__ uint32_t halo[SINGLE_WARP ? 1 : HALO_WORDS];
   __shared__ long long scratch[SINGLE_WARP ? 1 : 96];
   __shared__ uint32_t lut[256];
   for (int i = threadIdx.x; i < 256; i += NTHREADS) lut[i] = height_lut_entry(i);
+#if K1J_HALOCHECK
+  if (threadIdx.x == 0) g_halo_check = A.check;  // every CTA writes the same pointer
+#endif
   __syncthreads();
 
   // SPW == 1: CTA = sample, thread = UPT units.  SPW > 1: CTA = one warp = SPW samples, lane = (sample, units).

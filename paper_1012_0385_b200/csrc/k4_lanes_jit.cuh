@@ -28,10 +28,13 @@
 //
 // Compile-time configuration (-D, set by lanes_api.cu): K4J_W = L/32, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN
 // (thresholds in [0, 2^32]), K4J_OFFSET_MODE, K4J_TW0 and K4J_INDEP (site-wise crossing model), K4J_EAGER,
-// K4J_SMAX, K4J_TRIP, K4J_PRE, K4J_CHUNK, K4J_DIRECT.
+// K4J_SMAX, K4J_TRIP, K4J_PRE, K4J_CHUNK, K4J_DIRECT, K4J_VPROF.
 #pragma once
 #include "sweep_types.cuh"
 
+#ifndef K4J_HALOCHECK  // debug: sequence numbers on the shared-memory halo slots (see k1_sweep_jit.cuh, K1J_HALOCHECK)
+#define K4J_HALOCHECK 0
+#endif
 #ifndef K4J_W
 #error "k4_lanes_jit.cuh needs K4J_W, K4J_TPA, K4J_TPB, K4J_TOMEGA, K4J_TTURN, K4J_OFFSET_MODE"
 #endif
@@ -47,6 +50,10 @@
 #ifndef K4J_CHUNK
 #define K4J_CHUNK 16  // MCS per precomputed chunk (lanes_api.cu sizes the dynamic shared memory with the same number)
 #endif
+#ifndef K4J_VPROF
+#define K4J_VPROF 6   // occupancy profile: epoch-end snapshots are counted in this many bit-sliced planes in shared memory
+#endif                //   and flushed to the per-site counters every 2^K4J_VPROF - 1 snapshots (0: added to them directly)
+
 #ifndef K4J_DIRECT
 #define K4J_DIRECT 4  // planes every lane draws for each of its items before undecided items go to the queue
 #endif
@@ -71,6 +78,7 @@ constexpr int U = (W + 3) / 4;
 constexpr bool SINGLE_WARP = U <= 32;
 constexpr bool PARTIAL = (W % 4) != 0;
 constexpr int NTHREADS = (U + 31) / 32 * 32;
+constexpr int VPROF = (K4J_VPROF > 0 && NTHREADS <= 256) ? K4J_VPROF : 0;  // bit-sliced snapshot counters (see add_profile_v)
 // Small rings (the paper's L = 512 ... 2048): U <= 16 supergroups fill only U lanes, so a warp sweeps SPW = 32 / U
 // independent samples side by side; offsets and record sums become per-lane values (segments of U lanes).
 constexpr int SPW = (!PARTIAL && U <= 16 && (U & (U - 1)) == 0) ? 32 / U : 1;
@@ -241,15 +249,26 @@ __device__ __forceinline__ uint32_t spread_even(uint32_t x) {  // low 16 bits ->
 }
 
 // ---- neighbour exchange: the value held by thread `src` of this sample ---------------------------------------------
+// (`parity` counts the exchanges of the CTA; the slot set alternates with it)
+#if K4J_HALOCHECK
+__device__ unsigned int* g_halo_check;  // = LanesRunArgs.check
+#endif
+constexpr int HALO_WORDS = (K4J_HALOCHECK ? 4 : 2) * NTHREADS;
 __device__ __forceinline__ uint32_t unit_exchange(uint32_t mine, int src, uint32_t* halo, int& parity) {
   if (SINGLE_WARP) {
     return __shfl_sync(FULL, mine, src);
   } else {
-    uint32_t* slot = halo + parity * NTHREADS;
+    uint32_t* slot = halo + (parity & 1) * NTHREADS;
     slot[threadIdx.x] = mine;
+#if K4J_HALOCHECK
+    slot[2 * NTHREADS + threadIdx.x] = (uint32_t)parity;
+#endif
     __syncthreads();
     const uint32_t v = slot[src];
-    parity ^= 1;
+#if K4J_HALOCHECK
+    if (slot[2 * NTHREADS + src] != (uint32_t)parity) atomicAdd(g_halo_check, 1u);
+#endif
+    parity += 1;
     return v;
   }
 }
@@ -261,12 +280,19 @@ __device__ __forceinline__ void unit_exchange2(uint32_t mine, int src1, int src2
     v1 = __shfl_sync(FULL, mine, src1);
     v2 = __shfl_sync(FULL, mine, src2);
   } else {
-    uint32_t* slot = halo + parity * NTHREADS;
+    uint32_t* slot = halo + (parity & 1) * NTHREADS;
     slot[threadIdx.x] = mine;
+#if K4J_HALOCHECK
+    slot[2 * NTHREADS + threadIdx.x] = (uint32_t)parity;
+#endif
     __syncthreads();
     v1 = slot[src1];
     v2 = slot[src2];
-    parity ^= 1;
+#if K4J_HALOCHECK
+    if (slot[2 * NTHREADS + src1] != (uint32_t)parity || slot[2 * NTHREADS + src2] != (uint32_t)parity)
+      atomicAdd(g_halo_check, 1u);
+#endif
+    parity += 1;
   }
 }
 
@@ -430,8 +456,8 @@ __device__ __forceinline__ void queue_push(WarpSmem* ws, Queue& q, bool und, con
 // One trip of the warp over up to 32 queued entries: each lane draws the next plane of ITS entry (whatever lane, MCS
 // and step that entry belongs to), applies it, ORs newly accepted sites into the entry's mask and queues the entry
 // again while it is undecided.  Entries are unique per (lane, k, st), so the read-modify-write of acc needs no atomic.
-__device__ __forceinline__ void queue_trip(WarpSmem* ws, Queue& q, const PhiloxKeys& K, uint32_t G, uint32_t gs,
-                                           long long m0) {
+__device__ __forceinline__ void queue_trip(WarpSmem* ws, uint4 (*acc)[2][32], Queue& q, const PhiloxKeys& K, uint32_t G,
+                                           uint32_t gs, long long m0) {
   const int lane = threadIdx.x & 31;
   const uint32_t nv = q.tail - q.head < 32u ? q.tail - q.head : 32u;
   const bool valid = (uint32_t)lane < nv;
@@ -454,9 +480,9 @@ __device__ __forceinline__ void queue_trip(WarpSmem* ws, Queue& q, const PhiloxK
   uint32_t eq[4] = {valid ? e.x : 0u, valid ? e.y : 0u, valid ? e.z : 0u, valid ? e.w : 0u};
   change_step(lt, eq, R, F, pl);
   if ((lt[0] | lt[1] | lt[2] | lt[3]) != 0u) {
-    uint4 a = ws->acc[k][st][le];
+    uint4 a = acc[k][st][le];
     a.x |= lt[0]; a.y |= lt[1]; a.z |= lt[2]; a.w |= lt[3];
-    ws->acc[k][st][le] = a;
+    acc[k][st][le] = a;
   }
   __syncwarp();  // the popped slots may be reused by the pushes below
   queue_push(ws, q, (eq[0] | eq[1] | eq[2] | eq[3]) != 0u && pl + 1 < NPW, eq, id + (1u << 14));
@@ -465,8 +491,8 @@ __device__ __forceinline__ void queue_trip(WarpSmem* ws, Queue& q, const PhiloxK
 
 // Acceptance masks of this warp's supergroups for MCS m0 .. m0 + n - 1 (n <= CHUNK), both lane-change steps.
 // F0 / F1 = the lane's flag words of step 0 / 1 (turning points; u_i / v_i), fixed over the chunk.
-__device__ __forceinline__ void precompute_chunk(WarpSmem* ws, const PhiloxKeys& K, const Unit& un, const uint32_t (&F0)[4],
-                                                 const uint32_t (&F1)[4], long long m0, int n) {
+__device__ __forceinline__ void precompute_chunk(WarpSmem* ws, uint4 (*acc)[2][32], const PhiloxKeys& K, const Unit& un,
+                                                 const uint32_t (&F0)[4], const uint32_t (&F1)[4], long long m0, int n) {
   const int lane = threadIdx.x & 31;
   if constexpr (CROSS) {
     ws->flag[0][lane] = make_uint4(F0[0], F0[1], F0[2], F0[3]);
@@ -496,16 +522,16 @@ __device__ __forceinline__ void precompute_chunk(WarpSmem* ws, const PhiloxKeys&
         change_step(lt1, eq1, R1[pl], F1, pl);
       }
     }
-    ws->acc[k][0][lane] = make_uint4(lt0[0], lt0[1], lt0[2], lt0[3]);
-    ws->acc[k][1][lane] = make_uint4(lt1[0], lt1[1], lt1[2], lt1[3]);
+    acc[k][0][lane] = make_uint4(lt0[0], lt0[1], lt0[2], lt0[3]);
+    acc[k][1][lane] = make_uint4(lt1[0], lt1[1], lt1[2], lt1[3]);
     __syncwarp();
     const uint32_t id = (uint32_t)lane | ((uint32_t)k << 5) | ((uint32_t)DIRECT << 14);
     queue_push(ws, q, DIRECT < NPW && (eq0[0] | eq0[1] | eq0[2] | eq0[3]) != 0u, eq0, id);
     queue_push(ws, q, DIRECT < NPW && (eq1[0] | eq1[1] | eq1[2] | eq1[3]) != 0u, eq1, id | (1u << 13));
     __syncwarp();
-    while (q.tail - q.head >= 32u) queue_trip(ws, q, K, (uint32_t)un.u, un.gs, m0);
+    while (q.tail - q.head >= 32u) queue_trip(ws, acc, q, K, (uint32_t)un.u, un.gs, m0);
   }
-  while (q.tail != q.head) queue_trip(ws, q, K, (uint32_t)un.u, un.gs, m0);
+  while (q.tail != q.head) queue_trip(ws, acc, q, K, (uint32_t)un.u, un.gs, m0);
   __syncwarp();
 }
 
@@ -598,6 +624,46 @@ __device__ __forceinline__ void add_profile(const uint32_t (&X)[4], uint32_t* oc
   }
 }
 
+// The same through bit-sliced counters (K4J_VPROF planes per lane array, one uint4 per plane and thread, in shared memory):
+// an epoch-end snapshot is ONE ripple-carry addition of the thread's 128 occupation bits to its 128 vertical counters
+// (two planes touched on average) instead of 128 shuffles and up to 128 atomics per warp; flush_profile() adds the
+// counters to the per-site uint32 profile every 2^K4J_VPROF - 1 snapshots and at the end of the launch.  The sites of a
+// thread belong to it alone, so the flush is a plain read-modify-write.
+__device__ __forceinline__ void add_profile_v(const uint32_t (&X)[4], uint4* cnt /* [VPROF][NTHREADS], this thread's column */) {
+  uint32_t c[4] = {X[0], X[1], X[2], X[3]};
+#pragma unroll 1
+  for (int p = 0; p < VPROF; ++p) {
+    if ((c[0] | c[1] | c[2] | c[3]) == 0u) break;
+    const uint4 t = cnt[p * NTHREADS];
+    cnt[p * NTHREADS] = make_uint4(t.x ^ c[0], t.y ^ c[1], t.z ^ c[2], t.w ^ c[3]);
+    c[0] &= t.x; c[1] &= t.y; c[2] &= t.z; c[3] &= t.w;
+  }
+}
+__device__ __forceinline__ void flush_profile(uint4* cnt, uint32_t* occ_unit /* this thread's 128 counters */, int nwn) {
+  uint32_t pl[VPROF > 0 ? VPROF : 1][4];
+  uint32_t any = 0u;
+#pragma unroll
+  for (int p = 0; p < VPROF; ++p) {
+    const uint4 t = cnt[p * NTHREADS];
+    pl[p][0] = t.x; pl[p][1] = t.y; pl[p][2] = t.z; pl[p][3] = t.w;
+    any |= t.x | t.y | t.z | t.w;
+    cnt[p * NTHREADS] = make_uint4(0u, 0u, 0u, 0u);
+  }
+  if (any == 0u) return;
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    if (w < nwn) {
+#pragma unroll 1
+      for (int b = 0; b < 32; ++b) {
+        uint32_t v = 0u;
+#pragma unroll
+        for (int p = 0; p < VPROF; ++p) v |= ((pl[p][w] >> b) & 1u) << p;
+        if (v) occ_unit[32 * w + b] += v;
+      }
+    }
+  }
+}
+
 __device__ __forceinline__ uint32_t draw_offsets16(const PhiloxKeys& K, uint32_t gs, long long m) {
   const int lane = threadIdx.x & 31;
   const unsigned long long mb = ((unsigned long long)m & ~15ull) + (unsigned)(lane >> 1);
@@ -613,22 +679,32 @@ extern "C" __global__ void __launch_bounds__(kpz::k4j::NTHREADS)
 lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constant__ kpz::LanesRunArgs R) {
   using namespace kpz;
   using namespace kpz::k4j;
-  __shared__ uint32_t halo[SINGLE_WARP ? 1 : 2 * NTHREADS];
+  __shared__ uint32_t halo[SINGLE_WARP ? 1 : HALO_WORDS];
+#if K4J_HALOCHECK
+  if (threadIdx.x == 0) g_halo_check = R.check;  // every CTA writes the same pointer
+  __syncthreads();
+#endif
   __shared__ unsigned long long red[SINGLE_WARP ? 1 : 4 * 32];
   __shared__ PackSmem pack[NTHREADS / 32];
-  PackSmem* const xs = pack + (threadIdx.x >> 5);
-  extern __shared__ __align__(16) unsigned char k4_dyn_smem[];  // K4J_PRE: NTHREADS / 32 WarpSmem (lanes_api.cu sizes it)
-  WarpSmem* const ws = reinterpret_cast<WarpSmem*>(k4_dyn_smem) + (threadIdx.x >> 5);
+  const int tid = (int)threadIdx.x;
+  PackSmem* const xs = pack + (tid >> 5);
+  // dynamic shared memory (lanes_api.cu sizes it): K4J_PRE: NTHREADS / 32 WarpSmem; then the bit-sliced profile counters
+  extern __shared__ __align__(16) unsigned char k4_dyn_smem[];
+  WarpSmem* const ws = reinterpret_cast<WarpSmem*>(k4_dyn_smem) + (tid >> 5);
+  uint4* const vcnt = reinterpret_cast<uint4*>(k4_dyn_smem + (K4J_PRE ? sizeof(WarpSmem) * (NTHREADS / 32) : 0));
+  // vcnt[(lane array * VPROF + plane) * NTHREADS + tid]: a thread touches its own column only
+  if (VPROF > 0)
+    for (int p = 0; p < 2 * VPROF; ++p) vcnt[p * NTHREADS + tid] = make_uint4(0u, 0u, 0u, 0u);
   // SPW == 1: CTA = sample, thread = supergroup.  SPW > 1: CTA = one warp = SPW samples, lane = (sample, supergroup).
   int sub = 0, s = (int)blockIdx.x, lane0 = 0;
   const int lane = threadIdx.x & 31;
   Unit un;
-  un.u = threadIdx.x;
+  un.u = tid;
   bool active = un.u < U;
   if constexpr (SPW > 1) {
-    sub = (int)threadIdx.x / U;
+    sub = tid / U;
     s = (int)blockIdx.x * SPW + sub;
-    un.u = (int)threadIdx.x % U;
+    un.u = tid % U;
     lane0 = sub * U;
     active = s < D.S;
   }
@@ -644,9 +720,9 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
   if (active) {
     const uint4 a = *reinterpret_cast<const uint4*>(D.A + row);
     const uint4 b = *reinterpret_cast<const uint4*>(D.B + row);
-    const uint4 t = *reinterpret_cast<const uint4*>(D.T + row);
     A[0] = a.x; A[1] = a.y; A[2] = a.z; A[3] = a.w;
     B[0] = b.x; B[1] = b.y; B[2] = b.z; B[3] = b.w;
+    const uint4 t = *reinterpret_cast<const uint4*>(D.T + row);
     T[0] = t.x; T[1] = t.y; T[2] = t.z; T[3] = t.w;
     if (K4J_INDEP) {
       const uint4 v = *reinterpret_cast<const uint4*>(D.V + row);
@@ -687,7 +763,7 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
 #pragma unroll
       for (int k = 0; k < 4; ++k) out[k] = v[k];  // valid in the first lane of each sample
     } else {
-      const int warp = threadIdx.x >> 5;
+      const int warp = tid >> 5;
       __syncthreads();
       if (lane == 0)
 #pragma unroll
@@ -704,6 +780,7 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
 
   Eager EA, EB;
   if (!K4J_PRE) draw_eager(EA, D.keys, un, m);
+  int nflush = 0;  // snapshots in the bit-sliced profile counters
 
   auto redraw_flags = [&]() {  // a new epoch starts at MCS m
     if (period > 0 && m > 0 && in_epoch == 0) {
@@ -775,14 +852,26 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
     if (period > 0 && ++in_epoch == period) {
       in_epoch = 0;
       ++epoch;
-      add_profile(A, D.occA, D.S);  // occupancy profile at epoch ends
-      add_profile(B, D.occB, D.S);
+      if (VPROF > 0) {  // occupancy profile at epoch ends
+        add_profile_v(A, vcnt + tid);
+        add_profile_v(B, vcnt + VPROF * NTHREADS + tid);
+        if (++nflush == (1 << VPROF) - 1) {
+          if (active) {
+            flush_profile(vcnt + tid, D.occA + (size_t)s * (32 * W) + 128 * un.u, un.nwn);
+            flush_profile(vcnt + VPROF * NTHREADS + tid, D.occB + (size_t)s * (32 * W) + 128 * un.u, un.nwn);
+          }
+          nflush = 0;
+        }
+      } else {
+        add_profile(A, D.occA, D.S);
+        add_profile(B, D.occB, D.S);
+      }
     }
     if (m == next_rec) {
       unsigned long long tot[4];
       block_sum4(jA, jB, (unsigned long long)(__popc(A[0]) + __popc(A[1]) + __popc(A[2]) + __popc(A[3])),
                  (unsigned long long)(__popc(B[0]) + __popc(B[1]) + __popc(B[2]) + __popc(B[3])), tot);
-      if (SPW > 1 ? (un.u == 0 && active) : threadIdx.x == 0) {
+      if (SPW > 1 ? (un.u == 0 && active) : tid == 0) {
         const size_t cell = (size_t)ri * D.S + s, plane = (size_t)R.nt * D.S;
         R.rec[cell] = (long long)(D.JA[s] + tot[0]);
         R.rec[plane + cell] = (long long)(D.JB[s] + tot[1]);
@@ -800,7 +889,7 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
       long long n = t_end - m < (long long)CHUNK ? t_end - m : (long long)CHUNK;
       if (period > 0 && period - in_epoch < n) n = period - in_epoch;
       redraw_flags();
-      precompute_chunk(ws, D.keys, un, T, K4J_INDEP ? V : T, m, (int)n);
+      precompute_chunk(ws, ws->acc, D.keys, un, T, K4J_INDEP ? V : T, m, (int)n);
       for (int kc = 0; kc < (int)n; ++kc) mcs(EA, EA, kc);
     }
   } else {
@@ -814,10 +903,14 @@ lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constan
   {
     unsigned long long tot[4];
     block_sum4(jA, jB, 0, 0, tot);
-    if (SPW > 1 ? (un.u == 0 && active) : threadIdx.x == 0) {
+    if (SPW > 1 ? (un.u == 0 && active) : tid == 0) {
       D.JA[s] += tot[0];
       D.JB[s] += tot[1];
     }
+  }
+  if (VPROF > 0 && active && nflush > 0) {
+    flush_profile(vcnt + tid, D.occA + (size_t)s * (32 * W) + 128 * un.u, un.nwn);
+    flush_profile(vcnt + VPROF * NTHREADS + tid, D.occB + (size_t)s * (32 * W) + 128 * un.u, un.nwn);
   }
   if (active) {
     *reinterpret_cast<uint4*>(D.A + row) = make_uint4(A[0], A[1], A[2], A[3]);

@@ -225,10 +225,12 @@ K1Shape k1_shape(const KpzDev& D, int S, int dis) {
   }
   K1Shape sh;
   const bool partial = (D.PW % 4) != 0;
-  // units per thread (K1J_UPT): a ring of 64 or more units gives every thread two of them - half the warps, no
-  // barrier at all for L = 16384, two independent chains of pair logic per thread
-  sh.upt = debug_int("K1J_UPT", (!partial && D.U >= 64 && D.U % 2 == 0) ? 2 : 1);
-  if (partial || D.U % sh.upt != 0) sh.upt = 1;
+  // units per thread (K1J_UPT, k1_sweep_jit.cuh): 2 gives a ring of 64 units to ONE warp - no barrier, two independent
+  // chains of pair logic per thread.  Measured (profiles/r02_k1_upt.md): no gain at BASELINE's 512 rings of 16384
+  // sites (a lone warp per SMSP stays latency-bound), +8 % with K1J_VARIANT=2 once 1184 rings fill the chip, and a loss
+  // on the lazily evaluated path (twice the registers, same trips) - so the default stays 1; the knob is kept for tests.
+  sh.upt = debug_int("K1J_UPT", 1);
+  if (sh.upt < 1 || sh.upt > 2 || partial || D.U % sh.upt != 0) sh.upt = 1;
   const int UT = D.U / sh.upt;
   sh.block = (UT + 31) / 32 * 32;
   // small rings (SPW): UT <= 16 threads, a power of two, no ragged unit -> 32/UT samples per warp
@@ -237,10 +239,9 @@ K1Shape k1_shape(const KpzDev& D, int S, int dis) {
   sh.spw = pack ? 32 / UT : 1;
   sh.defs = k1_jit_defines(D, dis);
   char buf[32];
-  if (!debug_has("K1J_UPT")) {
-    snprintf(buf, sizeof buf, "K1J_UPT=%d", sh.upt);
-    sh.defs.push_back(buf);
-  }
+  drop_define(&sh.defs, "K1J_UPT");  // the value clamped above, not the raw debug setting
+  snprintf(buf, sizeof buf, "K1J_UPT=%d", sh.upt);
+  sh.defs.push_back(buf);
   if (!pack) sh.defs.push_back("K1J_PACK=0");
   if (!debug_has("K1J_VARIANT")) {
     // code shape by occupancy (k1_sweep_jit.cuh, K1J_VARIANT): with >= 4 resident warps per SMSP the other warps
@@ -777,9 +778,22 @@ int kpz_run(kpz_sim* sim, int64_t n_mcs) {
       void* kfn = nullptr;
       rc = jit_get("k1_sweep_jit.cuh", "kpz_k1_sweep_jit", sh.defs, &kfn);
       if (rc) return rc;
+      // debug (kpz_debug_config "K1J_HALOCHECK=1"): sequence numbers on the shared-memory halo slots, counted here
+      const bool halocheck = debug_int("K1J_HALOCHECK", 0) != 0;
+      unsigned int* check = (unsigned int*)(sim->scratch + D.PW + 32);
+      if (halocheck) {
+        KPZ_CUDA_CHECK(cudaMemsetAsync(check, 0, sizeof(unsigned int), sim->stream));
+        A.check = check;
+      }
       void* args[] = {(void*)&D, (void*)&A};
       KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((sim->S + sh.spw - 1) / sh.spw), dim3(sh.block), args, 0, sim->stream));
       KPZ_LAUNCH_CHECK("kpz_k1_sweep_jit");
+      if (halocheck) {
+        unsigned int bad = 0;
+        KPZ_CUDA_CHECK(cudaMemcpyAsync(&bad, check, sizeof bad, cudaMemcpyDeviceToHost, sim->stream));
+        KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
+        if (bad) return fail(KPZ_ECUDA, "halo sequence check: %u reads of a slot of another exchange", bad);
+      }
     } else {
       K1Fn fn = k1_pick(single, partial, dis, D.nplanes);
       fn<<<sim->S, block, 0, sim->stream>>>(D, A);

@@ -23,6 +23,7 @@ struct lanes_sim {
   int64_t nsnap = 0;  // profile snapshots taken (epoch ends passed by lanes_run)
   std::vector<int64_t> rec_times;
   int32_t nrec = 0;
+  unsigned int* check = nullptr;  // debug counter (K4J_HALOCHECK)
   char* base = nullptr;   // workspace start
   size_t zero_bytes = 0;  // lattices (incl. pad words), counters and profile sit in [base, base + zero_bytes)
   Thresh t_rho{};
@@ -31,7 +32,7 @@ struct lanes_sim {
 namespace {
 
 struct LLayout {
-  size_t off_A, off_B, off_T, off_V, off_JA, off_JB, off_occA, off_occB, off_rec_t, off_rec, total;
+  size_t off_A, off_B, off_T, off_V, off_JA, off_JB, off_occA, off_occB, off_rec_t, off_rec, off_check, total;
   int W, Wp, U;
 };
 
@@ -65,6 +66,7 @@ LLayout lanes_layout(int64_t L, int32_t S, int32_t max_records) {
   y.off_occB = take((size_t)S * L * 4);
   y.off_rec_t = take((size_t)std::max(max_records, 1) * 8);
   y.off_rec = take((size_t)4 * std::max(max_records, 1) * S * 8);
+  y.off_check = take(256);  // debug counter (K4J_HALOCHECK)
   y.total = off;
   return y;
 }
@@ -72,11 +74,28 @@ LLayout lanes_layout(int64_t L, int32_t S, int32_t max_records) {
 // ---- K4 v2: kernel specialised at run time on (L, thresholds, offset mode) — k4_lanes_jit.cuh ---------------------
 bool k4_use_jit(const LanesDev& D) { return jit_enabled() && (D.W + 3) / 4 <= 1024; }
 
-// MCS per precomputed chunk: as many as keep the CTA's shared memory near 100 KB (two CTAs per SM), at most 16.
-int k4_chunk(const LanesDev& D) {
-  const int nwarps = ((D.W + 3) / 4 + 31) / 32;
-  const int per_warp = 100 * 1024 / nwarps - (128 * 16 + 128 * 4 + 1024);
-  return std::max(1, std::min(16, per_warp / 1024));
+// Launch shape of the run-time specialised two-lane kernel (k4_lanes_jit.cuh): which of its code shapes, how many MCS
+// per precomputed chunk, block size, dynamic shared memory - the same numbers go to the compiler as definitions.
+struct K4Shape {
+  int pre = 1, chunk = 1, vprof = 0, block = 32;
+  size_t smem = 0;
+};
+K4Shape k4_shape(const LanesDev& D) {
+  K4Shape sh;
+  const int nthreads = ((D.W + 3) / 4 + 31) / 32 * 32;
+  const int nwarps = nthreads / 32;
+  sh.pre = debug_int("K4J_PRE", 1) ? 1 : 0;
+  sh.vprof = nthreads <= 256 ? std::max(0, std::min(12, debug_int("K4J_VPROF", 6))) : 0;
+  const size_t fixed = 128 * 16 + 128 * 4 + 2 * 32 * 16;  // queue and flags of one WarpSmem
+  const size_t vbytes = (size_t)2 * sh.vprof * nthreads * 16;
+  // MCS per chunk: as many as keep the CTA near 100 KB (two CTAs per SM), at most 16
+  const long long budget = 100 * 1024 - (long long)vbytes;
+  const long long per_warp = budget / nwarps - (long long)fixed;
+  int chunk = (int)std::max<long long>(1, std::min<long long>(16, per_warp / 1024));
+  sh.chunk = std::max(1, std::min(256, debug_int("K4J_CHUNK", chunk)));
+  sh.block = nthreads;
+  sh.smem = (sh.pre ? (size_t)nwarps * ((size_t)sh.chunk * 1024 + fixed) : 0) + vbytes;
+  return sh;
 }
 
 std::vector<std::string> k4_jit_defines(const LanesDev& D) {
@@ -100,20 +119,20 @@ std::vector<std::string> k4_jit_defines(const LanesDev& D) {
   snprintf(buf, sizeof buf, "K4J_INDEP=%d", D.independent);
   d.push_back(buf);
   debug_defines("K4J_", &d);  // kpz_debug_config: tests and tuning only (the run reads no environment)
-  if (!debug_has("K4J_CHUNK")) {
-    snprintf(buf, sizeof buf, "K4J_CHUNK=%d", k4_chunk(D));
-    d.push_back(buf);
+  // the launch shape as the host computed it (clamped), not the raw debug values
+  const K4Shape sh = k4_shape(D);
+  for (const char* name : {"K4J_PRE", "K4J_CHUNK", "K4J_VPROF"}) {
+    const std::string key = std::string(name) + "=";
+    d.erase(std::remove_if(d.begin(), d.end(), [&](const std::string& x) { return x.compare(0, key.size(), key) == 0; }),
+            d.end());
   }
+  snprintf(buf, sizeof buf, "K4J_PRE=%d", sh.pre);
+  d.push_back(buf);
+  snprintf(buf, sizeof buf, "K4J_CHUNK=%d", sh.chunk);
+  d.push_back(buf);
+  snprintf(buf, sizeof buf, "K4J_VPROF=%d", sh.vprof);
+  d.push_back(buf);
   return d;
-}
-
-// Dynamic shared memory of the kernel: one WarpSmem (k4_lanes_jit.cuh) per warp when the lane-change acceptance is
-// precomputed: acc[CHUNK][2][32] uint4 + a 128-entry queue (uint4 + uint32) + flag[2][32] uint4.
-size_t k4_smem_bytes(const LanesDev& D) {
-  if (!debug_int("K4J_PRE", 1)) return 0;
-  const int nwarps = ((D.W + 3) / 4 + 31) / 32;
-  const int chunk = debug_int("K4J_CHUNK", k4_chunk(D));
-  return (size_t)nwarps * ((size_t)chunk * 1024 + 128 * 16 + 128 * 4 + 1024);
 }
 
 int grid_for(size_t n, int block = 256) {
@@ -223,6 +242,7 @@ int lanes_create_crossing(lanes_sim** out, int64_t L, int32_t nsamples, double p
   D.occB = (uint32_t*)(base + y.off_occB);
   sim->rec_t = (long long*)(base + y.off_rec_t);
   sim->rec = (long long*)(base + y.off_rec);
+  sim->check = (unsigned int*)(base + y.off_check);
 
   sim->zero_bytes = y.off_rec_t;
   sim->base = base;
@@ -330,10 +350,23 @@ int lanes_run(lanes_sim* sim, int64_t n_mcs) {
     // small rings (k4_lanes_jit.cuh, SPW): U4 <= 16 supergroups, a power of two, no ragged word -> 32/U4 samples per warp
     const bool pack = (D.W % 4) == 0 && U4 <= 16 && (U4 & (U4 - 1)) == 0;
     const int spw = pack ? 32 / U4 : 1;
-    const size_t smem = k4_smem_bytes(D);
-    if (smem > 48 * 1024)
-      KPZ_CUDA_CHECK(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((sim->S + spw - 1) / spw), dim3(block4), args, smem, sim->stream));
+    const K4Shape sh = k4_shape(D);
+    (void)block4;
+    const bool halocheck = debug_int("K4J_HALOCHECK", 0) != 0;  // debug: sequence numbers on the halo slots
+    if (halocheck) {
+      KPZ_CUDA_CHECK(cudaMemsetAsync(sim->check, 0, sizeof(unsigned int), sim->stream));
+      A.check = sim->check;
+      args[1] = (void*)&A;
+    }
+    if (sh.smem > 32 * 1024)  // static shared memory (halo, sums, pack slots) comes on top
+      KPZ_CUDA_CHECK(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
+    KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((sim->S + spw - 1) / spw), dim3(sh.block), args, sh.smem, sim->stream));
+    if (halocheck) {
+      unsigned int bad = 0;
+      KPZ_CUDA_CHECK(cudaMemcpyAsync(&bad, sim->check, sizeof bad, cudaMemcpyDeviceToHost, sim->stream));
+      KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
+      if (bad) return fail(KPZ_ECUDA, "halo sequence check: %u reads of a slot of another exchange", bad);
+    }
   } else if (D.independent || D.t_w0.value != 0 || D.t_w0.always) {
     return fail(KPZ_EUNSUPPORTED, "the site-wise crossing model runs on the run-time specialised kernel only "
                                   "(L <= 131072, KPZ_B200_JIT not 0)");

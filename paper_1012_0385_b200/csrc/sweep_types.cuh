@@ -37,6 +37,7 @@ struct KpzRunArgs {
   int32_t nt;
   long long* rec_sum_h;    // [nt][S]
   long long* rec_sum_h2;   // [nt][S]
+  unsigned int* check;     // debug (K1J_HALOCHECK): counter of failed halo sequence checks, else nullptr
 };
 
 // K3 (pass-by-pass streamed sweep): one launch = one sub-lattice pass from (Ein, Oin) to (Eout, Oout).
@@ -88,6 +89,7 @@ struct LanesRunArgs {
   const long long* rec_t;
   int32_t rec_begin, nt;
   long long* rec;  // [4][nt][S]: J_A, J_B, N_A, N_B
+  unsigned int* check;  // debug (K4J_HALOCHECK): counter of failed halo sequence checks, else nullptr
 };
 
 }  // namespace kpz

@@ -465,11 +465,28 @@ def test_static_streamed_kernel_against_oracle(K):
 
 @pytest.mark.parametrize("cfg", ["jit=0", "K4J_PRE=0", "K4J_PRE=0;K4J_EAGER=0;K4J_SMAX=32", "K4J_PRE=0;K4J_EAGER=7;K4J_SMAX=2",
                                  "K4J_PRE=0;K4J_EAGER=3;K4J_SMAX=8", "K4J_CHUNK=3;K4J_DIRECT=1", "K4J_CHUNK=1;K4J_DIRECT=0",
-                                 "K4J_CHUNK=7;K4J_DIRECT=9"])
+                                 "K4J_CHUNK=7;K4J_DIRECT=9", "K4J_CHUNK=5;K4J_VPROF=0", "K4J_VPROF=2", "K4J_PRE=0;K4J_VPROF=1"])
 def test_k4_variants_against_oracle(K, cfg):
     with K.debug_config(cfg):
         run_both_lanes(K, 8192 + 64, 2, 1.0, 1.0, 0.3, 0.05, 6, 0.1, seed=31, times=[1, 6, 13], chunks=[6, 7])
         run_both_lanes(K, 2048, 2, 0.75, 0.5, 0.4, 0.3, 4, 0.3, seed=32, times=[9], chunks=[9])
+
+
+@pytest.mark.parametrize("extra", ["", ";K1J_REFRAME=1", ";K1J_VARIANT=2"])
+def test_k1_halo_slots_carry_the_number_of_their_exchange(K, extra):
+    """Stand-in for compute-sanitizer's racecheck (closed on this GPU pool): with K1J_HALOCHECK every word published
+    through the shared-memory halo of a multi-warp ring carries the number of its exchange, and a reader that finds another
+    number - a slot not yet written or already overwritten - makes kpz_run fail.  2-, 5- and 32-warp rings, ragged too."""
+    with K.debug_config("K1J_HALOCHECK=1" + extra):
+        run_both_kpz(K, 16384, 3, 0.75, 0.25, seed=71, times=[1, 9, 60], chunks=[25, 35])
+        run_both_kpz(K, 40960 + 64, 2, 1.0, 0.0, disorder=(0.1, 0.5, 0.0, 0.0), seed=72, times=[40], chunks=[40])
+        run_both_kpz(K, 262144, 1, 0.8, 0.1, disorder=(0.3, 0.2, 0.3, 0.05), seed=73, times=[6], chunks=[6])
+
+
+def test_k4_halo_slots_carry_the_number_of_their_exchange(K):
+    with K.debug_config("K4J_HALOCHECK=1"):
+        run_both_lanes(K, 16384, 2, 1.0, 1.0, 0.3, 0.05, 10, 0.1, seed=74, times=[1, 30], chunks=[30])
+        run_both_lanes(K, 40960 + 64, 1, 0.75, 0.5, 0.4, 0.3, 4, 0.3, seed=75, times=[9], chunks=[9])
 
 
 def test_k4_ring_beyond_the_specialised_kernel(K):
