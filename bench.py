@@ -432,8 +432,8 @@ def roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run):
         traffic = num("dram_bytes_read") + num("dram_bytes_write")
     measured = None
     if row:
-        measured = {k: num(k) for k in ("issue_active_pct", "pipe_alu_pct", "pipe_fmaheavy_pct", "warps_active_per_smsp")
-                    if num(k) is not None} or None
+        measured = {k: num(k) for k in ("issue_active_pct", "pipe_alu_pct", "pipe_fma_pct", "pipe_fmaheavy_pct_of_elapsed",
+                                        "warps_active_per_smsp", "registers", "gpu_time_us") if num(k) is not None} or None
     src = (f"profiles/ncu_counters.csv row {cfg_key}: {row.get('capture', '')}" if row else None)
     if path == 2:
         # streamed sweep: 2*n_mcs pass kernels per run; per launch one read + one write of the ring

@@ -99,12 +99,12 @@ def main() -> int:
     print(f"alu-pipe slot instructions (LOP3 + SHF + PRMT + SEL + LEA + IMAD.WIDE): {slots:,}"
           + (f" = {slots / w:.1f} per warp-MCS" if w else "") + f"; without IMAD.WIDE: {alu_only:,}")
     if cyc_elapsed:
-        per_smsp = slots / n_smsp
-        print(f"slots per SMSP x 2 clk = {2 * per_smsp:,.0f} clk of {cyc_elapsed:,.0f} elapsed SM cycles "
-              f"= {100.0 * 2 * per_smsp / cyc_elapsed:.1f} % of the alu-pipe slot peak (mean over 592 SMSPs); "
-              f"instructions that execute ON the alu pipe (those without IMAD.WIDE, plus ISETP / PLOP3 / VOTE ...) x 2 clk = "
-              f"{100.0 * 2 * alu_pipe / n_smsp / (cyc_active or cyc_elapsed):.1f} % of the active cycles - to be compared with "
-              f"ncu's sm__pipe_alu_cycles_active below")
+        act = cyc_active or cyc_elapsed
+        print(f"- slot instructions per SMSP x 2 clk = {2 * slots / n_smsp:,.0f} clk = {100.0 * 2 * slots / n_smsp / cyc_elapsed:.1f} % of the "
+              f"{cyc_elapsed:,.0f} elapsed SM cycles (mean over {n_smsp} SMSPs): the executed slot occupancy")
+        print(f"- check against ncu: LOP3 + SHF + PRMT + SEL + LEA x 2 clk = {100.0 * 2 * alu_only / n_smsp / act:.1f} % of the "
+              f"{act:,.0f} ACTIVE cycles per SMSP ({100.0 * 2 * alu_pipe / n_smsp / act:.1f} % with ISETP / PLOP3 / VOTE); "
+              f"ncu's `sm__pipe_alu_cycles_active` (per active cycle) is in the table below")
     print()
     print("| ncu counter | value |")
     print("|---|---|")
