@@ -14,6 +14,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "kpz_oracle.c")
 HDR = os.path.join(HERE, "kpz_oracle.h")
+SRC2D = os.path.join(HERE, "kpz2d_oracle.c")   # the 2+1D generalisation (calls the exported RNG functions of kpz_oracle.c)
+HDR2D = os.path.join(HERE, "kpz2d_oracle.h")
 LIB = os.path.join(HERE, "libkpz_oracle.so")
 
 
@@ -21,14 +23,14 @@ def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(f) > t for f in (SRC, HDR))
+    return any(os.path.getmtime(f) > t for f in (SRC, HDR, SRC2D, HDR2D))
 
 
 def build(force: bool = False, sanitize: bool = False) -> str:
     if force or sanitize or needs_build():
         tmp = LIB + f".tmp{os.getpid()}"
         opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"] if sanitize else ["-O3"]
-        cmd = ["gcc", "-std=c11", *opt, "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, SRC, "-lm"]
+        cmd = ["gcc", "-std=c11", *opt, "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, SRC, SRC2D, "-lm"]
         subprocess.run(cmd, check=True, cwd=HERE)
         os.replace(tmp, LIB)
     return LIB

@@ -300,3 +300,75 @@ def pack_sites(sites):
     if pad:
         s = np.concatenate([s, np.zeros((S, pad), dtype=np.uint8)], axis=1)
     return np.packbits(s, axis=1, bitorder="little").view(np.uint32).reshape(S, -1)
+
+
+class Kpz2dRef:
+    """The 2+1D generalisation (oracle/kpz2d_oracle.c)."""
+
+    def __init__(self, Lx, Ly, nsamples, p, q, seed=0, first_sample=0, offset_mode=0):
+        self.Lx, self.Ly, self.S = int(Lx), int(Ly), int(nsamples)
+        self.row_words = (self.Lx + 31) // 32
+        self._o = Options(int(first_sample), int(offset_mode), 0)
+        self._h = C.c_void_p()
+        self._nt = 0
+        _chk(lib().kpz2dref_create(C.byref(self._h), C.c_int32(self.Lx), C.c_int32(self.Ly), C.c_int32(self.S),
+                                   C.c_double(p), C.c_double(q), C.c_uint64(seed), C.byref(self._o)), "kpz2dref_create")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().kpz2dref_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_record_times(self, t):
+        t = _times(t)
+        self._nt = len(t)
+        _chk(lib().kpz2dref_set_record_times(self._h, _p(t, C.c_int64), C.c_int32(len(t))), "kpz2dref_set_record_times")
+
+    def run(self, n_mcs):
+        _chk(lib().kpz2dref_run(self._h, C.c_int64(n_mcs)), "kpz2dref_run")
+
+    @property
+    def time(self):
+        t = C.c_int64()
+        _chk(lib().kpz2dref_time(self._h, C.byref(t)), "kpz2dref_time")
+        return t.value
+
+    def slopes(self):
+        sx = np.zeros((self.S, self.Ly, self.row_words), dtype=np.uint32)
+        sy = np.zeros_like(sx)
+        _chk(lib().kpz2dref_slopes(self._h, _p(sx, C.c_uint32), _p(sy, C.c_uint32)), "kpz2dref_slopes")
+        return sx, sy
+
+    def set_slopes(self, sx, sy):
+        sx = np.ascontiguousarray(sx, dtype=np.uint32)
+        sy = np.ascontiguousarray(sy, dtype=np.uint32)
+        _chk(lib().kpz2dref_set_slopes(self._h, _p(sx, C.c_uint32), _p(sy, C.c_uint32)), "kpz2dref_set_slopes")
+
+    def heights(self, sample):
+        h = np.zeros((self.Ly, self.Lx), dtype=np.int32)
+        _chk(lib().kpz2dref_heights(self._h, C.c_int32(sample), _p(h, C.c_int32)), "kpz2dref_heights")
+        return h
+
+    def roughness(self):
+        cap = max(self._nt, 1)
+        nt = C.c_int32(cap)
+        t = np.zeros(cap, dtype=np.int64)
+        s1 = np.zeros((cap, self.S), dtype=np.int64)
+        s2 = np.zeros((cap, self.S), dtype=np.int64)
+        w2 = np.zeros(cap, dtype=np.float64)
+        _chk(lib().kpz2dref_roughness(self._h, C.byref(nt), _p(t, C.c_int64), _p(s1, C.c_int64), _p(s2, C.c_int64),
+                                      _p(w2, C.c_double)), "kpz2dref_roughness")
+        k = nt.value
+        return dict(t=t[:k], sum_h=s1[:k], sum_h2=s2[:k], w2_mean=w2[:k])
+
+    def hops(self):
+        f = np.zeros(self.S, dtype=np.int64)
+        b = np.zeros(self.S, dtype=np.int64)
+        _chk(lib().kpz2dref_hops(self._h, _p(f, C.c_int64), _p(b, C.c_int64)), "kpz2dref_hops")
+        return f, b

@@ -196,3 +196,77 @@ def lanes_finite_time(L, start_state, turn_mask, p_a, p_b, omega, n_mcs, ab_firs
             v = 0.5 * (T0 @ v + T1 @ v)
             v = S @ v
     return states, v, JA, JB
+
+
+# ------------------------------------------------------------------------------------------------
+# 2+1D generalisation: checkerboard passes of the dimer / octahedron move on a tiny
+# periodic Lx x Ly lattice.  A state is (sx, sy), two tuples of Ly rows of Lx bits; written without reference to the
+# oracle: site (x, y), colour (x + y) & 1; forward move iff x-pair and y-pair are both (1,0), backward iff both (0,1).
+# ------------------------------------------------------------------------------------------------
+def flat2d(Lx, Ly):
+    rows = tuple(tuple((x + y) & 1 for x in range(Lx)) for y in range(Ly))
+    return rows, rows
+
+
+def _moves2d(state, Lx, Ly, colour, need_both=True):
+    """Eligible moves of one colour pass: list of (x, y, kind) with kind +1 forward, -1 backward."""
+    sx, sy = state
+    out = []
+    for y in range(Ly):
+        for x in range(Lx):
+            if (x + y) & 1 != colour:
+                continue
+            xp = (sx[y][x], sx[y][(x + 1) % Lx])
+            yp = (sy[y][x], sy[(y + 1) % Ly][x])
+            if need_both:
+                if xp == (1, 0) and yp == (1, 0):
+                    out.append((x, y, +1))
+                elif xp == (0, 1) and yp == (0, 1):
+                    out.append((x, y, -1))
+            else:                       # a WRONG reading kept for the power check: the x-pair alone decides
+                if xp == (1, 0):
+                    out.append((x, y, +1))
+                elif xp == (0, 1):
+                    out.append((x, y, -1))
+    return out
+
+
+def _apply2d(state, Lx, Ly, chosen):
+    sx = [list(r) for r in state[0]]
+    sy = [list(r) for r in state[1]]
+    for x, y, kind in chosen:
+        a, b = (0, 1) if kind > 0 else (1, 0)
+        sx[y][x], sx[y][(x + 1) % Lx] = a, b
+        sy[y][x], sy[(y + 1) % Ly][x] = a, b
+    return tuple(tuple(r) for r in sx), tuple(tuple(r) for r in sy)
+
+
+def kpz2d_finite_time(Lx, Ly, p, q, n_mcs, mode="drawn", need_both=True):
+    """Exact distribution {state: probability} after n_mcs MCS from the flat state, and the expected numbers of accepted
+    forward / backward moves.  mode "drawn": every pass has colour 0 or 1 with probability 1/2; "alternating": 0 then 1."""
+    import itertools
+    dist = {flat2d(Lx, Ly): 1.0}
+    fwd = bwd = 0.0
+    for _ in range(n_mcs):
+        for ps in range(2):
+            new = {}
+            colours = [(0, 0.5), (1, 0.5)] if mode == "drawn" else [(ps, 1.0)]
+            for state, pr in dist.items():
+                for colour, pc in colours:
+                    mv = _moves2d(state, Lx, Ly, colour, need_both)
+                    for pick in itertools.product((0, 1), repeat=len(mv)):
+                        w = pr * pc
+                        chosen = []
+                        for take, (x, y, kind) in zip(pick, mv):
+                            rate = p if kind > 0 else q
+                            w *= rate if take else 1.0 - rate
+                            if take:
+                                chosen.append((x, y, kind))
+                        if w == 0.0:
+                            continue
+                        fwd += w * sum(1 for c in chosen if c[2] > 0)
+                        bwd += w * sum(1 for c in chosen if c[2] < 0)
+                        ns = _apply2d(state, Lx, Ly, chosen)
+                        new[ns] = new.get(ns, 0.0) + w
+            dist = new
+    return dist, fwd, bwd
