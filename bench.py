@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — site-update throughput of the KPZ/ASEP hot path on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1|2|3|4|5|4-aux-i|4-aux-ii|2-fill|3-fill|paper-...]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1|2|3|4|5|4-aux-i|4-aux-ii|2d-1024|2-fill|3-fill|paper-...]
                     [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: reset to the
@@ -76,6 +76,10 @@ ALU_SLOTS_PER_SU = {
     # cover 256 sites per call: 2 lanes x 2 passes x 0.5 call) + crossings 2 steps x (log2(32 live)+1.33 planes) x (34+12)
     "paper-lanes-4096": (2 * 34 + 2 * 6.33 * (34 + 12) + 2 * 2 * 4 * 5 + 2 * 4 * 4) / 256,
 }
+# 2+1D generalisation: per Philox supergroup (128 elements = the active half of 256 sites of a row) and
+# colour pass: p = 0.75 needs 2 planes (2 x 34 slots); per 32-site word 3 LOP3/SHF for the two-pair eligibility, 1 for the
+# acceptance, 2 for the flips of sx (the sy flips are memory operations); 2 passes per MCS over Lx Ly / 256 supergroups
+ALU_SLOTS_PER_SU["2d-1024"] = 2 * (2 * 34 + 8 * 6) / 256
 for _L in (512, 1024, 2048, 4096, 8192, 16384, 32768):   # the paper's size scan: same rates and schedule as paper-1024x30
     ALU_SLOTS_PER_SU[f"paper-scan-{_L}"] = ALU_SLOTS_PER_SU["paper-1024x30"]
 # default run: the headline first, then the other BASELINE configs and the auxiliary streamed runs of SURVEY §8(d)
@@ -181,6 +185,9 @@ def _oracle_sim(cfg, nsamples, first_sample=0):
                           cfg["omega"], seed=cfg["seed"], first_sample=first_sample,
                           offset_mode=cfg.get("offset_mode", 0), w_unflagged=cfg.get("w_unflagged"),
                           independent=cfg.get("independent", 0))
+    if cfg["kind"] == "kpz2d":
+        return R.Kpz2dRef(cfg["Lx"], cfg["Ly"], nsamples, cfg["p"], cfg["q"], seed=cfg["seed"], first_sample=first_sample,
+                          offset_mode=cfg.get("offset_mode", 0))
     return R.KpzRef(cfg["L"], nsamples, cfg["p"], cfg["q"], disorder=cfg["disorder"], seed=cfg["seed"],
                     first_sample=first_sample, offset_mode=cfg.get("offset_mode", 0))
 
@@ -188,6 +195,8 @@ def _oracle_sim(cfg, nsamples, first_sample=0):
 def oracle_sample_shape(cfg, target_su):
     """A bounded sample of the workload: whole samples first, then a prefix of the MCS; about target_su site updates."""
     per_mcs = (2 if cfg["kind"] == "lanes" else 1) * cfg["L"]
+    if cfg["kind"] == "kpz2d":
+        target_su //= 10   # the 2+1D oracle assembles every uniform on its own (32 Philox calls per site): ~2 MSU/s
     n_mcs = int(max(1, min(cfg["n_mcs"], target_su // per_mcs)))
     nsamp = int(max(1, min(cfg["S"], target_su // (per_mcs * n_mcs))))
     return nsamp, n_mcs
@@ -244,6 +253,9 @@ def make_sim(pkg, cfg, first_sample):
                            cfg["omega"], seed=cfg["seed"], first_sample=first_sample, max_records=nrec,
                            offset_mode=cfg.get("offset_mode", 0), w_unflagged=cfg.get("w_unflagged"),
                            independent=cfg.get("independent", 0))
+    elif cfg["kind"] == "kpz2d":
+        sim = pkg.Kpz2dSim(cfg["Lx"], cfg["Ly"], cfg["S"], cfg["p"], cfg["q"], seed=cfg["seed"], first_sample=first_sample,
+                           max_records=nrec, offset_mode=cfg.get("offset_mode", 0))
     else:
         sim = pkg.KpzSim(cfg["L"], cfg["S"], cfg["p"], cfg["q"], disorder=cfg["disorder"], seed=cfg["seed"],
                          first_sample=first_sample, max_records=nrec, path=cfg.get("path", 0),
@@ -341,6 +353,7 @@ def bench_one(ctx, args, cfg_key, with_cpu):
     value = world * su_step * args.steps / (ms_total * 1e-3) / 1e9
     e2e = time_e2e(ctx, args, cfg, sim, n_mcs, su_step)
     path = sim.path if cfg["kind"] == "kpz" else 1
+    path_name = {"kpz": PATH_NAMES.get(path), "lanes": "two-lane K4", "kpz2d": "2+1D checkerboard K5 (one launch per colour pass)"}[cfg["kind"]]
     ms_run = ms_run_total / args.steps
     roof = roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run)
     cpu = None
@@ -357,7 +370,7 @@ def bench_one(ctx, args, cfg_key, with_cpu):
                                                       and args.samples is None) else None,
         "config": {"workload": cfg["name"], "config_key": str(cfg_key), "L": cfg["L"], "samples_per_gpu": cfg["S"],
                    "n_mcs": n_mcs, "records": len(cfg["record_times"]),
-                   "path": PATH_NAMES[path] if cfg["kind"] == "kpz" else "two-lane K4",
+                   "path": path_name,
                    "l2": "flushed between timed steps (256 MiB fill)", "parallelism": f"samples x{world}"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
         "wall_s_timed_region": wall,
@@ -394,6 +407,37 @@ def time_e2e(ctx, args, cfg, sim, n_mcs, su_step):
         rec_bytes = int(rec["sum_h"].nbytes + rec["sum_h2"].nbytes)
         return {"value": ctx.world * su_step * args.steps / dt / 1e9, "unit": UNIT,
                 "h2d_bytes_per_step": int(h_in.numel() * 4), "d2h_bytes_per_step": int(h_out.numel() * 4) + rec_bytes}
+
+    if cfg["kind"] == "kpz2d":
+        import numpy as np
+        rw, Ly = cfg["Lx"] // 32, cfg["Ly"]
+        flat = np.empty((cfg["S"], Ly, rw), dtype=np.uint32)
+        flat[:, 0::2, :] = 0xAAAAAAAA
+        flat[:, 1::2, :] = 0x55555555
+        h_in = torch.from_numpy(flat.view(np.int32)).pin_memory()
+        h_out = [torch.empty((cfg["S"], Ly, rw), dtype=torch.int32).pin_memory() for _ in range(2)]
+        d_in = torch.empty((cfg["S"], Ly, rw), dtype=torch.int32, device=ctx.dev)
+
+        def e2e_step2d():
+            sim.reset()
+            d_in.copy_(h_in, non_blocking=True)
+            sim.set_slopes(d_in, d_in)
+            sim.run(n_mcs)
+            sx, sy = sim.slopes()
+            h_out[0].copy_(sx, non_blocking=True)
+            h_out[1].copy_(sy, non_blocking=True)
+            return sim.roughness()        # syncs; records -> host
+
+        e2e_step2d()
+        ctx.barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            rec = e2e_step2d()
+        ctx.barrier()
+        dt, = ctx.max_over_ranks([time.perf_counter() - t0])
+        rec_bytes = int(rec["sum_h"].nbytes + rec["sum_h2"].nbytes)
+        return {"value": ctx.world * su_step * args.steps / dt / 1e9, "unit": UNIT,
+                "h2d_bytes_per_step": int(h_in.numel() * 4), "d2h_bytes_per_step": int(2 * h_in.numel() * 4) + rec_bytes}
 
     def e2e_step():
         sim.reset()
@@ -445,7 +489,7 @@ def roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run):
                 "peak_source": peaks["source"], "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
     slots = ALU_SLOTS_PER_SU.get(cfg_key)
     kname = {1: "kpz_k1_sweep_jit", 3: "kpz_k3t_sweep_jit"}.get(path, "kpz_k1_sweep_jit") if cfg["kind"] == "kpz" \
-        else "lanes_k4_sweep_jit"
+        else ("k2d_pass" if cfg["kind"] == "kpz2d" else "lanes_k4_sweep_jit")
     if slots is None:
         return {"bound": "alu", "kernel": kname, "achieved": None, "peak": None, "unit": "Tslot/s", "frac": None,
                 "traffic": traffic, "reason": f"no algorithmic slot count is modelled for workload key {cfg_key!r}"}

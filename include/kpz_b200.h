@@ -169,6 +169,34 @@ int lanes_currents(lanes_sim*, int32_t* nt, int64_t* t, int64_t* j_a, int64_t* j
 int lanes_profile(lanes_sim*, uint32_t* d_occ_a, uint32_t* d_occ_b, int64_t* nsnap);
 int lanes_destroy(lanes_sim*); /* as kpz_destroy: host-side handle only */
 
+/* ---- 2+1D generalisation ------------------------------------- */
+/* "We used two-sub-lattice updates, which can be generalized to checker-board lattice decomposition in two dimensions"
+ * (PAPER.md:289), towards the 2+1D simulations of refs. [7, 28]: the dimer / octahedron move on a periodic
+ * Lx x Ly lattice.  Slopes as bits, sx[y][x] = 1 iff h(x,y) - h(x-1,y) = +1, sy[y][x] = 1 iff h(x,y) - h(x,y-1) = +1; site
+ * (x,y) moves forward with probability p when its x-pair (sx[y][x], sx[y][x+1]) and its y-pair (sy[y][x], sy[y+1][x]) are
+ * both (1,0) - both become (0,1) - and backward with q when both are (0,1).  One MCS = two colour passes of the
+ * checkerboard, sites with (x + y + o) even, o drawn per pass as in the 1+1D sweep (or o = pass with offset_mode 1); the
+ * j-th active site of row y draws element y * Lx/2 + j of stream PAIR.  Flat start h = (x + y) & 1.
+ * Layout of every slope buffer (device): [nsamples][Ly][Lx/32] uint32, bit (x & 31) of word x >> 5 of row y.
+ * Lx a multiple of 64, Ly even, Lx, Ly <= 32768, Lx * Ly <= 2^30.  Ownership, streams and error codes as above. */
+typedef struct kpz2d_sim kpz2d_sim;
+int kpz2d_workspace_bytes(int32_t Lx, int32_t Ly, int32_t nsamples, int32_t max_records, size_t* bytes);
+int kpz2d_create(kpz2d_sim** out, int32_t Lx, int32_t Ly, int32_t nsamples, double p, double q, uint64_t seed,
+                 const kpz_options* opt /* first_sample, offset_mode; path ignored */, int32_t max_records, void* d_workspace,
+                 size_t workspace_bytes, void* cuda_stream);
+int kpz2d_set_record_times(kpz2d_sim*, const int64_t* t, int32_t nt); /* as kpz_set_record_times */
+/* n_mcs checkerboard sweeps (two kernel launches per MCS, in place); captures (sum h, sum h^2) over the Lx * Ly heights
+ * h(x,0) = sum_{i<=x} (2 sx[0][i] - 1), h(x,y) = h(x,y-1) + 2 sy[y][x] - 1 at the record times.  Asynchronous. */
+int kpz2d_run(kpz2d_sim*, int64_t n_mcs);
+int kpz2d_time(const kpz2d_sim*, int64_t* t);
+int kpz2d_reset(kpz2d_sim*);                                          /* flat surface, t = 0, records dropped; async */
+int kpz2d_slopes(kpz2d_sim*, uint32_t* d_sx, uint32_t* d_sy);        /* copy out (either may be NULL); async */
+int kpz2d_set_slopes(kpz2d_sim*, const uint32_t* d_sx, const uint32_t* d_sy);
+int kpz2d_heights(kpz2d_sim*, int32_t sample, int32_t* d_h /* [Ly][Lx] int32, device */);
+/* As kpz_roughness: W^2 over the Lx * Ly sites of a sample (Eq. 3), mean over samples.  SYNCS. */
+int kpz2d_roughness(kpz2d_sim*, int32_t* nt, int64_t* t, int64_t* sum_h, int64_t* sum_h2, double* w2_mean);
+int kpz2d_destroy(kpz2d_sim*);
+
 /* ---- diagnostics ------------------------------------------------------------------------------------------ */
 /* Text of an error code.  The paper's programs report nothing of the kind; this serves the "no exception or abort
  * crosses the ABI" rule of SURVEY §8(b). */

@@ -80,6 +80,18 @@ SIGNATURES = {
     "lanes_currents": (C.c_int, [_P, C.POINTER(C.c_int32), _P, _P, _P, _P, _P]),
     "lanes_profile": (C.c_int, [_P, _P, _P, C.POINTER(C.c_int64)]),
     "lanes_destroy": (C.c_int, [_P]),
+    "kpz2d_workspace_bytes": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]),
+    "kpz2d_create": (C.c_int, [C.POINTER(_P), C.c_int32, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_uint64,
+                               C.POINTER(Options), C.c_int32, _P, C.c_size_t, _P]),
+    "kpz2d_set_record_times": (C.c_int, [_P, C.POINTER(C.c_int64), C.c_int32]),
+    "kpz2d_run": (C.c_int, [_P, C.c_int64]),
+    "kpz2d_time": (C.c_int, [_P, C.POINTER(C.c_int64)]),
+    "kpz2d_reset": (C.c_int, [_P]),
+    "kpz2d_slopes": (C.c_int, [_P, _P, _P]),
+    "kpz2d_set_slopes": (C.c_int, [_P, _P, _P]),
+    "kpz2d_heights": (C.c_int, [_P, C.c_int32, _P]),
+    "kpz2d_roughness": (C.c_int, [_P, C.POINTER(C.c_int32), _P, _P, _P, _P]),
+    "kpz2d_destroy": (C.c_int, [_P]),
     "kpz_strerror": (C.c_char_p, [C.c_int]),
     "kpz_last_error": (C.c_char_p, []),
     "kpz_kernel_launches": (C.c_int64, []),
@@ -290,6 +302,85 @@ class KpzSim:
         w2 = np.zeros(cap, dtype=np.float64)
         _chk(load_library().kpz_roughness(self._h, C.byref(nt), t.ctypes.data, s1.ctypes.data, s2.ctypes.data,
                                           w2.ctypes.data), "kpz_roughness")
+        k = nt.value
+        return dict(t=t[:k], sum_h=s1[:k], sum_h2=s2[:k], w2_mean=w2[:k])
+
+
+class Kpz2dSim:
+    """kpz2d_create / kpz2d_run / kpz2d_heights / kpz2d_roughness (the 2+1D generalisation) on the current
+    CUDA device and stream.  Argument marshalling only."""
+
+    def __init__(self, Lx, Ly, nsamples, p, q, seed=0, first_sample=0, offset_mode=0, max_records=64):
+        _require_cuda()
+        lib = load_library()
+        self.Lx, self.Ly, self.S = int(Lx), int(Ly), int(nsamples)
+        self.rw = self.Lx // 32
+        self.max_records = int(max_records)
+        self.device = torch.device("cuda", torch.cuda.current_device())
+        self._o = Options(int(first_sample), int(offset_mode), 0)
+        nbytes = C.c_size_t()
+        _chk(lib.kpz2d_workspace_bytes(self.Lx, self.Ly, self.S, self.max_records, C.byref(nbytes)), "kpz2d_workspace_bytes")
+        self.workspace = torch.empty(nbytes.value + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) // 256 * 256
+        self._h = C.c_void_p()
+        _chk(lib.kpz2d_create(C.byref(self._h), self.Lx, self.Ly, self.S, float(p), float(q), int(seed), C.byref(self._o),
+                              self.max_records, C.c_void_p(base), nbytes.value, _stream_ptr()), "kpz2d_create")
+        self._nt = 0
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load_library().kpz2d_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def time(self):
+        t = C.c_int64()
+        _chk(load_library().kpz2d_time(self._h, C.byref(t)), "kpz2d_time")
+        return int(t.value)
+
+    def set_record_times(self, t):
+        t = _times(t)
+        self._nt = len(t)
+        _chk(load_library().kpz2d_set_record_times(self._h, t.ctypes.data_as(C.POINTER(C.c_int64)), len(t)),
+             "kpz2d_set_record_times")
+
+    def run(self, n_mcs):
+        _chk(load_library().kpz2d_run(self._h, int(n_mcs)), "kpz2d_run")
+
+    def reset(self):
+        _chk(load_library().kpz2d_reset(self._h), "kpz2d_reset")
+
+    def slopes(self):
+        """(sx, sy): device tensors [S][Ly][Lx/32] (int32 storage of the uint32 words)."""
+        sx = torch.empty((self.S, self.Ly, self.rw), dtype=torch.int32, device=self.device)
+        sy = torch.empty_like(sx)
+        _chk(load_library().kpz2d_slopes(self._h, _dptr(sx), _dptr(sy)), "kpz2d_slopes")
+        return sx, sy
+
+    def set_slopes(self, sx, sy):
+        assert sx.is_cuda and sx.is_contiguous() and sx.numel() == self.S * self.Ly * self.rw and sy.numel() == sx.numel()
+        _chk(load_library().kpz2d_set_slopes(self._h, _dptr(sx), _dptr(sy)), "kpz2d_set_slopes")
+
+    def heights(self, sample):
+        out = torch.empty((self.Ly, self.Lx), dtype=torch.int32, device=self.device)
+        _chk(load_library().kpz2d_heights(self._h, int(sample), _dptr(out)), "kpz2d_heights")
+        return out
+
+    def roughness(self):
+        cap = max(self._nt, 1)
+        nt = C.c_int32(cap)
+        t = np.zeros(cap, dtype=np.int64)
+        s1 = np.zeros((cap, self.S), dtype=np.int64)
+        s2 = np.zeros((cap, self.S), dtype=np.int64)
+        w2 = np.zeros(cap, dtype=np.float64)
+        _chk(load_library().kpz2d_roughness(self._h, C.byref(nt), t.ctypes.data, s1.ctypes.data, s2.ctypes.data,
+                                            w2.ctypes.data), "kpz2d_roughness")
         k = nt.value
         return dict(t=t[:k], sum_h=s1[:k], sum_h2=s2[:k], w2_mean=w2[:k])
 

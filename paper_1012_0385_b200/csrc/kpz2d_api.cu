@@ -1,0 +1,269 @@
+// kpz2d_api.cu — host side of the 2+1D generalisation: the kpz2d_* entry
+// points of include/kpz_b200.h.  Validation, workspace carving, kernel launches; every step of the path runs in the
+// kernels of kpz2d_k5.cuh.  No CPU fallback.
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "kpz2d_k5.cuh"
+
+using namespace kpz;
+
+struct kpz2d_sim {
+  Kpz2dDev dev{};
+  int32_t max_records = 0;
+  cudaStream_t stream = nullptr;
+  long long *rec_t = nullptr, *rec_h = nullptr, *rec_h2 = nullptr;
+  unsigned char* off = nullptr;  // [kChunkPasses][S] colour offsets of a chunk of passes
+  int64_t t = 0;
+  std::vector<int64_t> rec_times;
+  int32_t nrec = 0;
+};
+
+namespace {
+
+constexpr int kChunkPasses = 1024;
+
+int grid_for2(size_t n, int block = 256) {
+  size_t g = (n + block - 1) / block;
+  return (int)std::min<size_t>(std::max<size_t>(g, 1), 148 * 16);
+}
+
+struct Layout2d {
+  size_t off_sx, off_sy, off_rec_t, off_h, off_h2, off_off, total;
+  int RW;
+};
+
+int validate2d(int32_t Lx, int32_t Ly, int32_t S, int32_t max_records) {
+  if (Lx < 2 || Ly < 2 || (Lx & 1) || (Ly & 1) || S < 1 || max_records < 0)
+    return fail(KPZ_EINVAL, "need even Lx, Ly >= 2, nsamples >= 1, max_records >= 0");
+  if (Lx % 64 != 0) return fail(KPZ_EUNSUPPORTED, "the CUDA path needs Lx to be a multiple of 64 (Lx=%d)", Lx);
+  if (Lx > 32768 || Ly > 32768 || (int64_t)Lx * Ly > ((int64_t)1 << 30))
+    return fail(KPZ_EUNSUPPORTED, "lattice too large (Lx, Ly <= 32768, Lx * Ly <= 2^30)");
+  if ((int64_t)S * Lx * Ly / 64 > ((int64_t)1 << 31) - 8) return fail(KPZ_EUNSUPPORTED, "nsamples * Lx * Ly too large");
+  return KPZ_OK;
+}
+
+Layout2d layout2d(int32_t Lx, int32_t Ly, int32_t S, int32_t max_records) {
+  Layout2d y{};
+  y.RW = Lx / 32;
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    size_t o = off;
+    off += align_up(bytes, 256);
+    return o;
+  };
+  const size_t plane = (size_t)S * Ly * y.RW * 4;
+  y.off_sx = take(plane);
+  y.off_sy = take(plane);
+  y.off_rec_t = take((size_t)std::max(max_records, 1) * 8);
+  y.off_h = take((size_t)std::max(max_records, 1) * S * 8);
+  y.off_h2 = take((size_t)std::max(max_records, 1) * S * 8);
+  y.off_off = take((size_t)kChunkPasses * S);
+  y.total = off;
+  return y;
+}
+
+int record2d(kpz2d_sim* sim, int ri) {
+  const Kpz2dDev& D = sim->dev;
+  unsigned long long* oh = (unsigned long long*)(sim->rec_h + (size_t)ri * D.S);
+  unsigned long long* oh2 = (unsigned long long*)(sim->rec_h2 + (size_t)ri * D.S);
+  KPZ_CUDA_CHECK(cudaMemsetAsync(oh, 0, (size_t)D.S * 8, sim->stream));
+  KPZ_CUDA_CHECK(cudaMemsetAsync(oh2, 0, (size_t)D.S * 8, sim->stream));
+  const int nxb = (D.Lx + 255) / 256;
+  k2d_heights<0><<<D.S * nxb, 256, 0, sim->stream>>>(D.sx, D.sy, D.Lx, D.Ly, D.RW, nxb, oh, oh2, nullptr);
+  KPZ_LAUNCH_CHECK("k2d_heights");
+  return KPZ_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int kpz2d_workspace_bytes(int32_t Lx, int32_t Ly, int32_t nsamples, int32_t max_records, size_t* bytes) {
+  if (!bytes) return fail(KPZ_EINVAL, "bytes is NULL");
+  int rc = validate2d(Lx, Ly, nsamples, max_records);
+  if (rc) return rc;
+  *bytes = layout2d(Lx, Ly, nsamples, max_records).total;
+  return KPZ_OK;
+}
+
+int kpz2d_reset(kpz2d_sim* sim) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  const Kpz2dDev& D = sim->dev;
+  k2d_init_flat<<<grid_for2((size_t)D.S * D.Ly * D.RW), 256, 0, sim->stream>>>(D.sx, D.sy, D.S, D.Ly, D.RW);
+  KPZ_LAUNCH_CHECK("k2d_init_flat");
+  sim->t = 0;
+  sim->nrec = 0;
+  return KPZ_OK;
+}
+
+int kpz2d_create(kpz2d_sim** out, int32_t Lx, int32_t Ly, int32_t nsamples, double p, double q, uint64_t seed,
+                 const kpz_options* opt, int32_t max_records, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return fail(KPZ_EINVAL, "out is NULL");
+  *out = nullptr;
+  int rc = validate2d(Lx, Ly, nsamples, max_records);
+  if (rc) return rc;
+  if (!valid_prob(p) || !valid_prob(q)) return fail(KPZ_EINVAL, "p and q must lie in [0,1]");
+  kpz_options o{0, 0, 0};
+  if (opt) o = *opt;
+  if (o.first_sample < 0 || (o.offset_mode != 0 && o.offset_mode != 1))
+    return fail(KPZ_EINVAL, "options: first_sample >= 0, offset_mode in {0,1}");
+  if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(KPZ_EINVAL, "d_workspace must be non-NULL and 256-byte aligned");
+  const Layout2d y = layout2d(Lx, Ly, nsamples, max_records);
+  if (workspace_bytes < y.total) return fail(KPZ_ENOMEM, "workspace has %zu bytes, %zu needed", workspace_bytes, y.total);
+  kpz2d_sim* sim = new (std::nothrow) kpz2d_sim();
+  if (!sim) return fail(KPZ_ENOMEM, "host allocation failed");
+  char* base = (char*)d_workspace;
+  Kpz2dDev& D = sim->dev;
+  D.keys = make_keys(seed);
+  D.t_p = make_thresh(p);
+  D.t_q = make_thresh(q);
+  D.offset_mode = o.offset_mode;
+  D.first_sample = o.first_sample;
+  D.S = nsamples;
+  D.Lx = Lx;
+  D.Ly = Ly;
+  D.RW = y.RW;
+  D.n_ew = (int32_t)((int64_t)Lx * Ly / 64);
+  D.n_sg = (D.n_ew + 3) / 4;
+  D.sx = (uint32_t*)(base + y.off_sx);
+  D.sy = (uint32_t*)(base + y.off_sy);
+  sim->max_records = max_records;
+  sim->stream = (cudaStream_t)cuda_stream;
+  sim->rec_t = (long long*)(base + y.off_rec_t);
+  sim->rec_h = (long long*)(base + y.off_h);
+  sim->rec_h2 = (long long*)(base + y.off_h2);
+  sim->off = (unsigned char*)(base + y.off_off);
+  rc = kpz2d_reset(sim);
+  if (rc) {
+    delete sim;
+    return rc;
+  }
+  *out = sim;
+  return KPZ_OK;
+}
+
+int kpz2d_destroy(kpz2d_sim* sim) {
+  delete sim;
+  return KPZ_OK;
+}
+
+int kpz2d_time(const kpz2d_sim* sim, int64_t* t) {
+  if (!sim || !t) return fail(KPZ_EINVAL, "NULL argument");
+  *t = sim->t;
+  return KPZ_OK;
+}
+
+int kpz2d_set_record_times(kpz2d_sim* sim, const int64_t* t, int32_t nt) {
+  if (!sim || nt < 0 || (nt > 0 && !t)) return fail(KPZ_EINVAL, "bad record-time list");
+  if (nt > sim->max_records) return fail(KPZ_ENOMEM, "%d record times but max_records=%d", nt, sim->max_records);
+  for (int32_t k = 0; k < nt; ++k)
+    if (t[k] < 1 || (k == 0 ? t[k] <= sim->t : t[k] <= t[k - 1]))
+      return fail(KPZ_EINVAL, "record times must be strictly increasing and later than the current time");
+  // no overflow guard is needed: |h| <= (Lx + Ly) / 2 + 1 <= 32769 and Lx * Ly <= 2^30, so sum h^2 < 2^61
+  sim->rec_times.assign(t, t + nt);
+  sim->nrec = 0;
+  return KPZ_OK;
+}
+
+int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
+  if (!sim || n_mcs < 0) return fail(KPZ_EINVAL, "bad arguments");
+  if (((uint64_t)(sim->t + n_mcs) >> 54) != 0) return fail(KPZ_EUNSUPPORTED, "time beyond 2^54 MCS");
+  const Kpz2dDev D = sim->dev;
+  const int nt = (int)sim->rec_times.size();
+  int ri = sim->nrec;
+  const long long p_begin = 2 * (long long)sim->t, p_end = 2 * (long long)(sim->t + n_mcs);
+  const long long nthreads = (long long)D.S * D.n_sg;
+  const unsigned nblocks = (unsigned)((nthreads + 127) / 128);
+  for (long long c0 = p_begin; c0 < p_end; c0 += kChunkPasses) {
+    const int np = (int)std::min<long long>(kChunkPasses, p_end - c0);
+    k2d_offsets<<<grid_for2((size_t)np * D.S), 256, 0, sim->stream>>>(D.keys, D.first_sample, D.S, c0, np, D.offset_mode,
+                                                                    sim->off);
+    KPZ_LAUNCH_CHECK("k2d_offsets");
+    for (int k = 0; k < np; ++k) {
+      const long long gp = c0 + k;
+      const long long m = gp >> 1;
+      const int ps = (int)(gp & 1);
+      k2d_pass<<<nblocks, 128, 0, sim->stream>>>(D, sim->off + (size_t)k * D.S, m, ps);
+      KPZ_LAUNCH_CHECK("k2d_pass");
+      if (ps == 1 && ri < nt && sim->rec_times[ri] == m + 1) {
+        int rc = record2d(sim, ri);
+        if (rc) return rc;
+        ++ri;
+      }
+    }
+  }
+  sim->t += n_mcs;
+  sim->nrec = ri;
+  return KPZ_OK;
+}
+
+int kpz2d_slopes(kpz2d_sim* sim, uint32_t* d_sx, uint32_t* d_sy) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  const Kpz2dDev& D = sim->dev;
+  const size_t bytes = (size_t)D.S * D.Ly * D.RW * 4;
+  if (d_sx) KPZ_CUDA_CHECK(cudaMemcpyAsync(d_sx, D.sx, bytes, cudaMemcpyDeviceToDevice, sim->stream));
+  if (d_sy) KPZ_CUDA_CHECK(cudaMemcpyAsync(d_sy, D.sy, bytes, cudaMemcpyDeviceToDevice, sim->stream));
+  return KPZ_OK;
+}
+
+int kpz2d_set_slopes(kpz2d_sim* sim, const uint32_t* d_sx, const uint32_t* d_sy) {
+  if (!sim) return fail(KPZ_EINVAL, "NULL handle");
+  const Kpz2dDev& D = sim->dev;
+  const size_t bytes = (size_t)D.S * D.Ly * D.RW * 4;
+  if (d_sx) KPZ_CUDA_CHECK(cudaMemcpyAsync(D.sx, d_sx, bytes, cudaMemcpyDeviceToDevice, sim->stream));
+  if (d_sy) KPZ_CUDA_CHECK(cudaMemcpyAsync(D.sy, d_sy, bytes, cudaMemcpyDeviceToDevice, sim->stream));
+  return KPZ_OK;
+}
+
+int kpz2d_heights(kpz2d_sim* sim, int32_t sample, int32_t* d_h) {
+  if (!sim || !d_h || sample < 0 || sample >= sim->dev.S) return fail(KPZ_EINVAL, "bad arguments");
+  const Kpz2dDev& D = sim->dev;
+  const int nxb = (D.Lx + 255) / 256;
+  const size_t row0 = (size_t)sample * D.Ly * D.RW;
+  k2d_heights<1><<<nxb, 256, 0, sim->stream>>>(D.sx + row0, D.sy + row0, D.Lx, D.Ly, D.RW, nxb, nullptr, nullptr, d_h);
+  KPZ_LAUNCH_CHECK("k2d_heights");
+  return KPZ_OK;
+}
+
+int kpz2d_roughness(kpz2d_sim* sim, int32_t* nt, int64_t* t, int64_t* sum_h, int64_t* sum_h2, double* w2_mean) {
+  if (!sim || !nt) return fail(KPZ_EINVAL, "NULL argument");
+  if (*nt < sim->nrec) return fail(KPZ_ENOMEM, "capacity %d < %d records", *nt, sim->nrec);
+  const int32_t n = sim->nrec, S = sim->dev.S;
+  const size_t cells = (size_t)n * S;
+  std::vector<int64_t> h, h2;
+  int64_t* ph = sum_h;
+  int64_t* ph2 = sum_h2;
+  if (n > 0) {
+    if (!ph) {
+      h.resize(cells);
+      ph = h.data();
+    }
+    if (!ph2) {
+      h2.resize(cells);
+      ph2 = h2.data();
+    }
+    KPZ_CUDA_CHECK(cudaMemcpyAsync(ph, sim->rec_h, cells * 8, cudaMemcpyDeviceToHost, sim->stream));
+    KPZ_CUDA_CHECK(cudaMemcpyAsync(ph2, sim->rec_h2, cells * 8, cudaMemcpyDeviceToHost, sim->stream));
+  }
+  KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
+  const double N = (double)sim->dev.Lx * (double)sim->dev.Ly;
+  for (int32_t k = 0; k < n; ++k) {
+    if (t) t[k] = sim->rec_times[k];
+    if (w2_mean) {
+      double acc = 0.0;  // Eq. 3 squared per sample over the Lx * Ly sites, averaged over samples
+      for (int32_t s = 0; s < S; ++s) {
+        const __int128 s1 = ph[(size_t)k * S + s], s2 = ph2[(size_t)k * S + s];
+        const __int128 num = (__int128)((int64_t)sim->dev.Lx * sim->dev.Ly) * s2 - s1 * s1;
+        acc += (double)num / (N * N);
+      }
+      w2_mean[k] = acc / (double)S;
+    }
+  }
+  *nt = n;
+  return KPZ_OK;
+}
+
+}  // extern "C"

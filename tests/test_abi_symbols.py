@@ -20,7 +20,7 @@ def lib():
 def _declared_symbols():
     text = open(os.path.join(ROOT, "include", "kpz_b200.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b((?:kpz|lanes)_[a-z_0-9]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b((?:kpz2d|kpz|lanes)_[a-z_0-9]+)\s*\(", text)))
 
 
 def test_header_symbols_are_all_exported_and_bound(lib):

@@ -1,0 +1,122 @@
+"""GPU parity of the 2+1D generalisation: kernel K5 through the C ABI
+against the CPU oracle, bit for bit - slope words of both fields, int32 heights, exact sums - plus properties at a size
+the oracle cannot reach.
+
+Run on the B200 box with:  python -m pytest tests -m gpu
+"""
+import numpy as np
+import pytest
+
+import workloads
+from oracle import kpzref as R
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def K():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1012_0385_b200 as pkg
+    pkg.load_library()
+    return pkg
+
+
+def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_mode=0, start=None):
+    total = sum(chunks)
+    times = [t for t in times if t <= total]
+    ref = R.Kpz2dRef(Lx, Ly, S, p, q, seed=seed, first_sample=first_sample, offset_mode=offset_mode)
+    gpu = K.Kpz2dSim(Lx, Ly, S, p, q, seed=seed, first_sample=first_sample, offset_mode=offset_mode,
+                     max_records=max(len(times), 1))
+    if start is not None:
+        ref.set_slopes(*start)
+        gpu.set_slopes(K.words_from_numpy(start[0], gpu.device), K.words_from_numpy(start[1], gpu.device))
+    ref.set_record_times(times)
+    gpu.set_record_times(times)
+
+    def same(tag):
+        for name, g, r in zip(("sx", "sy"), gpu.slopes(), ref.slopes()):
+            assert np.array_equal(K.words_to_numpy(g), r), f"{name} differs {tag}"
+    same("initially")
+    done = 0
+    for n in chunks:
+        ref.run(n)
+        gpu.run(n)
+        done += n
+        assert gpu.time == ref.time == done
+        same(f"at t={done}")
+    g, r = gpu.roughness(), ref.roughness()
+    assert list(g["t"]) == list(r["t"]) == times
+    assert np.array_equal(g["sum_h"], r["sum_h"]) and np.array_equal(g["sum_h2"], r["sum_h2"])
+    assert np.array_equal(g["w2_mean"], r["w2_mean"]) or np.allclose(g["w2_mean"], r["w2_mean"], rtol=1e-15, atol=0)
+    for s in (0, S - 1):
+        assert np.array_equal(gpu.heights(s).cpu().numpy(), ref.heights(s)), f"heights of sample {s} differ"
+    return gpu, g
+
+
+@pytest.mark.parametrize("Lx,Ly", [(64, 2), (64, 6), (128, 64), (192, 10), (256, 256), (320, 30), (1024, 4)])
+def test_sizes_ragged_supergroups_and_tiny_lattices(K, Lx, Ly):
+    """A row of 64 sites is a quarter of a Philox supergroup, 192 / 320 sites leave ragged ones; Ly = 2 couples every row
+    to itself through the periodic y-pair."""
+    run_both_2d(K, Lx, Ly, 3, 0.75, 0.25, seed=Lx + Ly, times=[1, 3, 12], chunks=[5, 7])
+
+
+@pytest.mark.parametrize("p,q", [(1.0, 0.0), (0.0, 1.0), (0.5, 0.5), (0.9, 0.1), (0.3, 0.6), (1.0, 1.0), (0.0, 0.0), (0.8, 0.0)])
+def test_rate_classes(K, p, q):
+    run_both_2d(K, 128, 32, 2, p, q, seed=7, times=[2, 9], chunks=[9])
+
+
+def test_alternating_colours_resume_first_sample_and_rough_start(K):
+    run_both_2d(K, 128, 16, 2, 0.75, 0.25, seed=9, times=[4, 11], chunks=[3, 1, 7], offset_mode=1)
+    run_both_2d(K, 128, 16, 1, 0.75, 0.25, seed=9, times=[11], chunks=[11], first_sample=5)
+    rough = R.Kpz2dRef(64, 8, 2, 0.6, 0.4, seed=1)
+    rough.run(25)
+    run_both_2d(K, 64, 8, 2, 0.2, 0.9, seed=3, times=[6], chunks=[6], start=rough.slopes())
+
+
+def test_time_keys_beyond_32_bits_are_not_needed_but_chunks_are_crossed(K):
+    """kpz2d_run draws the colour offsets for 1024 passes (512 MCS) at a time: one run across two chunk boundaries."""
+    run_both_2d(K, 64, 4, 2, 0.75, 0.25, seed=13, times=[511, 512, 513, 1100], chunks=[1100])
+
+
+def test_workload_shape_sampled_against_solo_oracle_runs(K):
+    """The bench workload `2d-1024` in its launch configuration (all samples), shortened: first and last sample against
+    solo oracle runs, every sample single-valued."""
+    c = workloads.CONFIGS["2d-1024"]
+    n, times = 6, [1, 2, 3, 4, 5, 6]
+    gpu = K.Kpz2dSim(c["Lx"], c["Ly"], c["S"], c["p"], c["q"], seed=c["seed"], max_records=len(times))
+    gpu.set_record_times(times)
+    gpu.run(n)
+    sx, sy = [K.words_to_numpy(t) for t in gpu.slopes()]
+    r = gpu.roughness()
+    for k in (0, c["S"] - 1):
+        ref = R.Kpz2dRef(c["Lx"], c["Ly"], 1, c["p"], c["q"], seed=c["seed"], first_sample=k)
+        ref.set_record_times(times)
+        ref.run(n)
+        rx, ry = ref.slopes()
+        assert np.array_equal(sx[k], rx[0]) and np.array_equal(sy[k], ry[0])
+        rr = ref.roughness()
+        assert np.array_equal(r["sum_h"][:, k], rr["sum_h"][:, 0]) and np.array_equal(r["sum_h2"][:, k], rr["sum_h2"][:, 0])
+    bits = np.unpackbits(sx.view(np.uint8), bitorder="little").reshape(c["S"], c["Ly"], c["Lx"])
+    assert np.all(bits.sum(axis=2) == c["Lx"] // 2)                 # every row closes periodically
+    bits = np.unpackbits(sy.view(np.uint8), bitorder="little").reshape(c["S"], c["Ly"], c["Lx"])
+    assert np.all(bits.sum(axis=1) == c["Ly"] // 2)                 # every column too
+
+
+def test_growth_at_a_size_the_oracle_cannot_reach(K):
+    """2+1D KPZ (refs. [7, 28] of the paper): W^2 - 1/4 grows with an effective exponent 2 beta well below the 1+1D 2/3;
+    the exact sums of kpz2d_roughness equal a torch reduction of kpz2d_heights."""
+    L, S = 1024, 4
+    times = [2 ** k for k in range(2, 11)]
+    gpu = K.Kpz2dSim(L, L, S, 0.75, 0.0, seed=31, max_records=len(times))
+    gpu.set_record_times(times)
+    gpu.run(times[-1])
+    r = gpu.roughness()
+    h = gpu.heights(S - 1).to(torch.int64)
+    assert int(h.sum()) == r["sum_h"][-1, S - 1] and int((h * h).sum()) == r["sum_h2"][-1, S - 1]
+    w2 = r["w2_mean"] - 0.25
+    assert np.all(np.diff(w2) > 0)
+    local = np.diff(np.log(w2)) / np.diff(np.log(np.array(times, dtype=np.float64)))
+    assert np.all((local[3:] > 0.2) & (local[3:] < 0.6)), local
