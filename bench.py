@@ -79,7 +79,7 @@ ALU_SLOTS_PER_SU = {
 # 2+1D generalisation: per Philox supergroup (128 elements = the active half of 256 sites of a row) and
 # colour pass: p = 0.75 needs 2 planes (2 x 34 slots); per 32-site word 3 LOP3/SHF for the two-pair eligibility, 1 for the
 # acceptance, 2 for the flips of sx (the sy flips are memory operations); 2 passes per MCS over Lx Ly / 256 supergroups
-ALU_SLOTS_PER_SU["2d-1024"] = 2 * (2 * 34 + 8 * 6) / 256
+ALU_SLOTS_PER_SU["2d-1024"] = ALU_SLOTS_PER_SU["2d-512"] = 2 * (2 * 34 + 8 * 6) / 256
 for _L in (512, 1024, 2048, 4096, 8192, 16384, 32768):   # the paper's size scan: same rates and schedule as paper-1024x30
     ALU_SLOTS_PER_SU[f"paper-scan-{_L}"] = ALU_SLOTS_PER_SU["paper-1024x30"]
 # default run: the headline first, then the other BASELINE configs and the auxiliary streamed runs of SURVEY §8(d)
@@ -353,9 +353,11 @@ def bench_one(ctx, args, cfg_key, with_cpu):
     value = world * su_step * args.steps / (ms_total * 1e-3) / 1e9
     e2e = time_e2e(ctx, args, cfg, sim, n_mcs, su_step)
     path = sim.path if cfg["kind"] == "kpz" else 1
-    path_name = {"kpz": PATH_NAMES.get(path), "lanes": "two-lane K4", "kpz2d": "2+1D checkerboard K5 (one launch per colour pass)"}[cfg["kind"]]
+    path_name = {"kpz": PATH_NAMES.get(path), "lanes": "two-lane K4", "kpz2d": "2+1D checkerboard K5"}[cfg["kind"]]
+    if cfg["kind"] == "kpz2d":
+        path_name += " (a sample in shared memory, one launch per run)" if sim.path == 1 else " (one launch per colour pass)"
     ms_run = ms_run_total / args.steps
-    roof = roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run)
+    roof = roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run, sim_path=sim.path if cfg["kind"] == "kpz2d" else 0)
     cpu = None
     if with_cpu and ctx.rank == 0 and world == 1 and not args.no_cpu_baseline:
         nsamp, nm = oracle_sample_shape(cfg, args.cpu_su)
@@ -458,7 +460,7 @@ def time_e2e(ctx, args, cfg, sim, n_mcs, su_step):
             "note": "the two-lane initial state is generated on the device from the seed; no host input exists"}
 
 
-def roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run):
+def roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run, sim_path=0):
     """The dominant kernel against its bound.  `achieved` uses the ALGORITHMIC slots / bytes of the method
     and the device time of kpz_run / lanes_run measured in this run; `traffic` and `measured` come from the committed ncu
     capture table (one launch of the same kernel and launch shape), never from this run."""
@@ -489,7 +491,7 @@ def roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run):
                 "peak_source": peaks["source"], "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
     slots = ALU_SLOTS_PER_SU.get(cfg_key)
     kname = {1: "kpz_k1_sweep_jit", 3: "kpz_k3t_sweep_jit"}.get(path, "kpz_k1_sweep_jit") if cfg["kind"] == "kpz" \
-        else ("k2d_pass" if cfg["kind"] == "kpz2d" else "lanes_k4_sweep_jit")
+        else (("k2d_onchip" if sim_path == 1 else "k2d_pass") if cfg["kind"] == "kpz2d" else "lanes_k4_sweep_jit")
     if slots is None:
         return {"bound": "alu", "kernel": kname, "achieved": None, "peak": None, "unit": "Tslot/s", "frac": None,
                 "traffic": traffic, "reason": f"no algorithmic slot count is modelled for workload key {cfg_key!r}"}

@@ -182,13 +182,16 @@ int lanes_destroy(lanes_sim*); /* as kpz_destroy: host-side handle only (PAPER.m
 typedef struct kpz2d_sim kpz2d_sim;
 int kpz2d_workspace_bytes(int32_t Lx, int32_t Ly, int32_t nsamples, int32_t max_records, size_t* bytes);
 int kpz2d_create(kpz2d_sim** out, int32_t Lx, int32_t Ly, int32_t nsamples, double p, double q, uint64_t seed,
-                 const kpz_options* opt /* first_sample, offset_mode; path ignored */, int32_t max_records, void* d_workspace,
+                 const kpz_options* opt /* first_sample, offset_mode, path: see kpz2d_path */, int32_t max_records, void* d_workspace,
                  size_t workspace_bytes, void* cuda_stream);
 int kpz2d_set_record_times(kpz2d_sim*, const int64_t* t, int32_t nt); /* as kpz_set_record_times */
-/* n_mcs checkerboard sweeps (two kernel launches per MCS, in place); captures (sum h, sum h^2) over the Lx * Ly heights
+/* n_mcs checkerboard sweeps (see kpz2d_path); captures (sum h, sum h^2) over the Lx * Ly heights
  * h(x,0) = sum_{i<=x} (2 sx[0][i] - 1), h(x,y) = h(x,y-1) + 2 sy[y][x] - 1 at the record times.  Asynchronous. */
 int kpz2d_run(kpz2d_sim*, int64_t n_mcs);
 int kpz2d_time(const kpz2d_sim*, int64_t* t);
+/* 1 = a whole sample in shared memory, one persistent launch per kpz2d_run (auto up to 96 KiB of slopes per sample, e.g.
+ * 512 x 512; options.path = 1 forces it up to 200 KiB), 2 = one in-place launch per colour pass (options.path = 2). */
+int kpz2d_path(const kpz2d_sim*, int32_t* path);
 int kpz2d_reset(kpz2d_sim*);                                          /* flat surface, t = 0, records dropped; async */
 int kpz2d_slopes(kpz2d_sim*, uint32_t* d_sx, uint32_t* d_sy);        /* copy out (either may be NULL); async */
 int kpz2d_set_slopes(kpz2d_sim*, const uint32_t* d_sx, const uint32_t* d_sy);

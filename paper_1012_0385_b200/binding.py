@@ -86,6 +86,7 @@ SIGNATURES = {
     "kpz2d_set_record_times": (C.c_int, [_P, C.POINTER(C.c_int64), C.c_int32]),
     "kpz2d_run": (C.c_int, [_P, C.c_int64]),
     "kpz2d_time": (C.c_int, [_P, C.POINTER(C.c_int64)]),
+    "kpz2d_path": (C.c_int, [_P, C.POINTER(C.c_int32)]),
     "kpz2d_reset": (C.c_int, [_P]),
     "kpz2d_slopes": (C.c_int, [_P, _P, _P]),
     "kpz2d_set_slopes": (C.c_int, [_P, _P, _P]),
@@ -310,14 +311,14 @@ class Kpz2dSim:
     """kpz2d_create / kpz2d_run / kpz2d_heights / kpz2d_roughness (the 2+1D generalisation) on the current
     CUDA device and stream.  Argument marshalling only."""
 
-    def __init__(self, Lx, Ly, nsamples, p, q, seed=0, first_sample=0, offset_mode=0, max_records=64):
+    def __init__(self, Lx, Ly, nsamples, p, q, seed=0, first_sample=0, offset_mode=0, max_records=64, path=KPZ_PATH_AUTO):
         _require_cuda()
         lib = load_library()
         self.Lx, self.Ly, self.S = int(Lx), int(Ly), int(nsamples)
         self.rw = self.Lx // 32
         self.max_records = int(max_records)
         self.device = torch.device("cuda", torch.cuda.current_device())
-        self._o = Options(int(first_sample), int(offset_mode), 0)
+        self._o = Options(int(first_sample), int(offset_mode), int(path))
         nbytes = C.c_size_t()
         _chk(lib.kpz2d_workspace_bytes(self.Lx, self.Ly, self.S, self.max_records, C.byref(nbytes)), "kpz2d_workspace_bytes")
         self.workspace = torch.empty(nbytes.value + 256, dtype=torch.uint8, device=self.device)
@@ -337,6 +338,12 @@ class Kpz2dSim:
             self.close()
         except Exception:
             pass
+
+    @property
+    def path(self):
+        p = C.c_int32()
+        _chk(load_library().kpz2d_path(self._h, C.byref(p)), "kpz2d_path")
+        return int(p.value)
 
     @property
     def time(self):

@@ -12,6 +12,7 @@ using namespace kpz;
 
 struct kpz2d_sim {
   Kpz2dDev dev{};
+  int path = KPZ_PATH_STREAM;  // KPZ_PATH_ONCHIP: a sample in shared memory (k2d_onchip), else one launch per pass
   int32_t max_records = 0;
   cudaStream_t stream = nullptr;
   long long *rec_t = nullptr, *rec_h = nullptr, *rec_h2 = nullptr;
@@ -24,6 +25,19 @@ struct kpz2d_sim {
 namespace {
 
 constexpr int kChunkPasses = 1024;
+constexpr size_t kOnchipBytes = 96 * 1024;  // both slope fields of a sample in shared memory, two CTAs per SM
+
+// options.path: 0 auto (on chip when the sample fits), 1 on chip (k2d_onchip), 2 streamed (k2d_pass per colour pass)
+int choose_path2d(int32_t Lx, int32_t Ly, const kpz_options* opt, int* path) {
+  const size_t bytes = (size_t)2 * Ly * (Lx / 32 + Lx / 256) * 4;  // padded rows, see k2d_onchip
+  int want = opt ? opt->path : KPZ_PATH_AUTO;
+  if (want == KPZ_PATH_AUTO) want = bytes <= kOnchipBytes ? KPZ_PATH_ONCHIP : KPZ_PATH_STREAM;
+  if (want == KPZ_PATH_ONCHIP && bytes > 200 * 1024)
+    return fail(KPZ_EUNSUPPORTED, "the on-chip 2+1D path holds at most 200 KiB of slopes per sample (%zu needed)", bytes);
+  if (want != KPZ_PATH_ONCHIP && want != KPZ_PATH_STREAM) return fail(KPZ_EINVAL, "options.path must be 0, 1 or 2 here");
+  *path = want;
+  return KPZ_OK;
+}
 
 int grid_for2(size_t n, int block = 256) {
   size_t g = (n + block - 1) / block;
@@ -110,6 +124,9 @@ int kpz2d_create(kpz2d_sim** out, int32_t Lx, int32_t Ly, int32_t nsamples, doub
   if (opt) o = *opt;
   if (o.first_sample < 0 || (o.offset_mode != 0 && o.offset_mode != 1))
     return fail(KPZ_EINVAL, "options: first_sample >= 0, offset_mode in {0,1}");
+  int path;
+  rc = choose_path2d(Lx, Ly, &o, &path);
+  if (rc) return rc;
   if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(KPZ_EINVAL, "d_workspace must be non-NULL and 256-byte aligned");
   const Layout2d y = layout2d(Lx, Ly, nsamples, max_records);
   if (workspace_bytes < y.total) return fail(KPZ_ENOMEM, "workspace has %zu bytes, %zu needed", workspace_bytes, y.total);
@@ -131,6 +148,7 @@ int kpz2d_create(kpz2d_sim** out, int32_t Lx, int32_t Ly, int32_t nsamples, doub
   D.sx = (uint32_t*)(base + y.off_sx);
   D.sy = (uint32_t*)(base + y.off_sy);
   sim->max_records = max_records;
+  sim->path = path;
   sim->stream = (cudaStream_t)cuda_stream;
   sim->rec_t = (long long*)(base + y.off_rec_t);
   sim->rec_h = (long long*)(base + y.off_h);
@@ -165,6 +183,16 @@ int kpz2d_set_record_times(kpz2d_sim* sim, const int64_t* t, int32_t nt) {
   // no overflow guard is needed: |h| <= (Lx + Ly) / 2 + 1 <= 32769 and Lx * Ly <= 2^30, so sum h^2 < 2^61
   sim->rec_times.assign(t, t + nt);
   sim->nrec = 0;
+  if (nt > 0) {
+    KPZ_CUDA_CHECK(cudaMemcpyAsync(sim->rec_t, sim->rec_times.data(), (size_t)nt * 8, cudaMemcpyHostToDevice, sim->stream));
+    KPZ_CUDA_CHECK(cudaStreamSynchronize(sim->stream));
+  }
+  return KPZ_OK;
+}
+
+int kpz2d_path(const kpz2d_sim* sim, int32_t* path) {
+  if (!sim || !path) return fail(KPZ_EINVAL, "NULL argument");
+  *path = sim->path;
   return KPZ_OK;
 }
 
@@ -174,6 +202,24 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
   const Kpz2dDev D = sim->dev;
   const int nt = (int)sim->rec_times.size();
   int ri = sim->nrec;
+  if (n_mcs == 0) return KPZ_OK;
+  if (sim->path == KPZ_PATH_ONCHIP) {
+    Kpz2dRun A{};
+    A.t0 = sim->t;
+    A.n_mcs = n_mcs;
+    A.rec_t = sim->rec_t;
+    A.rec_begin = ri;
+    A.nt = nt;
+    A.rec_h = sim->rec_h;
+    A.rec_h2 = sim->rec_h2;
+    const size_t smem = (size_t)4 * D.Ly * (D.RW / 2 + D.RW / 8) * 4;  // 4 parity planes, one pad word per 4 words
+    KPZ_CUDA_CHECK(cudaFuncSetAttribute(k2d_onchip, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k2d_onchip<<<D.S, kK5SThreads, smem, sim->stream>>>(D, A);
+    KPZ_LAUNCH_CHECK("k2d_onchip");
+    sim->t += n_mcs;
+    while (sim->nrec < nt && sim->rec_times[sim->nrec] <= sim->t) sim->nrec++;
+    return KPZ_OK;
+  }
   const long long p_begin = 2 * (long long)sim->t, p_end = 2 * (long long)(sim->t + n_mcs);
   const long long nthreads = (long long)D.S * D.n_sg;
   const unsigned nblocks = (unsigned)((nthreads + 127) / 128);

@@ -24,12 +24,14 @@ def K():
     return pkg
 
 
-def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_mode=0, start=None):
+def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_mode=0, start=None, path=0):
     total = sum(chunks)
     times = [t for t in times if t <= total]
     ref = R.Kpz2dRef(Lx, Ly, S, p, q, seed=seed, first_sample=first_sample, offset_mode=offset_mode)
     gpu = K.Kpz2dSim(Lx, Ly, S, p, q, seed=seed, first_sample=first_sample, offset_mode=offset_mode,
-                     max_records=max(len(times), 1))
+                     max_records=max(len(times), 1), path=path)
+    if path:
+        assert gpu.path == path
     if start is not None:
         ref.set_slopes(*start)
         gpu.set_slopes(K.words_from_numpy(start[0], gpu.device), K.words_from_numpy(start[1], gpu.device))
@@ -56,35 +58,60 @@ def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_
     return gpu, g
 
 
+PATHS = [1, 2]   # 1 = a sample in shared memory (k2d_onchip), 2 = one launch per colour pass (k2d_pass)
+
+
+@pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("Lx,Ly", [(64, 2), (64, 6), (128, 64), (192, 10), (256, 256), (320, 30), (1024, 4)])
-def test_sizes_ragged_supergroups_and_tiny_lattices(K, Lx, Ly):
+def test_sizes_ragged_supergroups_and_tiny_lattices(K, Lx, Ly, path):
     """A row of 64 sites is a quarter of a Philox supergroup, 192 / 320 sites leave ragged ones; Ly = 2 couples every row
-    to itself through the periodic y-pair."""
-    run_both_2d(K, Lx, Ly, 3, 0.75, 0.25, seed=Lx + Ly, times=[1, 3, 12], chunks=[5, 7])
+    to itself through the periodic y-pair; 256 x 256 gives the 512 threads of the on-chip kernel one supergroup each."""
+    run_both_2d(K, Lx, Ly, 3, 0.75, 0.25, seed=Lx + Ly, times=[1, 3, 12], chunks=[5, 7], path=path)
 
 
+@pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("p,q", [(1.0, 0.0), (0.0, 1.0), (0.5, 0.5), (0.9, 0.1), (0.3, 0.6), (1.0, 1.0), (0.0, 0.0), (0.8, 0.0)])
-def test_rate_classes(K, p, q):
-    run_both_2d(K, 128, 32, 2, p, q, seed=7, times=[2, 9], chunks=[9])
+def test_rate_classes(K, p, q, path):
+    run_both_2d(K, 128, 32, 2, p, q, seed=7, times=[2, 9], chunks=[9], path=path)
 
 
-def test_alternating_colours_resume_first_sample_and_rough_start(K):
-    run_both_2d(K, 128, 16, 2, 0.75, 0.25, seed=9, times=[4, 11], chunks=[3, 1, 7], offset_mode=1)
-    run_both_2d(K, 128, 16, 1, 0.75, 0.25, seed=9, times=[11], chunks=[11], first_sample=5)
+@pytest.mark.parametrize("path", PATHS)
+def test_alternating_colours_resume_first_sample_and_rough_start(K, path):
+    run_both_2d(K, 128, 16, 2, 0.75, 0.25, seed=9, times=[4, 11], chunks=[3, 1, 7], offset_mode=1, path=path)
+    run_both_2d(K, 128, 16, 1, 0.75, 0.25, seed=9, times=[11], chunks=[11], first_sample=5, path=path)
     rough = R.Kpz2dRef(64, 8, 2, 0.6, 0.4, seed=1)
     rough.run(25)
-    run_both_2d(K, 64, 8, 2, 0.2, 0.9, seed=3, times=[6], chunks=[6], start=rough.slopes())
+    run_both_2d(K, 64, 8, 2, 0.2, 0.9, seed=3, times=[6], chunks=[6], start=rough.slopes(), path=path)
 
 
-def test_time_keys_beyond_32_bits_are_not_needed_but_chunks_are_crossed(K):
-    """kpz2d_run draws the colour offsets for 1024 passes (512 MCS) at a time: one run across two chunk boundaries."""
-    run_both_2d(K, 64, 4, 2, 0.75, 0.25, seed=13, times=[511, 512, 513, 1100], chunks=[1100])
+@pytest.mark.parametrize("path", PATHS)
+def test_offset_batches_and_chunks_are_crossed(K, path):
+    """kpz2d_run draws the colour offsets for 1024 passes (512 MCS) at a time on the streamed path, for 16 MCS at a time in
+    the on-chip kernel: one run across those boundaries, records on and around them."""
+    run_both_2d(K, 64, 4, 2, 0.75, 0.25, seed=13, times=[15, 16, 17, 511, 512, 513, 1100], chunks=[1100], path=path)
 
 
-def test_workload_shape_sampled_against_solo_oracle_runs(K):
-    """The bench workload `2d-1024` in its launch configuration (all samples), shortened: first and last sample against
-    solo oracle runs, every sample single-valued."""
-    c = workloads.CONFIGS["2d-1024"]
+def test_path_selection_and_both_paths_agree_at_512(K):
+    a = K.Kpz2dSim(512, 512, 2, 0.75, 0.0, seed=5, max_records=1)
+    assert a.path == K.KPZ_PATH_ONCHIP                             # 64 KiB of slopes per sample
+    b = K.Kpz2dSim(512, 512, 2, 0.75, 0.0, seed=5, max_records=1, path=K.KPZ_PATH_STREAM)
+    assert K.Kpz2dSim(1024, 1024, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ_PATH_STREAM
+    with pytest.raises(K.KpzError):
+        K.Kpz2dSim(2048, 2048, 1, 0.75, 0.0, seed=5, max_records=1, path=K.KPZ_PATH_ONCHIP)
+    for g in (a, b):
+        g.set_record_times([40])
+        g.run(40)
+    for x, y in zip(a.slopes(), b.slopes()):
+        assert torch.equal(x, y)
+    ra, rb = a.roughness(), b.roughness()
+    assert np.array_equal(ra["sum_h"], rb["sum_h"]) and np.array_equal(ra["sum_h2"], rb["sum_h2"])
+
+
+@pytest.mark.parametrize("key", ["2d-512", "2d-1024"])
+def test_workload_shape_sampled_against_solo_oracle_runs(K, key):
+    """The bench workloads `2d-512` (on chip) and `2d-1024` (streamed) in their launch configuration (all samples),
+    shortened: first and last sample against solo oracle runs, every sample single-valued."""
+    c = workloads.CONFIGS[key]
     n, times = 6, [1, 2, 3, 4, 5, 6]
     gpu = K.Kpz2dSim(c["Lx"], c["Ly"], c["S"], c["p"], c["q"], seed=c["seed"], max_records=len(times))
     gpu.set_record_times(times)

@@ -98,6 +98,8 @@ CONFIGS = {
 
 # the 2+1D generalisation: 64 independent 1024 x 1024 surfaces of the dimer
 # / octahedron model, p = 0.75, q = 0, 1000 MCS, 20 log-spaced record times.  "site updates" = Lx * Ly per MCS and sample.
+CONFIGS["2d-512"] = dict(name="kpz2d_L512x512_S256_p075", kind="kpz2d", Lx=512, Ly=512, L=512 * 512, S=256, p=0.75, q=0.0,
+                         n_mcs=1000, record_times=_T20_1E3, seed=12)   # a sample (64 KiB of slopes) stays in shared memory
 CONFIGS["2d-1024"] = dict(name="kpz2d_L1024x1024_S64_p075", kind="kpz2d", Lx=1024, Ly=1024, L=1024 * 1024, S=64, p=0.75,
                           q=0.0, n_mcs=1000, record_times=_T20_1E3, seed=12)
 
