@@ -29,7 +29,7 @@ constexpr size_t kOnchipBytes = 96 * 1024;  // both slope fields of a sample in 
 
 // options.path: 0 auto (on chip when the sample fits), 1 on chip (k2d_onchip), 2 streamed (k2d_pass per colour pass)
 int choose_path2d(int32_t Lx, int32_t Ly, const kpz_options* opt, int* path) {
-  const size_t bytes = (size_t)2 * Ly * (Lx / 32 + Lx / 256) * 4;  // padded rows, see k2d_onchip
+  const size_t bytes = (size_t)4 * Ly * (Lx / 64 + Lx / 256) * 4;  // 4 parity planes with padded rows, see k2d_onchip
   int want = opt ? opt->path : KPZ_PATH_AUTO;
   if (want == KPZ_PATH_AUTO) want = bytes <= kOnchipBytes ? KPZ_PATH_ONCHIP : KPZ_PATH_STREAM;
   if (want == KPZ_PATH_ONCHIP && bytes > 200 * 1024)
@@ -45,8 +45,8 @@ int grid_for2(size_t n, int block = 256) {
 }
 
 struct Layout2d {
-  size_t off_sx, off_sy, off_rec_t, off_h, off_h2, off_off, total;
-  int RW;
+  size_t off_EX, off_OX, off_EY, off_OY, off_rec_t, off_h, off_h2, off_off, total;
+  int RH;
 };
 
 int validate2d(int32_t Lx, int32_t Ly, int32_t S, int32_t max_records) {
@@ -61,16 +61,18 @@ int validate2d(int32_t Lx, int32_t Ly, int32_t S, int32_t max_records) {
 
 Layout2d layout2d(int32_t Lx, int32_t Ly, int32_t S, int32_t max_records) {
   Layout2d y{};
-  y.RW = Lx / 32;
+  y.RH = Lx / 64;
   size_t off = 0;
   auto take = [&](size_t bytes) {
     size_t o = off;
     off += align_up(bytes, 256);
     return o;
   };
-  const size_t plane = (size_t)S * Ly * y.RW * 4;
-  y.off_sx = take(plane);
-  y.off_sy = take(plane);
+  const size_t plane = (size_t)S * Ly * y.RH * 4;  // one parity plane of one slope field
+  y.off_EX = take(plane);
+  y.off_OX = take(plane);
+  y.off_EY = take(plane);
+  y.off_OY = take(plane);
   y.off_rec_t = take((size_t)std::max(max_records, 1) * 8);
   y.off_h = take((size_t)std::max(max_records, 1) * S * 8);
   y.off_h2 = take((size_t)std::max(max_records, 1) * S * 8);
@@ -79,6 +81,10 @@ Layout2d layout2d(int32_t Lx, int32_t Ly, int32_t S, int32_t max_records) {
   return y;
 }
 
+// both thresholds depend on their two leading bit-planes at most (p = 0.75, 0.5, 0.25, 0, 1 ...): the kernels then draw
+// those two planes unconditionally
+bool two_planes(const Kpz2dDev& D) { return planes_needed(D.t_p) <= 2 && planes_needed(D.t_q) <= 2; }
+
 int record2d(kpz2d_sim* sim, int ri) {
   const Kpz2dDev& D = sim->dev;
   unsigned long long* oh = (unsigned long long*)(sim->rec_h + (size_t)ri * D.S);
@@ -86,7 +92,7 @@ int record2d(kpz2d_sim* sim, int ri) {
   KPZ_CUDA_CHECK(cudaMemsetAsync(oh, 0, (size_t)D.S * 8, sim->stream));
   KPZ_CUDA_CHECK(cudaMemsetAsync(oh2, 0, (size_t)D.S * 8, sim->stream));
   const int nxb = (D.Lx + 255) / 256;
-  k2d_heights<0><<<D.S * nxb, 256, 0, sim->stream>>>(D.sx, D.sy, D.Lx, D.Ly, D.RW, nxb, oh, oh2, nullptr);
+  k2d_heights<0><<<D.S * nxb, 256, 0, sim->stream>>>(D.EX, D.OX, D.EY, D.OY, D.Lx, D.Ly, D.RH, nxb, oh, oh2, nullptr);
   KPZ_LAUNCH_CHECK("k2d_heights");
   return KPZ_OK;
 }
@@ -106,7 +112,7 @@ int kpz2d_workspace_bytes(int32_t Lx, int32_t Ly, int32_t nsamples, int32_t max_
 int kpz2d_reset(kpz2d_sim* sim) {
   if (!sim) return fail(KPZ_EINVAL, "NULL handle");
   const Kpz2dDev& D = sim->dev;
-  k2d_init_flat<<<grid_for2((size_t)D.S * D.Ly * D.RW), 256, 0, sim->stream>>>(D.sx, D.sy, D.S, D.Ly, D.RW);
+  k2d_init_flat<<<grid_for2((size_t)D.S * D.Ly * D.RH), 256, 0, sim->stream>>>(D.EX, D.OX, D.EY, D.OY, D.S, D.Ly, D.RH);
   KPZ_LAUNCH_CHECK("k2d_init_flat");
   sim->t = 0;
   sim->nrec = 0;
@@ -142,11 +148,13 @@ int kpz2d_create(kpz2d_sim** out, int32_t Lx, int32_t Ly, int32_t nsamples, doub
   D.S = nsamples;
   D.Lx = Lx;
   D.Ly = Ly;
-  D.RW = y.RW;
+  D.RH = y.RH;
   D.n_ew = (int32_t)((int64_t)Lx * Ly / 64);
   D.n_sg = (D.n_ew + 3) / 4;
-  D.sx = (uint32_t*)(base + y.off_sx);
-  D.sy = (uint32_t*)(base + y.off_sy);
+  D.EX = (uint32_t*)(base + y.off_EX);
+  D.OX = (uint32_t*)(base + y.off_OX);
+  D.EY = (uint32_t*)(base + y.off_EY);
+  D.OY = (uint32_t*)(base + y.off_OY);
   sim->max_records = max_records;
   sim->path = path;
   sim->stream = (cudaStream_t)cuda_stream;
@@ -212,14 +220,20 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
     A.nt = nt;
     A.rec_h = sim->rec_h;
     A.rec_h2 = sim->rec_h2;
-    const size_t smem = (size_t)4 * D.Ly * (D.RW / 2 + D.RW / 8) * 4;  // 4 parity planes, one pad word per 4 words
-    KPZ_CUDA_CHECK(cudaFuncSetAttribute(k2d_onchip, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k2d_onchip<<<D.S, kK5SThreads, smem, sim->stream>>>(D, A);
+    const size_t smem = (size_t)4 * D.Ly * (D.RH + D.RH / 4) * 4;  // 4 parity planes, one pad word per 4 words
+    using OnchipFn = void (*)(const Kpz2dDev, const Kpz2dRun);
+    const OnchipFn fn = D.RH % 4 == 0 ? (two_planes(D) ? k2d_onchip<true, true> : k2d_onchip<true, false>)
+                                      : (two_planes(D) ? k2d_onchip<false, true> : k2d_onchip<false, false>);
+    KPZ_CUDA_CHECK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    fn<<<D.S, kK5SThreads, smem, sim->stream>>>(D, A);
     KPZ_LAUNCH_CHECK("k2d_onchip");
     sim->t += n_mcs;
     while (sim->nrec < nt && sim->rec_times[sim->nrec] <= sim->t) sim->nrec++;
     return KPZ_OK;
   }
+  using PassFn = void (*)(const Kpz2dDev, const unsigned char*, long long, int);
+  const PassFn pass_fn = D.RH % 4 == 0 ? (two_planes(D) ? k2d_pass<true, true> : k2d_pass<true, false>)
+                                       : (two_planes(D) ? k2d_pass<false, true> : k2d_pass<false, false>);
   const long long p_begin = 2 * (long long)sim->t, p_end = 2 * (long long)(sim->t + n_mcs);
   const long long nthreads = (long long)D.S * D.n_sg;
   const unsigned nblocks = (unsigned)((nthreads + 127) / 128);
@@ -232,7 +246,7 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
       const long long gp = c0 + k;
       const long long m = gp >> 1;
       const int ps = (int)(gp & 1);
-      k2d_pass<<<nblocks, 128, 0, sim->stream>>>(D, sim->off + (size_t)k * D.S, m, ps);
+      pass_fn<<<nblocks, 128, 0, sim->stream>>>(D, sim->off + (size_t)k * D.S, m, ps);
       KPZ_LAUNCH_CHECK("k2d_pass");
       if (ps == 1 && ri < nt && sim->rec_times[ri] == m + 1) {
         int rc = record2d(sim, ri);
@@ -249,18 +263,30 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
 int kpz2d_slopes(kpz2d_sim* sim, uint32_t* d_sx, uint32_t* d_sy) {
   if (!sim) return fail(KPZ_EINVAL, "NULL handle");
   const Kpz2dDev& D = sim->dev;
-  const size_t bytes = (size_t)D.S * D.Ly * D.RW * 4;
-  if (d_sx) KPZ_CUDA_CHECK(cudaMemcpyAsync(d_sx, D.sx, bytes, cudaMemcpyDeviceToDevice, sim->stream));
-  if (d_sy) KPZ_CUDA_CHECK(cudaMemcpyAsync(d_sy, D.sy, bytes, cudaMemcpyDeviceToDevice, sim->stream));
+  const size_t n = (size_t)D.S * D.Ly * D.RH;
+  if (d_sx) {
+    k2d_eo_to_nat<<<grid_for2(n), 256, 0, sim->stream>>>(D.EX, D.OX, n, d_sx);
+    KPZ_LAUNCH_CHECK("k2d_eo_to_nat");
+  }
+  if (d_sy) {
+    k2d_eo_to_nat<<<grid_for2(n), 256, 0, sim->stream>>>(D.EY, D.OY, n, d_sy);
+    KPZ_LAUNCH_CHECK("k2d_eo_to_nat");
+  }
   return KPZ_OK;
 }
 
 int kpz2d_set_slopes(kpz2d_sim* sim, const uint32_t* d_sx, const uint32_t* d_sy) {
   if (!sim) return fail(KPZ_EINVAL, "NULL handle");
   const Kpz2dDev& D = sim->dev;
-  const size_t bytes = (size_t)D.S * D.Ly * D.RW * 4;
-  if (d_sx) KPZ_CUDA_CHECK(cudaMemcpyAsync(D.sx, d_sx, bytes, cudaMemcpyDeviceToDevice, sim->stream));
-  if (d_sy) KPZ_CUDA_CHECK(cudaMemcpyAsync(D.sy, d_sy, bytes, cudaMemcpyDeviceToDevice, sim->stream));
+  const size_t n = (size_t)D.S * D.Ly * D.RH;
+  if (d_sx) {
+    k2d_nat_to_eo<<<grid_for2(n), 256, 0, sim->stream>>>(d_sx, n, D.EX, D.OX);
+    KPZ_LAUNCH_CHECK("k2d_nat_to_eo");
+  }
+  if (d_sy) {
+    k2d_nat_to_eo<<<grid_for2(n), 256, 0, sim->stream>>>(d_sy, n, D.EY, D.OY);
+    KPZ_LAUNCH_CHECK("k2d_nat_to_eo");
+  }
   return KPZ_OK;
 }
 
@@ -268,8 +294,9 @@ int kpz2d_heights(kpz2d_sim* sim, int32_t sample, int32_t* d_h) {
   if (!sim || !d_h || sample < 0 || sample >= sim->dev.S) return fail(KPZ_EINVAL, "bad arguments");
   const Kpz2dDev& D = sim->dev;
   const int nxb = (D.Lx + 255) / 256;
-  const size_t row0 = (size_t)sample * D.Ly * D.RW;
-  k2d_heights<1><<<nxb, 256, 0, sim->stream>>>(D.sx + row0, D.sy + row0, D.Lx, D.Ly, D.RW, nxb, nullptr, nullptr, d_h);
+  const size_t row0 = (size_t)sample * D.Ly * D.RH;
+  k2d_heights<1><<<nxb, 256, 0, sim->stream>>>(D.EX + row0, D.OX + row0, D.EY + row0, D.OY + row0, D.Lx, D.Ly, D.RH, nxb, nullptr,
+                                              nullptr, d_h);
   KPZ_LAUNCH_CHECK("k2d_heights");
   return KPZ_OK;
 }
