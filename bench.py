@@ -11,8 +11,8 @@ device memory.
 Default (`--config all`): BASELINE.json's `metric` names no configuration, so the headline (top-level `value`,
 `ms_per_step`, `config.workload`, `roofline`, `cpu_baseline`, `e2e`, `clocks`) is the LARGEST single-GPU configuration,
 config 3 (512 rings x 16384 sites x 10^5 MCS = 8.39e11 site updates), and the same line carries one full sub-record
-per other BASELINE configuration (1, 2, 4, 5) and for the two auxiliary streamed runs of SURVEY §8(d) (4-aux-i: L=2^28
-ring in L2; 4-aux-ii: L=2^32, the HBM roofline case) under `"per_config"`, each timed with its own K steps after W
+per other BASELINE configuration (1, 2, 4, 5), for the two auxiliary streamed runs of SURVEY §8(d) (4-aux-i: L=2^28
+ring in L2; 4-aux-ii: L=2^32, the HBM roofline case) and for the 2+1D workload 2d-512 under `"per_config"`, each timed with its own K steps after W
 warm-up steps.  `--config X` runs one workload only.
 
 value      site updates / s (GSU/s) of the whole job, device-timed (CUDA events on the launching stream), inputs
@@ -84,7 +84,7 @@ for _L in (512, 1024, 2048, 4096, 8192, 16384, 32768):   # the paper's size scan
     ALU_SLOTS_PER_SU[f"paper-scan-{_L}"] = ALU_SLOTS_PER_SU["paper-1024x30"]
 # default run: the headline first, then the other BASELINE configs and the auxiliary streamed runs of SURVEY §8(d)
 HEADLINE = 3
-DEFAULT_SET = [3, 1, 2, 4, 5, "4-aux-i", "4-aux-ii"]
+DEFAULT_SET = [3, 1, 2, 4, 5, "4-aux-i", "4-aux-ii", "2d-512"]   # the last one: SURVEY 8(f)-4, not a BASELINE config
 ALU_SLOTS_PER_CLK_SMSP = 0.5
 # streamed sweep: one read + one write of the bit-packed ring per sub-lattice pass = 2 passes * 2 * 1/8 B
 STREAM_BYTES_PER_SU = 0.5
