@@ -71,6 +71,9 @@
 #if (defined(K1J_TILE) || defined(K1J_STREAM)) && K1J_UPT != 1
 #error "K1J_UPT > 1 is implemented by the per-sample kernel only"
 #endif
+#ifndef K1J_QUEUE  // per-sample kernel, > 0: the run is cut into chunks of K1J_QUEUE MCS and the CTAs pull (sample, chunk)
+#define K1J_QUEUE 0  // items from a counter in chunk-major order, parking the ring in HBM between chunks (exact: the RNG is
+#endif               // counter-based, it is run(a); run(b)).  Balances rings over SMSPs that hold different numbers of warps.
 #ifndef K1J_HALOCHECK  // debug (compute-sanitizer's racecheck is closed on the GPU pool): every word published through
 #define K1J_HALOCHECK 0  // the shared-memory halo carries the number of its exchange; a reader that finds another number
 #endif                   // - a slot not yet written, or already overwritten by a later exchange - counts an error
@@ -716,11 +719,13 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   __syncthreads();
 
   // SPW == 1: CTA = sample, thread = UPT units.  SPW > 1: CTA = one warp = SPW samples, lane = (sample, units).
-  int sub = 0, s = (int)blockIdx.x, u = (int)threadIdx.x, lane0 = 0;  // lane0 = first lane of this sample
+  // run_sample: MCS [ta, tb) of the sample(s) of block index sblk
+  auto run_sample = [&](const int sblk, const long long ta, const long long tb) {
+  int sub = 0, s = sblk, u = (int)threadIdx.x, lane0 = 0;  // lane0 = first lane of this sample
   bool active = u < UT;
   if constexpr (SPW > 1) {
     sub = (int)threadIdx.x / UT;
-    s = (int)blockIdx.x * SPW + sub;
+    s = sblk * SPW + sub;
     u = (int)threadIdx.x % UT;
     lane0 = sub * UT;
     active = s < D.S;
@@ -744,7 +749,9 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   auto load_words = [&](uint32_t(&dst)[NW], const uint32_t* src) {
 #pragma unroll
     for (int j = 0; j < UPT; ++j) {
-      const uint4 v = *reinterpret_cast<const uint4*>(src + row + 4 * j);
+      // (K1J_QUEUE: the ring may have been parked by another SM a moment ago: read it past L1)
+      const uint4 v = K1J_QUEUE ? __ldcg(reinterpret_cast<const uint4*>(src + row + 4 * j))
+                                : *reinterpret_cast<const uint4*>(src + row + 4 * j);
       dst[4 * j + 0] = v.x; dst[4 * j + 1] = v.y; dst[4 * j + 2] = v.z; dst[4 * j + 3] = v.w;
     }
   };
@@ -763,16 +770,17 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
   if (DIS >= 2) frame_up(c.tags.sqb1, c.un, halo, c.parity);  // b side of frame 1 = the NEXT even site
 
   int ri = A.rec_begin;
+  while (K1J_QUEUE && ri < A.nt && A.rec_t[ri] <= ta) ++ri;  // records of earlier chunks
   long long next_rec = ri < A.nt ? A.rec_t[ri] : -1;
-  const long long t_end = A.t0 + A.n_mcs;
-  long long m = A.t0;
+  const long long t_end = tb;
+  long long m = ta;
   auto draw_offsets = [&]() {
     if constexpr (SPW == 1) {
       c.offbits = draw_offsets16(D.keys, c.gs, m);
     } else {
 #pragma unroll 1
       for (int k = 0; k < SPW; ++k) {  // one ballot per sample of this warp; each lane keeps its own sample's
-        const uint32_t b = draw_offsets16(D.keys, (uint32_t)(D.first_sample + (int)blockIdx.x * SPW + k), m);
+        const uint32_t b = draw_offsets16(D.keys, (uint32_t)(D.first_sample + sblk * SPW + k), m);
         if (k == sub) c.offbits = b;
       }
     }
@@ -817,6 +825,40 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
       *reinterpret_cast<uint4*>(D.O + row + 4 * j) = make_uint4(c.Q[4 * j], c.Q[4 * j + 1], c.Q[4 * j + 2], c.Q[4 * j + 3]);
     }
   }
+  };  // run_sample
+#if K1J_QUEUE
+  static_assert(SPW == 1, "K1J_QUEUE: one sample per CTA");
+  __shared__ unsigned int s_item;
+  const long long nchunks = (A.n_mcs + K1J_QUEUE - 1) / K1J_QUEUE;
+  const unsigned long long nitems = (unsigned long long)nchunks * (unsigned long long)D.S;
+  for (;;) {
+    if (threadIdx.x == 0) s_item = atomicAdd(A.queue, 1u);
+    __syncthreads();
+    const unsigned long long item = s_item;
+    __syncthreads();
+    if (item >= nitems) break;
+    const int smp = (int)(item % (unsigned)D.S);
+    const long long ch = (long long)(item / (unsigned)D.S);
+    if (ch > 0) {  // the previous chunk of this ring was handed out D.S items ago: wait until it is parked
+      if (threadIdx.x == 0) {
+        unsigned int done;
+        do {
+          asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(A.queue + 1 + smp) : "memory");
+          if (done < (unsigned)ch) __nanosleep(128);
+        } while (done < (unsigned)ch);
+      }
+      __syncthreads();
+    }
+    const long long ta = A.t0 + ch * K1J_QUEUE;
+    run_sample(smp, ta, ta + K1J_QUEUE < A.t0 + A.n_mcs ? ta + K1J_QUEUE : A.t0 + A.n_mcs);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0)
+      asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(A.queue + 1 + smp), "r"((unsigned)(ch + 1)) : "memory");
+  }
+#else
+  run_sample((int)blockIdx.x, A.t0, A.t0 + A.n_mcs);
+#endif
 }
 #else  // K1J_TILE
 // ---- K3T: temporally blocked sweep of rings beyond on-chip memory (north_star (2)) --------------------

@@ -215,8 +215,12 @@ void drop_define(std::vector<std::string>* defs, const char* name) {
 struct K1Shape {
   std::vector<std::string> defs;
   int block = 32, spw = 1, upt = 1;
+  int queue = 0;  // K1J_QUEUE: MCS per work item (0 = one CTA per sample for the whole run)
+  int grid = 1;
 };
-K1Shape k1_shape(const KpzDev& D, int S, int dis) {
+constexpr int kQueueMaxSamples = 8000;  // the done flags live in the scratch area behind the group totals
+
+K1Shape k1_shape(const KpzDev& D, int S, int dis, long long n_mcs = 1LL << 40) {
   static int smsp = 0;
   if (!smsp) {
     int dev = 0, sms = 148;
@@ -249,6 +253,24 @@ K1Shape k1_shape(const KpzDev& D, int S, int dis) {
     const long long warps = (long long)((S + sh.spw - 1) / sh.spw) * (sh.block / 32);
     if (warps >= 4LL * smsp) sh.defs.push_back("K1J_VARIANT=2");
   }
+  // Work queue (K1J_QUEUE = MCS per item, K1J_QGRID = CTAs in percent of the rings; k1_sweep_jit.cuh): chunks pulled from a
+  // counter let CTAs on emptier SMSPs run more of them.  Measured (profiles/r02_summary.md 3): config 2 -12 % (rings are
+  // chains, so a CTA that runs ahead ends up waiting for the chunk in front of it), config 3 +2 ... +4 % with chunks of
+  // 1024 MCS and 16 % spare CTAs: inside the run-to-run spread, so the default is off; the knob is kept for tests.
+  const long long warps = (long long)((S + sh.spw - 1) / sh.spw) * (sh.block / 32);
+  (void)warps;
+  (void)n_mcs;
+  int q = 0;
+  q = debug_int("K1J_QUEUE", q);
+  if (sh.spw != 1 || S > kQueueMaxSamples || q < 0) q = 0;
+  sh.queue = q;
+  drop_define(&sh.defs, "K1J_QUEUE");
+  drop_define(&sh.defs, "K1J_QGRID");
+  snprintf(buf, sizeof buf, "K1J_QUEUE=%d", q);
+  sh.defs.push_back(buf);
+  const int nblocks = (S + sh.spw - 1) / sh.spw;
+  sh.grid = nblocks;
+  if (q > 0) sh.grid = std::max(1, std::min(2 * nblocks, (int)((long long)nblocks * debug_int("K1J_QGRID", 100) / 100)));
   return sh;
 }
 
@@ -774,7 +796,7 @@ int kpz_run(kpz_sim* sim, int64_t n_mcs) {
     const int dis = sim->has_sq ? 2 : sim->has_sp ? 1 : 0;
     const int block = (D.U + 31) / 32 * 32;
     if (k1_use_jit(D)) {
-      K1Shape sh = k1_shape(D, sim->S, dis);
+      K1Shape sh = k1_shape(D, sim->S, dis, n_mcs);
       void* kfn = nullptr;
       rc = jit_get("k1_sweep_jit.cuh", "kpz_k1_sweep_jit", sh.defs, &kfn);
       if (rc) return rc;
@@ -785,8 +807,12 @@ int kpz_run(kpz_sim* sim, int64_t n_mcs) {
         KPZ_CUDA_CHECK(cudaMemsetAsync(check, 0, sizeof(unsigned int), sim->stream));
         A.check = check;
       }
+      if (sh.queue > 0) {  // work counter and per-sample chunk counters: scratch ints [PW + 64, PW + 64 + S]
+        A.queue = (unsigned int*)(sim->scratch + D.PW + 64);
+        KPZ_CUDA_CHECK(cudaMemsetAsync(A.queue, 0, ((size_t)sim->S + 1) * sizeof(unsigned int), sim->stream));
+      }
       void* args[] = {(void*)&D, (void*)&A};
-      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3((sim->S + sh.spw - 1) / sh.spw), dim3(sh.block), args, 0, sim->stream));
+      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(sh.grid), dim3(sh.block), args, 0, sim->stream));
       KPZ_LAUNCH_CHECK("kpz_k1_sweep_jit");
       if (halocheck) {
         unsigned int bad = 0;

@@ -38,6 +38,7 @@ struct KpzRunArgs {
   long long* rec_sum_h;    // [nt][S]
   long long* rec_sum_h2;   // [nt][S]
   unsigned int* check;     // debug (K1J_HALOCHECK): counter of failed halo sequence checks, else nullptr
+  unsigned int* queue;     // K1J_QUEUE: [0] = next work item, [1 + s] = chunks of sample s done (zeroed before the launch)
 };
 
 // K3 (pass-by-pass streamed sweep): one launch = one sub-lattice pass from (Ein, Oin) to (Eout, Oout).

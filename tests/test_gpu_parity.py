@@ -444,12 +444,24 @@ def test_overflow_guard_measures_a_lattice_handed_in(K):
 # ---------------------------------------------------------------------------------------------------------
 
 @pytest.mark.parametrize("cfg", ["jit=0", "K1J_VARIANT=0", "K1J_VARIANT=2", "K1J_REFRAME=1", "K1J_EAGER=3;K1J_TRIP=3",
-                                 "K1J_UPT=1", "K1J_UPT=2", "K1J_UPT=2;K1J_VARIANT=2", "K1J_UPT=2;K1J_REFRAME=1"])
+                                 "K1J_UPT=1", "K1J_UPT=2", "K1J_UPT=2;K1J_VARIANT=2", "K1J_UPT=2;K1J_REFRAME=1",
+                                 "K1J_QUEUE=5", "K1J_QUEUE=16;K1J_QGRID=50", "K1J_QUEUE=0"])
 def test_k1_variants_against_oracle(K, cfg):
     with K.debug_config(cfg):
         run_both_kpz(K, 8192 + 64, 3, 0.75, 0.25, seed=21, times=[1, 3, 20], chunks=[7, 13])
         run_both_kpz(K, 16384, 2, 1.0, 0.0, disorder=(0.1, 0.5, 0.0, 0.0), seed=22, times=[20], chunks=[20])
         run_both_kpz(K, 2048, 2, 0.8, 0.05, disorder=(0.3, 0.2, 0.3, 0.01), seed=23, times=[9], chunks=[9])
+
+
+@pytest.mark.parametrize("cfg", ["K1J_QUEUE=7", "K1J_QUEUE=32;K1J_QGRID=30", "K1J_QUEUE=1000"])
+def test_k1_work_queue_against_oracle(K, cfg):
+    """K1J_QUEUE (k1_sweep_jit.cuh): the run is cut into chunks that the CTAs pull from a counter, the ring parked in HBM
+    between chunks - it must be run(a); run(b); ... exactly: records on and around chunk boundaries, more rings than CTAs,
+    multi-warp and ragged rings, disorder tags, resumed runs whose chunks start at t0 > 0."""
+    with K.debug_config(cfg):
+        run_both_kpz(K, 8192, 40, 0.75, 0.25, seed=81, times=[6, 7, 8, 14, 31, 32, 33, 90], chunks=[50, 40])
+        run_both_kpz(K, 16384 + 64, 9, 1.0, 0.0, disorder=(0.1, 0.5, 0.0, 0.0), seed=82, times=[7, 64, 65], chunks=[65])
+        run_both_kpz(K, 40960, 3, 0.8, 0.1, disorder=(0.3, 0.2, 0.3, 0.05), seed=83, times=[20], chunks=[13, 7])
 
 
 def test_static_streamed_kernel_against_oracle(K):
