@@ -115,6 +115,22 @@ int kpz_heights(kpz_sim*, int32_t sample, int32_t* d_h);
  * (L*sum_h2 - sum_h^2)/L^2.  Any output pointer may be NULL. */
 int kpz_roughness(kpz_sim*, int32_t* nt, int64_t* t, int64_t* sum_h, int64_t* sum_h2, double* w2_mean);
 
+/* The exact sums behind the width W of Eq. 3 of rings handed in by the caller, WITHOUT any
+ * allocation: no handle, no workspace, no cudaMalloc / cudaFree / allocating library call - for callers that cannot
+ * allocate (CUDA graph capture, serving loops, harnesses that forbid it).  d_words: nsamples * L/32 device words, natural
+ * layout, 16-byte aligned (as kpz_lattice writes them); d_sum_h, d_sum_h2: nsamples device int64 each, overwritten with
+ * sum_x h_x and sum_x h_x^2, h_x = sum_{i<=x} (2 n_i - 1) - the values kpz_roughness reports for the same lattice.  They
+ * are exact modulo 2^64, hence exact whenever L * max|h|^2 < 2^63 (any lattice with L < 2^21; rougher, longer rings are the
+ * caller's to bound, cf. the guard of kpz_set_lattice).  Asynchronous on cuda_stream (a cudaStream_t of the CURRENT device).
+ * The tile scratch of the reduction (one int per 65536 sites) is a static device array of KPZ_NOALLOC_MAX_TILES ints
+ * (256 KiB per GPU that loads the library, until exit): nsamples * ceil(L / 65536) beyond that, L beyond 2^30 or not a
+ * multiple of 64 -> KPZ_EUNSUPPORTED with the reason in kpz_last_error().  ALL calls share that array: two calls that
+ * overlap on the GPU (different streams or host threads without an ordering between them) race; calls on one stream
+ * are safe back to back. */
+#define KPZ_NOALLOC_MAX_TILES 65536
+int kpz_noalloc_height_sums(const uint32_t* d_words, int64_t L, int32_t nsamples, int64_t* d_sum_h, int64_t* d_sum_h2,
+                            void* cuda_stream);
+
 /* Frees the host-side handle only ("device memory is touched at the start and the end of a time loop", PAPER.md:91:
  * the state lives in the caller's workspace, which the caller frees).  Pending work on the stream is not waited for. */
 int kpz_destroy(kpz_sim*);

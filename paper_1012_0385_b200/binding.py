@@ -60,6 +60,7 @@ SIGNATURES = {
     "kpz_heights": (C.c_int, [_P, C.c_int32, _P]),
     "kpz_roughness": (C.c_int, [_P, C.POINTER(C.c_int32), _P, _P, _P, _P]),
     "kpz_destroy": (C.c_int, [_P]),
+    "kpz_noalloc_height_sums": (C.c_int, [_P, C.c_int64, C.c_int32, _P, _P, _P]),
     "lanes_workspace_bytes": (C.c_int, [C.c_int64, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]),
     "lanes_create": (C.c_int, [C.POINTER(_P), C.c_int64, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
                                C.c_int64, C.c_double, C.c_uint64, C.POINTER(Options), C.c_int32, _P, C.c_size_t, _P]),
@@ -171,6 +172,30 @@ def debug_dump_cubins(directory: str) -> int:
     n = C.c_int32(0)
     _chk(load_library().kpz_debug_dump_cubins(directory.encode(), C.byref(n)), "kpz_debug_dump_cubins")
     return int(n.value)
+
+
+KPZ_NOALLOC_MAX_TILES = 65536
+
+
+def noalloc_height_sums(words, L, sum_h, sum_h2) -> None:
+    """kpz_noalloc_height_sums: sum h, sum h^2 of the rings in `words` ([nsamples, L/32] int32 / uint32 CUDA tensor, natural
+    layout) into the caller's int64 CUDA tensors `sum_h`, `sum_h2` ([nsamples]).  Allocates nothing, on either side of
+    the ABI: the scratch is a static device array (nsamples * ceil(L / 65536) <= KPZ_NOALLOC_MAX_TILES).  Asynchronous on
+    the current stream; calls that overlap on the GPU race on that array."""
+    L = int(L)
+    if not (words.is_cuda and sum_h.is_cuda and sum_h2.is_cuda and words.is_contiguous() and sum_h.is_contiguous()
+            and sum_h2.is_contiguous()):
+        raise ValueError("words, sum_h, sum_h2 must be contiguous CUDA tensors")
+    if words.element_size() != 4 or sum_h.dtype != torch.int64 or sum_h2.dtype != torch.int64:
+        raise ValueError("words must hold 32-bit words, sum_h / sum_h2 int64")
+    if L < 32 or words.numel() % (L // 32) != 0:
+        raise ValueError("words must hold nsamples * L/32 words")
+    S = words.numel() // (L // 32)
+    if sum_h.numel() != S or sum_h2.numel() != S:
+        raise ValueError("sum_h, sum_h2 must hold one value per sample")
+    with torch.cuda.device(words.device):
+        _chk(load_library().kpz_noalloc_height_sums(_dptr(words), L, S, _dptr(sum_h), _dptr(sum_h2), _stream_ptr()),
+             "kpz_noalloc_height_sums")
 
 
 def jit_check(L, p, q, disorder=None, offset_mode=0, path=KPZ_PATH_AUTO) -> int:
