@@ -227,9 +227,9 @@ int kpz_path(const kpz_sim*, int32_t* path);
 
 /* Test and tuning hook, not part of the paper's problem statement: a ';'-separated list of NAME=VALUE items that
  * replaces the process-wide debug configuration (NULL or "" restores the defaults).  "jit=0" selects the statically
- * compiled generic kernels instead of the run-time specialised ones; "K1J_<X>=v" / "K4J_<X>=v" are appended as
- * definitions to every later run-time compilation of the KPZ / two-lane sweep kernels (the knobs documented at the top
- * of csrc/k1_sweep_jit.cuh and csrc/k4_lanes_jit.cuh).  Every setting computes the same results (tests/ check that);
+ * compiled generic kernels instead of the run-time specialised ones; "K1J_<X>=v" / "K4J_<X>=v" / "K5J_<X>=v" are appended
+ * as definitions to every later run-time compilation of the KPZ / two-lane / 2+1D sweep kernels (the knobs documented at
+ * the top of csrc/k1_sweep_jit.cuh and csrc/k4_lanes_jit.cuh; K5J_RIW=0: no shuffles in the 2+1D on-chip kernel).  Every setting computes the same results (tests/ check that);
  * kpz_run / lanes_run read no environment variable.  KPZ_EINVAL for anything else. */
 int kpz_debug_config(const char* spec);
 /* Writes every kernel image compiled by this process so far (kpz_run, lanes_run, *_jit_check) to
@@ -247,6 +247,9 @@ int lanes_jit_check(int64_t L, double p_a, double p_b, double turn_prob, int64_t
                     const kpz_options* opt, size_t* cubin_bytes); /* same for the two-lane kernel */
 int lanes_crossing_jit_check(int64_t L, double p_a, double p_b, const lanes_crossing* crossing, int64_t turn_period,
                              const kpz_options* opt, size_t* cubin_bytes);
+/* Same for the 2+1D kernels (K5 / K5S, specialised on Lx, Ly and the thresholds of p, q): the kernel kpz2d_run would use
+ * for these parameters and options.path. */
+int kpz2d_jit_check(int32_t Lx, int32_t Ly, double p, double q, const kpz_options* opt, size_t* cubin_bytes);
 
 #ifdef __cplusplus
 }

@@ -102,6 +102,7 @@ SIGNATURES = {
     "kpz_debug_dump_cubins": (C.c_int, [C.c_char_p, C.POINTER(C.c_int32)]),
     "kpz_jit_check": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.POINTER(Disorder), C.POINTER(Options),
                                 C.POINTER(C.c_size_t)]),
+    "kpz2d_jit_check": (C.c_int, [C.c_int32, C.c_int32, C.c_double, C.c_double, C.POINTER(Options), C.POINTER(C.c_size_t)]),
     "lanes_jit_check": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int64, C.c_double,
                                   C.POINTER(Options), C.POINTER(C.c_size_t)]),
 }
@@ -205,6 +206,14 @@ def jit_check(L, p, q, disorder=None, offset_mode=0, path=KPZ_PATH_AUTO) -> int:
     n = C.c_size_t()
     _chk(load_library().kpz_jit_check(int(L), float(p), float(q), C.byref(d) if d is not None else None, C.byref(o),
                                       C.byref(n)), "kpz_jit_check")
+    return int(n.value)
+
+
+def kpz2d_jit_check(Lx, Ly, p, q, offset_mode=0, path=KPZ_PATH_AUTO) -> int:
+    """kpz2d_jit_check: compile (no GPU needed) the specialised 2+1D kernel for these parameters; cubin size in bytes."""
+    o = Options(0, int(offset_mode), int(path))
+    n = C.c_size_t()
+    _chk(load_library().kpz2d_jit_check(int(Lx), int(Ly), float(p), float(q), C.byref(o), C.byref(n)), "kpz2d_jit_check")
     return int(n.value)
 
 

@@ -83,10 +83,10 @@ int debug_config(const char* spec) {
         return fail(KPZ_EINVAL, "debug config: bad character in '%s'", tok.c_str());
     if (tok.compare(0, eq, "jit") == 0) {
       jit_on = tok[eq + 1] != '0';
-    } else if (tok.compare(0, 4, "K1J_") == 0 || tok.compare(0, 4, "K4J_") == 0) {
+    } else if (tok.compare(0, 4, "K1J_") == 0 || tok.compare(0, 4, "K4J_") == 0 || tok.compare(0, 4, "K5J_") == 0) {
       defs.push_back(tok);
     } else {
-      return fail(KPZ_EINVAL, "debug config: unknown name in '%s' (jit, K1J_*, K4J_*)", tok.c_str());
+      return fail(KPZ_EINVAL, "debug config: unknown name in '%s' (jit, K1J_*, K4J_*, K5J_*)", tok.c_str());
     }
   }
   std::lock_guard<std::mutex> lock(g_dbg_mu);

@@ -3,10 +3,12 @@
 // kernels of kpz2d_k5.cuh.  No CPU fallback.
 #include <algorithm>
 #include <new>
+#include <string>
 #include <vector>
 
 #include "common.cuh"
-#include "kpz2d_k5.cuh"
+#include "jit.h"
+#include "kpz2d_util.cuh"
 
 using namespace kpz;
 
@@ -27,9 +29,11 @@ namespace {
 constexpr int kChunkPasses = 1024;
 constexpr size_t kOnchipBytes = 96 * 1024;  // both slope fields of a sample in shared memory, two CTAs per SM
 
+size_t onchip_bytes(int32_t Lx, int32_t Ly) { return (size_t)4 * Ly * (Lx / 64) * 4; }  // 4 parity planes of Ly * Lx/64 words
+
 // options.path: 0 auto (on chip when the sample fits), 1 on chip (k2d_onchip), 2 streamed (k2d_pass per colour pass)
 int choose_path2d(int32_t Lx, int32_t Ly, const kpz_options* opt, int* path) {
-  const size_t bytes = (size_t)4 * Ly * (Lx / 64 + Lx / 256) * 4;  // 4 parity planes with padded rows, see k2d_onchip
+  const size_t bytes = onchip_bytes(Lx, Ly);
   int want = opt ? opt->path : KPZ_PATH_AUTO;
   if (want == KPZ_PATH_AUTO) want = bytes <= kOnchipBytes ? KPZ_PATH_ONCHIP : KPZ_PATH_STREAM;
   if (want == KPZ_PATH_ONCHIP && bytes > 200 * 1024)
@@ -84,6 +88,29 @@ Layout2d layout2d(int32_t Lx, int32_t Ly, int32_t S, int32_t max_records) {
 // both thresholds depend on their two leading bit-planes at most (p = 0.75, 0.5, 0.25, 0, 1 ...): the kernels then draw
 // those two planes unconditionally
 bool two_planes(const Kpz2dDev& D) { return planes_needed(D.t_p) <= 2 && planes_needed(D.t_q) <= 2; }
+
+// Definitions of the run-time specialised kernels (kpz2d_k5.cuh under NVRTC): shape, thresholds, launch shape.
+std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, size_t smem) {
+  char buf[64];
+  std::vector<std::string> d;
+  auto add = [&](const char* name, long long v) {
+    snprintf(buf, sizeof buf, "%s=%lld", name, v);
+    d.push_back(buf);
+  };
+  add("K5J_LX", D.Lx);
+  add("K5J_LY", D.Ly);
+  snprintf(buf, sizeof buf, "K5J_TP=0x%xu", D.t_p.value);
+  d.push_back(buf);
+  add("K5J_TP_ALWAYS", D.t_p.always);
+  snprintf(buf, sizeof buf, "K5J_TQ=0x%xu", D.t_q.value);
+  d.push_back(buf);
+  add("K5J_TQ_ALWAYS", D.t_q.always);
+  add("K5J_TWO", two_planes(D) ? 1 : 0);
+  // CTAs per SM the on-chip kernel is compiled for: two when two samples fit the shared memory of an SM
+  add("K5J_MINB", smem != 0 && 2 * (smem + 1024) <= 227 * 1024 ? 2 : 1);
+  add("K5J_RIW", debug_int("K5J_RIW", 1));
+  return d;
+}
 
 int record2d(kpz2d_sim* sim, int ri) {
   const Kpz2dDev& D = sim->dev;
@@ -171,6 +198,30 @@ int kpz2d_create(kpz2d_sim** out, int32_t Lx, int32_t Ly, int32_t nsamples, doub
   return KPZ_OK;
 }
 
+int kpz2d_jit_check(int32_t Lx, int32_t Ly, double p, double q, const kpz_options* opt, size_t* cubin_bytes) {
+  if (!cubin_bytes) return fail(KPZ_EINVAL, "cubin_bytes is NULL");
+  *cubin_bytes = 0;
+  int rc = validate2d(Lx, Ly, 1, 0);
+  if (rc) return rc;
+  if (!valid_prob(p) || !valid_prob(q)) return fail(KPZ_EINVAL, "p and q must lie in [0,1]");
+  int path;
+  rc = choose_path2d(Lx, Ly, opt, &path);
+  if (rc) return rc;
+  if (!jit_enabled()) return KPZ_OK;
+  Kpz2dDev D{};
+  D.t_p = make_thresh(p);
+  D.t_q = make_thresh(q);
+  D.Lx = Lx;
+  D.Ly = Ly;
+  std::vector<char> cubin;
+  const bool onchip = path == KPZ_PATH_ONCHIP;
+  rc = jit_compile("kpz2d_k5.cuh", onchip ? "kpz2d_k5s_jit" : "kpz2d_k5_pass_jit",
+                   k5_jit_defines(D, onchip ? onchip_bytes(Lx, Ly) : 0), &cubin, nullptr);
+  if (rc) return rc;
+  *cubin_bytes = cubin.size();
+  return KPZ_OK;
+}
+
 int kpz2d_destroy(kpz2d_sim* sim) {
   delete sim;
   return KPZ_OK;
@@ -220,13 +271,23 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
     A.nt = nt;
     A.rec_h = sim->rec_h;
     A.rec_h2 = sim->rec_h2;
-    const size_t smem = (size_t)4 * D.Ly * (D.RH + D.RH / 4) * 4;  // 4 parity planes, one pad word per 4 words
-    using OnchipFn = void (*)(const Kpz2dDev, const Kpz2dRun);
-    const OnchipFn fn = D.RH % 4 == 0 ? (two_planes(D) ? k2d_onchip<true, true> : k2d_onchip<true, false>)
-                                      : (two_planes(D) ? k2d_onchip<false, true> : k2d_onchip<false, false>);
-    KPZ_CUDA_CHECK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    fn<<<D.S, kK5SThreads, smem, sim->stream>>>(D, A);
-    KPZ_LAUNCH_CHECK("k2d_onchip");
+    const size_t smem = onchip_bytes(D.Lx, D.Ly);
+    if (jit_enabled()) {  // specialised on the shape and the thresholds (NVRTC)
+      void* kfn = nullptr;
+      int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5s_jit", k5_jit_defines(D, smem), &kfn);
+      if (rc) return rc;
+      void* args[] = {(void*)&D, (void*)&A};
+      KPZ_CUDA_CHECK(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(D.S), dim3(kK5SThreads), args, smem, sim->stream));
+      count_launch();
+    } else {
+      using OnchipFn = void (*)(const Kpz2dDev, const Kpz2dRun);
+      const OnchipFn fn = D.RH % 4 == 0 ? (two_planes(D) ? k2d_onchip<true, true> : k2d_onchip<true, false>)
+                                        : (two_planes(D) ? k2d_onchip<false, true> : k2d_onchip<false, false>);
+      KPZ_CUDA_CHECK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      fn<<<D.S, kK5SThreads, smem, sim->stream>>>(D, A);
+      KPZ_LAUNCH_CHECK("k2d_onchip");
+    }
     sim->t += n_mcs;
     while (sim->nrec < nt && sim->rec_times[sim->nrec] <= sim->t) sim->nrec++;
     return KPZ_OK;
@@ -234,6 +295,11 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
   using PassFn = void (*)(const Kpz2dDev, const unsigned char*, long long, int);
   const PassFn pass_fn = D.RH % 4 == 0 ? (two_planes(D) ? k2d_pass<true, true> : k2d_pass<true, false>)
                                        : (two_planes(D) ? k2d_pass<false, true> : k2d_pass<false, false>);
+  void* pass_jit = nullptr;
+  if (jit_enabled()) {
+    int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5_pass_jit", k5_jit_defines(D, 0), &pass_jit);
+    if (rc) return rc;
+  }
   const long long p_begin = 2 * (long long)sim->t, p_end = 2 * (long long)(sim->t + n_mcs);
   const long long nthreads = (long long)D.S * D.n_sg;
   const unsigned nblocks = (unsigned)((nthreads + 127) / 128);
@@ -246,8 +312,17 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
       const long long gp = c0 + k;
       const long long m = gp >> 1;
       const int ps = (int)(gp & 1);
-      pass_fn<<<nblocks, 128, 0, sim->stream>>>(D, sim->off + (size_t)k * D.S, m, ps);
-      KPZ_LAUNCH_CHECK("k2d_pass");
+      if (pass_jit) {
+        const unsigned char* off_k = sim->off + (size_t)k * D.S;
+        long long m_arg = m;
+        int ps_arg = ps;
+        void* args[] = {(void*)&D, (void*)&off_k, (void*)&m_arg, (void*)&ps_arg};
+        KPZ_CUDA_CHECK(cudaLaunchKernel(pass_jit, dim3(nblocks), dim3(128), args, 0, sim->stream));
+        count_launch();
+      } else {
+        pass_fn<<<nblocks, 128, 0, sim->stream>>>(D, sim->off + (size_t)k * D.S, m, ps);
+        KPZ_LAUNCH_CHECK("k2d_pass");
+      }
       if (ps == 1 && ri < nt && sim->rec_times[ri] == m + 1) {
         int rc = record2d(sim, ri);
         if (rc) return rc;

@@ -1,0 +1,77 @@
+// kpz2d_util.cuh — the helper kernels of the 2+1D path that only the library build needs (initialisation, layout
+// conversion at the ABI, colour offsets of a chunk of passes, heights / exact sums from the planes in HBM).  The sweep
+// kernels themselves are in kpz2d_k5.cuh (also compiled at run time).
+#pragma once
+#include "common.cuh"
+#include "kpz2d_k5.cuh"
+
+namespace kpz {
+
+// flat start h = (x + y) & 1: sx = sy = (x + y) & 1, i.e. even sites carry y & 1, odd sites its complement
+__global__ void k2d_init_flat(uint32_t* EX, uint32_t* OX, uint32_t* EY, uint32_t* OY, int S, int Ly, int RH) {
+  const size_t n = (size_t)S * Ly * RH;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const int y = (int)((i / RH) % Ly);
+    const uint32_t e = (y & 1) ? 0xFFFFFFFFu : 0u;
+    EX[i] = e;
+    OX[i] = ~e;
+    EY[i] = e;
+    OY[i] = ~e;
+  }
+}
+
+// natural words [rows][2 RH] <-> parity planes [rows][RH]
+__global__ void k2d_nat_to_eo(const uint32_t* words, size_t n /* rows * RH */, uint32_t* E, uint32_t* O) {
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const uint2 w = reinterpret_cast<const uint2*>(words)[i];
+    uint32_t e, o;
+    nat_to_eo(w.x, w.y, e, o);
+    E[i] = e;
+    O[i] = o;
+  }
+}
+__global__ void k2d_eo_to_nat(const uint32_t* E, const uint32_t* O, size_t n, uint32_t* words) {
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    uint32_t w0, w1;
+    eo_to_nat(E[i], O[i], w0, w1);
+    reinterpret_cast<uint2*>(words)[i] = make_uint2(w0, w1);
+  }
+}
+
+// offsets of np passes starting at global pass index p0 (pass = 2 m + ps): out[k * S + s]
+__global__ void k2d_offsets(const __grid_constant__ PhiloxKeys K, int first_sample, int S, long long p0, int np, int offset_mode,
+                            unsigned char* out) {
+  const size_t n = (size_t)np * S;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const int k = (int)(i / S), s = (int)(i % S);
+    const unsigned long long gp = (unsigned long long)(p0 + k);
+    const unsigned long long m = gp >> 1;
+    const uint32_t ps = (uint32_t)(gp & 1ull);
+    uint32_t o = ps;
+    if (offset_mode == 0)
+      o = philox4x32_10(0u, (uint32_t)(first_sample + s), (uint32_t)m, ctr3(TAG_OFFSET, ps, 0, (uint32_t)(m >> 32)), K).x & 1u;
+    out[i] = (unsigned char)o;
+  }
+}
+
+// MODE 0: exact sums over a sample (grid = S * nxb blocks of 256 columns, atomicAdd per block); MODE 1: heights of one sample.
+template <int MODE>
+__global__ void __launch_bounds__(256) k2d_heights(const uint32_t* __restrict__ EX, const uint32_t* __restrict__ OX,
+                                                   const uint32_t* __restrict__ EY, const uint32_t* __restrict__ OY, int Lx, int Ly,
+                                                   int RH, int nxb, unsigned long long* out_h, unsigned long long* out_h2,
+                                                   int32_t* h_out) {
+  __shared__ long long red[16];
+  const int s = blockIdx.x / nxb, x = (blockIdx.x % nxb) * 256 + threadIdx.x;
+  const size_t base = (size_t)s * Ly * RH;
+  long long s1 = 0, s2 = 0;
+  column_sums<MODE>(EX + base, OX + base, EY + base, OY + base, RH, 0, Lx, Ly, x < Lx ? x : Lx, Lx, s1, s2, h_out);
+  if (MODE == 0) {
+    block_sum2<8>(s1, s2, red);
+    if (threadIdx.x == 0) {
+      atomicAdd(out_h + s, (unsigned long long)s1);  // exact: two's-complement wrap-around addition
+      atomicAdd(out_h2 + s, (unsigned long long)s2);
+    }
+  }
+}
+
+}  // namespace kpz

@@ -25,6 +25,9 @@ def K():
 
 
 def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_mode=0, start=None, path=0):
+    if isinstance(path, tuple):          # (path, kpz_debug_config spec): see PATHS
+        with K.debug_config(path[1]):
+            return run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample, offset_mode, start, path[0])
     total = sum(chunks)
     times = [t for t in times if t <= total]
     ref = R.Kpz2dRef(Lx, Ly, S, p, q, seed=seed, first_sample=first_sample, offset_mode=offset_mode)
@@ -58,14 +61,21 @@ def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_
     return gpu, g
 
 
-PATHS = [1, 2]   # 1 = a sample in shared memory (k2d_onchip), 2 = one launch per colour pass (k2d_pass)
+# 1 = a sample in shared memory (K5S), 2 = one launch per colour pass (K5); each as the run-time specialised kernel
+# (NVRTC: shape and thresholds are constants) and as the generic kernel of the library build ("jit=0"); K5J_RIW=0 takes
+# the shuffles out of the specialised on-chip kernel (neighbour word loaded, carries by atomics)
+PATHS = [(1, ""), (2, ""), (1, "jit=0"), (2, "jit=0"), (1, "K5J_RIW=0")]
 
 
 @pytest.mark.parametrize("path", PATHS)
-@pytest.mark.parametrize("Lx,Ly", [(64, 2), (64, 6), (128, 64), (192, 10), (256, 256), (320, 30), (1024, 4)])
+@pytest.mark.parametrize("Lx,Ly", [(64, 2), (64, 6), (128, 64), (192, 10), (256, 256), (320, 30), (1024, 4), (256, 2), (512, 64),
+                                   (768, 6), (2048, 8), (8192, 2), (16384, 2), (512, 130)])
 def test_sizes_ragged_supergroups_and_tiny_lattices(K, Lx, Ly, path):
     """A row of 64 sites is a quarter of a Philox supergroup, 192 / 320 sites leave ragged ones; Ly = 2 couples every row
-    to itself through the periodic y-pair; 256 x 256 gives the 512 threads of the on-chip kernel one supergroup each."""
+    to itself through the periodic y-pair; 256 x 256 gives the 512 threads of the on-chip kernel one supergroup each.
+    Fast path (Lx a multiple of 256, threads taken by row parity): 512 x 64, 2048 x 8 and 8192 x 2 keep a row inside a
+    warp (2, 8, 32 lanes: shuffles), 768 x 6 has three supergroups per row and warps of mixed colour on the streamed
+    path, 16384 x 2 rows longer than a warp, 512 x 130 a last warp that is partly idle."""
     run_both_2d(K, Lx, Ly, 3, 0.75, 0.25, seed=Lx + Ly, times=[1, 3, 12], chunks=[5, 7], path=path)
 
 
@@ -107,15 +117,17 @@ def test_path_selection_and_both_paths_agree_at_512(K):
     assert np.array_equal(ra["sum_h"], rb["sum_h"]) and np.array_equal(ra["sum_h2"], rb["sum_h2"])
 
 
+@pytest.mark.parametrize("spec", ["", "jit=0"])
 @pytest.mark.parametrize("key", ["2d-512", "2d-1024"])
-def test_workload_shape_sampled_against_solo_oracle_runs(K, key):
+def test_workload_shape_sampled_against_solo_oracle_runs(K, key, spec):
     """The bench workloads `2d-512` (on chip) and `2d-1024` (streamed) in their launch configuration (all samples),
     shortened: first and last sample against solo oracle runs, every sample single-valued."""
     c = workloads.CONFIGS[key]
     n, times = 6, [1, 2, 3, 4, 5, 6]
-    gpu = K.Kpz2dSim(c["Lx"], c["Ly"], c["S"], c["p"], c["q"], seed=c["seed"], max_records=len(times))
-    gpu.set_record_times(times)
-    gpu.run(n)
+    with K.debug_config(spec):
+        gpu = K.Kpz2dSim(c["Lx"], c["Ly"], c["S"], c["p"], c["q"], seed=c["seed"], max_records=len(times))
+        gpu.set_record_times(times)
+        gpu.run(n)
     sx, sy = [K.words_to_numpy(t) for t in gpu.slopes()]
     r = gpu.roughness()
     for k in (0, c["S"] - 1):

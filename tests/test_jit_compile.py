@@ -58,7 +58,29 @@ def test_paper_two_lane_model_compiles(K, L, indep, period):
     assert K.lanes_crossing_jit_check(L, 0.5, 0.5, 0.5, 0.2, 0.8, indep, period) > 10_000
 
 
+@pytest.mark.parametrize("Lx,Ly,p,q,path", [
+    (512, 512, 0.75, 0.0, 0),       # bench workload 2d-512: on chip, two planes, a row = two lanes of a warp
+    (1024, 1024, 0.75, 0.0, 0),     # 2d-1024: streamed
+    (512, 512, 0.8, 0.1, 1),        # lazy plane loop on chip
+    (64, 16, 0.75, 0.25, 0),        # ragged: a supergroup spans rows
+    (320, 10, 0.3, 0.2, 2),
+    (256, 2, 1.0, 0.0, 1),          # one supergroup per row, Ly = 2
+    (768, 64, 0.5, 0.5, 1),         # three supergroups per row: no shuffles
+    (8192, 4, 0.75, 0.0, 1),        # a row longer than a warp
+])
+def test_2d_kernels_compile(K, Lx, Ly, p, q, path):
+    assert K.kpz2d_jit_check(Lx, Ly, p, q, path=path) > 10_000
+    with K.debug_config("K5J_RIW=0"):
+        assert K.kpz2d_jit_check(Lx, Ly, p, q, path=path) > 10_000
+    with K.debug_config("jit=0"):
+        assert K.kpz2d_jit_check(Lx, Ly, p, q, path=path) == 0
+
+
 def test_bad_arguments_are_refused_without_compiling(K):
+    with pytest.raises(K.KpzError):
+        K.kpz2d_jit_check(100, 64, 0.5, 0.5)    # Lx not a multiple of 64
+    with pytest.raises(K.KpzError):
+        K.kpz2d_jit_check(2048, 2048, 0.5, 0.5, path=1)   # beyond the shared memory of an SM
     with pytest.raises(K.KpzError):
         K.jit_check(100, 0.5, 0.5)              # L not a multiple of 64
     with pytest.raises(K.KpzError):
@@ -94,5 +116,5 @@ def test_compiled_images_can_be_dumped(K, tmp_path):
     assert n >= 1
     names = sorted(p.name for p in tmp_path.iterdir())
     assert any(x.startswith("kpz_k1_sweep_jit_") and x.endswith(".cubin") for x in names)
-    txt = next(p for p in tmp_path.iterdir() if p.name.startswith("kpz_k1_sweep_jit_") and p.suffix == ".txt")
-    assert "-DK1J_PW=128" in txt.read_text()
+    txts = [p.read_text() for p in tmp_path.iterdir() if p.name.startswith("kpz_k1_sweep_jit_") and p.suffix == ".txt"]
+    assert any("-DK1J_PW=128" in t for t in txts)       # L = 8192: 128 words per parity plane
