@@ -210,6 +210,10 @@ int kpz2d_time(const kpz2d_sim*, int64_t* t);
 int kpz2d_path(const kpz2d_sim*, int32_t* path);
 int kpz2d_reset(kpz2d_sim*);                                          /* flat surface, t = 0, records dropped; async */
 int kpz2d_slopes(kpz2d_sim*, uint32_t* d_sx, uint32_t* d_sy);        /* copy out (either may be NULL); async */
+/* Copy in.  The two fields must describe a single-valued surface (every plaquette curl-free: sx[y][x] + sy[y+1][x] =
+ * sx[y+1][x] + sy[y+1][x-1], both ways round a plaquette give the same height), as every state reached from the flat start
+ * does: the sums captured at record times integrate the heights row by row, kpz2d_heights column by column, and the
+ * two agree exactly on such surfaces only. */
 int kpz2d_set_slopes(kpz2d_sim*, const uint32_t* d_sx, const uint32_t* d_sy);
 int kpz2d_heights(kpz2d_sim*, int32_t sample, int32_t* d_h /* [Ly][Lx] int32, device */);
 /* As kpz_roughness: W^2 over the Lx * Ly sites of a sample (Eq. 3), mean over samples.  SYNCS. */

@@ -118,9 +118,9 @@ int record2d(kpz2d_sim* sim, int ri) {
   unsigned long long* oh2 = (unsigned long long*)(sim->rec_h2 + (size_t)ri * D.S);
   KPZ_CUDA_CHECK(cudaMemsetAsync(oh, 0, (size_t)D.S * 8, sim->stream));
   KPZ_CUDA_CHECK(cudaMemsetAsync(oh2, 0, (size_t)D.S * 8, sim->stream));
-  const int nxb = (D.Lx + 255) / 256;
-  k2d_heights<0><<<D.S * nxb, 256, 0, sim->stream>>>(D.EX, D.OX, D.EY, D.OY, D.Lx, D.Ly, D.RH, nxb, oh, oh2, nullptr);
-  KPZ_LAUNCH_CHECK("k2d_heights");
+  const int nyb = (D.Ly + 255) / 256;
+  k2d_row_sums<<<D.S * nyb, 256, 0, sim->stream>>>(D.EX, D.OX, D.EY, D.Lx, D.Ly, D.RH, nyb, oh, oh2);
+  KPZ_LAUNCH_CHECK("k2d_row_sums");
   return KPZ_OK;
 }
 

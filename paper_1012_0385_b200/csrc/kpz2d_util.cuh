@@ -74,4 +74,63 @@ __global__ void __launch_bounds__(256) k2d_heights(const uint32_t* __restrict__ 
   }
 }
 
+// Exact sums over every sample from the planes in HBM, row by row (see row_sums_onchip): grid = S * nyb blocks of 256
+// rows; a block first adds up column 0 of sy over the rows before its own (the height of its first row's site 0).
+__global__ void __launch_bounds__(256) k2d_row_sums(const uint32_t* __restrict__ EX, const uint32_t* __restrict__ OX,
+                                                    const uint32_t* __restrict__ EY, int Lx, int Ly, int RH, int nyb,
+                                                    unsigned long long* out_h, unsigned long long* out_h2) {
+  __shared__ long long red[16];
+  __shared__ uint32_t lut[256];
+  __shared__ int scan[8];
+  lut[threadIdx.x] = height_lut_entry((int)threadIdx.x);
+  const int s = blockIdx.x / nyb, y_first = (blockIdx.x % nyb) * 256;
+  const size_t base = (size_t)s * Ly * RH;
+  const uint32_t *ex = EX + base, *ox = OX + base, *ey = EY + base;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  auto block_total = [&](int v) {  // sum over the block, to every thread
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, d);
+    __syncthreads();
+    if (lane == 0) scan[warp] = v;
+    __syncthreads();
+    int t = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) t += scan[k];
+    return t;
+  };
+  int pre = 0;
+  for (int yy = 1 + (int)threadIdx.x; yy < y_first; yy += 256) pre += 2 * (int)(ey[(size_t)yy * RH] & 1u) - 1;
+  const int h_before = 2 * (int)(ex[0] & 1u) - 1 + block_total(pre);  // h(0, y_first - 1), or h(0,0) for the first block
+  const int y = y_first + (int)threadIdx.x;
+  const bool live = y < Ly;
+  const size_t row = (size_t)(live ? y : 0) * RH;
+  const int d = (live && y > 0) ? 2 * (int)(ey[row] & 1u) - 1 : 0;
+  int incl = d;
+#pragma unroll
+  for (int k = 1; k < 32; k <<= 1) {
+    const int v = __shfl_up_sync(0xFFFFFFFFu, incl, k);
+    if (lane >= k) incl += v;
+  }
+  __syncthreads();
+  if (lane == 31) scan[warp] = incl;
+  __syncthreads();
+  int add = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k)
+    if (k < warp) add += scan[k];
+  long long s1 = 0, s2 = 0;
+  if (live) {
+    const long long B = (long long)(h_before + add + incl) - (2 * (int)(ex[row] & 1u) - 1);
+    long long S1, S2;
+    row_relative_sums(ex + row, ox + row, RH, lut, S1, S2);
+    s1 = (long long)Lx * B + S1;
+    s2 = (long long)Lx * B * B + 2 * B * S1 + S2;
+  }
+  block_sum2<8>(s1, s2, red);
+  if (threadIdx.x == 0) {
+    atomicAdd(out_h + s, (unsigned long long)s1);  // exact: two's-complement wrap-around addition
+    atomicAdd(out_h2 + s, (unsigned long long)s2);
+  }
+}
+
 }  // namespace kpz
