@@ -109,6 +109,7 @@ std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, size_t smem) {
   // CTAs per SM the on-chip kernel is compiled for: two when two samples fit the shared memory of an SM
   add("K5J_MINB", smem != 0 && 2 * (smem + 1024) <= 227 * 1024 ? 2 : 1);
   add("K5J_RIW", debug_int("K5J_RIW", 1));
+  add("K5J_PIPE", debug_int("K5J_PIPE", 1));
   return d;
 }
 

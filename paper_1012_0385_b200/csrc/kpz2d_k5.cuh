@@ -115,21 +115,35 @@ __device__ __forceinline__ Rates2d make_rates2d(const Kpz2dDev& D) {
   return r;
 }
 
+// The two leading bit-planes of the 128 uniforms of supergroup G in colour pass (time, ps): two independent Philox calls.
+struct Planes2 {
+  uint4 v0, v1;
+};
+__device__ __forceinline__ Planes2 draw_two(const PhiloxKeys& K, uint32_t G, uint32_t gs, uint32_t tlo, uint32_t thi, uint32_t ps) {
+  Planes2 R;
+  R.v0 = philox4x32_10(G, gs, tlo, ctr3(TAG_PAIR, ps, 0u, thi), K);
+  R.v1 = philox4x32_10(G, gs, tlo, ctr3(TAG_PAIR, ps, 1u, thi), K);
+  return R;
+}
+// [U < T] from the two leading planes: plane 0 decides unless it equals T's bit, then plane 1
+__device__ __forceinline__ void accept_two(uint32_t (&hop)[4], const uint32_t (&cf)[4], const uint32_t (&cb)[4], const Rates2d& r,
+                                           const Planes2& R) {
+  const uint32_t R0[4] = {R.v0.x, R.v0.y, R.v0.z, R.v0.w}, R1[4] = {R.v1.x, R.v1.y, R.v1.z, R.v1.w};
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const uint32_t lf = r.pf_always | (r.pf0 & ~R0[k]) | (~(R0[k] ^ r.pf0) & r.pf1 & ~R1[k] & r.pf_two);
+    const uint32_t lb = r.pb_always | (r.pb0 & ~R0[k]) | (~(R0[k] ^ r.pb0) & r.pb1 & ~R1[k] & r.pb_two);
+    hop[k] = (cf[k] & lf) | (cb[k] & lb);
+  }
+}
+
 // Accepted moves of one supergroup: cf / cb = forward- / backward-eligible elements of its 4 element-words.
 // Must be called by whole warps (the lazy loop votes).  TWO: both thresholds need at most two planes.
 template <bool TWO>
 __device__ __forceinline__ void accept2d(uint32_t (&hop)[4], const uint32_t (&cf)[4], const uint32_t (&cb)[4], const Rates2d& r,
                                          const PhiloxKeys& K, uint32_t G, uint32_t gs, uint32_t tlo, uint32_t thi, uint32_t ps) {
-  if constexpr (TWO) {  // [U < T] from the two leading planes: plane 0 decides unless it equals T's bit, then plane 1
-    const uint4 v0 = philox4x32_10(G, gs, tlo, ctr3(TAG_PAIR, ps, 0u, thi), K);
-    const uint4 v1 = philox4x32_10(G, gs, tlo, ctr3(TAG_PAIR, ps, 1u, thi), K);
-    const uint32_t R0[4] = {v0.x, v0.y, v0.z, v0.w}, R1[4] = {v1.x, v1.y, v1.z, v1.w};
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const uint32_t lf = r.pf_always | (r.pf0 & ~R0[k]) | (~(R0[k] ^ r.pf0) & r.pf1 & ~R1[k] & r.pf_two);
-      const uint32_t lb = r.pb_always | (r.pb0 & ~R0[k]) | (~(R0[k] ^ r.pb0) & r.pb1 & ~R1[k] & r.pb_two);
-      hop[k] = (cf[k] & lf) | (cb[k] & lb);
-    }
+  if constexpr (TWO) {
+    accept_two(hop, cf, cb, r, draw_two(K, G, gs, tlo, thi, ps));
   } else {
     uint32_t eqf[4], eqb[4];
 #pragma unroll
@@ -173,10 +187,12 @@ __device__ __forceinline__ void st4(uint32_t* p, uint32_t x, uint32_t y, uint32_
 // RIW ("row in warp"): the sgr supergroups of a row are sgr consecutive lanes of ONE warp and the warp is whole: the
 // word to the right and the carry from the left then travel by shuffle and every store is a plain 128-bit store;
 // otherwise word NX is loaded and the two carries are atomic XORs.
+// pre != nullptr (a compile-time fact at every call site): the two planes were drawn earlier (software pipeline).
 template <bool TWO, int C, bool RIW>
 __device__ __forceinline__ void sweep_row_supergroup(uint32_t* EX, uint32_t* OX, uint32_t* EY, uint32_t* OY, int P0, int P1, int NX,
                                                      int kq, int sgr, uint32_t G, bool live, const Rates2d& r, const PhiloxKeys& K,
-                                                     uint32_t gs, uint32_t tlo, uint32_t thi, uint32_t ps) {
+                                                     uint32_t gs, uint32_t tlo, uint32_t thi, uint32_t ps,
+                                                     const Planes2* pre = nullptr) {
   uint32_t* PA = C ? OX : EX;  // the a side of the x-pair: the active sites themselves
   uint32_t* PB = C ? EX : OX;  // the b side: the neighbour to the right
   uint32_t* PY = C ? OY : EY;
@@ -200,7 +216,10 @@ __device__ __forceinline__ void sweep_row_supergroup(uint32_t* EX, uint32_t* OX,
     cf[k] = a[k] & ~b[k] & ya[k] & ~yb[k];                 // both pairs (1,0)
     cb[k] = ~a[k] & b[k] & ~ya[k] & yb[k];                 // both pairs (0,1)
   }
-  accept2d<TWO>(hop, cf, cb, r, K, G, gs, tlo, thi, ps);
+  if (pre)
+    accept_two(hop, cf, cb, r, *pre);
+  else
+    accept2d<TWO>(hop, cf, cb, r, K, G, gs, tlo, thi, ps);
   uint32_t cin = 0;
   if (C && RIW) cin = __shfl_sync(0xFFFFFFFFu, hop[3] >> 31, kq == 0 ? lane + (sgr - 1) : lane - 1);
   if (!live) return;
@@ -437,12 +456,35 @@ __device__ __forceinline__ void row_sums_onchip(const uint32_t* EX, const uint32
   }
 }
 
+// Split barrier of a CTA (one arrival per warp): arrive after a pass's stores, wait before the next pass's loads, with
+// work that needs no shared memory (the next pass's Philox calls) in between.
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}" ::"r"(bar) : "memory");
+}
+// keep: values that must have been computed BEFORE the wait (the compiler may not sink them past it)
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, const Planes2& keep) {
+  asm volatile(
+      "{\n.reg .pred p;\n"
+      "K5_WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@!p bra K5_WAIT_%=;\n}" ::"r"(bar),
+      "r"(parity), "r"(keep.v0.x), "r"(keep.v0.y), "r"(keep.v0.z), "r"(keep.v0.w), "r"(keep.v1.x), "r"(keep.v1.y), "r"(keep.v1.z),
+      "r"(keep.v1.w)
+      : "memory");
+}
+
 // K5S: a whole sample on chip.  A pass is the sweep on shared memory followed by ONE __syncthreads (a pass reads only
 // bits no other thread of the pass touches, so nothing else orders it); colour offsets are drawn in the kernel 16 MCS at a
 // time (one Philox call per lane + ballot); records are taken from shared memory.
 constexpr int kK5SThreads = 512;
 
-template <bool ROWALIGNED, bool TWO, bool RIW>
+// PIPE (fast path with two-plane thresholds and at most one supergroup per thread and row parity): the planes of the
+// next sweep are drawn one sweep ahead, and the CTA barrier after a pass is split (mbarrier) around that draw.
+template <bool ROWALIGNED, bool TWO, bool RIW, bool PIPE>
 __device__ __forceinline__ void onchip_body(const Kpz2dDev& D, const Kpz2dRun& A) {
   extern __shared__ __align__(16) uint32_t k5s_smem[];
   __shared__ long long red[2 * (kK5SThreads / 32)];
@@ -480,10 +522,51 @@ __device__ __forceinline__ void onchip_body(const Kpz2dDev& D, const Kpz2dRun& A
   };
   if (D.offset_mode == 0) draw_offsets(A.t0);
   const int sgr = RH / 4, nh = sh.n_sg / 2;  // fast path: supergroups per row; per row parity
+  // PIPE: this thread's supergroup of each row parity, fixed for the whole run
+  __shared__ unsigned long long mbar_word;
+  const uint32_t mbar = smem_addr(&mbar_word);
+  uint32_t phase = 0;
+  const bool pl_live = (int)threadIdx.x < nh;
+  const int pl_i = pl_live ? (int)threadIdx.x : 0, pl_rr = pl_i / sgr, pl_kq = pl_i - pl_rr * sgr;
+  const uint32_t pl_G0 = (uint32_t)(2 * pl_rr * sgr + pl_kq), pl_G1 = pl_G0 + (uint32_t)sgr;
+  Planes2 pl_R;
+  if constexpr (PIPE) {
+    if (threadIdx.x == 0) mbar_init(mbar, kK5SThreads / 32);
+    __syncthreads();
+    pl_R = draw_two(D.keys, pl_G0, gs, (uint32_t)A.t0, (uint32_t)((unsigned long long)A.t0 >> 32), 0u);
+  }
   for (long long m = A.t0; m < A.t0 + A.n_mcs; ++m) {
     const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
     for (int ps = 0; ps < 2; ++ps) {
       const uint32_t o = D.offset_mode ? (uint32_t)ps : ((offbits >> (2 * ((int)m & 15) + ps)) & 1u);
+      if constexpr (PIPE) {
+        const int P0e = pl_rr * RH + 4 * pl_kq, P0o = P0e + half * RH;  // own row: even rows first, then odd rows
+        const int P1o = (pl_rr + 1 == half ? 0 : pl_rr + 1) * RH + 4 * pl_kq;  // row y + 1 of an odd row: the next even row
+        const int nxw = pl_kq + 1 == sgr ? 0 : 4 * (pl_kq + 1);
+        // even rows (colour o), with the planes drawn one sweep ago; then draw those of the odd rows
+        if (o)
+          sweep_row_supergroup<TWO, 1, RIW>(EX, OX, EY, OY, P0e, P0o, pl_rr * RH + nxw, pl_kq, sgr, pl_G0, pl_live, r, D.keys, gs, tlo, thi,
+                                            (uint32_t)ps, &pl_R);
+        else
+          sweep_row_supergroup<TWO, 0, RIW>(EX, OX, EY, OY, P0e, P0o, pl_rr * RH + nxw, pl_kq, sgr, pl_G0, pl_live, r, D.keys, gs, tlo, thi,
+                                            (uint32_t)ps, &pl_R);
+        pl_R = draw_two(D.keys, pl_G1, gs, tlo, thi, (uint32_t)ps);
+        if (o)
+          sweep_row_supergroup<TWO, 0, RIW>(EX, OX, EY, OY, P0o, P1o, (pl_rr + half) * RH + nxw, pl_kq, sgr, pl_G1, pl_live, r, D.keys, gs,
+                                            tlo, thi, (uint32_t)ps, &pl_R);
+        else
+          sweep_row_supergroup<TWO, 1, RIW>(EX, OX, EY, OY, P0o, P1o, (pl_rr + half) * RH + nxw, pl_kq, sgr, pl_G1, pl_live, r, D.keys, gs,
+                                            tlo, thi, (uint32_t)ps, &pl_R);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(mbar);
+        {  // the first sweep of the next pass, drawn while the other warps finish this one
+          const long long mn = ps ? m + 1 : m;
+          pl_R = draw_two(D.keys, pl_G0, gs, (uint32_t)mn, (uint32_t)((unsigned long long)mn >> 32), (uint32_t)(ps ^ 1));
+        }
+        mbar_wait(mbar, phase, pl_R);
+        phase ^= 1u;
+        continue;
+      }
       if constexpr (ROWALIGNED) {
         for (int h = 0; h < 2; ++h) {  // even rows, then odd rows: one colour for the whole CTA
           const bool c1 = (((uint32_t)h + o) & 1u) != 0u;
@@ -539,10 +622,11 @@ constexpr bool kJRowAligned = (K5J_LX % 256) == 0;
 constexpr int kJSgr = K5J_LX / 256;                   // supergroups per row (fast path)
 constexpr int kJNh = K5J_LX / 256 * K5J_LY / 2;       // supergroups per row parity
 constexpr bool kJRiw = kJRowAligned && kJSgr <= 32 && (32 % (kJSgr > 0 ? kJSgr : 1)) == 0 && (kJNh % 32) == 0 && K5J_RIW;
+constexpr bool kJPipe = kJRowAligned && (K5J_TWO != 0) && kJNh <= kK5SThreads && K5J_PIPE;
 
 extern "C" __global__ void __launch_bounds__(kK5SThreads, K5J_MINB)
     kpz2d_k5s_jit(const __grid_constant__ Kpz2dDev D, const __grid_constant__ Kpz2dRun A) {
-  onchip_body<kJRowAligned, K5J_TWO != 0, kJRiw>(D, A);
+  onchip_body<kJRowAligned, K5J_TWO != 0, kJRiw, kJPipe>(D, A);
 }
 extern "C" __global__ void __launch_bounds__(128)
     kpz2d_k5_pass_jit(const __grid_constant__ Kpz2dDev D, const unsigned char* __restrict__ off, long long m, int ps) {
@@ -557,7 +641,7 @@ __global__ void __launch_bounds__(128) k2d_pass(const __grid_constant__ Kpz2dDev
 }
 template <bool ROWALIGNED, bool TWO>
 __global__ void __launch_bounds__(kK5SThreads, 2) k2d_onchip(const __grid_constant__ Kpz2dDev D, const __grid_constant__ Kpz2dRun A) {
-  onchip_body<ROWALIGNED, TWO, false>(D, A);
+  onchip_body<ROWALIGNED, TWO, false, false>(D, A);
 }
 #endif
 

@@ -63,8 +63,9 @@ def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_
 
 # 1 = a sample in shared memory (K5S), 2 = one launch per colour pass (K5); each as the run-time specialised kernel
 # (NVRTC: shape and thresholds are constants) and as the generic kernel of the library build ("jit=0"); K5J_RIW=0 takes
-# the shuffles out of the specialised on-chip kernel (neighbour word loaded, carries by atomics)
-PATHS = [(1, ""), (2, ""), (1, "jit=0"), (2, "jit=0"), (1, "K5J_RIW=0")]
+# the shuffles out of the specialised on-chip kernel (neighbour word loaded, carries by atomics), K5J_PIPE=0 its
+# software pipeline (planes drawn one sweep ahead around a split barrier)
+PATHS = [(1, ""), (2, ""), (1, "jit=0"), (2, "jit=0"), (1, "K5J_RIW=0"), (1, "K5J_PIPE=0")]
 
 
 @pytest.mark.parametrize("path", PATHS)
