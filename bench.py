@@ -79,7 +79,7 @@ ALU_SLOTS_PER_SU = {
 # 2+1D generalisation: per Philox supergroup (128 elements = the active half of 256 sites of a row) and
 # colour pass: p = 0.75 needs 2 planes (2 x 34 slots); per 32-site word 3 LOP3/SHF for the two-pair eligibility, 1 for the
 # acceptance, 2 for the flips of sx (the sy flips are memory operations); 2 passes per MCS over Lx Ly / 256 supergroups
-ALU_SLOTS_PER_SU["2d-1024"] = ALU_SLOTS_PER_SU["2d-512"] = 2 * (2 * 34 + 8 * 6) / 256
+ALU_SLOTS_PER_SU["2d-1024"] = ALU_SLOTS_PER_SU["2d-512"] = ALU_SLOTS_PER_SU["2d-512-cluster"] = 2 * (2 * 34 + 8 * 6) / 256
 for _L in (512, 1024, 2048, 4096, 8192, 16384, 32768):   # the paper's size scan: same rates and schedule as paper-1024x30
     ALU_SLOTS_PER_SU[f"paper-scan-{_L}"] = ALU_SLOTS_PER_SU["paper-1024x30"]
 # default run: the headline first, then the other BASELINE configs and the auxiliary streamed runs of SURVEY §8(d)
@@ -255,7 +255,7 @@ def make_sim(pkg, cfg, first_sample):
                            independent=cfg.get("independent", 0))
     elif cfg["kind"] == "kpz2d":
         sim = pkg.Kpz2dSim(cfg["Lx"], cfg["Ly"], cfg["S"], cfg["p"], cfg["q"], seed=cfg["seed"], first_sample=first_sample,
-                           max_records=nrec, offset_mode=cfg.get("offset_mode", 0))
+                           max_records=nrec, offset_mode=cfg.get("offset_mode", 0), path=cfg.get("path", 0))
     else:
         sim = pkg.KpzSim(cfg["L"], cfg["S"], cfg["p"], cfg["q"], disorder=cfg["disorder"], seed=cfg["seed"],
                          first_sample=first_sample, max_records=nrec, path=cfg.get("path", 0),
@@ -355,7 +355,9 @@ def bench_one(ctx, args, cfg_key, with_cpu):
     path = sim.path if cfg["kind"] == "kpz" else 1
     path_name = {"kpz": PATH_NAMES.get(path), "lanes": "two-lane K4", "kpz2d": "2+1D checkerboard K5"}[cfg["kind"]]
     if cfg["kind"] == "kpz2d":
-        path_name += " (a sample in shared memory, one launch per run)" if sim.path == 1 else " (one launch per colour pass)"
+        path_name += {1: " (K5S: a sample in the shared memory of a CTA, one launch per run)",
+                      3: " (K5C: a sample over the shared memories of a thread-block cluster, one launch per run)"
+                      }.get(sim.path, " (K5: one launch per colour pass)")
     ms_run = ms_run_total / args.steps
     roof = roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run, sim_path=sim.path if cfg["kind"] == "kpz2d" else 0)
     cpu = None
@@ -491,7 +493,8 @@ def roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run, sim_path=0):
                 "peak_source": peaks["source"], "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
     slots = ALU_SLOTS_PER_SU.get(cfg_key)
     kname = {1: "kpz_k1_sweep_jit", 3: "kpz_k3t_sweep_jit"}.get(path, "kpz_k1_sweep_jit") if cfg["kind"] == "kpz" \
-        else (("k2d_onchip" if sim_path == 1 else "k2d_pass") if cfg["kind"] == "kpz2d" else "lanes_k4_sweep_jit")
+        else ({1: "kpz2d_k5s_jit", 3: "kpz2d_k5c_jit"}.get(sim_path, "kpz2d_k5_pass_jit") if cfg["kind"] == "kpz2d"
+              else "lanes_k4_sweep_jit")
     if slots is None:
         return {"bound": "alu", "kernel": kname, "achieved": None, "peak": None, "unit": "Tslot/s", "frac": None,
                 "traffic": traffic, "reason": f"no algorithmic slot count is modelled for workload key {cfg_key!r}"}

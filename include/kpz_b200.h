@@ -58,6 +58,7 @@ typedef struct {
 #define KPZ_PATH_ONCHIP 1
 #define KPZ_PATH_STREAM 2
 #define KPZ_PATH_BLOCKED 3
+#define KPZ2D_PATH_CLUSTER 3 /* kpz2d_* only: a sample on chip, spread over a thread-block cluster (K5C) */
 
 /* ---- KPZ / ASEP ring ensemble ----------------------------------------------------------------------------- */
 
@@ -205,8 +206,11 @@ int kpz2d_set_record_times(kpz2d_sim*, const int64_t* t, int32_t nt); /* as kpz_
  * h(x,0) = sum_{i<=x} (2 sx[0][i] - 1), h(x,y) = h(x,y-1) + 2 sy[y][x] - 1 at the record times.  Asynchronous. */
 int kpz2d_run(kpz2d_sim*, int64_t n_mcs);
 int kpz2d_time(const kpz2d_sim*, int64_t* t);
-/* 1 = a whole sample in shared memory, one persistent launch per kpz2d_run (auto up to 96 KiB of slopes per sample, e.g.
- * 512 x 512; options.path = 1 forces it up to 200 KiB), 2 = one in-place launch per colour pass (options.path = 2). */
+/* 1 = a whole sample in the shared memory of one CTA, one persistent launch per kpz2d_run (auto up to 96 KiB of slopes
+ * per sample, e.g. 512 x 512; options.path = 1 forces it up to 200 KiB); 3 (KPZ2D_PATH_CLUSTER) = a sample spread over
+ * the shared memories of a thread-block cluster of 2, 4 or 8 CTAs, neighbour rows through distributed shared memory, one
+ * persistent launch (auto beyond 96 KiB when Lx is a multiple of 256 and the rows divide, up to 800 KiB per sample, e.g.
+ * 1024 x 1024; run-time specialised kernels only); 2 = one in-place launch per colour pass (everything else). */
 int kpz2d_path(const kpz2d_sim*, int32_t* path);
 int kpz2d_reset(kpz2d_sim*);                                          /* flat surface, t = 0, records dropped; async */
 int kpz2d_slopes(kpz2d_sim*, uint32_t* d_sx, uint32_t* d_sy);        /* copy out (either may be NULL); async */

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(HERE, "libkpz_b200.so")
 HOOKS_PATH = os.path.join(HERE, "libkpz_b200_testhooks.so")
 
 KPZ_PATH_AUTO, KPZ_PATH_ONCHIP, KPZ_PATH_STREAM, KPZ_PATH_BLOCKED = 0, 1, 2, 3
+KPZ2D_PATH_CLUSTER = 3     # kpz2d_* only: a sample on chip, spread over a thread-block cluster
 
 
 class KpzError(RuntimeError):

@@ -31,14 +31,55 @@ constexpr size_t kOnchipBytes = 96 * 1024;  // both slope fields of a sample in 
 
 size_t onchip_bytes(int32_t Lx, int32_t Ly) { return (size_t)4 * Ly * (Lx / 64) * 4; }  // 4 parity planes of Ly * Lx/64 words
 
-// options.path: 0 auto (on chip when the sample fits), 1 on chip (k2d_onchip), 2 streamed (k2d_pass per colour pass)
+// K5C: a sample spread over a cluster of cs CTAs (kpz2d_k5.cuh): one supergroup per thread and row parity.
+struct ClusterShape {
+  int cs = 0, threads = 0, minb = 1;
+  size_t smem = 0;  // dynamic shared memory per CTA
+};
+constexpr int KPZ2D_CLUSTER = KPZ2D_PATH_CLUSTER;
+
+// The smallest cluster (2, 4, 8 CTAs; "K5J_CS=n" forces one) whose CTAs hold their rows in at most 100 KiB (two CTAs per
+// SM) with at most 512 supergroups per row parity.  False when no such cluster exists for this shape.
+bool cluster_shape(int32_t Lx, int32_t Ly, ClusterShape* out) {
+  if (Lx % 256 != 0) return false;
+  const int forced = debug_int("K5J_CS", 0);
+  // measured (profiles/r02_summary.md §6): CTAs of at most 256 threads run best, so that size is looked for first
+  for (int pass = 0; pass < 2; ++pass)
+  for (int cs : {2, 4, 8}) {
+    if (forced && cs != forced) continue;
+    if (Ly % (2 * cs) != 0) continue;
+    const size_t smem = onchip_bytes(Lx, Ly) / cs;
+    const int nh = Lx / 256 * (Ly / cs) / 2;
+    if (nh > (pass == 0 && !forced ? 256 : 512) || smem > 100 * 1024) continue;
+    ClusterShape c;
+    c.cs = cs;
+    c.smem = smem;
+    c.threads = std::max(32, (nh + 31) / 32 * 32);
+    const int by_regs = 1024 / c.threads;  // 64 registers per thread
+    const int by_smem = (int)((227 * 1024) / (smem + 3 * 1024));
+    c.minb = std::max(1, std::min({by_regs, by_smem, 16}));
+    *out = c;
+    return true;
+  }
+  return false;
+}
+
+// options.path: 0 auto, 1 on chip (K5S: a sample in the shared memory of one CTA), 2 streamed (K5: one launch per colour
+// pass), 3 on chip over a thread-block cluster (K5C).  auto: K5S when the sample fits 96 KiB, else K5C when a cluster
+// shape exists (and run-time specialisation is on), else K5.
 int choose_path2d(int32_t Lx, int32_t Ly, const kpz_options* opt, int* path) {
   const size_t bytes = onchip_bytes(Lx, Ly);
   int want = opt ? opt->path : KPZ_PATH_AUTO;
-  if (want == KPZ_PATH_AUTO) want = bytes <= kOnchipBytes ? KPZ_PATH_ONCHIP : KPZ_PATH_STREAM;
+  ClusterShape cshape;
+  const bool can_cluster = jit_enabled() && cluster_shape(Lx, Ly, &cshape);
+  if (want == KPZ_PATH_AUTO) want = bytes <= kOnchipBytes ? KPZ_PATH_ONCHIP : (can_cluster ? KPZ2D_CLUSTER : KPZ_PATH_STREAM);
   if (want == KPZ_PATH_ONCHIP && bytes > 200 * 1024)
     return fail(KPZ_EUNSUPPORTED, "the on-chip 2+1D path holds at most 200 KiB of slopes per sample (%zu needed)", bytes);
-  if (want != KPZ_PATH_ONCHIP && want != KPZ_PATH_STREAM) return fail(KPZ_EINVAL, "options.path must be 0, 1 or 2 here");
+  if (want == KPZ2D_CLUSTER && !can_cluster)
+    return fail(KPZ_EUNSUPPORTED, "no thread-block cluster shape for %d x %d (needs Lx %% 256 == 0, Ly %% 4 == 0, at most 800 KiB of "
+                                  "slopes per sample, run-time specialisation on)", Lx, Ly);
+  if (want != KPZ_PATH_ONCHIP && want != KPZ_PATH_STREAM && want != KPZ2D_CLUSTER)
+    return fail(KPZ_EINVAL, "options.path must be 0, 1, 2 or 3 here");
   *path = want;
   return KPZ_OK;
 }
@@ -90,7 +131,7 @@ Layout2d layout2d(int32_t Lx, int32_t Ly, int32_t S, int32_t max_records) {
 bool two_planes(const Kpz2dDev& D) { return planes_needed(D.t_p) <= 2 && planes_needed(D.t_q) <= 2; }
 
 // Definitions of the run-time specialised kernels (kpz2d_k5.cuh under NVRTC): shape, thresholds, launch shape.
-std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, size_t smem) {
+std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, size_t smem, const ClusterShape* cl = nullptr) {
   char buf[64];
   std::vector<std::string> d;
   auto add = [&](const char* name, long long v) {
@@ -107,9 +148,12 @@ std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, size_t smem) {
   add("K5J_TQ_ALWAYS", D.t_q.always);
   add("K5J_TWO", two_planes(D) ? 1 : 0);
   // CTAs per SM the on-chip kernel is compiled for: two when two samples fit the shared memory of an SM
-  add("K5J_MINB", smem != 0 && 2 * (smem + 1024) <= 227 * 1024 ? 2 : 1);
+  add("K5J_MINB", cl ? cl->minb : (smem != 0 && 2 * (smem + 1024) <= 227 * 1024 ? 2 : 1));
+  add("K5J_CS", cl ? cl->cs : 1);
+  add("K5J_THREADS", cl ? cl->threads : 512);
   add("K5J_RIW", debug_int("K5J_RIW", 1));
   add("K5J_PIPE", debug_int("K5J_PIPE", 1));
+  if (debug_has("K5J_XRALL")) add("K5J_XRALL", debug_int("K5J_XRALL", 0));
   return d;
 }
 
@@ -216,8 +260,14 @@ int kpz2d_jit_check(int32_t Lx, int32_t Ly, double p, double q, const kpz_option
   D.Ly = Ly;
   std::vector<char> cubin;
   const bool onchip = path == KPZ_PATH_ONCHIP;
-  rc = jit_compile("kpz2d_k5.cuh", onchip ? "kpz2d_k5s_jit" : "kpz2d_k5_pass_jit",
-                   k5_jit_defines(D, onchip ? onchip_bytes(Lx, Ly) : 0), &cubin, nullptr);
+  if (path == KPZ2D_CLUSTER) {
+    ClusterShape cl;
+    cluster_shape(Lx, Ly, &cl);
+    rc = jit_compile("kpz2d_k5.cuh", "kpz2d_k5c_jit", k5_jit_defines(D, cl.smem, &cl), &cubin, nullptr);
+  } else {
+    rc = jit_compile("kpz2d_k5.cuh", onchip ? "kpz2d_k5s_jit" : "kpz2d_k5_pass_jit",
+                     k5_jit_defines(D, onchip ? onchip_bytes(Lx, Ly) : 0), &cubin, nullptr);
+  }
   if (rc) return rc;
   *cubin_bytes = cubin.size();
   return KPZ_OK;
@@ -263,7 +313,7 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
   const int nt = (int)sim->rec_times.size();
   int ri = sim->nrec;
   if (n_mcs == 0) return KPZ_OK;
-  if (sim->path == KPZ_PATH_ONCHIP) {
+  if (sim->path == KPZ_PATH_ONCHIP || sim->path == KPZ2D_CLUSTER) {
     Kpz2dRun A{};
     A.t0 = sim->t;
     A.n_mcs = n_mcs;
@@ -273,7 +323,23 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
     A.rec_h = sim->rec_h;
     A.rec_h2 = sim->rec_h2;
     const size_t smem = onchip_bytes(D.Lx, D.Ly);
-    if (jit_enabled()) {  // specialised on the shape and the thresholds (NVRTC)
+    if (sim->path == KPZ2D_CLUSTER) {  // K5C: the CTAs of a cluster add their rows' sums into the records
+      ClusterShape cl;
+      if (!jit_enabled() || !cluster_shape(D.Lx, D.Ly, &cl))
+        return fail(KPZ_EUNSUPPORTED, "the cluster path needs run-time specialisation (kpz_debug_config jit=0 is set)");
+      if (ri < nt) {
+        const size_t off = (size_t)ri * D.S * 8, len = (size_t)(nt - ri) * D.S * 8;
+        KPZ_CUDA_CHECK(cudaMemsetAsync((char*)sim->rec_h + off, 0, len, sim->stream));
+        KPZ_CUDA_CHECK(cudaMemsetAsync((char*)sim->rec_h2 + off, 0, len, sim->stream));
+      }
+      void* kfn = nullptr;
+      int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5c_jit", k5_jit_defines(D, cl.smem, &cl), &kfn);
+      if (rc) return rc;
+      void* args[] = {(void*)&D, (void*)&A};
+      KPZ_CUDA_CHECK(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cl.smem));
+      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(D.S * cl.cs), dim3(cl.threads), args, cl.smem, sim->stream));
+      count_launch();
+    } else if (jit_enabled()) {  // specialised on the shape and the thresholds (NVRTC)
       void* kfn = nullptr;
       int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5s_jit", k5_jit_defines(D, smem), &kfn);
       if (rc) return rc;

@@ -38,6 +38,10 @@
 #include "sweep_types.cuh"
 #include "height_lut.cuh"
 
+#ifndef K5J_XRALL
+#define K5J_XRALL 0  // 1: every warp of K5C reaches row y + 1 through shared::cluster addresses (debug)
+#endif
+
 namespace kpz {
 
 struct Kpz2dDev {
@@ -175,6 +179,35 @@ __device__ __forceinline__ void accept2d(uint32_t (&hop)[4], const uint32_t (&cf
   }
 }
 
+// Distributed shared memory of a thread-block cluster (K5C): a 32-bit shared::cluster address names a word of any CTA
+// of the cluster (mapa), loads / stores on it reach that CTA's shared memory; barrier.cluster orders them.
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t mapa(uint32_t cta_addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(cta_addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ uint4 ld4_cluster(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.shared::cluster.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st4_cluster(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+  asm volatile("st.shared::cluster.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+__device__ __forceinline__ int ld_cluster_s32(uint32_t a) {
+  int v;
+  asm volatile("ld.shared::cluster.s32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
 __device__ __forceinline__ uint4 ld4(const uint32_t* p) { return *reinterpret_cast<const uint4*>(p); }
 __device__ __forceinline__ void st4(uint32_t* p, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
   *reinterpret_cast<uint4*>(p) = make_uint4(x, y, z, w);
@@ -188,11 +221,13 @@ __device__ __forceinline__ void st4(uint32_t* p, uint32_t x, uint32_t y, uint32_
 // word to the right and the carry from the left then travel by shuffle and every store is a plain 128-bit store;
 // otherwise word NX is loaded and the two carries are atomic XORs.
 // pre != nullptr (a compile-time fact at every call site): the two planes were drawn earlier (software pipeline).
-template <bool TWO, int C, bool RIW>
+// XR: the words of row y + 1 are reached through the shared::cluster address xr1 (they may lie in the next CTA of the
+// cluster: K5C) instead of PY + P1.
+template <bool TWO, int C, bool RIW, bool XR = false>
 __device__ __forceinline__ void sweep_row_supergroup(uint32_t* EX, uint32_t* OX, uint32_t* EY, uint32_t* OY, int P0, int P1, int NX,
                                                      int kq, int sgr, uint32_t G, bool live, const Rates2d& r, const PhiloxKeys& K,
                                                      uint32_t gs, uint32_t tlo, uint32_t thi, uint32_t ps,
-                                                     const Planes2* pre = nullptr) {
+                                                     const Planes2* pre = nullptr, uint32_t xr1 = 0) {
   uint32_t* PA = C ? OX : EX;  // the a side of the x-pair: the active sites themselves
   uint32_t* PB = C ? EX : OX;  // the b side: the neighbour to the right
   uint32_t* PY = C ? OY : EY;
@@ -202,7 +237,7 @@ __device__ __forceinline__ void sweep_row_supergroup(uint32_t* EX, uint32_t* OX,
     va = ld4(PA + P0);
     vb = ld4(PB + P0);
     v0 = ld4(PY + P0);
-    v1 = ld4(PY + P1);
+    v1 = XR ? ld4_cluster(xr1) : ld4(PY + P1);
     if (C && !RIW) e4 = PB[NX];
   }
   const int lane = (int)(threadIdx.x & 31u);
@@ -225,7 +260,10 @@ __device__ __forceinline__ void sweep_row_supergroup(uint32_t* EX, uint32_t* OX,
   if (!live) return;
   st4(PA + P0, a[0] ^ hop[0], a[1] ^ hop[1], a[2] ^ hop[2], a[3] ^ hop[3]);
   st4(PY + P0, ya[0] ^ hop[0], ya[1] ^ hop[1], ya[2] ^ hop[2], ya[3] ^ hop[3]);
-  st4(PY + P1, yb[0] ^ hop[0], yb[1] ^ hop[1], yb[2] ^ hop[2], yb[3] ^ hop[3]);
+  if (XR)
+    st4_cluster(xr1, yb[0] ^ hop[0], yb[1] ^ hop[1], yb[2] ^ hop[2], yb[3] ^ hop[3]);
+  else
+    st4(PY + P1, yb[0] ^ hop[0], yb[1] ^ hop[1], yb[2] ^ hop[2], yb[3] ^ hop[3]);
   if (C) {  // the b side is bit j + 1 of EX: the flips move up by one bit, the top bit into the next word
     const uint32_t f1 = __funnelshift_l(hop[0], hop[1], 1), f2 = __funnelshift_l(hop[1], hop[2], 1),
                    f3 = __funnelshift_l(hop[2], hop[3], 1);
@@ -418,17 +456,18 @@ __device__ __forceinline__ void row_relative_sums(const uint32_t* ex, const uint
 // (2 sy[y'][0] - 1).  Equal to the column-wise definition on every single-valued surface - which the
 // dynamics preserve (every move flips the four slopes around one site) - and about ten times cheaper than walking each
 // column bit by bit.  NT threads, all call.
+// The planes hold rows yg0 .. yg0 + Ly - 1 of the sample (K5C: the rows of one CTA of the cluster; else yg0 = 0);
+// carry = h(0, yg0 - 1), or h(0,0) when yg0 = 0.
 template <int NT>
 __device__ __forceinline__ void row_sums_onchip(const uint32_t* EX, const uint32_t* OX, const uint32_t* EY, int RH, int half, int Lx,
-                                                int Ly, const uint32_t* lut, int* scan /* [NT / 32] shared */, long long& s1,
-                                                long long& s2) {
+                                                int Ly, int yg0, int carry, const uint32_t* lut, int* scan /* [NT / 32] shared */,
+                                                long long& s1, long long& s2) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  int carry = 2 * (int)(EX[0] & 1u) - 1;  // h(0,0); row 0 is slot 0 in both row orders
   for (int y0 = 0; y0 < Ly; y0 += NT) {   // block-uniform trip count
     const int y = y0 + (int)threadIdx.x;
     const bool live = y < Ly;
     const int row = (live ? (half ? (y >> 1) + (y & 1) * half : y) : 0) * RH;
-    const int d = (live && y > 0) ? 2 * (int)(EY[row] & 1u) - 1 : 0;  // h(0,y) - h(0,y-1)
+    const int d = (live && yg0 + y > 0) ? 2 * (int)(EY[row] & 1u) - 1 : 0;  // h(0,y) - h(0,y-1)
     int incl = d;
 #pragma unroll
     for (int k = 1; k < 32; k <<= 1) {
@@ -458,7 +497,6 @@ __device__ __forceinline__ void row_sums_onchip(const uint32_t* EX, const uint32
 
 // Split barrier of a CTA (one arrival per warp): arrive after a pass's stores, wait before the next pass's loads, with
 // work that needs no shared memory (the next pass's Philox calls) in between.
-__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
@@ -526,7 +564,7 @@ __device__ __forceinline__ void onchip_body(const Kpz2dDev& D, const Kpz2dRun& A
   __shared__ unsigned long long mbar_word;
   const uint32_t mbar = smem_addr(&mbar_word);
   uint32_t phase = 0;
-  const bool pl_live = (int)threadIdx.x < nh;
+  const bool pl_live = nh >= kK5SThreads || (int)threadIdx.x < nh;  // a constant when every thread holds a supergroup
   const int pl_i = pl_live ? (int)threadIdx.x : 0, pl_rr = pl_i / sgr, pl_kq = pl_i - pl_rr * sgr;
   const uint32_t pl_G0 = (uint32_t)(2 * pl_rr * sgr + pl_kq), pl_G1 = pl_G0 + (uint32_t)sgr;
   Planes2 pl_R;
@@ -596,7 +634,7 @@ __device__ __forceinline__ void onchip_body(const Kpz2dDev& D, const Kpz2dRun& A
     const long long t = m + 1;
     if (t == next_rec) {  // block-uniform
       long long s1 = 0, s2 = 0;
-      row_sums_onchip<kK5SThreads>(EX, OX, EY, RH, half, sh.Lx, Ly, lut, scan, s1, s2);
+      row_sums_onchip<kK5SThreads>(EX, OX, EY, RH, half, sh.Lx, Ly, 0, 2 * (int)(EX[0] & 1u) - 1, lut, scan, s1, s2);  // row 0 = slot 0
       block_sum2<kK5SThreads / 32>(s1, s2, red);
       if (threadIdx.x == 0) {
         A.rec_h[(size_t)ri * D.S + s] = s1;
@@ -616,6 +654,142 @@ __device__ __forceinline__ void onchip_body(const Kpz2dDev& D, const Kpz2dRun& A
   }
 }
 
+// K5C: a sample spread over a thread-block cluster of CS CTAs (lattices beyond the shared memory of one SM, e.g.
+// 1024 x 1024 = 256 KiB of slopes; also: more, smaller CTAs balance better over the 148 SMs).  CTA q holds rows
+// q Ly/CS .. (q + 1) Ly/CS - 1 in its own shared memory, by parity as K5S does; the only words of another CTA a sweep
+// touches are the first even row of CTA q + 1 (row y + 1 of this CTA's last odd row), read and written through
+// distributed shared memory.  One barrier.cluster per colour pass, split (arrive ... wait) around the Philox calls of
+// the next pass.  One supergroup per thread and row parity (NT >= Ly/CS/2 * Lx/256); run-time specialised only.
+template <bool TWO, bool RIW, int CS, int NT>
+__device__ __forceinline__ void cluster_body(const Kpz2dDev& D, const Kpz2dRun& A) {
+  extern __shared__ __align__(16) uint32_t k5s_smem[];
+  __shared__ long long red[2 * (NT / 32)];
+  __shared__ uint32_t lut[256];
+  __shared__ int scan[NT / 32];
+  __shared__ int col0[2];  // [0]: sum over this CTA's rows of h(0,y) - h(0,y-1); [1]: h(0,0) (CTA 0)
+  for (int i = threadIdx.x; i < 256; i += NT) lut[i] = height_lut_entry(i);
+  const Shape2d sh = shape2d(D);
+  const uint32_t q = cluster_ctarank();
+  const int s = blockIdx.x / CS;
+  const int RH = sh.RH, LyC = sh.Ly / CS, half = LyC / 2, plane = LyC * RH, yg0 = (int)q * LyC;
+  uint32_t* EX = k5s_smem;
+  uint32_t* OX = EX + plane;
+  uint32_t* EY = OX + plane;
+  uint32_t* OY = EY + plane;
+  const size_t base = (size_t)s * sh.Ly * RH + (size_t)q * plane;  // this CTA's rows in the workspace
+  for (int i = threadIdx.x; i < plane; i += NT) {
+    const int y = i / RH, k = i - y * RH, j = ((y >> 1) + (y & 1) * half) * RH + k;
+    EX[j] = D.EX[base + i];
+    OX[j] = D.OX[base + i];
+    EY[j] = D.EY[base + i];
+    OY[j] = D.OY[base + i];
+  }
+  cluster_arrive();  // every CTA of the cluster holds its rows before a neighbour reaches into them
+  cluster_wait();
+  const int lane = threadIdx.x & 31;
+  const uint32_t gs = (uint32_t)(D.first_sample + s);
+  const Rates2d r = make_rates2d(D);
+  int ri = A.rec_begin;
+  long long next_rec = ri < A.nt ? A.rec_t[ri] : -1;
+  uint32_t offbits = 0;
+  auto draw_offsets = [&](long long m) {  // bit 2 k + ps = offset of pass ps of MCS (m & ~15) + k
+    const unsigned long long mb = ((unsigned long long)m & ~15ull) + (unsigned)(lane >> 1);
+    const uint4 w = philox4x32_10(0u, gs, (uint32_t)mb, ctr3(TAG_OFFSET, lane & 1, 0, (uint32_t)(mb >> 32)), D.keys);
+    offbits = __ballot_sync(0xFFFFFFFFu, w.x & 1u);
+  };
+  if (D.offset_mode == 0) draw_offsets(A.t0);
+  // this thread's supergroup of each row parity, fixed for the whole run
+  const int sgr = RH / 4, nh = half * sgr;
+  const bool live = nh >= NT || (int)threadIdx.x < nh;
+  const int ti = live ? (int)threadIdx.x : 0, rr = ti / sgr, kq = ti - rr * sgr;
+  const uint32_t G0 = (uint32_t)((yg0 + 2 * rr) * sgr + kq), G1 = G0 + (uint32_t)sgr;
+  const int P0e = rr * RH + 4 * kq, P0o = P0e + half * RH, nxw = kq + 1 == sgr ? 0 : 4 * (kq + 1);
+  // row y + 1 of an odd row: the next even row - of the next CTA (cyclically) for this CTA's last odd row
+  const bool edge = rr + 1 == half;
+  const int P1o = (edge ? 0 : rr + 1) * RH + 4 * kq;
+  const uint32_t nbr = edge ? (q + 1 == (uint32_t)CS ? 0u : q + 1u) : q;
+  const uint32_t xrE = mapa(smem_addr(EY + P1o), nbr), xrO = mapa(smem_addr(OY + P1o), nbr);
+  const bool warp_edge = __any_sync(0xFFFFFFFFu, live && edge) || K5J_XRALL;
+  Planes2 R;
+  const Planes2* pre = TWO ? &R : nullptr;
+  if constexpr (TWO) R = draw_two(D.keys, G0, gs, (uint32_t)A.t0, (uint32_t)((unsigned long long)A.t0 >> 32), 0u);
+  for (long long m = A.t0; m < A.t0 + A.n_mcs; ++m) {
+    const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
+    for (int ps = 0; ps < 2; ++ps) {
+      const uint32_t o = D.offset_mode ? (uint32_t)ps : ((offbits >> (2 * ((int)m & 15) + ps)) & 1u);
+      if (o)  // even rows: colour o
+        sweep_row_supergroup<TWO, 1, RIW>(EX, OX, EY, OY, P0e, P0o, rr * RH + nxw, kq, sgr, G0, live, r, D.keys, gs, tlo, thi,
+                                          (uint32_t)ps, pre);
+      else
+        sweep_row_supergroup<TWO, 0, RIW>(EX, OX, EY, OY, P0e, P0o, rr * RH + nxw, kq, sgr, G0, live, r, D.keys, gs, tlo, thi,
+                                          (uint32_t)ps, pre);
+      if constexpr (TWO) R = draw_two(D.keys, G1, gs, tlo, thi, (uint32_t)ps);
+      // odd rows: colour 1 - o; only the warp that holds the CTA's last odd row goes through shared::cluster addresses
+      if (warp_edge) {
+        if (o)
+          sweep_row_supergroup<TWO, 0, RIW, true>(EX, OX, EY, OY, P0o, P1o, (rr + half) * RH + nxw, kq, sgr, G1, live, r, D.keys, gs,
+                                                  tlo, thi, (uint32_t)ps, pre, xrE);
+        else
+          sweep_row_supergroup<TWO, 1, RIW, true>(EX, OX, EY, OY, P0o, P1o, (rr + half) * RH + nxw, kq, sgr, G1, live, r, D.keys, gs,
+                                                  tlo, thi, (uint32_t)ps, pre, xrO);
+      } else {
+        if (o)
+          sweep_row_supergroup<TWO, 0, RIW>(EX, OX, EY, OY, P0o, P1o, (rr + half) * RH + nxw, kq, sgr, G1, live, r, D.keys, gs, tlo,
+                                            thi, (uint32_t)ps, pre);
+        else
+          sweep_row_supergroup<TWO, 1, RIW>(EX, OX, EY, OY, P0o, P1o, (rr + half) * RH + nxw, kq, sgr, G1, live, r, D.keys, gs, tlo,
+                                            thi, (uint32_t)ps, pre);
+      }
+      cluster_arrive();
+      if constexpr (TWO) {  // the first sweep of the next pass, drawn while the other CTAs finish this one
+        const long long mn = ps ? m + 1 : m;
+        R = draw_two(D.keys, G0, gs, (uint32_t)mn, (uint32_t)((unsigned long long)mn >> 32), (uint32_t)(ps ^ 1));
+        asm volatile("" ::"r"(R.v0.x), "r"(R.v0.y), "r"(R.v0.z), "r"(R.v0.w), "r"(R.v1.x), "r"(R.v1.y), "r"(R.v1.z), "r"(R.v1.w));
+      }
+      cluster_wait();
+    }
+    const long long t = m + 1;
+    if (t == next_rec) {  // cluster-uniform
+      int d = 0;  // column 0 of sy over this CTA's rows
+      for (int y = threadIdx.x; y < LyC; y += NT)
+        if (yg0 + y > 0) d += 2 * (int)(EY[((y >> 1) + (y & 1) * half) * RH] & 1u) - 1;
+#pragma unroll
+      for (int k = 16; k >= 1; k >>= 1) d += __shfl_xor_sync(0xFFFFFFFFu, d, k);
+      if (lane == 0) scan[threadIdx.x >> 5] = d;
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        int tot = 0;
+        for (int k = 0; k < NT / 32; ++k) tot += scan[k];
+        col0[0] = tot;
+        col0[1] = 2 * (int)(EX[0] & 1u) - 1;  // meaningful in CTA 0: its slot 0 is row 0 of the sample
+      }
+      cluster_arrive();
+      cluster_wait();
+      int carry = ld_cluster_s32(mapa(smem_addr(&col0[1]), 0u));  // h(0,0)
+      for (uint32_t k = 0; k < q; ++k) carry += ld_cluster_s32(mapa(smem_addr(&col0[0]), k));
+      long long s1 = 0, s2 = 0;
+      row_sums_onchip<NT>(EX, OX, EY, RH, half, sh.Lx, LyC, yg0, carry, lut, scan, s1, s2);
+      block_sum2<NT / 32>(s1, s2, red);
+      if (threadIdx.x == 0) {  // the host cleared the records of this run: exact two's-complement wrap-around addition
+        atomicAdd((unsigned long long*)A.rec_h + (size_t)ri * D.S + s, (unsigned long long)s1);
+        atomicAdd((unsigned long long*)A.rec_h2 + (size_t)ri * D.S + s, (unsigned long long)s2);
+      }
+      ++ri;
+      next_rec = ri < A.nt ? A.rec_t[ri] : -1;
+    }
+    if (D.offset_mode == 0 && ((int)t & 15) == 0) draw_offsets(t);
+  }
+  for (int i = threadIdx.x; i < plane; i += NT) {
+    const int y = i / RH, k = i - y * RH, j = ((y >> 1) + (y & 1) * half) * RH + k;
+    D.EX[base + i] = EX[j];
+    D.OX[base + i] = OX[j];
+    D.EY[base + i] = EY[j];
+    D.OY[base + i] = OY[j];
+  }
+  cluster_arrive();  // no CTA leaves while a neighbour may still read its col0
+  cluster_wait();
+}
+
 #ifdef K5J_LX
 // ---- entry points of the run-time specialised build (NVRTC; csrc/jit.cu) -----------------------------------------
 constexpr bool kJRowAligned = (K5J_LX % 256) == 0;
@@ -628,6 +802,15 @@ extern "C" __global__ void __launch_bounds__(kK5SThreads, K5J_MINB)
     kpz2d_k5s_jit(const __grid_constant__ Kpz2dDev D, const __grid_constant__ Kpz2dRun A) {
   onchip_body<kJRowAligned, K5J_TWO != 0, kJRiw, kJPipe>(D, A);
 }
+#if K5J_CS > 1
+constexpr int kJNhC = K5J_LX / 256 * (K5J_LY / K5J_CS) / 2;  // supergroups per row parity and CTA
+constexpr bool kJRiwC = kJRowAligned && kJSgr <= 32 && (32 % (kJSgr > 0 ? kJSgr : 1)) == 0 && (kJNhC % 32) == 0 && K5J_RIW;
+static_assert(kJRowAligned && (K5J_LY % (2 * K5J_CS)) == 0 && kJNhC <= K5J_THREADS, "K5C: shape the host must not ask for");
+extern "C" __global__ void __cluster_dims__(K5J_CS, 1, 1) __launch_bounds__(K5J_THREADS, K5J_MINB)
+    kpz2d_k5c_jit(const __grid_constant__ Kpz2dDev D, const __grid_constant__ Kpz2dRun A) {
+  cluster_body<K5J_TWO != 0, kJRiwC, K5J_CS, K5J_THREADS>(D, A);
+}
+#endif
 extern "C" __global__ void __launch_bounds__(128)
     kpz2d_k5_pass_jit(const __grid_constant__ Kpz2dDev D, const unsigned char* __restrict__ off, long long m, int ps) {
   pass_body<kJRowAligned, K5J_TWO != 0>(D, off, m, ps);

@@ -30,9 +30,14 @@ def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_
             return run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample, offset_mode, start, path[0])
     total = sum(chunks)
     times = [t for t in times if t <= total]
+    try:
+        gpu = K.Kpz2dSim(Lx, Ly, S, p, q, seed=seed, first_sample=first_sample, offset_mode=offset_mode,
+                         max_records=max(len(times), 1), path=path)
+    except K.KpzError as e:
+        if path == K.KPZ2D_PATH_CLUSTER and e.code == -2:
+            pytest.skip("no cluster shape for this lattice")      # Lx % 256, Ly % (2 CS): refused, not mis-run
+        raise
     ref = R.Kpz2dRef(Lx, Ly, S, p, q, seed=seed, first_sample=first_sample, offset_mode=offset_mode)
-    gpu = K.Kpz2dSim(Lx, Ly, S, p, q, seed=seed, first_sample=first_sample, offset_mode=offset_mode,
-                     max_records=max(len(times), 1), path=path)
     if path:
         assert gpu.path == path
     if start is not None:
@@ -65,12 +70,15 @@ def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_
 # (NVRTC: shape and thresholds are constants) and as the generic kernel of the library build ("jit=0"); K5J_RIW=0 takes
 # the shuffles out of the specialised on-chip kernel (neighbour word loaded, carries by atomics), K5J_PIPE=0 its
 # software pipeline (planes drawn one sweep ahead around a split barrier)
-PATHS = [(1, ""), (2, ""), (1, "jit=0"), (2, "jit=0"), (1, "K5J_RIW=0"), (1, "K5J_PIPE=0")]
+# 3 = a sample spread over a thread-block cluster (K5C; 2 CTAs unless K5J_CS forces 4 or 8), rows of the neighbour CTA
+# through distributed shared memory; shapes without a cluster decomposition are refused (and skipped here)
+PATHS = [(1, ""), (2, ""), (1, "jit=0"), (2, "jit=0"), (1, "K5J_RIW=0"), (1, "K5J_PIPE=0"), (3, ""), (3, "K5J_CS=4"),
+         (3, "K5J_CS=8"), (3, "K5J_RIW=0")]
 
 
 @pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("Lx,Ly", [(64, 2), (64, 6), (128, 64), (192, 10), (256, 256), (320, 30), (1024, 4), (256, 2), (512, 64),
-                                   (768, 6), (2048, 8), (8192, 2), (16384, 2), (512, 130)])
+                                   (768, 6), (2048, 8), (8192, 2), (16384, 2), (512, 130), (768, 48), (256, 16), (1024, 32)])
 def test_sizes_ragged_supergroups_and_tiny_lattices(K, Lx, Ly, path):
     """A row of 64 sites is a quarter of a Philox supergroup, 192 / 320 sites leave ragged ones; Ly = 2 couples every row
     to itself through the periodic y-pair; 256 x 256 gives the 512 threads of the on-chip kernel one supergroup each.
@@ -106,22 +114,28 @@ def test_path_selection_and_both_paths_agree_at_512(K):
     a = K.Kpz2dSim(512, 512, 2, 0.75, 0.0, seed=5, max_records=1)
     assert a.path == K.KPZ_PATH_ONCHIP                             # 64 KiB of slopes per sample
     b = K.Kpz2dSim(512, 512, 2, 0.75, 0.0, seed=5, max_records=1, path=K.KPZ_PATH_STREAM)
-    assert K.Kpz2dSim(1024, 1024, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ_PATH_STREAM
+    assert K.Kpz2dSim(1024, 1024, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ2D_PATH_CLUSTER   # 256 KiB: 4 CTAs
+    with K.debug_config("jit=0"):
+        assert K.Kpz2dSim(1024, 1024, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ_PATH_STREAM
+    assert K.Kpz2dSim(2048, 2048, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ_PATH_STREAM           # 1 MiB
+    assert K.Kpz2dSim(1024, 1022, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ_PATH_STREAM           # rows do not divide
     with pytest.raises(K.KpzError):
         K.Kpz2dSim(2048, 2048, 1, 0.75, 0.0, seed=5, max_records=1, path=K.KPZ_PATH_ONCHIP)
-    for g in (a, b):
+    c = K.Kpz2dSim(512, 512, 2, 0.75, 0.0, seed=5, max_records=1, path=K.KPZ2D_PATH_CLUSTER)
+    for g in (a, b, c):
         g.set_record_times([40])
         g.run(40)
-    for x, y in zip(a.slopes(), b.slopes()):
-        assert torch.equal(x, y)
-    ra, rb = a.roughness(), b.roughness()
-    assert np.array_equal(ra["sum_h"], rb["sum_h"]) and np.array_equal(ra["sum_h2"], rb["sum_h2"])
+    for other in (b, c):
+        for x, y in zip(a.slopes(), other.slopes()):
+            assert torch.equal(x, y)
+        ra, rb = a.roughness(), other.roughness()
+        assert np.array_equal(ra["sum_h"], rb["sum_h"]) and np.array_equal(ra["sum_h2"], rb["sum_h2"])
 
 
-@pytest.mark.parametrize("spec", ["", "jit=0"])
+@pytest.mark.parametrize("spec", ["", "jit=0", "K5J_CS=8"])
 @pytest.mark.parametrize("key", ["2d-512", "2d-1024"])
 def test_workload_shape_sampled_against_solo_oracle_runs(K, key, spec):
-    """The bench workloads `2d-512` (on chip) and `2d-1024` (streamed) in their launch configuration (all samples),
+    """The bench workloads `2d-512` (on chip) and `2d-1024` (over a cluster; streamed with jit=0) in their launch configuration (all samples),
     shortened: first and last sample against solo oracle runs, every sample single-valued."""
     c = workloads.CONFIGS[key]
     n, times = 6, [1, 2, 3, 4, 5, 6]
