@@ -153,6 +153,7 @@ std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, size_t smem, const Cl
   add("K5J_THREADS", cl ? cl->threads : 512);
   add("K5J_RIW", debug_int("K5J_RIW", 1));
   add("K5J_PIPE", debug_int("K5J_PIPE", 1));
+  add("K5J_NBR", debug_int("K5J_NBR", 0));  // neighbour-only mbarriers: measured slower than barrier.cluster (r02_summary §6)
   if (debug_has("K5J_XRALL")) add("K5J_XRALL", debug_int("K5J_XRALL", 0));
   return d;
 }

@@ -654,13 +654,41 @@ __device__ __forceinline__ void onchip_body(const Kpz2dDev& D, const Kpz2dRun& A
   }
 }
 
+// mbarrier operations at cluster scope (K5C neighbour synchronisation): a CTA's barrier also takes arrivals from the
+// two neighbouring CTAs of the cluster, sent through its shared::cluster address.
+__device__ __forceinline__ void mbar_init_cluster(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive_rel_cluster(uint32_t bar) {
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.release.cluster.shared::cta.b64 st, [%0];\n}" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_bar) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_acq_cluster(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n.reg .pred p;\n"
+      "K5C_WAIT_%=:\n"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+      "@!p bra K5C_WAIT_%=;\n}" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+
 // K5C: a sample spread over a thread-block cluster of CS CTAs (lattices beyond the shared memory of one SM, e.g.
 // 1024 x 1024 = 256 KiB of slopes; also: more, smaller CTAs balance better over the 148 SMs).  CTA q holds rows
 // q Ly/CS .. (q + 1) Ly/CS - 1 in its own shared memory, by parity as K5S does; the only words of another CTA a sweep
 // touches are the first even row of CTA q + 1 (row y + 1 of this CTA's last odd row), read and written through
-// distributed shared memory.  One barrier.cluster per colour pass, split (arrive ... wait) around the Philox calls of
-// the next pass.  One supergroup per thread and row parity (NT >= Ly/CS/2 * Lx/256); run-time specialised only.
-template <bool TWO, bool RIW, int CS, int NT>
+// distributed shared memory.  Synchronisation after a colour pass, split (arrive ... wait) around the Philox calls of the
+// next pass: NBR = false (the default: measured faster): one barrier.cluster; NBR = true ("K5J_NBR=1"): the CTAs
+// synchronise with their two NEIGHBOURS only - CTA q
+// may start pass k + 1 when its own warps, the warps of CTA q - 1 that hold that CTA's last odd row (they write q's row
+// 0) and the warps of CTA q + 1 that hold its row 0 (q's last odd row reads it) have finished pass k.  That is an
+// mbarrier per CTA with NW + n_edge + n_row0 arrivals, the foreign ones sent through distributed shared memory; two
+// barriers alternate, since a neighbour may run one pass ahead (never two: its own barrier waits for this CTA's warps).
+// One supergroup per thread and row parity (NT >= Ly/CS/2 * Lx/256); run-time specialised only.
+template <bool TWO, bool RIW, int CS, int NT, bool NBR>
 __device__ __forceinline__ void cluster_body(const Kpz2dDev& D, const Kpz2dRun& A) {
   extern __shared__ __align__(16) uint32_t k5s_smem[];
   __shared__ long long red[2 * (NT / 32)];
@@ -709,7 +737,25 @@ __device__ __forceinline__ void cluster_body(const Kpz2dDev& D, const Kpz2dRun& 
   const int P1o = (edge ? 0 : rr + 1) * RH + 4 * kq;
   const uint32_t nbr = edge ? (q + 1 == (uint32_t)CS ? 0u : q + 1u) : q;
   const uint32_t xrE = mapa(smem_addr(EY + P1o), nbr), xrO = mapa(smem_addr(OY + P1o), nbr);
-  const bool warp_edge = __any_sync(0xFFFFFFFFu, live && edge) || K5J_XRALL;
+  const bool has_edge = __any_sync(0xFFFFFFFFu, live && edge);      // this warp holds (part of) the CTA's last odd row
+  const bool has_row0 = __any_sync(0xFFFFFFFFu, live && rr == 0);    // ... of the CTA's first even row
+  const bool warp_edge = has_edge || K5J_XRALL;
+  __shared__ unsigned long long nbar[2];
+  const uint32_t bar0 = smem_addr(&nbar[0]), bar1 = smem_addr(&nbar[1]);
+  const uint32_t q_next = q + 1 == (uint32_t)CS ? 0u : q + 1u, q_prev = q == 0 ? (uint32_t)CS - 1u : q - 1u;
+  const uint32_t nx0 = mapa(bar0, q_next), nx1 = mapa(bar1, q_next), pv0 = mapa(bar0, q_prev), pv1 = mapa(bar1, q_prev);
+  uint32_t npass = 0;  // colour passes done by this launch
+  if constexpr (NBR) {
+    if (threadIdx.x == 0) {
+      const int a = (half - 1) * sgr, b = half * sgr - 1;  // threads of the last odd row; row 0: threads 0 .. sgr - 1
+      const uint32_t count = (uint32_t)(NT / 32 + (b / 32 - a / 32 + 1) + (sgr + 31) / 32);
+      mbar_init_cluster(bar0, count);
+      mbar_init_cluster(bar1, count);
+      mbar_fence_init();
+    }
+    cluster_arrive();  // the barriers exist before a neighbour arrives on them
+    cluster_wait();
+  }
   Planes2 R;
   const Planes2* pre = TWO ? &R : nullptr;
   if constexpr (TWO) R = draw_two(D.keys, G0, gs, (uint32_t)A.t0, (uint32_t)((unsigned long long)A.t0 >> 32), 0u);
@@ -740,13 +786,27 @@ __device__ __forceinline__ void cluster_body(const Kpz2dDev& D, const Kpz2dRun& 
           sweep_row_supergroup<TWO, 1, RIW>(EX, OX, EY, OY, P0o, P1o, (rr + half) * RH + nxw, kq, sgr, G1, live, r, D.keys, gs, tlo,
                                             thi, (uint32_t)ps, pre);
       }
-      cluster_arrive();
+      const bool odd_pass = (npass & 1u) != 0u;
+      if constexpr (NBR) {
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive_rel_cluster(odd_pass ? bar1 : bar0);
+          if (has_edge) mbar_arrive_remote(odd_pass ? nx1 : nx0);
+          if (has_row0) mbar_arrive_remote(odd_pass ? pv1 : pv0);
+        }
+      } else {
+        cluster_arrive();
+      }
       if constexpr (TWO) {  // the first sweep of the next pass, drawn while the other CTAs finish this one
         const long long mn = ps ? m + 1 : m;
         R = draw_two(D.keys, G0, gs, (uint32_t)mn, (uint32_t)((unsigned long long)mn >> 32), (uint32_t)(ps ^ 1));
         asm volatile("" ::"r"(R.v0.x), "r"(R.v0.y), "r"(R.v0.z), "r"(R.v0.w), "r"(R.v1.x), "r"(R.v1.y), "r"(R.v1.z), "r"(R.v1.w));
       }
-      cluster_wait();
+      if constexpr (NBR)
+        mbar_wait_acq_cluster(odd_pass ? bar1 : bar0, (npass >> 1) & 1u);
+      else
+        cluster_wait();
+      ++npass;
     }
     const long long t = m + 1;
     if (t == next_rec) {  // cluster-uniform
@@ -808,7 +868,7 @@ constexpr bool kJRiwC = kJRowAligned && kJSgr <= 32 && (32 % (kJSgr > 0 ? kJSgr 
 static_assert(kJRowAligned && (K5J_LY % (2 * K5J_CS)) == 0 && kJNhC <= K5J_THREADS, "K5C: shape the host must not ask for");
 extern "C" __global__ void __cluster_dims__(K5J_CS, 1, 1) __launch_bounds__(K5J_THREADS, K5J_MINB)
     kpz2d_k5c_jit(const __grid_constant__ Kpz2dDev D, const __grid_constant__ Kpz2dRun A) {
-  cluster_body<K5J_TWO != 0, kJRiwC, K5J_CS, K5J_THREADS>(D, A);
+  cluster_body<K5J_TWO != 0, kJRiwC, K5J_CS, K5J_THREADS, K5J_NBR != 0>(D, A);
 }
 #endif
 extern "C" __global__ void __launch_bounds__(128)
