@@ -84,7 +84,7 @@ for _L in (512, 1024, 2048, 4096, 8192, 16384, 32768):   # the paper's size scan
     ALU_SLOTS_PER_SU[f"paper-scan-{_L}"] = ALU_SLOTS_PER_SU["paper-1024x30"]
 # default run: the headline first, then the other BASELINE configs and the auxiliary streamed runs of SURVEY §8(d)
 HEADLINE = 3
-DEFAULT_SET = [3, 1, 2, 4, 5, "4-aux-i", "4-aux-ii", "2d-512"]   # the last one: SURVEY 8(f)-4, not a BASELINE config
+DEFAULT_SET = [3, 1, 2, 4, 5, "4-aux-i", "4-aux-ii", "2d-512", "2d-1024"]   # the last two: SURVEY 8(f)-4, not BASELINE configs
 ALU_SLOTS_PER_CLK_SMSP = 0.5
 # streamed sweep: one read + one write of the bit-packed ring per sub-lattice pass = 2 passes * 2 * 1/8 B
 STREAM_BYTES_PER_SU = 0.5

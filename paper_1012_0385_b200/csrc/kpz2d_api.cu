@@ -438,8 +438,7 @@ int kpz2d_heights(kpz2d_sim* sim, int32_t sample, int32_t* d_h) {
   const Kpz2dDev& D = sim->dev;
   const int nxb = (D.Lx + 255) / 256;
   const size_t row0 = (size_t)sample * D.Ly * D.RH;
-  k2d_heights<1><<<nxb, 256, 0, sim->stream>>>(D.EX + row0, D.OX + row0, D.EY + row0, D.OY + row0, D.Lx, D.Ly, D.RH, nxb, nullptr,
-                                              nullptr, d_h);
+  k2d_heights<<<nxb, 256, 0, sim->stream>>>(D.EX + row0, D.OX + row0, D.EY + row0, D.OY + row0, D.Lx, D.Ly, D.RH, d_h);
   KPZ_LAUNCH_CHECK("k2d_heights");
   return KPZ_OK;
 }

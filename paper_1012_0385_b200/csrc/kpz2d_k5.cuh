@@ -375,34 +375,6 @@ __device__ __forceinline__ void pass_body(const Kpz2dDev& D, const unsigned char
   }
 }
 
-// Exact sums of h and h^2 of one sample from its planes: thread = column x, strided by nthr.  half > 0: the rows are
-// stored by parity, row y in slot (y >> 1) + (y & 1) * half (the on-chip fast path); half = 0: natural order.
-// h(x,0) = 2 (occupied bonds among sx[0][0..x]) - (x + 1): even sites 0..x are bits 0..x/2 of EX[0], odd ones bits
-// 0..(x-1)/2 of OX[0]; h(x,y) = h(x,y-1) + 2 sy[y][x] - 1.  MODE 1 also writes h[y][x].
-template <int MODE>
-__device__ __forceinline__ void column_sums(const uint32_t* EX, const uint32_t* OX, const uint32_t* EY, const uint32_t* OY, int RH,
-                                            int half, int Lx, int Ly, int x0, int nthr, long long& s1, long long& s2,
-                                            int32_t* h_out) {
-  for (int x = x0; x < Lx; x += nthr) {
-    const int ne = x / 2 + 1, no = (x + 1) / 2;
-    int cnt = 0;  // row 0 is slot 0 in both orders
-    for (int w = 0; w < (ne >> 5); ++w) cnt += __popc(EX[w]);
-    if (ne & 31) cnt += __popc(EX[ne >> 5] & ((1u << (ne & 31)) - 1u));
-    for (int w = 0; w < (no >> 5); ++w) cnt += __popc(OX[w]);
-    if (no & 31) cnt += __popc(OX[no >> 5] & ((1u << (no & 31)) - 1u));
-    int h = 2 * cnt - (x + 1);
-    const uint32_t* col = (x & 1) ? OY : EY;
-    const int jw = (x >> 1) >> 5, jb = (x >> 1) & 31;
-    for (int y = 0; y < Ly; ++y) {
-      const int slot = half ? (y >> 1) + (y & 1) * half : y;
-      if (y > 0) h += 2 * (int)((col[(size_t)slot * RH + jw] >> jb) & 1u) - 1;
-      if (MODE == 1) h_out[(size_t)y * Lx + x] = h;
-      s1 += h;
-      s2 += (long long)h * h;
-    }
-  }
-}
-
 // block-wide sum of (s1, s2) into thread 0 (NW warps)
 template <int NW>
 __device__ __forceinline__ void block_sum2(long long& s1, long long& s2, long long* red /* [2 * NW] shared */) {

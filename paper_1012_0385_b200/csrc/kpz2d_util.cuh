@@ -54,23 +54,27 @@ __global__ void k2d_offsets(const __grid_constant__ PhiloxKeys K, int first_samp
   }
 }
 
-// MODE 0: exact sums over a sample (grid = S * nxb blocks of 256 columns, atomicAdd per block); MODE 1: heights of one sample.
-template <int MODE>
+// Heights of one sample, column by column - the definition of DESIGN §R19 written out (thread = column x):
+// h(x,0) = 2 (occupied bonds among sx[0][0..x]) - (x + 1): even sites 0..x are bits 0..x/2 of EX[0], odd ones bits
+// 0..(x-1)/2 of OX[0]; h(x,y) = h(x,y-1) + 2 sy[y][x] - 1.  (The exact sums at record times integrate row by row:
+// k2d_row_sums below, row_sums_onchip in kpz2d_k5.cuh; a GPU test compares the two.)
 __global__ void __launch_bounds__(256) k2d_heights(const uint32_t* __restrict__ EX, const uint32_t* __restrict__ OX,
                                                    const uint32_t* __restrict__ EY, const uint32_t* __restrict__ OY, int Lx, int Ly,
-                                                   int RH, int nxb, unsigned long long* out_h, unsigned long long* out_h2,
-                                                   int32_t* h_out) {
-  __shared__ long long red[16];
-  const int s = blockIdx.x / nxb, x = (blockIdx.x % nxb) * 256 + threadIdx.x;
-  const size_t base = (size_t)s * Ly * RH;
-  long long s1 = 0, s2 = 0;
-  column_sums<MODE>(EX + base, OX + base, EY + base, OY + base, RH, 0, Lx, Ly, x < Lx ? x : Lx, Lx, s1, s2, h_out);
-  if (MODE == 0) {
-    block_sum2<8>(s1, s2, red);
-    if (threadIdx.x == 0) {
-      atomicAdd(out_h + s, (unsigned long long)s1);  // exact: two's-complement wrap-around addition
-      atomicAdd(out_h2 + s, (unsigned long long)s2);
-    }
+                                                   int RH, int32_t* h_out) {
+  const int x = blockIdx.x * 256 + threadIdx.x;
+  if (x >= Lx) return;
+  const int ne = x / 2 + 1, no = (x + 1) / 2;
+  int cnt = 0;
+  for (int w = 0; w < (ne >> 5); ++w) cnt += __popc(EX[w]);
+  if (ne & 31) cnt += __popc(EX[ne >> 5] & ((1u << (ne & 31)) - 1u));
+  for (int w = 0; w < (no >> 5); ++w) cnt += __popc(OX[w]);
+  if (no & 31) cnt += __popc(OX[no >> 5] & ((1u << (no & 31)) - 1u));
+  int h = 2 * cnt - (x + 1);
+  const uint32_t* col = (x & 1) ? OY : EY;
+  const int jw = (x >> 1) >> 5, jb = (x >> 1) & 31;
+  for (int y = 0; y < Ly; ++y) {
+    if (y > 0) h += 2 * (int)((col[(size_t)y * RH + jw] >> jb) & 1u) - 1;
+    h_out[(size_t)y * Lx + x] = h;
   }
 }
 
