@@ -14,7 +14,7 @@ using namespace kpz;
 
 struct kpz2d_sim {
   Kpz2dDev dev{};
-  int path = KPZ_PATH_STREAM;  // KPZ_PATH_ONCHIP: a sample in shared memory (k2d_onchip), else one launch per pass
+  int path = KPZ_PATH_STREAM;  // KPZ_PATH_ONCHIP: K5S (a sample per CTA), KPZ2D_PATH_CLUSTER: K5C, else K5 (a launch per pass)
   int32_t max_records = 0;
   cudaStream_t stream = nullptr;
   long long *rec_t = nullptr, *rec_h = nullptr, *rec_h2 = nullptr;
@@ -38,19 +38,15 @@ struct ClusterShape {
 };
 constexpr int KPZ2D_CLUSTER = KPZ2D_PATH_CLUSTER;
 
-// The smallest cluster (2, 4, 8 CTAs; "K5J_CS=n" forces one) whose CTAs hold their rows in at most 100 KiB (two CTAs per
-// SM) with at most 512 supergroups per row parity.  False when no such cluster exists for this shape.
-bool cluster_shape(int32_t Lx, int32_t Ly, ClusterShape* out) {
-  if (Lx % 256 != 0) return false;
-  const int forced = debug_int("K5J_CS", 0);
-  // measured (profiles/r02_summary.md §6): CTAs of at most 256 threads run best, so that size is looked for first
-  for (int pass = 0; pass < 2; ++pass)
+// A cluster of 2, 4 or 8 CTAs ("K5J_CS=n" forces one) whose CTAs hold their rows in at most 100 KiB (two CTAs per SM) with
+// at most max_nh supergroups per row parity (= threads per CTA); the smallest such cluster.  False when there is none.
+bool cluster_shape_upto(int32_t Lx, int32_t Ly, int forced, int max_nh, ClusterShape* out) {
   for (int cs : {2, 4, 8}) {
     if (forced && cs != forced) continue;
     if (Ly % (2 * cs) != 0) continue;
     const size_t smem = onchip_bytes(Lx, Ly) / cs;
     const int nh = Lx / 256 * (Ly / cs) / 2;
-    if (nh > (pass == 0 && !forced ? 256 : 512) || smem > 100 * 1024) continue;
+    if (nh > max_nh || smem > 100 * 1024) continue;
     ClusterShape c;
     c.cs = cs;
     c.smem = smem;
@@ -62,6 +58,14 @@ bool cluster_shape(int32_t Lx, int32_t Ly, ClusterShape* out) {
     return true;
   }
   return false;
+}
+
+// Measured (profiles/r02_summary.md §6): CTAs of at most 256 threads run best, so that size is looked for first.
+bool cluster_shape(int32_t Lx, int32_t Ly, ClusterShape* out) {
+  if (Lx % 256 != 0) return false;
+  const int forced = debug_int("K5J_CS", 0);
+  if (!forced && cluster_shape_upto(Lx, Ly, 0, 256, out)) return true;
+  return cluster_shape_upto(Lx, Ly, forced, 512, out);
 }
 
 // options.path: 0 auto, 1 on chip (K5S: a sample in the shared memory of one CTA), 2 streamed (K5: one launch per colour
