@@ -1,6 +1,6 @@
 """GPU parity at the sizes the throughput claims are made on (VERDICT r1 "parity depth at full size").
 
-The oracle needs minutes for these runs (it does ~2.6e7 site updates per second on one core), so its three long jobs
+The oracle needs minutes for these runs (it does ~2.6e7 site updates per second on one core), so its long jobs
 start together in background threads when the first test of this module asks for one (the C library releases the GIL)
 and every test waits for its own job only:
 
@@ -8,6 +8,8 @@ and every test waits for its own job only:
                  at t = 1, 4, 32 and every record time up to 32 (a full 32-MCS chunk of the blocked path)     ~5 min
   job "config3"  sample S-1 of configs[2] alone, the full 10^5 MCS with all 50 records                          ~70 s
   job "config5"  sample S-1 of configs[4] alone, the full 10^5 MCS: state, currents, populations, profile       ~4 min
+  job "2d-512"   sample S-1 of workload 2d-512 alone, the full 1000 MCS with all 20 records      ~2 min
+  job "2d-1024"  sample S-1 of workload 2d-1024 alone, 100 MCS with the records up to there                      ~1 min
 
 Run on the B200 box with:  python -m pytest tests -m gpu
 """
@@ -71,12 +73,24 @@ def _oracle_config5():
     return out
 
 
+def _oracle_2d(key, n_mcs):
+    c = workloads.CONFIGS[key]
+    times = [t for t in c["record_times"] if t <= n_mcs]
+    ref = R.Kpz2dRef(c["Lx"], c["Ly"], 1, c["p"], c["q"], seed=c["seed"], first_sample=c["S"] - 1)
+    ref.set_record_times(times)
+    ref.run(n_mcs)
+    out = {"slopes": [x.copy() for x in ref.slopes()], "rough": ref.roughness(), "times": times}
+    ref.close()
+    return out
+
+
 @pytest.fixture(scope="module")
 def oracle_jobs():
     R.lib()                       # build / load once, before the threads start
-    pool = cf.ThreadPoolExecutor(max_workers=3)
+    pool = cf.ThreadPoolExecutor(max_workers=5)
     jobs = {"config4": pool.submit(_oracle_config4), "config3": pool.submit(_oracle_config3),
-            "config5": pool.submit(_oracle_config5)}
+            "config5": pool.submit(_oracle_config5), "2d-512": pool.submit(_oracle_2d, "2d-512", 1000),
+            "2d-1024": pool.submit(_oracle_2d, "2d-1024", 100)}
     yield jobs
     pool.shutdown(wait=True)
 
@@ -209,3 +223,24 @@ def test_config4_full_size_against_oracle(K, oracle_jobs, path):
     nt = len(times)
     assert list(g["t"]) == list(r["t"][:nt]) == times
     assert np.array_equal(g["sum_h"], r["sum_h"][:nt]) and np.array_equal(g["sum_h2"], r["sum_h2"][:nt])
+
+
+@pytest.mark.parametrize("key,n_mcs", [("2d-512", 1000), ("2d-1024", 100)])
+def test_2d_workloads_last_sample_in_the_full_launch(K, oracle_jobs, key, n_mcs):
+    """The 2+1D bench workloads in their launch configuration (all samples: 256 CTAs of K5S / 64 clusters of 8 CTAs of
+    K5C): the LAST sample against a solo oracle run - `2d-512` for its full 1000 MCS with all 20 records, `2d-1024` for
+    100 MCS - slope words of both fields and the exact sums."""
+    c = workloads.CONFIGS[key]
+    times = [t for t in c["record_times"] if t <= n_mcs]
+    gpu = K.Kpz2dSim(c["Lx"], c["Ly"], c["S"], c["p"], c["q"], seed=c["seed"], max_records=len(times))
+    assert gpu.path == (K.KPZ_PATH_ONCHIP if key == "2d-512" else K.KPZ2D_PATH_CLUSTER)
+    gpu.set_record_times(times)
+    gpu.run(n_mcs)
+    sx, sy = [K.words_to_numpy(t) for t in gpu.slopes()]
+    g = gpu.roughness()
+    ref = oracle_jobs[key].result()
+    k = c["S"] - 1
+    assert np.array_equal(sx[k], ref["slopes"][0][0]) and np.array_equal(sy[k], ref["slopes"][1][0])
+    r = ref["rough"]
+    assert list(g["t"]) == list(r["t"]) == times == ref["times"]
+    assert np.array_equal(g["sum_h"][:, k], r["sum_h"][:, 0]) and np.array_equal(g["sum_h2"][:, k], r["sum_h2"][:, 0])
