@@ -35,6 +35,7 @@ size_t onchip_bytes(int32_t Lx, int32_t Ly) { return (size_t)4 * Ly * (Lx / 64) 
 struct ClusterShape {
   int cs = 0, threads = 0, minb = 1;
   size_t smem = 0;  // dynamic shared memory per CTA
+  int dual = 0;     // 1: two samples per cluster, swept alternately (cluster_body_dual)
 };
 constexpr int KPZ2D_CLUSTER = KPZ2D_PATH_CLUSTER;
 
@@ -64,8 +65,14 @@ bool cluster_shape_upto(int32_t Lx, int32_t Ly, int forced, int max_nh, ClusterS
 bool cluster_shape(int32_t Lx, int32_t Ly, ClusterShape* out) {
   if (Lx % 256 != 0) return false;
   const int forced = debug_int("K5J_CS", 0);
-  if (!forced && cluster_shape_upto(Lx, Ly, 0, 256, out)) return true;
-  return cluster_shape_upto(Lx, Ly, forced, 512, out);
+  bool ok = !forced && cluster_shape_upto(Lx, Ly, 0, 256, out);
+  if (!ok) ok = cluster_shape_upto(Lx, Ly, forced, 512, out);
+  if (ok && debug_int("K5J_DUAL", 0) != 0 && 2 * out->smem <= 200 * 1024) {  // two samples per cluster
+    out->dual = 1;
+    out->smem *= 2;
+    out->minb = std::max(1, std::min({1024 / out->threads, (int)((227 * 1024) / (out->smem + 3 * 1024)), 16}));
+  }
+  return ok;
 }
 
 // options.path: 0 auto, 1 on chip (K5S: a sample in the shared memory of one CTA), 2 streamed (K5: one launch per colour
@@ -155,6 +162,7 @@ std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, size_t smem, const Cl
   add("K5J_MINB", cl ? cl->minb : (smem != 0 && 2 * (smem + 1024) <= 227 * 1024 ? 2 : 1));
   add("K5J_CS", cl ? cl->cs : 1);
   add("K5J_THREADS", cl ? cl->threads : 512);
+  add("K5J_DUAL", cl ? cl->dual : 0);
   add("K5J_RIW", debug_int("K5J_RIW", 1));
   add("K5J_PIPE", debug_int("K5J_PIPE", 1));
   add("K5J_NBR", debug_int("K5J_NBR", 0));  // neighbour-only mbarriers: measured slower than barrier.cluster (r02_summary §6)
@@ -342,7 +350,8 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
       if (rc) return rc;
       void* args[] = {(void*)&D, (void*)&A};
       KPZ_CUDA_CHECK(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cl.smem));
-      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(D.S * cl.cs), dim3(cl.threads), args, cl.smem, sim->stream));
+      const int nclusters = cl.dual ? (D.S + 1) / 2 : D.S;
+      KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(nclusters * cl.cs), dim3(cl.threads), args, cl.smem, sim->stream));
       count_launch();
     } else if (jit_enabled()) {  // specialised on the shape and the thresholds (NVRTC)
       void* kfn = nullptr;

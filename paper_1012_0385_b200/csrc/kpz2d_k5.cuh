@@ -822,6 +822,159 @@ __device__ __forceinline__ void cluster_body(const Kpz2dDev& D, const Kpz2dRun& 
   cluster_wait();
 }
 
+// K5C, two samples per cluster ("K5J_DUAL"): every CTA holds its rows of TWO samples and sweeps them alternately - A's
+// pass k, B's pass k, A's pass k + 1, ... - so the cluster barrier that publishes a pass of one sample completes while
+// the CTA sweeps the other sample: sweep(p); [wait for sweep p - 1's barrier]; arrive for sweep p; sweep(p + 1) ...
+// The last cluster of an odd ensemble holds one sample and waits before every sweep.  Same rows, addresses and
+// distributed-shared-memory accesses as cluster_body; the planes are drawn inside the sweep.
+template <bool TWO, bool RIW, int CS, int NT>
+__device__ __forceinline__ void cluster_body_dual(const Kpz2dDev& D, const Kpz2dRun& A) {
+  extern __shared__ __align__(16) uint32_t k5s_smem[];
+  __shared__ long long red[2 * (NT / 32)];
+  __shared__ uint32_t lut[256];
+  __shared__ int scan[NT / 32];
+  __shared__ int col0[2];
+  for (int i = threadIdx.x; i < 256; i += NT) lut[i] = height_lut_entry(i);
+  const Shape2d sh = shape2d(D);
+  const uint32_t q = cluster_ctarank();
+  const int s0 = (int)(blockIdx.x / CS) * 2, ns = D.S - s0 < 2 ? D.S - s0 : 2;
+  const int RH = sh.RH, LyC = sh.Ly / CS, half = LyC / 2, plane = LyC * RH, yg0 = (int)q * LyC;
+  const int set = 4 * plane;  // words of one sample's four planes: EX, OX, EY, OY at 0, plane, 2 plane, 3 plane
+  for (int j = 0; j < ns; ++j) {
+    const size_t base = (size_t)(s0 + j) * sh.Ly * RH + (size_t)q * plane;
+    uint32_t* P = k5s_smem + j * set;
+    for (int i = threadIdx.x; i < plane; i += NT) {
+      const int y = i / RH, k = i - y * RH, w = ((y >> 1) + (y & 1) * half) * RH + k;
+      P[w] = D.EX[base + i];
+      P[plane + w] = D.OX[base + i];
+      P[2 * plane + w] = D.EY[base + i];
+      P[3 * plane + w] = D.OY[base + i];
+    }
+  }
+  cluster_arrive();
+  cluster_wait();
+  const int lane = threadIdx.x & 31;
+  const Rates2d r = make_rates2d(D);
+  int ri = A.rec_begin;
+  long long next_rec = ri < A.nt ? A.rec_t[ri] : -1;
+  uint32_t offbits[2] = {0u, 0u};
+  auto draw_offsets = [&](long long m) {
+    for (int j = 0; j < ns; ++j) {
+      const unsigned long long mb = ((unsigned long long)m & ~15ull) + (unsigned)(lane >> 1);
+      const uint4 w = philox4x32_10(0u, (uint32_t)(D.first_sample + s0 + j), (uint32_t)mb,
+                                    ctr3(TAG_OFFSET, lane & 1, 0, (uint32_t)(mb >> 32)), D.keys);
+      offbits[j] = __ballot_sync(0xFFFFFFFFu, w.x & 1u);
+    }
+  };
+  if (D.offset_mode == 0) draw_offsets(A.t0);
+  const int sgr = RH / 4, nh = half * sgr;
+  const bool live = nh >= NT || (int)threadIdx.x < nh;
+  const int ti = live ? (int)threadIdx.x : 0, rr = ti / sgr, kq = ti - rr * sgr;
+  const uint32_t G0 = (uint32_t)((yg0 + 2 * rr) * sgr + kq), G1 = G0 + (uint32_t)sgr;
+  const int P0e = rr * RH + 4 * kq, P0o = P0e + half * RH, nxw = kq + 1 == sgr ? 0 : 4 * (kq + 1);
+  const bool edge = rr + 1 == half;
+  const int P1o = (edge ? 0 : rr + 1) * RH + 4 * kq;
+  const uint32_t nbr = edge ? (q + 1 == (uint32_t)CS ? 0u : q + 1u) : q;
+  const bool warp_edge = __any_sync(0xFFFFFFFFu, live && edge);
+  bool pending = false;  // an arrival on the cluster barrier that has not been waited for, made after a sweep of sample pend_j
+  int pend_j = 0;
+  auto settle = [&]() {
+    if (pending) cluster_wait();
+    pending = false;
+  };
+  auto sweep = [&](int j, uint32_t tlo, uint32_t thi, uint32_t ps, uint32_t o) {
+    uint32_t* EX = k5s_smem + j * set;
+    uint32_t* OX = EX + plane;
+    uint32_t* EY = OX + plane;
+    uint32_t* OY = EY + plane;
+    const uint32_t gs = (uint32_t)(D.first_sample + s0 + j);
+    if (o)
+      sweep_row_supergroup<TWO, 1, RIW>(EX, OX, EY, OY, P0e, P0o, rr * RH + nxw, kq, sgr, G0, live, r, D.keys, gs, tlo, thi, ps);
+    else
+      sweep_row_supergroup<TWO, 0, RIW>(EX, OX, EY, OY, P0e, P0o, rr * RH + nxw, kq, sgr, G0, live, r, D.keys, gs, tlo, thi, ps);
+    if (warp_edge) {
+      if (o)
+        sweep_row_supergroup<TWO, 0, RIW, true>(EX, OX, EY, OY, P0o, P1o, (rr + half) * RH + nxw, kq, sgr, G1, live, r, D.keys, gs,
+                                                tlo, thi, ps, nullptr, mapa(smem_addr(EY + P1o), nbr));
+      else
+        sweep_row_supergroup<TWO, 1, RIW, true>(EX, OX, EY, OY, P0o, P1o, (rr + half) * RH + nxw, kq, sgr, G1, live, r, D.keys, gs,
+                                                tlo, thi, ps, nullptr, mapa(smem_addr(OY + P1o), nbr));
+    } else {
+      if (o)
+        sweep_row_supergroup<TWO, 0, RIW>(EX, OX, EY, OY, P0o, P1o, (rr + half) * RH + nxw, kq, sgr, G1, live, r, D.keys, gs, tlo, thi, ps);
+      else
+        sweep_row_supergroup<TWO, 1, RIW>(EX, OX, EY, OY, P0o, P1o, (rr + half) * RH + nxw, kq, sgr, G1, live, r, D.keys, gs, tlo, thi, ps);
+    }
+  };
+  for (long long m = A.t0; m < A.t0 + A.n_mcs; ++m) {
+    const uint32_t tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
+    for (int ps = 0; ps < 2; ++ps) {
+      for (int j = 0; j < ns; ++j) {
+        if (pending && pend_j == j) settle();  // this sample's previous pass must be published (one-sample cluster only)
+        const uint32_t o = D.offset_mode ? (uint32_t)ps : ((offbits[j] >> (2 * ((int)m & 15) + ps)) & 1u);
+        sweep(j, tlo, thi, (uint32_t)ps, o);
+        settle();  // the other sample's barrier has had this whole sweep to complete
+        cluster_arrive();
+        pending = true;
+        pend_j = j;
+      }
+    }
+    const long long t = m + 1;
+    if (t == next_rec) {  // cluster-uniform
+      settle();
+      for (int j = 0; j < ns; ++j) {
+        const uint32_t* EX = k5s_smem + j * set;
+        const uint32_t* OX = EX + plane;
+        const uint32_t* EY = OX + plane;
+        int d = 0;
+        for (int y = threadIdx.x; y < LyC; y += NT)
+          if (yg0 + y > 0) d += 2 * (int)(EY[((y >> 1) + (y & 1) * half) * RH] & 1u) - 1;
+#pragma unroll
+        for (int k = 16; k >= 1; k >>= 1) d += __shfl_xor_sync(0xFFFFFFFFu, d, k);
+        __syncthreads();  // scan / col0 of the previous sample have been read
+        if (lane == 0) scan[threadIdx.x >> 5] = d;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+          int tot = 0;
+          for (int k = 0; k < NT / 32; ++k) tot += scan[k];
+          col0[0] = tot;
+          col0[1] = 2 * (int)(EX[0] & 1u) - 1;
+        }
+        cluster_arrive();
+        cluster_wait();
+        int carry = ld_cluster_s32(mapa(smem_addr(&col0[1]), 0u));
+        for (uint32_t k = 0; k < q; ++k) carry += ld_cluster_s32(mapa(smem_addr(&col0[0]), k));
+        cluster_arrive();  // every CTA has read col0 before it is written for the next sample
+        cluster_wait();
+        long long s1 = 0, s2 = 0;
+        row_sums_onchip<NT>(EX, OX, EY, RH, half, sh.Lx, LyC, yg0, carry, lut, scan, s1, s2);
+        block_sum2<NT / 32>(s1, s2, red);
+        if (threadIdx.x == 0) {
+          atomicAdd((unsigned long long*)A.rec_h + (size_t)ri * D.S + s0 + j, (unsigned long long)s1);
+          atomicAdd((unsigned long long*)A.rec_h2 + (size_t)ri * D.S + s0 + j, (unsigned long long)s2);
+        }
+      }
+      ++ri;
+      next_rec = ri < A.nt ? A.rec_t[ri] : -1;
+    }
+    if (D.offset_mode == 0 && ((int)t & 15) == 0) draw_offsets(t);
+  }
+  settle();
+  for (int j = 0; j < ns; ++j) {
+    const size_t base = (size_t)(s0 + j) * sh.Ly * RH + (size_t)q * plane;
+    const uint32_t* P = k5s_smem + j * set;
+    for (int i = threadIdx.x; i < plane; i += NT) {
+      const int y = i / RH, k = i - y * RH, w = ((y >> 1) + (y & 1) * half) * RH + k;
+      D.EX[base + i] = P[w];
+      D.OX[base + i] = P[plane + w];
+      D.EY[base + i] = P[2 * plane + w];
+      D.OY[base + i] = P[3 * plane + w];
+    }
+  }
+  cluster_arrive();
+  cluster_wait();
+}
+
 #ifdef K5J_LX
 // ---- entry points of the run-time specialised build (NVRTC; csrc/jit.cu) -----------------------------------------
 constexpr bool kJRowAligned = (K5J_LX % 256) == 0;
@@ -840,7 +993,10 @@ constexpr bool kJRiwC = kJRowAligned && kJSgr <= 32 && (32 % (kJSgr > 0 ? kJSgr 
 static_assert(kJRowAligned && (K5J_LY % (2 * K5J_CS)) == 0 && kJNhC <= K5J_THREADS, "K5C: shape the host must not ask for");
 extern "C" __global__ void __cluster_dims__(K5J_CS, 1, 1) __launch_bounds__(K5J_THREADS, K5J_MINB)
     kpz2d_k5c_jit(const __grid_constant__ Kpz2dDev D, const __grid_constant__ Kpz2dRun A) {
-  cluster_body<K5J_TWO != 0, kJRiwC, K5J_CS, K5J_THREADS, K5J_NBR != 0>(D, A);
+  if constexpr (K5J_DUAL != 0)
+    cluster_body_dual<K5J_TWO != 0, kJRiwC, K5J_CS, K5J_THREADS>(D, A);
+  else
+    cluster_body<K5J_TWO != 0, kJRiwC, K5J_CS, K5J_THREADS, K5J_NBR != 0>(D, A);
 }
 #endif
 extern "C" __global__ void __launch_bounds__(128)

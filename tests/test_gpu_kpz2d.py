@@ -74,7 +74,7 @@ def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_
 # through distributed shared memory, one barrier.cluster per pass (K5J_NBR=1: the CTAs synchronise with their two neighbours
 # only, through mbarriers); shapes without a cluster decomposition are refused (and skipped here)
 PATHS = [(1, ""), (2, ""), (1, "jit=0"), (2, "jit=0"), (1, "K5J_RIW=0"), (1, "K5J_PIPE=0"), (3, ""), (3, "K5J_CS=4"),
-         (3, "K5J_CS=8"), (3, "K5J_RIW=0"), (3, "K5J_NBR=1")]
+         (3, "K5J_CS=8"), (3, "K5J_RIW=0"), (3, "K5J_NBR=1"), (3, "K5J_DUAL=1"), (3, "K5J_DUAL=1;K5J_CS=4")]
 
 
 @pytest.mark.parametrize("path", PATHS)
