@@ -79,7 +79,7 @@ ALU_SLOTS_PER_SU = {
 # 2+1D generalisation: per Philox supergroup (128 elements = the active half of 256 sites of a row) and
 # colour pass: p = 0.75 needs 2 planes (2 x 34 slots); per 32-site word 3 LOP3/SHF for the two-pair eligibility, 1 for the
 # acceptance, 2 for the flips of sx (the sy flips are memory operations); 2 passes per MCS over Lx Ly / 256 supergroups
-ALU_SLOTS_PER_SU["2d-1024"] = ALU_SLOTS_PER_SU["2d-512"] = ALU_SLOTS_PER_SU["2d-512-cluster"] = 2 * (2 * 34 + 8 * 6) / 256
+ALU_SLOTS_PER_SU["2d-2048"] = ALU_SLOTS_PER_SU["2d-1024"] = ALU_SLOTS_PER_SU["2d-512"] = ALU_SLOTS_PER_SU["2d-512-cluster"] = 2 * (2 * 34 + 8 * 6) / 256
 for _L in (512, 1024, 2048, 4096, 8192, 16384, 32768):   # the paper's size scan: same rates and schedule as paper-1024x30
     ALU_SLOTS_PER_SU[f"paper-scan-{_L}"] = ALU_SLOTS_PER_SU["paper-1024x30"]
 # default run: the headline first, then the other BASELINE configs and the auxiliary streamed runs of SURVEY §8(d)

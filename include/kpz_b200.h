@@ -208,9 +208,10 @@ int kpz2d_run(kpz2d_sim*, int64_t n_mcs);
 int kpz2d_time(const kpz2d_sim*, int64_t* t);
 /* 1 = a whole sample in the shared memory of one CTA, one persistent launch per kpz2d_run (auto up to 96 KiB of slopes
  * per sample, e.g. 512 x 512; options.path = 1 forces it up to 200 KiB); 3 (KPZ2D_PATH_CLUSTER) = a sample spread over
- * the shared memories of a thread-block cluster of 2, 4 or 8 CTAs, neighbour rows through distributed shared memory, one
- * persistent launch (auto beyond 96 KiB when Lx is a multiple of 256 and the rows divide, up to 800 KiB per sample, e.g.
- * 1024 x 1024; run-time specialised kernels only); 2 = one in-place launch per colour pass (everything else). */
+ * the shared memories of a thread-block cluster of 2, 4, 8 or 16 CTAs, neighbour rows through distributed shared memory,
+ * one persistent launch (auto beyond 96 KiB when Lx is a multiple of 256 and the rows divide, up to 1600 KiB per sample,
+ * e.g. 1024 x 1024 on 8 CTAs, 2048 x 2048 on 16 - the non-portable cluster size, used when the device says it can hold
+ * one; run-time specialised kernels only); 2 = one in-place launch per colour pass (everything else). */
 int kpz2d_path(const kpz2d_sim*, int32_t* path);
 int kpz2d_reset(kpz2d_sim*);                                          /* flat surface, t = 0, records dropped; async */
 int kpz2d_slopes(kpz2d_sim*, uint32_t* d_sx, uint32_t* d_sy);        /* copy out (either may be NULL); async */
@@ -238,7 +239,7 @@ int kpz_path(const kpz_sim*, int32_t* path);
  * compiled generic kernels instead of the run-time specialised ones; "K1J_<X>=v" / "K4J_<X>=v" / "K5J_<X>=v" are appended
  * as definitions to every later run-time compilation of the KPZ / two-lane / 2+1D sweep kernels (the knobs documented at
  * the top of csrc/k1_sweep_jit.cuh and csrc/k4_lanes_jit.cuh; 2+1D: K5J_RIW=0 no shuffles, K5J_PIPE=0 no software
- * pipeline in the on-chip kernel, K5J_CS=2|4|8 cluster size, K5J_NBR=1 neighbour-only barriers, K5J_DUAL=1 two samples per cluster, K5J_XRALL=1 every warp
+ * pipeline in the on-chip kernel, K5J_CS=2|4|8|16 cluster size, K5J_NBR=1 neighbour-only barriers, K5J_DUAL=1 two samples per cluster, K5J_XRALL=1 every warp
  * through shared::cluster addresses in the cluster kernel).  Every setting computes the same results (tests/ check that);
  * kpz_run / lanes_run read no environment variable.  KPZ_EINVAL for anything else. */
 int kpz_debug_config(const char* spec);

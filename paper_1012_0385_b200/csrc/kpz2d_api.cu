@@ -39,10 +39,12 @@ struct ClusterShape {
 };
 constexpr int KPZ2D_CLUSTER = KPZ2D_PATH_CLUSTER;
 
-// A cluster of 2, 4 or 8 CTAs ("K5J_CS=n" forces one) whose CTAs hold their rows in at most 100 KiB (two CTAs per SM) with
-// at most max_nh supergroups per row parity (= threads per CTA); the smallest such cluster.  False when there is none.
+// A cluster of 2, 4, 8 or 16 CTAs ("K5J_CS=n" forces one; 16 is beyond the portable cluster size and needs the kernel's
+// consent: cudaFuncAttributeNonPortableClusterSizeAllowed) whose CTAs hold their rows in at most 100 KiB (two CTAs per
+// SM) with at most max_nh supergroups per row parity (= threads per CTA); the smallest such cluster.  False when there
+// is none.
 bool cluster_shape_upto(int32_t Lx, int32_t Ly, int forced, int max_nh, ClusterShape* out) {
-  for (int cs : {2, 4, 8}) {
+  for (int cs : {2, 4, 8, 16}) {
     if (forced && cs != forced) continue;
     if (Ly % (2 * cs) != 0) continue;
     const size_t smem = onchip_bytes(Lx, Ly) / cs;
@@ -87,7 +89,7 @@ int choose_path2d(int32_t Lx, int32_t Ly, const kpz_options* opt, int* path) {
   if (want == KPZ_PATH_ONCHIP && bytes > 200 * 1024)
     return fail(KPZ_EUNSUPPORTED, "the on-chip 2+1D path holds at most 200 KiB of slopes per sample (%zu needed)", bytes);
   if (want == KPZ2D_CLUSTER && !can_cluster)
-    return fail(KPZ_EUNSUPPORTED, "no thread-block cluster shape for %d x %d (needs Lx %% 256 == 0, Ly %% 4 == 0, at most 800 KiB of "
+    return fail(KPZ_EUNSUPPORTED, "no thread-block cluster shape for %d x %d (needs Lx %% 256 == 0, Ly %% 4 == 0, at most 1600 KiB of "
                                   "slopes per sample, run-time specialisation on)", Lx, Ly);
   if (want != KPZ_PATH_ONCHIP && want != KPZ_PATH_STREAM && want != KPZ2D_CLUSTER)
     return fail(KPZ_EINVAL, "options.path must be 0, 1, 2 or 3 here");
@@ -170,6 +172,31 @@ std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, size_t smem, const Cl
   return d;
 }
 
+// The specialised K5C kernel for this handle, ready to launch (attributes set).  KPZ_EUNSUPPORTED when the device cannot
+// hold one cluster of that shape at all (clusters of 16 on a partitioned GPU, say).
+int k5c_kernel(const Kpz2dDev& D, const ClusterShape& cl, void** kfn) {
+  int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5c_jit", k5_jit_defines(D, cl.smem, &cl), kfn);
+  if (rc) return rc;
+  KPZ_CUDA_CHECK(cudaFuncSetAttribute(*kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cl.smem));
+  if (cl.cs > 8) KPZ_CUDA_CHECK(cudaFuncSetAttribute(*kfn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(cl.cs);
+  cfg.blockDim = dim3(cl.threads);
+  cfg.dynamicSmemBytes = cl.smem;
+  cudaLaunchAttribute at{};
+  at.id = cudaLaunchAttributeClusterDimension;
+  at.val.clusterDim.x = cl.cs;
+  at.val.clusterDim.y = at.val.clusterDim.z = 1;
+  cfg.attrs = &at;
+  cfg.numAttrs = 1;
+  int nclusters = 0;
+  KPZ_CUDA_CHECK(cudaOccupancyMaxActiveClusters(&nclusters, *kfn, &cfg));
+  if (nclusters < 1)
+    return fail(KPZ_EUNSUPPORTED, "this device cannot hold a cluster of %d CTAs of %d threads with %zu bytes of shared memory",
+                cl.cs, cl.threads, cl.smem);
+  return KPZ_OK;
+}
+
 int record2d(kpz2d_sim* sim, int ri) {
   const Kpz2dDev& D = sim->dev;
   unsigned long long* oh = (unsigned long long*)(sim->rec_h + (size_t)ri * D.S);
@@ -240,6 +267,17 @@ int kpz2d_create(kpz2d_sim** out, int32_t Lx, int32_t Ly, int32_t nsamples, doub
   D.OX = (uint32_t*)(base + y.off_OX);
   D.EY = (uint32_t*)(base + y.off_EY);
   D.OY = (uint32_t*)(base + y.off_OY);
+  if (path == KPZ2D_CLUSTER) {  // a cluster of 16 CTAs is beyond the portable size: ask the device before promising it
+    ClusterShape cl;
+    void* kfn = nullptr;
+    if (cluster_shape(Lx, Ly, &cl) && cl.cs > 8 && k5c_kernel(D, cl, &kfn) != KPZ_OK) {
+      if (o.path != KPZ_PATH_AUTO) {
+        delete sim;
+        return KPZ_EUNSUPPORTED;  // text set by k5c_kernel
+      }
+      path = KPZ_PATH_STREAM;
+    }
+  }
   sim->max_records = max_records;
   sim->path = path;
   sim->stream = (cudaStream_t)cuda_stream;
@@ -346,10 +384,9 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
         KPZ_CUDA_CHECK(cudaMemsetAsync((char*)sim->rec_h2 + off, 0, len, sim->stream));
       }
       void* kfn = nullptr;
-      int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5c_jit", k5_jit_defines(D, cl.smem, &cl), &kfn);
+      int rc = k5c_kernel(D, cl, &kfn);
       if (rc) return rc;
       void* args[] = {(void*)&D, (void*)&A};
-      KPZ_CUDA_CHECK(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cl.smem));
       const int nclusters = cl.dual ? (D.S + 1) / 2 : D.S;
       KPZ_CUDA_CHECK(cudaLaunchKernel(kfn, dim3(nclusters * cl.cs), dim3(cl.threads), args, cl.smem, sim->stream));
       count_launch();

@@ -70,16 +70,16 @@ def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_
 # (NVRTC: shape and thresholds are constants) and as the generic kernel of the library build ("jit=0"); K5J_RIW=0 takes
 # the shuffles out of the specialised on-chip kernel (neighbour word loaded, carries by atomics), K5J_PIPE=0 its
 # software pipeline (planes drawn one sweep ahead around a split barrier)
-# 3 = a sample spread over a thread-block cluster (K5C; 2 CTAs unless K5J_CS forces 4 or 8), rows of the neighbour CTA
+# 3 = a sample spread over a thread-block cluster (K5C; 2 CTAs unless K5J_CS forces 4, 8 or 16), rows of the neighbour CTA
 # through distributed shared memory, one barrier.cluster per pass (K5J_NBR=1: the CTAs synchronise with their two neighbours
 # only, through mbarriers); shapes without a cluster decomposition are refused (and skipped here)
 PATHS = [(1, ""), (2, ""), (1, "jit=0"), (2, "jit=0"), (1, "K5J_RIW=0"), (1, "K5J_PIPE=0"), (3, ""), (3, "K5J_CS=4"),
-         (3, "K5J_CS=8"), (3, "K5J_RIW=0"), (3, "K5J_NBR=1"), (3, "K5J_DUAL=1"), (3, "K5J_DUAL=1;K5J_CS=4")]
+         (3, "K5J_CS=8"), (3, "K5J_CS=16"), (3, "K5J_RIW=0"), (3, "K5J_NBR=1"), (3, "K5J_DUAL=1"), (3, "K5J_DUAL=1;K5J_CS=4")]
 
 
 @pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("Lx,Ly", [(64, 2), (64, 6), (128, 64), (192, 10), (256, 256), (320, 30), (1024, 4), (256, 2), (512, 64),
-                                   (768, 6), (2048, 8), (8192, 2), (16384, 2), (512, 130), (768, 48), (256, 16), (1024, 32), (16384, 8)])
+                                   (768, 6), (2048, 8), (8192, 2), (16384, 2), (512, 130), (768, 48), (256, 16), (1024, 32), (16384, 8), (2048, 64)])
 def test_sizes_ragged_supergroups_and_tiny_lattices(K, Lx, Ly, path):
     """A row of 64 sites is a quarter of a Philox supergroup, 192 / 320 sites leave ragged ones; Ly = 2 couples every row
     to itself through the periodic y-pair; 256 x 256 gives the 512 threads of the on-chip kernel one supergroup each.
@@ -118,7 +118,8 @@ def test_path_selection_and_both_paths_agree_at_512(K):
     assert K.Kpz2dSim(1024, 1024, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ2D_PATH_CLUSTER   # 256 KiB: 4 CTAs
     with K.debug_config("jit=0"):
         assert K.Kpz2dSim(1024, 1024, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ_PATH_STREAM
-    assert K.Kpz2dSim(2048, 2048, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ_PATH_STREAM           # 1 MiB
+    assert K.Kpz2dSim(2048, 2048, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ2D_PATH_CLUSTER       # 1 MiB: 16 CTAs
+    assert K.Kpz2dSim(4096, 4096, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ_PATH_STREAM           # 4 MiB
     assert K.Kpz2dSim(1024, 1022, 1, 0.75, 0.0, seed=5, max_records=1).path == K.KPZ_PATH_STREAM           # rows do not divide
     with pytest.raises(K.KpzError):
         K.Kpz2dSim(2048, 2048, 1, 0.75, 0.0, seed=5, max_records=1, path=K.KPZ_PATH_ONCHIP)

@@ -102,6 +102,9 @@ CONFIGS["2d-512"] = dict(name="kpz2d_L512x512_S256_p075", kind="kpz2d", Lx=512, 
                          n_mcs=1000, record_times=_T20_1E3, seed=12)   # a sample (64 KiB of slopes) stays in shared memory
 CONFIGS["2d-1024"] = dict(name="kpz2d_L1024x1024_S64_p075", kind="kpz2d", Lx=1024, Ly=1024, L=1024 * 1024, S=64, p=0.75,
                           q=0.0, n_mcs=1000, record_times=_T20_1E3, seed=12)
+# 16 surfaces of 2048 x 2048 (1 MiB of slopes each): a sample over a cluster of 16 CTAs (the non-portable cluster size)
+CONFIGS["2d-2048"] = dict(name="kpz2d_L2048x2048_S16_p075", kind="kpz2d", Lx=2048, Ly=2048, L=2048 * 2048, S=16, p=0.75,
+                          q=0.0, n_mcs=1000, record_times=_T20_1E3, seed=12)
 # the same 512 x 512 ensemble with every sample spread over a thread-block cluster (K5C; options.path = 3): smaller CTAs,
 # which balance better over 148 SMs
 CONFIGS["2d-512-cluster"] = dict(CONFIGS["2d-512"], name="kpz2d_L512x512_S256_p075_cluster", path=3)
