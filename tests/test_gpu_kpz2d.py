@@ -105,6 +105,17 @@ def test_alternating_colours_resume_first_sample_and_rough_start(K, path):
 
 
 @pytest.mark.parametrize("path", PATHS)
+def test_fast_path_alternating_colours_first_sample_and_rough_start(K, path):
+    """The same on a lattice every kernel takes on its fast path (Lx = 512: K5S pipeline, K5C clusters): alternating
+    colours, a resumed run, a handle that starts at global sample 5, a rough start handed in through kpz2d_set_slopes."""
+    run_both_2d(K, 512, 32, 2, 0.75, 0.25, seed=9, times=[4, 11], chunks=[3, 1, 7], offset_mode=1, path=path)
+    run_both_2d(K, 512, 32, 1, 0.75, 0.0, seed=9, times=[11], chunks=[11], first_sample=5, path=path)
+    rough = R.Kpz2dRef(512, 32, 3, 0.6, 0.4, seed=1)
+    rough.run(25)
+    run_both_2d(K, 512, 32, 3, 0.2, 0.9, seed=3, times=[6, 18], chunks=[6, 12], start=rough.slopes(), path=path)
+
+
+@pytest.mark.parametrize("path", PATHS)
 def test_offset_batches_and_chunks_are_crossed(K, path):
     """kpz2d_run draws the colour offsets for 1024 passes (512 MCS) at a time on the streamed path, for 16 MCS at a time in
     the on-chip kernel: one run across those boundaries, records on and around them."""
