@@ -144,13 +144,15 @@ Layout2d layout2d(int32_t Lx, int32_t Ly, int32_t S, int32_t max_records) {
 bool two_planes(const Kpz2dDev& D) { return planes_needed(D.t_p) <= 2 && planes_needed(D.t_q) <= 2; }
 
 // Definitions of the run-time specialised kernels (kpz2d_k5.cuh under NVRTC): shape, thresholds, launch shape.
-std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, size_t smem, const ClusterShape* cl = nullptr) {
+// entry: 1 kpz2d_k5s_jit (smem = its dynamic shared memory), 2 kpz2d_k5c_jit (cl), 3 kpz2d_k5_pass_jit.
+std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, int entry, size_t smem, const ClusterShape* cl = nullptr) {
   char buf[64];
   std::vector<std::string> d;
   auto add = [&](const char* name, long long v) {
     snprintf(buf, sizeof buf, "%s=%lld", name, v);
     d.push_back(buf);
   };
+  add("K5J_ENTRY", entry);
   add("K5J_LX", D.Lx);
   add("K5J_LY", D.Ly);
   snprintf(buf, sizeof buf, "K5J_TP=0x%xu", D.t_p.value);
@@ -175,7 +177,7 @@ std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, size_t smem, const Cl
 // The specialised K5C kernel for this handle, ready to launch (attributes set).  KPZ_EUNSUPPORTED when the device cannot
 // hold one cluster of that shape at all (clusters of 16 on a partitioned GPU, say).
 int k5c_kernel(const Kpz2dDev& D, const ClusterShape& cl, void** kfn) {
-  int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5c_jit", k5_jit_defines(D, cl.smem, &cl), kfn);
+  int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5c_jit", k5_jit_defines(D, 2, cl.smem, &cl), kfn);
   if (rc) return rc;
   KPZ_CUDA_CHECK(cudaFuncSetAttribute(*kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cl.smem));
   if (cl.cs > 8) KPZ_CUDA_CHECK(cudaFuncSetAttribute(*kfn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
@@ -314,10 +316,10 @@ int kpz2d_jit_check(int32_t Lx, int32_t Ly, double p, double q, const kpz_option
   if (path == KPZ2D_CLUSTER) {
     ClusterShape cl;
     cluster_shape(Lx, Ly, &cl);
-    rc = jit_compile("kpz2d_k5.cuh", "kpz2d_k5c_jit", k5_jit_defines(D, cl.smem, &cl), &cubin, nullptr);
+    rc = jit_compile("kpz2d_k5.cuh", "kpz2d_k5c_jit", k5_jit_defines(D, 2, cl.smem, &cl), &cubin, nullptr);
   } else {
     rc = jit_compile("kpz2d_k5.cuh", onchip ? "kpz2d_k5s_jit" : "kpz2d_k5_pass_jit",
-                     k5_jit_defines(D, onchip ? onchip_bytes(Lx, Ly) : 0), &cubin, nullptr);
+                     k5_jit_defines(D, onchip ? 1 : 3, onchip ? onchip_bytes(Lx, Ly) : 0), &cubin, nullptr);
   }
   if (rc) return rc;
   *cubin_bytes = cubin.size();
@@ -392,7 +394,7 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
       count_launch();
     } else if (jit_enabled()) {  // specialised on the shape and the thresholds (NVRTC)
       void* kfn = nullptr;
-      int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5s_jit", k5_jit_defines(D, smem), &kfn);
+      int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5s_jit", k5_jit_defines(D, 1, smem), &kfn);
       if (rc) return rc;
       void* args[] = {(void*)&D, (void*)&A};
       KPZ_CUDA_CHECK(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -415,7 +417,7 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
                                        : (two_planes(D) ? k2d_pass<false, true> : k2d_pass<false, false>);
   void* pass_jit = nullptr;
   if (jit_enabled()) {
-    int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5_pass_jit", k5_jit_defines(D, 0), &pass_jit);
+    int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5_pass_jit", k5_jit_defines(D, 3, 0), &pass_jit);
     if (rc) return rc;
   }
   const long long p_begin = 2 * (long long)sim->t, p_end = 2 * (long long)(sim->t + n_mcs);

@@ -983,11 +983,18 @@ constexpr int kJNh = K5J_LX / 256 * K5J_LY / 2;       // supergroups per row par
 constexpr bool kJRiw = kJRowAligned && kJSgr <= 32 && (32 % (kJSgr > 0 ? kJSgr : 1)) == 0 && (kJNh % 32) == 0 && K5J_RIW;
 constexpr bool kJPipe = kJRowAligned && (K5J_TWO != 0) && kJNh <= kK5SThreads && K5J_PIPE;
 
+// K5J_ENTRY: the one entry point this compilation is for (1 K5S, 2 K5C, 3 K5) - the others are left out, which
+// shortens the NVRTC run; 0 or undefined: all of them.
+#ifndef K5J_ENTRY
+#define K5J_ENTRY 0
+#endif
+#if K5J_ENTRY == 0 || K5J_ENTRY == 1
 extern "C" __global__ void __launch_bounds__(kK5SThreads, K5J_MINB)
     kpz2d_k5s_jit(const __grid_constant__ Kpz2dDev D, const __grid_constant__ Kpz2dRun A) {
   onchip_body<kJRowAligned, K5J_TWO != 0, kJRiw, kJPipe>(D, A);
 }
-#if K5J_CS > 1
+#endif
+#if K5J_CS > 1 && (K5J_ENTRY == 0 || K5J_ENTRY == 2)
 constexpr int kJNhC = K5J_LX / 256 * (K5J_LY / K5J_CS) / 2;  // supergroups per row parity and CTA
 constexpr bool kJRiwC = kJRowAligned && kJSgr <= 32 && (32 % (kJSgr > 0 ? kJSgr : 1)) == 0 && (kJNhC % 32) == 0 && K5J_RIW;
 static_assert(kJRowAligned && (K5J_LY % (2 * K5J_CS)) == 0 && kJNhC <= K5J_THREADS, "K5C: shape the host must not ask for");
@@ -999,10 +1006,12 @@ extern "C" __global__ void __cluster_dims__(K5J_CS, 1, 1) __launch_bounds__(K5J_
     cluster_body<K5J_TWO != 0, kJRiwC, K5J_CS, K5J_THREADS, K5J_NBR != 0>(D, A);
 }
 #endif
+#if K5J_ENTRY == 0 || K5J_ENTRY == 3
 extern "C" __global__ void __launch_bounds__(128)
     kpz2d_k5_pass_jit(const __grid_constant__ Kpz2dDev D, const unsigned char* __restrict__ off, long long m, int ps) {
   pass_body<kJRowAligned, K5J_TWO != 0>(D, off, m, ps);
 }
+#endif
 #else
 // ---- the generic kernels of the library build --------------------------------------------------------------------
 template <bool ROWALIGNED, bool TWO>
