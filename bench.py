@@ -361,7 +361,9 @@ def bench_one(ctx, args, cfg_key, with_cpu):
     ms_run = ms_run_total / args.steps
     roof = roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run, sim_path=sim.path if cfg["kind"] == "kpz2d" else 0)
     cpu = None
-    if with_cpu and ctx.rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if cfg.get("no_cpu_baseline"):
+        cpu = {"value": None, "unit": UNIT, "cores": 0, "kind": "oracle", "sample": f"not run: {cfg['no_cpu_baseline']}"}
+    elif with_cpu and ctx.rank == 0 and world == 1 and not args.no_cpu_baseline:
         nsamp, nm = oracle_sample_shape(cfg, args.cpu_su)
         v, dt = time_oracle(cfg, nsamp, nm)
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
@@ -489,6 +491,15 @@ def roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run, sim_path=0):
         bytes_launch = 2 * cfg["S"] * cfg["L"] / 8
         achieved = bytes_launch * n_launch / (ms_run * 1e-3) / 1e9
         return {"bound": "hbm", "kernel": "kpz_k3_pass_jit", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "traffic_source": src, "measured": measured,
+                "peak_source": peaks["source"], "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
+    if cfg["kind"] == "kpz2d" and sim_path == 2 and cfg["S"] * cfg["L"] / 4 > 126e6:
+        # 2+1D streamed beyond the L2 (4 planes of S * Lx * Ly / 16 bytes): per colour pass every plane word is read once
+        # and written once (DESIGN.md §5 K5)
+        n_launch = 2 * n_mcs
+        bytes_launch = cfg["S"] * cfg["L"] / 2
+        achieved = bytes_launch * n_launch / (ms_run * 1e-3) / 1e9
+        return {"bound": "hbm", "kernel": "kpz2d_k5_pass_jit", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "traffic_source": src, "measured": measured,
                 "peak_source": peaks["source"], "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
     slots = ALU_SLOTS_PER_SU.get(cfg_key)

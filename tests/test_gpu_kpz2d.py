@@ -212,3 +212,21 @@ def test_growth_exponents_kpz_and_edwards_wilkinson_classes(K):
     w = out["ew"][1]
     step = np.diff(w[5:])                              # W^2 = a + b ln t: equal increments per octave
     assert np.all(step > 0) and step.max() / step.min() < 1.5, step
+
+
+def test_streamed_kernel_on_a_lattice_beyond_every_on_chip_variant(K):
+    """8192 x 8192 (8 MiB of slope planes: no cluster holds it) runs on K5, one launch per colour pass, as the 2^30-site
+    bench workload `2d-32768` does.  No oracle run is feasible (30 s per MCS), so: every row and column still closes
+    periodically, the surface has moved, and the row-wise exact sums equal a torch reduction of the column-wise heights."""
+    L = 8192
+    g = K.Kpz2dSim(L, L, 1, 0.75, 0.0, seed=8, max_records=2)
+    assert g.path == K.KPZ_PATH_STREAM
+    g.set_record_times([3, 6])
+    g.run(6)
+    r = g.roughness()
+    h = g.heights(0).to(torch.int64)
+    assert int(h.sum()) == r["sum_h"][1, 0] and int((h * h).sum()) == r["sum_h2"][1, 0]
+    assert 0.3 < r["w2_mean"][0] < r["w2_mean"][1] < 1.5
+    h = h.view(L, L)
+    assert torch.all((h[:, 1:] - h[:, :-1]).abs() == 1) and torch.all((h[1:, :] - h[:-1, :]).abs() == 1)
+    assert torch.all((h[:, 0] - h[:, -1]).abs() == 1) and torch.all((h[0, :] - h[-1, :]).abs() == 1)   # periodic closure

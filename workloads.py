@@ -105,6 +105,12 @@ CONFIGS["2d-1024"] = dict(name="kpz2d_L1024x1024_S64_p075", kind="kpz2d", Lx=102
 # 16 surfaces of 2048 x 2048 (1 MiB of slopes each): a sample over a cluster of 16 CTAs (the non-portable cluster size)
 CONFIGS["2d-2048"] = dict(name="kpz2d_L2048x2048_S16_p075", kind="kpz2d", Lx=2048, Ly=2048, L=2048 * 2048, S=16, p=0.75,
                           q=0.0, n_mcs=1000, record_times=_T20_1E3, seed=12)
+# one surface of 32768 x 32768 (2^30 sites, 512 MiB of slope planes): beyond the L2 and every on-chip variant - the streamed
+# kernel K5, one launch per colour pass, against the HBM roofline (1 byte per site update: every plane word is read once
+# and written once per pass)
+CONFIGS["2d-32768"] = dict(name="kpz2d_L32768x32768_S1_p075", kind="kpz2d", Lx=32768, Ly=32768, L=32768 * 32768, S=1, p=0.75,
+                           q=0.0, n_mcs=20, record_times=[4, 20], seed=12, no_cpu_baseline="one MCS of this lattice takes the "
+                           "oracle about 8 minutes")
 # the same 512 x 512 ensemble with every sample spread over a thread-block cluster (K5C; options.path = 3): smaller CTAs,
 # which balance better over 148 SMs
 CONFIGS["2d-512-cluster"] = dict(CONFIGS["2d-512"], name="kpz2d_L512x512_S256_p075_cluster", path=3)
