@@ -485,8 +485,10 @@ def roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run, sim_path=0):
         measured = {k: num(k) for k in ("issue_active_pct", "pipe_alu_pct", "pipe_fma_pct", "pipe_fmaheavy_pct_of_elapsed",
                                         "warps_active_per_smsp", "registers", "gpu_time_us") if num(k) is not None} or None
     src = (f"profiles/ncu_counters.csv row {cfg_key}: {row.get('capture', '')}" if row else None)
-    if path == 2:
-        # streamed sweep: 2*n_mcs pass kernels per run; per launch one read + one write of the ring
+    if path == 2 and 2 * cfg["S"] * cfg["L"] / 8 > 126e6:
+        # streamed sweep of a ring beyond the L2 (ping-pong pair of S * L / 8 bytes each; a pair that fits the 126 MB L2
+        # never reaches HBM and is measured against the alu-slot roofline below): 2*n_mcs pass kernels per run; per
+        # launch one read + one write of the ring
         n_launch = 2 * n_mcs
         bytes_launch = 2 * cfg["S"] * cfg["L"] / 8
         achieved = bytes_launch * n_launch / (ms_run * 1e-3) / 1e9
@@ -503,7 +505,7 @@ def roofline(ctx, cfg, cfg_key, path, n_mcs, su_step, ms_run, sim_path=0):
                 "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "traffic_source": src, "measured": measured,
                 "peak_source": peaks["source"], "launches_per_step": n_launch, "algorithmic_bytes_per_launch": bytes_launch}
     slots = ALU_SLOTS_PER_SU.get(cfg_key)
-    kname = {1: "kpz_k1_sweep_jit", 3: "kpz_k3t_sweep_jit"}.get(path, "kpz_k1_sweep_jit") if cfg["kind"] == "kpz" \
+    kname = {1: "kpz_k1_sweep_jit", 2: "kpz_k3_pass_jit", 3: "kpz_k3t_sweep_jit"}.get(path, "kpz_k1_sweep_jit") if cfg["kind"] == "kpz" \
         else ({1: "kpz2d_k5s_jit", 3: "kpz2d_k5c_jit"}.get(sim_path, "kpz2d_k5_pass_jit") if cfg["kind"] == "kpz2d"
               else "lanes_k4_sweep_jit")
     if slots is None:

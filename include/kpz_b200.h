@@ -239,7 +239,7 @@ int kpz_path(const kpz_sim*, int32_t* path);
  * compiled generic kernels instead of the run-time specialised ones; "K1J_<X>=v" / "K4J_<X>=v" / "K5J_<X>=v" are appended
  * as definitions to every later run-time compilation of the KPZ / two-lane / 2+1D sweep kernels (the knobs documented at
  * the top of csrc/k1_sweep_jit.cuh and csrc/k4_lanes_jit.cuh; 2+1D: K5J_RIW=0 no shuffles, K5J_PIPE=0 no software
- * pipeline in the on-chip kernel, K5J_CS=2|4|8|16 cluster size, K5J_NBR=1 neighbour-only barriers, K5J_DUAL=1 two samples per cluster, K5J_XRALL=1 every warp
+ * pipeline in the on-chip kernel, K5J_CS=2|4|8|16 cluster size, K5J_NBR=1 neighbour-only barriers, K5J_DUAL=1 two samples per cluster, K5J_PDL=0 no programmatic dependent launch of the streamed passes, K5J_XRALL=1 every warp
  * through shared::cluster addresses in the cluster kernel).  Every setting computes the same results (tests/ check that);
  * kpz_run / lanes_run read no environment variable.  KPZ_EINVAL for anything else. */
 int kpz_debug_config(const char* spec);

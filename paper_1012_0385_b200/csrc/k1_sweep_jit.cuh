@@ -74,6 +74,9 @@
 #ifndef K1J_QUEUE  // per-sample kernel, > 0: the run is cut into chunks of K1J_QUEUE MCS and the CTAs pull (sample, chunk)
 #define K1J_QUEUE 0  // items from a counter in chunk-major order, parking the ring in HBM between chunks (exact: the RNG is
 #endif               // counter-based, it is run(a); run(b)).  Balances rings over SMSPs that hold different numbers of warps.
+#ifndef K1J_PDL  // pass-by-pass stream (K3): programmatic dependent launch of consecutive passes (set by the host)
+#define K1J_PDL 0
+#endif
 #ifndef K1J_HALOCHECK  // debug (compute-sanitizer's racecheck is closed on the GPU pool): every word published through
 #define K1J_HALOCHECK 0  // the shared-memory halo carries the number of its exchange; a reader that finds another number
 #endif                   // - a slot not yet written, or already overwritten by a later exchange - counts an error
@@ -628,6 +631,12 @@ extern "C" __global__ void __launch_bounds__(256)
 kpz_k3_pass_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::K3Pass A) {
   using namespace kpz;
   using namespace kpz::k1j;
+#if K1J_PDL
+  // Programmatic dependent launch (the host sets the launch attribute): the NEXT pass may start to launch while this
+  // one runs; its threads draw their planes - which depend on nothing in memory - and only then wait for this pass to
+  // be complete and visible.  Hides the launch gap between two passes.
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
   const unsigned long long gid = (unsigned long long)blockIdx.x * 256ull + threadIdx.x;
   if (gid >= (unsigned long long)D.S * U) return;
   const int s = (int)(gid / U);
@@ -635,6 +644,25 @@ kpz_k3_pass_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ k
   const int nw = PARTIAL ? min(4, PW - 4 * u) : 4;
   const unsigned long long srow = (unsigned long long)s * PWp;
   const unsigned long long row = srow + 4ull * u;
+  const uint32_t gs = (uint32_t)(D.first_sample + s);
+  const uint32_t tlo = (uint32_t)A.m, thi = (uint32_t)((unsigned long long)A.m >> 32);
+  uint32_t r[NPSA][4];
+  if (A.fo) {  // a kernel parameter: no memory is read before the wait below
+    uint32_t keep = 0u;
+#pragma unroll
+    for (int pl = 0; pl < NEAG; ++pl) {
+      const uint4 v = philox4x32_10((uint32_t)u, gs, tlo, ctr3(TAG_PAIR, (uint32_t)A.pass, (uint32_t)pl, thi), D.keys);
+      r[pl][0] = v.x; r[pl][1] = v.y; r[pl][2] = v.z; r[pl][3] = v.w;
+      keep ^= v.x ^ v.y ^ v.z ^ v.w;
+    }
+#if K1J_PDL
+    asm volatile("" ::"r"(keep));  // the planes are computed BEFORE the wait
+#endif
+    (void)keep;
+  }
+#if K1J_PDL
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
   const uint32_t fin = A.fin[s];
   const uint32_t o = A.fo ? A.fo[s] : 0u;
   uint32_t P[4], Q[4];
@@ -664,14 +692,6 @@ kpz_k3_pass_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ k
       const uint4 x = *reinterpret_cast<const uint4*>((o ? D.SQE : D.SQO) + row);
       sqb[0] = x.x; sqb[1] = x.y; sqb[2] = x.z; sqb[3] = x.w;
       if (o) shift_up_words(sqb, nw, D.SQE[srow + 4ull * nxt], 1u);
-    }
-    const uint32_t gs = (uint32_t)(D.first_sample + s);
-    const uint32_t tlo = (uint32_t)A.m, thi = (uint32_t)((unsigned long long)A.m >> 32);
-    uint32_t r[NPSA][4];
-#pragma unroll
-    for (int pl = 0; pl < NEAG; ++pl) {
-      const uint4 v = philox4x32_10((uint32_t)u, gs, tlo, ctr3(TAG_PAIR, (uint32_t)A.pass, (uint32_t)pl, thi), D.keys);
-      r[pl][0] = v.x; r[pl][1] = v.y; r[pl][2] = v.z; r[pl][3] = v.w;
     }
     const uint32_t M = 0u - o;
     if constexpr (!GENERAL) {

@@ -169,6 +169,7 @@ std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, int entry, size_t sme
   add("K5J_DUAL", cl ? cl->dual : 0);
   add("K5J_RIW", debug_int("K5J_RIW", 1));
   add("K5J_PIPE", debug_int("K5J_PIPE", 1));
+  add("K5J_PDL", debug_int("K5J_PDL", 1));  // streamed kernel: programmatic dependent launch of consecutive passes
   add("K5J_NBR", debug_int("K5J_NBR", 0));  // neighbour-only mbarriers: measured slower than barrier.cluster (r02_summary §6)
   if (debug_has("K5J_XRALL")) add("K5J_XRALL", debug_int("K5J_XRALL", 0));
   return d;
@@ -416,6 +417,7 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
   const PassFn pass_fn = D.RH % 4 == 0 ? (two_planes(D) ? k2d_pass<true, true> : k2d_pass<true, false>)
                                        : (two_planes(D) ? k2d_pass<false, true> : k2d_pass<false, false>);
   void* pass_jit = nullptr;
+  const bool pdl = debug_int("K5J_PDL", 1) != 0;
   if (jit_enabled()) {
     int rc = jit_get("kpz2d_k5.cuh", "kpz2d_k5_pass_jit", k5_jit_defines(D, 3, 0), &pass_jit);
     if (rc) return rc;
@@ -437,7 +439,16 @@ int kpz2d_run(kpz2d_sim* sim, int64_t n_mcs) {
         long long m_arg = m;
         int ps_arg = ps;
         void* args[] = {(void*)&D, (void*)&off_k, (void*)&m_arg, (void*)&ps_arg};
-        KPZ_CUDA_CHECK(cudaLaunchKernel(pass_jit, dim3(nblocks), dim3(128), args, 0, sim->stream));
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(nblocks);
+        cfg.blockDim = dim3(128);
+        cfg.stream = sim->stream;
+        cudaLaunchAttribute at{};
+        at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at.val.programmaticStreamSerializationAllowed = 1;  // the next pass may start to launch while this one runs
+        cfg.attrs = &at;
+        cfg.numAttrs = pdl ? 1 : 0;
+        KPZ_CUDA_CHECK(cudaLaunchKernelExC(&cfg, pass_jit, args));
         count_launch();
       } else {
         pass_fn<<<nblocks, 128, 0, sim->stream>>>(D, sim->off + (size_t)k * D.S, m, ps);

@@ -343,8 +343,12 @@ __device__ __forceinline__ void sweep_ragged_supergroup(uint32_t* EX, uint32_t* 
 
 // K5: one colour pass (MCS m, pass ps) of every sample, in place.  off[s] = colour offset o of this pass.  Thread =
 // (sample, supergroup); on the fast path the supergroups of a sample are taken by row parity, so a warp has one colour.
-template <bool ROWALIGNED, bool TWO>
+// PDL (programmatic dependent launch; the host sets the launch attribute): the launch of the NEXT pass may begin while this
+// one is still running - its threads draw their planes, which depend on nothing in memory, and only then wait
+// (griddepcontrol.wait) for this pass to be complete and visible.  Hides the launch gap between two passes.
+template <bool ROWALIGNED, bool TWO, bool PDL = false>
 __device__ __forceinline__ void pass_body(const Kpz2dDev& D, const unsigned char* __restrict__ off, long long m, int ps) {
+  if constexpr (PDL) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const Shape2d sh = shape2d(D);
   const long long gid = (long long)blockIdx.x * 128 + threadIdx.x;
   const bool live = gid < (long long)D.S * sh.n_sg;
@@ -354,7 +358,6 @@ __device__ __forceinline__ void pass_body(const Kpz2dDev& D, const unsigned char
   uint32_t *EX = D.EX + base, *OX = D.OX + base, *EY = D.EY + base, *OY = D.OY + base;
   const Rates2d r = make_rates2d(D);
   const uint32_t gs = (uint32_t)(D.first_sample + s), tlo = (uint32_t)m, thi = (uint32_t)((unsigned long long)m >> 32);
-  const uint32_t o = off[s];
   if constexpr (ROWALIGNED) {
     const int sgr = sh.RH / 4, nh = sh.n_sg / 2;  // supergroups per row; per row parity
     const int h = i >= nh ? 1 : 0, ii = i - h * nh;
@@ -362,16 +365,26 @@ __device__ __forceinline__ void pass_body(const Kpz2dDev& D, const unsigned char
     const int P0 = y * sh.RH + 4 * kq, P1 = (y + 1 == sh.Ly ? 0 : y + 1) * sh.RH + 4 * kq;
     const int NX = y * sh.RH + (kq + 1 == sgr ? 0 : 4 * (kq + 1));
     const uint32_t G = (uint32_t)(y * sgr + kq);
+    Planes2 R;
+    const Planes2* pre = nullptr;
+    if constexpr (PDL && TWO) {  // drawn before anything of the previous pass is needed
+      R = draw_two(D.keys, G, gs, tlo, thi, (uint32_t)ps);
+      asm volatile("" ::"r"(R.v0.x), "r"(R.v0.y), "r"(R.v0.z), "r"(R.v0.w), "r"(R.v1.x), "r"(R.v1.y), "r"(R.v1.z), "r"(R.v1.w));
+      pre = &R;
+    }
+    if constexpr (PDL) asm volatile("griddepcontrol.wait;" ::: "memory");
+    const uint32_t o = off[s];
     // one colour per warp whenever nh is a multiple of 32; a warp that straddles samples or parities goes word by word
     const unsigned c1 = __ballot_sync(0xFFFFFFFFu, (((uint32_t)h + o) & 1u) != 0u);
     if (c1 == 0xFFFFFFFFu)
-      sweep_row_supergroup<TWO, 1, false>(EX, OX, EY, OY, P0, P1, NX, kq, sgr, G, live, r, D.keys, gs, tlo, thi, (uint32_t)ps);
+      sweep_row_supergroup<TWO, 1, false>(EX, OX, EY, OY, P0, P1, NX, kq, sgr, G, live, r, D.keys, gs, tlo, thi, (uint32_t)ps, pre);
     else if (c1 == 0u)
-      sweep_row_supergroup<TWO, 0, false>(EX, OX, EY, OY, P0, P1, NX, kq, sgr, G, live, r, D.keys, gs, tlo, thi, (uint32_t)ps);
+      sweep_row_supergroup<TWO, 0, false>(EX, OX, EY, OY, P0, P1, NX, kq, sgr, G, live, r, D.keys, gs, tlo, thi, (uint32_t)ps, pre);
     else
       sweep_ragged_supergroup<TWO>(EX, OX, EY, OY, sh.RH, sh.Ly, sh.n_ew, (int)G, live, o, r, D.keys, gs, tlo, thi, (uint32_t)ps);
   } else {
-    sweep_ragged_supergroup<TWO>(EX, OX, EY, OY, sh.RH, sh.Ly, sh.n_ew, i, live, o, r, D.keys, gs, tlo, thi, (uint32_t)ps);
+    if constexpr (PDL) asm volatile("griddepcontrol.wait;" ::: "memory");
+    sweep_ragged_supergroup<TWO>(EX, OX, EY, OY, sh.RH, sh.Ly, sh.n_ew, i, live, off[s], r, D.keys, gs, tlo, thi, (uint32_t)ps);
   }
 }
 
@@ -1009,7 +1022,7 @@ extern "C" __global__ void __cluster_dims__(K5J_CS, 1, 1) __launch_bounds__(K5J_
 #if K5J_ENTRY == 0 || K5J_ENTRY == 3
 extern "C" __global__ void __launch_bounds__(128)
     kpz2d_k5_pass_jit(const __grid_constant__ Kpz2dDev D, const unsigned char* __restrict__ off, long long m, int ps) {
-  pass_body<kJRowAligned, K5J_TWO != 0>(D, off, m, ps);
+  pass_body<kJRowAligned, K5J_TWO != 0, K5J_PDL != 0>(D, off, m, ps);
 }
 #endif
 #else

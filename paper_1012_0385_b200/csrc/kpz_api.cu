@@ -332,6 +332,9 @@ K3Fn k3_pick_dis(int dis, int nps) {
   }
 }
 
+// "K1J_PDL=0" (kpz_debug_config) launches consecutive passes of the streamed kernel without programmatic dependent launch
+bool k3_pdl() { return debug_int("K1J_PDL", 1) != 0; }
+
 int k3_launch_pass(kpz_sim* sim, K3Fn fn, void* jitfn, const unsigned char* fin, const unsigned char* fo, long long m,
                    int pass) {
   KpzDev D = sim->dev;
@@ -347,7 +350,16 @@ int k3_launch_pass(kpz_sim* sim, K3Fn fn, void* jitfn, const unsigned char* fin,
   const size_t nunits = (size_t)D.S * D.U;
   if (jitfn) {
     void* args[] = {(void*)&D, (void*)&A};
-    KPZ_CUDA_CHECK(cudaLaunchKernel(jitfn, dim3((unsigned)((nunits + 255) / 256)), dim3(256), args, 0, sim->stream));
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)((nunits + 255) / 256));
+    cfg.blockDim = dim3(256);
+    cfg.stream = sim->stream;
+    cudaLaunchAttribute at{};
+    at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at.val.programmaticStreamSerializationAllowed = 1;  // the next pass may start to launch while this one runs (K1J_PDL)
+    cfg.attrs = &at;
+    cfg.numAttrs = k3_pdl() ? 1 : 0;
+    KPZ_CUDA_CHECK(cudaLaunchKernelExC(&cfg, jitfn, args));
   } else {
     fn<<<(unsigned)((nunits + 255) / 256), 256, 0, sim->stream>>>(D, A);
   }
@@ -390,7 +402,9 @@ int k3_run(kpz_sim* sim, int64_t n_mcs) {
   if (jit_enabled()) {
     std::vector<std::string> defs = k1_jit_defines(D0, dis);
     drop_define(&defs, "K1J_UPT");
+    drop_define(&defs, "K1J_PDL");
     defs.push_back("K1J_STREAM=1");
+    defs.push_back(k3_pdl() ? "K1J_PDL=1" : "K1J_PDL=0");
     int rcj = jit_get("k1_sweep_jit.cuh", "kpz_k3_pass_jit", defs, &jitfn);
     if (rcj) return rcj;
   }
@@ -677,7 +691,6 @@ int kpz_jit_check(int64_t L, double p, double q, const kpz_disorder* disorder, c
   int path;
   rc = choose_path(L, opt, &path);
   if (rc) return rc;
-  if (path == KPZ_PATH_STREAM) return KPZ_OK;
   kpz_sim tmp;
   tmp.has_sp = disorder && d.prob_slow_p > 0.0;
   tmp.has_sq = disorder && d.prob_slow_q > 0.0;
@@ -694,13 +707,19 @@ int kpz_jit_check(int64_t L, double p, double q, const kpz_disorder* disorder, c
   D.PWp = (D.PW + 3) / 4 * 4;
   D.U = D.PWp / 4;
   const int dis_c = tmp.has_sq ? 2 : tmp.has_sp ? 1 : 0;
-  std::vector<std::string> defs = path == KPZ_PATH_BLOCKED ? k1_jit_defines(D, dis_c) : k1_shape(D, 1, dis_c).defs;
+  std::vector<std::string> defs = path == KPZ_PATH_ONCHIP ? k1_shape(D, 1, dis_c).defs : k1_jit_defines(D, dis_c);
   if (path == KPZ_PATH_BLOCKED) {
     drop_define(&defs, "K1J_UPT");
     defs.push_back("K1J_TILE=1");
+  } else if (path == KPZ_PATH_STREAM) {  // as k3_run asks for it
+    drop_define(&defs, "K1J_UPT");
+    drop_define(&defs, "K1J_PDL");
+    defs.push_back("K1J_STREAM=1");
+    defs.push_back(k3_pdl() ? "K1J_PDL=1" : "K1J_PDL=0");
   }
-  rc = jit_compile("k1_sweep_jit.cuh", path == KPZ_PATH_BLOCKED ? "kpz_k3t_sweep_jit" : "kpz_k1_sweep_jit", defs, &cubin,
-                   nullptr);
+  rc = jit_compile("k1_sweep_jit.cuh",
+                   path == KPZ_PATH_BLOCKED ? "kpz_k3t_sweep_jit" : path == KPZ_PATH_STREAM ? "kpz_k3_pass_jit" : "kpz_k1_sweep_jit",
+                   defs, &cubin, nullptr);
   if (rc) return rc;
   *cubin_bytes = cubin.size();
   return KPZ_OK;

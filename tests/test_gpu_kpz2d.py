@@ -70,10 +70,11 @@ def run_both_2d(K, Lx, Ly, S, p, q, seed, times, chunks, first_sample=0, offset_
 # (NVRTC: shape and thresholds are constants) and as the generic kernel of the library build ("jit=0"); K5J_RIW=0 takes
 # the shuffles out of the specialised on-chip kernel (neighbour word loaded, carries by atomics), K5J_PIPE=0 its
 # software pipeline (planes drawn one sweep ahead around a split barrier)
+# K5J_PDL=0: consecutive passes of the streamed kernel launched without programmatic dependent launch
 # 3 = a sample spread over a thread-block cluster (K5C; 2 CTAs unless K5J_CS forces 4, 8 or 16), rows of the neighbour CTA
 # through distributed shared memory, one barrier.cluster per pass (K5J_NBR=1: the CTAs synchronise with their two neighbours
 # only, through mbarriers); shapes without a cluster decomposition are refused (and skipped here)
-PATHS = [(1, ""), (2, ""), (1, "jit=0"), (2, "jit=0"), (1, "K5J_RIW=0"), (1, "K5J_PIPE=0"), (3, ""), (3, "K5J_CS=4"),
+PATHS = [(1, ""), (2, ""), (2, "K5J_PDL=0"), (1, "jit=0"), (2, "jit=0"), (1, "K5J_RIW=0"), (1, "K5J_PIPE=0"), (3, ""), (3, "K5J_CS=4"),
          (3, "K5J_CS=8"), (3, "K5J_CS=16"), (3, "K5J_RIW=0"), (3, "K5J_NBR=1"), (3, "K5J_DUAL=1"), (3, "K5J_DUAL=1;K5J_CS=4")]
 
 

@@ -464,6 +464,15 @@ def test_k1_work_queue_against_oracle(K, cfg):
         run_both_kpz(K, 40960, 3, 0.8, 0.1, disorder=(0.3, 0.2, 0.3, 0.05), seed=83, times=[20], chunks=[13, 7])
 
 
+def test_streamed_kernel_without_programmatic_dependent_launch(K):
+    """The specialised pass-by-pass kernel launches consecutive passes with programmatic dependent launch (a pass draws
+    its planes while the pass before it finishes, then waits for it); K1J_PDL=0 is the plain stream order.  The default
+    (PDL) is what every other path-2 test runs."""
+    with K.debug_config("K1J_PDL=0"):
+        run_both_kpz(K, 65536 + 64, 2, 0.9, 0.1, seed=24, times=[2, 9], chunks=[4, 5], path=2)
+        run_both_kpz(K, 320, 3, 0.75, 0.25, disorder=(0.2, 0.25, 0.3, 0.5), seed=5, times=[2, 40], chunks=[40], path=2)
+
+
 def test_static_streamed_kernel_against_oracle(K):
     with K.debug_config("jit=0"):
         gpu, _ = run_both_kpz(K, 65536 + 64, 2, 0.9, 0.1, seed=24, times=[2, 9], chunks=[4, 5], path=2)
