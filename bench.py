@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — site-update throughput of the KPZ/ASEP hot path on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1|2|3|4|5|4-aux-i|4-aux-ii|2d-1024|2-fill|3-fill|paper-...]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1|2|3|4|5|4-aux-i|4-aux-ii|2d-512|2d-1024|2d-2048|2d-32768|2-fill|3-fill|paper-...]
                     [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: reset to the
@@ -12,7 +12,7 @@ Default (`--config all`): BASELINE.json's `metric` names no configuration, so th
 `ms_per_step`, `config.workload`, `roofline`, `cpu_baseline`, `e2e`, `clocks`) is the LARGEST single-GPU configuration,
 config 3 (512 rings x 16384 sites x 10^5 MCS = 8.39e11 site updates), and the same line carries one full sub-record
 per other BASELINE configuration (1, 2, 4, 5), for the two auxiliary streamed runs of SURVEY §8(d) (4-aux-i: L=2^28
-ring in L2; 4-aux-ii: L=2^32, the HBM roofline case) and for the 2+1D workload 2d-512 under `"per_config"`, each timed with its own K steps after W
+ring in L2; 4-aux-ii: L=2^32, the HBM roofline case) and for the 2+1D workloads 2d-512 / 2d-1024 under `"per_config"`, each timed with its own K steps after W
 warm-up steps.  `--config X` runs one workload only.
 
 value      site updates / s (GSU/s) of the whole job, device-timed (CUDA events on the launching stream), inputs
