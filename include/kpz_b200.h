@@ -211,7 +211,8 @@ int kpz2d_time(const kpz2d_sim*, int64_t* t);
  * the shared memories of a thread-block cluster of 2, 4, 8 or 16 CTAs, neighbour rows through distributed shared memory,
  * one persistent launch (auto beyond 96 KiB when Lx is a multiple of 256 and the rows divide, up to 1600 KiB per sample,
  * e.g. 1024 x 1024 on 8 CTAs, 2048 x 2048 on 16 - the non-portable cluster size, used when the device says it can hold
- * one; run-time specialised kernels only); 2 = one in-place launch per colour pass (everything else). */
+ * one; run-time specialised kernels only); 2 = one in-place launch per colour pass (everything else), consecutive passes
+ * launched with programmatic dependent launch. */
 int kpz2d_path(const kpz2d_sim*, int32_t* path);
 int kpz2d_reset(kpz2d_sim*);                                          /* flat surface, t = 0, records dropped; async */
 int kpz2d_slopes(kpz2d_sim*, uint32_t* d_sx, uint32_t* d_sy);        /* copy out (either may be NULL); async */
@@ -258,7 +259,7 @@ int lanes_jit_check(int64_t L, double p_a, double p_b, double turn_prob, int64_t
                     const kpz_options* opt, size_t* cubin_bytes); /* same for the two-lane kernel */
 int lanes_crossing_jit_check(int64_t L, double p_a, double p_b, const lanes_crossing* crossing, int64_t turn_period,
                              const kpz_options* opt, size_t* cubin_bytes);
-/* Same for the 2+1D kernels (K5 / K5S, specialised on Lx, Ly and the thresholds of p, q): the kernel kpz2d_run would use
+/* Same for the 2+1D kernels (K5 / K5S / K5C, specialised on Lx, Ly and the thresholds of p, q): the kernel kpz2d_run would use
  * for these parameters and options.path. */
 int kpz2d_jit_check(int32_t Lx, int32_t Ly, double p, double q, const kpz_options* opt, size_t* cubin_bytes);
 
