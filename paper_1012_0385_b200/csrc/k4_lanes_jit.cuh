@@ -675,7 +675,14 @@ __device__ __forceinline__ uint32_t draw_offsets16(const PhiloxKeys& K, uint32_t
 }  // namespace kpz
 
 // grid = S samples, block = NTHREADS; thread u = supergroup u (idle when u >= U, but it joins every barrier / shuffle).
+#ifndef K4J_MINB  // CTAs per SM the kernel is compiled for (0: left to the compiler).  1: with ~1.7 warps per SMSP registers
+#define K4J_MINB 1  // are free, and the compiler's looser schedule is worth +2 % on config 5 (measured)
+#endif
+#if K4J_MINB > 0
+extern "C" __global__ void __launch_bounds__(kpz::k4j::NTHREADS, K4J_MINB)
+#else
 extern "C" __global__ void __launch_bounds__(kpz::k4j::NTHREADS)
+#endif
 lanes_k4_sweep_jit(const __grid_constant__ kpz::LanesDev D, const __grid_constant__ kpz::LanesRunArgs R) {
   using namespace kpz;
   using namespace kpz::k4j;
