@@ -888,7 +888,14 @@ kpz_k1_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ 
 // information by one site, so after k passes only the outer k+1 sites of the window are contaminated: the two end
 // units (256 sites each) absorb up to 127 MCS.  The random numbers are counter-based - keyed by the GLOBAL unit index
 // - so the halo units a neighbouring warp recomputes are bit-identical, and the result equals the pass-by-pass sweep.
+#ifndef K1J_TILE_MINB  // CTAs per SM this kernel is compiled for (0: left to the compiler, which takes 114 registers; 4: 120
+#define K1J_TILE_MINB 4  // registers and a slightly better schedule: config 4 +1.7 %; 5 ... 8 CTAs: no further gain, measured)
+#endif
+#if K1J_TILE_MINB > 0
+extern "C" __global__ void __launch_bounds__(128, K1J_TILE_MINB)
+#else
 extern "C" __global__ void __launch_bounds__(128)
+#endif
 kpz_k3t_sweep_jit(const __grid_constant__ kpz::KpzDev D, const __grid_constant__ kpz::K3TArgs A) {
   using namespace kpz;
   using namespace kpz::k1j;
