@@ -163,7 +163,7 @@ std::vector<std::string> k5_jit_defines(const Kpz2dDev& D, int entry, size_t sme
   add("K5J_TQ_ALWAYS", D.t_q.always);
   add("K5J_TWO", two_planes(D) ? 1 : 0);
   // CTAs per SM the on-chip kernel is compiled for: two when two samples fit the shared memory of an SM
-  add("K5J_MINB", cl ? cl->minb : (smem != 0 && 2 * (smem + 1024) <= 227 * 1024 ? 2 : 1));
+  add("K5J_MINB", debug_int("K5J_MINB", cl ? cl->minb : (smem != 0 && 2 * (smem + 1024) <= 227 * 1024 ? 2 : 1)));
   add("K5J_CS", cl ? cl->cs : 1);
   add("K5J_THREADS", cl ? cl->threads : 512);
   add("K5J_DUAL", cl ? cl->dual : 0);
