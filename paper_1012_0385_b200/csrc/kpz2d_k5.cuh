@@ -1,4 +1,4 @@
-// kpz2d_k5.cuh — K5 / K5S: checkerboard sweep of the 2+1D generalisation ("two-sub-lattice
+// kpz2d_k5.cuh — K5 / K5S / K5C: checkerboard sweep of the 2+1D generalisation ("two-sub-lattice
 // updates, which can be generalized to checker-board lattice decomposition in two dimensions"): the dimer /
 // octahedron move of ref. [7] - a site moves when its x-pair AND its y-pair of slopes are both (1,0) (forward, rate p) or
 // both (0,1) (backward, rate q).  Product code (CUDA path); shares nothing with oracle/.
@@ -28,10 +28,13 @@
 // blocks, so a warp's access is conflict-free without padding).  Threads are mapped to supergroups BY ROW PARITY (first
 // all even rows, then all odd rows), so the colour is uniform over a warp - over the whole CTA on chip - and each colour
 // runs its own straight-line code.
-//   k2d_pass    one launch = one colour pass of every sample, in place in HBM / L2 (lattices beyond shared memory);
-//   k2d_onchip  one CTA per sample, persistent over the whole kpz2d_run, all four planes in shared memory (64 KiB for
-//               512 x 512), rows stored by parity (even rows first): global memory is touched at the start and the end
-//               of the launch only.
+//   K5  (pass_body: k2d_pass / kpz2d_k5_pass_jit)  one launch = one colour pass of every sample, in place in HBM / L2
+//       (lattices beyond every on-chip variant); consecutive passes by programmatic dependent launch;
+//   K5S (onchip_body: k2d_onchip / kpz2d_k5s_jit)  one CTA per sample, persistent over the whole kpz2d_run, all four planes
+//       in shared memory (64 KiB for 512 x 512), rows stored by parity (even rows first): global memory is touched at the
+//       start and the end of the launch only; planes drawn one sweep ahead around a split barrier;
+//   K5C (cluster_body: kpz2d_k5c_jit)  the same with a sample spread over a thread-block cluster of 2 ... 16 CTAs, the
+//       neighbour CTA's first row through distributed shared memory (1024 x 1024, 2048 x 2048).
 #pragma once
 #include "rtc_prelude.cuh"
 #include "philox.cuh"
